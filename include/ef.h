@@ -1,0 +1,183 @@
+/*
+ * ef.h -- C ABI of libef: the MoE expert layer running against a GPU-resident expert cache
+ * (ExpertFlow, arxiv 2410.17954), hand-written CUDA for sm_100a (B200).
+ *
+ * Citations: P:L<n> = PAPER.md line n.  R<n> = reading n in DESIGN.md §3 (where the paper is silent).
+ *
+ * Conventions
+ *   - Every function returns int32_t: EF_OK (0) or a negative EF_ERR_* code.  No exceptions, no
+ *     aborts, no output on stdout.  ef_last_error(ctx) returns text for the last failure.
+ *   - "device" pointers are CUDA device pointers on ctx's device, 16-byte aligned, row-major,
+ *     contiguous.  "host" pointers are ordinary host memory unless "pinned" is stated.
+ *   - bf16 tensors are passed as `const void*` / `void*` (2 bytes per element).
+ *   - `stream` is a cudaStream_t passed as void* (e.g. torch.cuda.current_stream().cuda_stream).
+ *     All device work of a call is enqueued on it and the call returns without waiting, unless
+ *     "synchronous" is stated.  Weight copies run on the library's own copy stream and are ordered
+ *     against `stream` with events.
+ *   - Ownership: the caller owns every activation / index buffer.  The library owns the slot
+ *     arena, copy stream, events, workspaces, the slot table and -- after ef_host_expert_register --
+ *     a packed copy of each expert in its own pinned host pool (every expert is backed up
+ *     on the host, so eviction needs no write-back).
+ *   - One ctx per GPU; calls on one ctx must not run concurrently.
+ *   - Shape limits: d_model % 64 == 0, d_ff % 128 == 0, 1 <= top_k <= 8, top_k <= n_experts <= 256.
+ *
+ * Logical clock: visit = step * n_layers + layer.  The cache policy depends only on the sequence
+ * of calls and their arguments, never on whether a copy or kernel has physically finished (R9).
+ */
+#ifndef EF_H_
+#define EF_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EF_OK 0
+#define EF_ERR_INVALID_ARG (-1)
+#define EF_ERR_UNSUPPORTED (-2)    /* shape / alignment outside the limits above */
+#define EF_ERR_CUDA (-3)           /* a CUDA call failed; sticky */
+#define EF_ERR_OOM (-4)
+#define EF_ERR_NOT_REGISTERED (-5) /* an expert that must be loaded was never registered */
+#define EF_ERR_CAPACITY (-6)       /* more tokens than max_tokens, more groups than slots, ... */
+
+typedef struct ef_ctx ef_ctx;
+
+typedef struct {
+    int32_t n_layers;          /* L: layers sharing the one global slot pool (R7) */
+    int32_t n_experts;         /* E: routed experts per layer */
+    int32_t top_k;             /* k */
+    int32_t d_model;           /* d */
+    int32_t d_ff;              /* f */
+    int32_t n_slots;           /* S: cache slots, each holds one routed expert (3*d*f*2 bytes) */
+    int32_t n_shared;          /* always-resident shared experts per layer, outside the pool (R19) */
+    int32_t max_tokens;        /* largest T of any call */
+    int32_t prefetch_horizon;  /* H: visits ahead ef_cache_prefetch may load for; <= 0: as far as supplied (R10) */
+    int32_t device;            /* CUDA device ordinal */
+} ef_config;
+
+typedef struct {
+    uint64_t lookups;          /* active (visit, expert) pairs seen by ef_expert_ffn_grouped (R6) */
+    uint64_t hits;             /* ... found in the slot table (present or in flight) */
+    uint64_t misses;           /* ... not found: loaded on demand ("on-demand experts") */
+    uint64_t prefetch_issued;  /* loads started by ef_cache_prefetch */
+    uint64_t prefetch_used;    /* prefetched experts whose first use was a hit */
+    uint64_t prefetch_wasted;  /* prefetched experts evicted before any use ("mis-prefetched") */
+    uint64_t ondemand_loads;   /* == misses */
+    uint64_t evictions;        /* occupied slots overwritten or dropped */
+    uint64_t bytes_h2d;        /* bytes copied host -> device for expert weights */
+} ef_cache_stats;
+
+/* ---- lifetime ------------------------------------------------------------------------------ */
+
+/* Allocates the slot arena ((S + L*n_shared) * 3*d*f*2 bytes), workspaces, copy stream, events.
+ * Synchronous.  *out is NULL on failure. */
+int32_t ef_create(const ef_config* cfg, ef_ctx** out);
+int32_t ef_destroy(ef_ctx* ctx);
+
+/* Register expert `expert` of `layer` (expert < 0: shared expert -1-expert, which is also copied to
+ * its resident device slot).  w_gate, w_up: [f, d] bf16; w_down: [d, f] bf16; HOST pointers, read
+ * during the call only (the library packs them into its pinned pool).  Synchronous. */
+int32_t ef_host_expert_register(ef_ctx* ctx, int32_t layer, int32_t expert, const void* w_gate,
+                                const void* w_up, const void* w_down);
+
+/* Make (layer, expert) share the packed host buffer already registered for (src_layer, src_expert):
+ * lets a 90 GB logical pool (BASELINE.json cfg 5) run on a host that cannot pin that much.  Bytes
+ * moved, policy and accounting are unchanged. */
+int32_t ef_host_expert_alias(ef_ctx* ctx, int32_t layer, int32_t expert, int32_t src_layer, int32_t src_expert);
+
+/* ---- a1: router (Eq. 1-2; top-k per P:L52; R1-R3) -------------------------------- */
+
+/* logits[t,e] = sum_c x[t,c] * w_router[e,c] + bias[t*bias_token_stride + e]   (fp32 accumulate)
+ * topk_idx[t,:] = the k largest logits' experts, descending, ties -> lower index (R2)
+ * topk_w[t,j]   = exp(l_j - max) / Z,  Z over the k selected (renorm=1) or over all E (renorm=0, Eq. 1)
+ * x: [T, d] bf16 device.  w_router: [E, d] bf16 device.  bias: fp32 device, nullable;
+ * bias_token_stride 0 (per expert, [E]) or E (per token, [T,E]).  topk_idx: [T,k] int32, topk_w: [T,k]
+ * fp32, logits_out: [T,E] fp32 nullable -- all device.  T may be 0. */
+int32_t ef_route_topk(ef_ctx* ctx, void* stream, const void* x, const void* w_router, const float* bias,
+                      int64_t bias_token_stride, int32_t T, int32_t renorm, int32_t* topk_idx, float* topk_w,
+                      float* logits_out);
+
+/* ---- a2: permute (dispatch implied by P:L21; R5) ------------------------------------- */
+
+/* Stable counting sort of the flat pairs p = t*k + j by topk_idx[p]:
+ *   counts[E], offsets[E+1] (exclusive scan), inv[p] = row, src[row] = p, x_perm[row,:] = x[p / k,:].
+ * All device.  counts_host_pinned: nullable PINNED host int32[E] that also receives counts; when
+ * NULL the library mirrors counts into its own pinned buffer.  Either way an internal event marks
+ * the mirror complete and ef_expert_ffn_grouped(counts_host = NULL) waits on it. */
+int32_t ef_permute(ef_ctx* ctx, void* stream, const int32_t* topk_idx, const void* x, int32_t T, void* x_perm,
+                   int32_t* counts, int32_t* offsets, int32_t* src, int32_t* inv, int32_t* counts_host_pinned);
+
+/* ---- a3 + a4: cache lookup, real-time correction, grouped SwiGLU expert FFN ----------------- */
+
+/* For each expert e of `layer` with counts[e] > 0, rows [offsets[e], offsets[e+1]) of x_perm:
+ *   y_perm[r,:] = ( silu(x_perm[r,:] Wg_e^T) * (x_perm[r,:] Wu_e^T) ) Wd_e^T      (bf16 in, fp32 accumulate)
+ * with the weights read from the cache slot holding (layer, e).  Experts not resident are loaded on
+ * demand into victim slots (victim classes R8-R13) on the copy stream while resident
+ * experts compute; compute is issued in waves gated by per-slot events.  Updates the counters.
+ * counts_host: host int32[E] (what the gate actually selected); NULL = use the mirror written by the
+ * last ef_permute, which makes this call wait for that kernel (the one device->host sync per visit,
+ * P:L128 "based on the MoE gate's output").  x_perm: [T*k, d] bf16 device; y_perm: [T*k, d] bf16 device.
+ * The intermediate h lives in a library workspace. */
+int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visit, int32_t layer, const void* x_perm,
+                              const int32_t* counts_host, void* y_perm);
+
+/* Kernel-only variant for roofline timing and stage tests: no lookup, no loads, no counters.
+ * Group i applies the expert held in cache slot slots[i] to rows [row_begin[i], row_begin[i]+rows[i]).
+ * row_begin, rows, slots: HOST int32[n_groups]. */
+int32_t ef_expert_ffn_grouped_resident(ef_ctx* ctx, void* stream, const void* x_perm, int32_t n_groups,
+                                       const int32_t* row_begin, const int32_t* rows, const int32_t* slots,
+                                       void* y_perm);
+
+/* Shared experts of `layer` applied to every token (R19): y_shared[s*T + t, :] = FFN_shared_s(x[t,:]).
+ * x: [T,d] bf16 device; y_shared: [n_shared*T, d] bf16 device. */
+int32_t ef_shared_ffn(ef_ctx* ctx, void* stream, int32_t layer, const void* x, int32_t T, void* y_shared);
+
+/* ---- a5: combine (Eq. 2 summed over the k selected experts) --------------------------------- */
+
+/* out[t,:] = residual[t,:] + sum_j topk_w[t,j] * y_perm[inv[t*k+j],:] + sum_s y_shared[s*T+t,:]
+ * accumulated in fp32, rounded to bf16 once.  residual, y_shared nullable.  All device. */
+int32_t ef_combine(ef_ctx* ctx, void* stream, const void* y_perm, const int32_t* inv, const float* topk_w,
+                   int32_t T, const void* residual, const void* y_shared, void* out);
+
+/* ---- a8: RMSNorm with unit gain between layers (BASELINE.json cfg 5; R19) ------------------- */
+int32_t ef_rmsnorm(ef_ctx* ctx, void* stream, const void* x, int32_t T, float eps, void* out);
+
+/* ---- a6 / a7: cache manager (P:L116-124 PLEC, P:L183-187 overlap, P:L338 no write-back) ------ */
+
+/* PLEC refill after visit `visit_now` (-1 before the first visit).  predicted: HOST uint8[n_ahead, E],
+ * row i = batch-level predicted path of visit visit_now+1+i (nonzero = predicted active).  For each
+ * visit in order (at most prefetch_horizon of them), each predicted expert (ascending) that is not
+ * resident gets a victim slot (empty -> mis-prefetched -> completed with a later next use) and an H2D
+ * copy on the copy stream; stops at the first expert with no victim.  Returns immediately. */
+int32_t ef_cache_prefetch(ef_ctx* ctx, int64_t visit_now, const uint8_t* predicted, int32_t n_ahead);
+
+/* Drop experts of `layer` from the slot table (no write-back).  experts: HOST int32[n]. */
+int32_t ef_cache_evict(ef_ctx* ctx, int32_t layer, const int32_t* experts, int32_t n);
+
+int32_t ef_cache_get_stats(ef_ctx* ctx, ef_cache_stats* out);
+int32_t ef_cache_reset_stats(ef_ctx* ctx);
+/* slot_to_expert: HOST int32[S]; global expert id layer*E + e, or -1 if empty. */
+int32_t ef_cache_snapshot(ef_ctx* ctx, int32_t* slot_to_expert);
+/* Empty the slot table and forget supplied predictions (counters untouched). */
+int32_t ef_cache_clear(ef_ctx* ctx);
+
+/* Device time the copy stream spent on expert loads since the last reset, from events (milliseconds),
+ * and the wall time of the window in which the copy queue was non-empty are not part of parity;
+ * ef_copy_busy_ms waits for the copy stream.  Synchronous. */
+int32_t ef_copy_busy_ms(ef_ctx* ctx, float* ms_out);
+
+/* ---- misc ---------------------------------------------------------------------------------- */
+/* Wait for the copy stream and the device.  Synchronous. */
+int32_t ef_sync(ef_ctx* ctx);
+/* Text of the last error on ctx (ctx may be NULL: last ef_create failure).  Never NULL. */
+const char* ef_last_error(ef_ctx* ctx);
+/* Number of kernels this ctx has launched since creation (for bench.py's gpu_launches). */
+int64_t ef_launch_count(ef_ctx* ctx);
+/* 0 = tcgen05 kernels (default); 1 = plain-FMA debug kernels for the grouped FFN (bring-up aid, slow). */
+int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EF_H_ */

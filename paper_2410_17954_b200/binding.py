@@ -1,0 +1,234 @@
+"""ctypes binding of libef.so: same names as include/ef.h, argument marshalling only.
+
+Device tensors are torch tensors (their ``data_ptr()`` is passed through); host arrays are numpy.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+DECLARED_SYMBOLS = [
+    "ef_create", "ef_destroy", "ef_host_expert_register", "ef_host_expert_alias", "ef_route_topk", "ef_permute",
+    "ef_expert_ffn_grouped", "ef_expert_ffn_grouped_resident", "ef_shared_ffn", "ef_combine", "ef_rmsnorm",
+    "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
+    "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn",
+]
+
+
+class EfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libef error {code}: {msg}")
+        self.code = code
+
+
+class EfConfig(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("n_layers", "n_experts", "top_k", "d_model", "d_ff", "n_slots",
+                                               "n_shared", "max_tokens", "prefetch_horizon", "device")]
+
+
+class CacheStats(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_uint64) for n in ("lookups", "hits", "misses", "prefetch_issued", "prefetch_used",
+                                                "prefetch_wasted", "ondemand_loads", "evictions", "bytes_h2d")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+def library_path() -> str:
+    return os.path.join(_PKG, "libef.so")
+
+
+def load_library() -> ctypes.CDLL:
+    """Load libef.so (built by ``python -m paper_2410_17954_b200.build``).  Fails loudly if absent."""
+    global _LIB
+    if _LIB is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise EfError(-100, f"{path} not found: build it with `python -m paper_2410_17954_b200.build` "
+                                "(there is no CPU fallback)")
+        lib = ctypes.CDLL(path)
+        vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+        sig = {
+            "ef_create": [ctypes.POINTER(EfConfig), ctypes.POINTER(vp)],
+            "ef_destroy": [vp],
+            "ef_host_expert_register": [vp, i32, i32, vp, vp, vp],
+            "ef_host_expert_alias": [vp, i32, i32, i32, i32],
+            "ef_route_topk": [vp, vp, vp, vp, vp, i64, i32, i32, vp, vp, vp],
+            "ef_permute": [vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp],
+            "ef_expert_ffn_grouped": [vp, vp, i64, i32, vp, vp, vp],
+            "ef_expert_ffn_grouped_resident": [vp, vp, vp, i32, vp, vp, vp, vp],
+            "ef_shared_ffn": [vp, vp, i32, vp, i32, vp],
+            "ef_combine": [vp, vp, vp, vp, vp, i32, vp, vp, vp],
+            "ef_rmsnorm": [vp, vp, vp, i32, ctypes.c_float, vp],
+            "ef_cache_prefetch": [vp, i64, vp, i32],
+            "ef_cache_evict": [vp, i32, vp, i32],
+            "ef_cache_get_stats": [vp, ctypes.POINTER(CacheStats)],
+            "ef_cache_reset_stats": [vp],
+            "ef_cache_snapshot": [vp, vp],
+            "ef_cache_clear": [vp],
+            "ef_copy_busy_ms": [vp, ctypes.POINTER(ctypes.c_float)],
+            "ef_sync": [vp],
+            "ef_set_debug_simt_ffn": [vp, i32],
+        }
+        for name, args in sig.items():
+            fn = getattr(lib, name)
+            fn.argtypes = args
+            fn.restype = i32
+        lib.ef_last_error.argtypes = [vp]
+        lib.ef_last_error.restype = ctypes.c_char_p
+        lib.ef_launch_count.argtypes = [vp]
+        lib.ef_launch_count.restype = i64
+        _LIB = lib
+    return _LIB
+
+
+def exported_symbols() -> list[str]:
+    lib = load_library()
+    return [s for s in DECLARED_SYMBOLS if hasattr(lib, s)]
+
+
+def _dp(t):
+    """device pointer of a torch tensor (or None)"""
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "device tensors must be contiguous CUDA tensors"
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _hp(a):
+    if a is None:
+        return None
+    assert isinstance(a, np.ndarray) and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _stream():
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class EfContext:
+    """One ef_ctx.  Method names and argument order follow include/ef.h."""
+
+    def __init__(self, n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared=0, max_tokens=1,
+                 prefetch_horizon=0, device=0):
+        self.lib = load_library()
+        self.cfg = EfConfig(n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared, max_tokens,
+                            prefetch_horizon, device)
+        h = ctypes.c_void_p()
+        rc = self.lib.ef_create(ctypes.byref(self.cfg), ctypes.byref(h))
+        if rc != 0:
+            raise EfError(rc, self.lib.ef_last_error(None).decode())
+        self.h = h
+
+    # -- plumbing
+    def _chk(self, rc):
+        if rc != 0:
+            raise EfError(rc, self.lib.ef_last_error(self.h).decode())
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.ef_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- registration
+    def ef_host_expert_register(self, layer, expert, w_gate, w_up, w_down):
+        for a in (w_gate, w_up, w_down):
+            assert a.dtype == np.uint16 and a.flags["C_CONTIGUOUS"]
+        self._chk(self.lib.ef_host_expert_register(self.h, layer, expert, _hp(w_gate), _hp(w_up), _hp(w_down)))
+
+    def ef_host_expert_alias(self, layer, expert, src_layer, src_expert):
+        self._chk(self.lib.ef_host_expert_alias(self.h, layer, expert, src_layer, src_expert))
+
+    # -- a1
+    def ef_route_topk(self, x, w_router, bias, T, renorm, topk_idx, topk_w, logits_out=None):
+        stride = 0
+        if bias is not None and bias.dim() == 2:
+            stride = bias.shape[1]
+        self._chk(self.lib.ef_route_topk(self.h, _stream(), _dp(x), _dp(w_router), _dp(bias), stride, T, renorm,
+                                         _dp(topk_idx), _dp(topk_w), _dp(logits_out)))
+
+    # -- a2
+    def ef_permute(self, topk_idx, x, T, x_perm, counts, offsets, src, inv, counts_host_pinned=None):
+        chp = None
+        if counts_host_pinned is not None:
+            assert counts_host_pinned.is_pinned()
+            chp = ctypes.c_void_p(counts_host_pinned.data_ptr())
+        self._chk(self.lib.ef_permute(self.h, _stream(), _dp(topk_idx), _dp(x), T, _dp(x_perm), _dp(counts),
+                                      _dp(offsets), _dp(src), _dp(inv), chp))
+
+    # -- a3 + a4
+    def ef_expert_ffn_grouped(self, visit, layer, x_perm, counts_host, y_perm):
+        ch = None if counts_host is None else _hp(np.ascontiguousarray(counts_host, dtype=np.int32))
+        self._chk(self.lib.ef_expert_ffn_grouped(self.h, _stream(), visit, layer, _dp(x_perm), ch, _dp(y_perm)))
+
+    def ef_expert_ffn_grouped_resident(self, x_perm, row_begin, rows, slots, y_perm):
+        rb = np.ascontiguousarray(row_begin, dtype=np.int32)
+        rw = np.ascontiguousarray(rows, dtype=np.int32)
+        sl = np.ascontiguousarray(slots, dtype=np.int32)
+        self._chk(self.lib.ef_expert_ffn_grouped_resident(self.h, _stream(), _dp(x_perm), len(rb), _hp(rb), _hp(rw),
+                                                          _hp(sl), _dp(y_perm)))
+
+    def ef_shared_ffn(self, layer, x, T, y_shared):
+        self._chk(self.lib.ef_shared_ffn(self.h, _stream(), layer, _dp(x), T, _dp(y_shared)))
+
+    # -- a5, a8
+    def ef_combine(self, y_perm, inv, topk_w, T, residual, y_shared, out):
+        self._chk(self.lib.ef_combine(self.h, _stream(), _dp(y_perm), _dp(inv), _dp(topk_w), T, _dp(residual),
+                                      _dp(y_shared), _dp(out)))
+
+    def ef_rmsnorm(self, x, T, eps, out):
+        self._chk(self.lib.ef_rmsnorm(self.h, _stream(), _dp(x), T, eps, _dp(out)))
+
+    # -- a6, a7
+    def ef_cache_prefetch(self, visit_now, predicted):
+        p = np.ascontiguousarray(predicted, dtype=np.uint8)
+        if p.ndim == 1:
+            p = p[None, :]
+        self._chk(self.lib.ef_cache_prefetch(self.h, visit_now, _hp(p), p.shape[0]))
+
+    def ef_cache_evict(self, layer, experts):
+        e = np.ascontiguousarray(experts, dtype=np.int32)
+        self._chk(self.lib.ef_cache_evict(self.h, layer, _hp(e), len(e)))
+
+    def ef_cache_get_stats(self) -> dict:
+        st = CacheStats()
+        self._chk(self.lib.ef_cache_get_stats(self.h, ctypes.byref(st)))
+        return st.as_dict()
+
+    def ef_cache_reset_stats(self):
+        self._chk(self.lib.ef_cache_reset_stats(self.h))
+
+    def ef_cache_snapshot(self) -> list[int]:
+        a = np.empty(self.cfg.n_slots, dtype=np.int32)
+        self._chk(self.lib.ef_cache_snapshot(self.h, _hp(a)))
+        return a.tolist()
+
+    def ef_cache_clear(self):
+        self._chk(self.lib.ef_cache_clear(self.h))
+
+    def ef_copy_busy_ms(self) -> float:
+        ms = ctypes.c_float()
+        self._chk(self.lib.ef_copy_busy_ms(self.h, ctypes.byref(ms)))
+        return float(ms.value)
+
+    def ef_sync(self):
+        self._chk(self.lib.ef_sync(self.h))
+
+    def ef_launch_count(self) -> int:
+        return int(self.lib.ef_launch_count(self.h))
+
+    def ef_set_debug_simt_ffn(self, on: bool):
+        self._chk(self.lib.ef_set_debug_simt_ffn(self.h, 1 if on else 0))

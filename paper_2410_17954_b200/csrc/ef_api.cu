@@ -1,0 +1,611 @@
+// libef: context, host expert pool, cache manager (policy + copy-stream pipeline) and the C ABI.
+//
+// The cache manager implements DESIGN.md §4 (§3.2.1 PLEC, §3.2.2 real-time correction,
+// §4.1 multi-stream overlap) on its own; oracle/cache_sim.py is an independent restatement used
+// only by the tests.  Every policy decision depends on the call sequence alone (R9): "completed"
+// means enqueued, physical ordering is enforced with events:
+//   ready event  -- recorded on the copy stream after an expert's H2D; the compute stream waits on it
+//   free  event  -- recorded on the compute stream after the last wave reading a slot; the copy
+//                   stream waits on it before overwriting the slot.
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <tuple>
+
+#include "ef_internal.h"
+
+static std::string g_create_err;
+
+int32_t ef_fail(ef_ctx* ctx, int32_t code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf; else g_create_err = buf;
+    return code;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// event ring with generations
+// ---------------------------------------------------------------------------------------------------
+constexpr int kRing = 2048;
+
+static EvHandle ring_record(ef_ctx* ctx, cudaStream_t st, cudaError_t* err) {
+    const int i = ctx->ev_next;
+    ctx->ev_next = (ctx->ev_next + 1) % kRing;
+    ctx->ev_gen[i]++;
+    *err = cudaEventRecord(ctx->ev_ring[i], st);
+    return EvHandle{i, ctx->ev_gen[i]};
+}
+
+// make `waiter` wait for handle h (recorded on `origin`); if h was recycled, wait for everything
+// enqueued on `origin` so far, which is a superset.
+static cudaError_t ring_wait(ef_ctx* ctx, cudaStream_t waiter, const EvHandle& h, cudaStream_t origin) {
+    if (h.idx < 0) return cudaSuccess;
+    if (ctx->ev_gen[h.idx] == h.gen) return cudaStreamWaitEvent(waiter, ctx->ev_ring[h.idx], 0);
+    if (!origin || origin == waiter) return cudaSuccess;
+    cudaError_t e;
+    EvHandle f = ring_record(ctx, origin, &e);
+    if (e != cudaSuccess) return e;
+    return cudaStreamWaitEvent(waiter, ctx->ev_ring[f.idx], 0);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// lifetime
+// ---------------------------------------------------------------------------------------------------
+extern "C" int32_t ef_create(const ef_config* cfg, ef_ctx** out) {
+    if (out) *out = nullptr;
+    if (!cfg || !out) return ef_fail(nullptr, EF_ERR_INVALID_ARG, "ef_create: null argument");
+    const ef_config& c = *cfg;
+    if (c.n_layers < 1 || c.n_experts < 1 || c.top_k < 1 || c.d_model < 1 || c.d_ff < 1 || c.n_slots < 1 ||
+        c.n_shared < 0 || c.max_tokens < 1 || c.device < 0)
+        return ef_fail(nullptr, EF_ERR_INVALID_ARG, "ef_create: non-positive field in ef_config");
+    if (c.d_model % 64 || c.d_ff % 128 || c.top_k > 8 || c.top_k > c.n_experts || c.n_experts > 256)
+        return ef_fail(nullptr, EF_ERR_UNSUPPORTED,
+                       "ef_create: need d_model%%64==0, d_ff%%128==0, top_k<=8, top_k<=n_experts<=256");
+    ef_ctx* ctx = new ef_ctx();
+    ctx->cfg = c;
+    ctx->W = (int64_t)3 * c.d_model * c.d_ff * 2;
+    auto bail = [&](int32_t code, const char* what, cudaError_t e) {
+        ef_fail(nullptr, code, "ef_create: %s: %s", what, cudaGetErrorString(e));
+        ef_destroy(ctx);
+        return code;
+    };
+    cudaError_t e;
+    if ((e = cudaSetDevice(c.device)) != cudaSuccess) return bail(EF_ERR_CUDA, "cudaSetDevice", e);
+    int sms = 0;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c.device)) != cudaSuccess)
+        return bail(EF_ERR_CUDA, "cudaDeviceGetAttribute", e);
+    ctx->n_sms = sms;
+    ctx->n_arena_slots = c.n_slots + c.n_layers * c.n_shared;
+    if ((e = cudaMalloc(&ctx->arena, (size_t)ctx->n_arena_slots * ctx->W)) != cudaSuccess)
+        return bail(EF_ERR_OOM, "slot arena", e);
+    ctx->h_rows = (int64_t)c.max_tokens * (c.top_k + c.n_shared);
+    if ((e = cudaMalloc(&ctx->h_ws, (size_t)ctx->h_rows * c.d_ff * 2)) != cudaSuccess)
+        return bail(EF_ERR_OOM, "h workspace", e);
+    if ((e = cudaHostAlloc((void**)&ctx->counts_pinned, sizeof(int32_t) * c.n_experts, cudaHostAllocDefault)) !=
+        cudaSuccess)
+        return bail(EF_ERR_OOM, "pinned counts", e);
+    if ((e = cudaEventCreateWithFlags(&ctx->counts_event, cudaEventDisableTiming)) != cudaSuccess)
+        return bail(EF_ERR_CUDA, "event", e);
+    if ((e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
+        return bail(EF_ERR_CUDA, "copy stream", e);
+    ctx->ev_ring.resize(kRing, nullptr);
+    ctx->ev_gen.assign(kRing, 0);
+    for (int i = 0; i < kRing; ++i)
+        if ((e = cudaEventCreateWithFlags(&ctx->ev_ring[i], cudaEventDisableTiming)) != cudaSuccess)
+            return bail(EF_ERR_CUDA, "event ring", e);
+    ctx->host_expert.assign((size_t)c.n_layers * c.n_experts, nullptr);
+    ctx->host_owned.assign((size_t)c.n_layers * c.n_experts, 0);
+    ctx->shared_registered.assign((size_t)c.n_layers * std::max(1, c.n_shared), 0);
+    ctx->slots.assign(c.n_slots, EfSlot());
+    ctx->slot_of.assign((size_t)c.n_layers * c.n_experts, -1);
+    ctx->phys.assign(c.n_slots, EfPhys());
+    int32_t rc = efk_ffn_tc_init(ctx);
+    if (rc != EF_OK) {
+        g_create_err = "ef_create: " + ctx->err;
+        ef_destroy(ctx);
+        return rc;
+    }
+    *out = ctx;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_destroy(ef_ctx* ctx) {
+    if (!ctx) return EF_OK;
+    cudaSetDevice(ctx->cfg.device);
+    cudaDeviceSynchronize();
+    for (auto& sp : ctx->copy_spans) { cudaEventDestroy(sp.first); cudaEventDestroy(sp.second); }
+    for (auto ev : ctx->ev_ring) if (ev) cudaEventDestroy(ev);
+    if (ctx->counts_event) cudaEventDestroy(ctx->counts_event);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    for (size_t i = 0; i < ctx->host_expert.size(); ++i)
+        if (ctx->host_expert[i] && ctx->host_owned[i]) cudaFreeHost(ctx->host_expert[i]);
+    if (ctx->counts_pinned) cudaFreeHost(ctx->counts_pinned);
+    if (ctx->h_ws) cudaFree(ctx->h_ws);
+    if (ctx->arena) cudaFree(ctx->arena);
+    delete ctx;
+    return EF_OK;
+}
+
+// pack (Wg, Wu, Wd) into the library layout (ef_internal.h)
+static void pack_expert(const ef_config& c, const void* wg, const void* wu, const void* wd, char* dst) {
+    const size_t row = (size_t)c.d_model * 2;
+    const size_t blk = (size_t)EF_W13_BLOCK * row;
+    const char* g = (const char*)wg;
+    const char* u = (const char*)wu;
+    for (int j = 0; j < c.d_ff / EF_W13_BLOCK; ++j) {
+        memcpy(dst + (size_t)(2 * j) * blk, g + (size_t)j * blk, blk);
+        memcpy(dst + (size_t)(2 * j + 1) * blk, u + (size_t)j * blk, blk);
+    }
+    memcpy(dst + (size_t)2 * c.d_ff * row, wd, (size_t)c.d_model * c.d_ff * 2);
+}
+
+extern "C" int32_t ef_host_expert_register(ef_ctx* ctx, int32_t layer, int32_t expert, const void* w_gate,
+                                           const void* w_up, const void* w_down) {
+    EF_CHECK_CTX(ctx);
+    const ef_config& c = ctx->cfg;
+    if (!w_gate || !w_up || !w_down || layer < 0 || layer >= c.n_layers || expert >= c.n_experts ||
+        expert < -c.n_shared)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_register: bad layer/expert/pointer");
+    EF_CUDA(ctx, cudaSetDevice(c.device));
+    void* buf = nullptr;
+    cudaError_t e = cudaHostAlloc(&buf, (size_t)ctx->W, cudaHostAllocDefault);
+    if (e != cudaSuccess) return ef_fail(ctx, EF_ERR_OOM, "pinned host pool: %s", cudaGetErrorString(e));
+    pack_expert(c, w_gate, w_up, w_down, (char*)buf);
+    if (expert >= 0) {
+        size_t g = (size_t)layer * c.n_experts + expert;
+        if (ctx->host_expert[g] && ctx->host_owned[g]) cudaFreeHost(ctx->host_expert[g]);
+        ctx->host_expert[g] = buf;
+        ctx->host_owned[g] = 1;
+        return EF_OK;
+    }
+    const int s = -1 - expert;
+    const int slot = c.n_slots + layer * c.n_shared + s;
+    e = cudaMemcpy(ctx->arena + (size_t)slot * ctx->W, buf, (size_t)ctx->W, cudaMemcpyHostToDevice);
+    cudaFreeHost(buf);
+    if (e != cudaSuccess) { ctx->sticky = EF_ERR_CUDA; return ef_fail(ctx, EF_ERR_CUDA, "shared expert upload: %s", cudaGetErrorString(e)); }
+    ctx->shared_registered[(size_t)layer * c.n_shared + s] = 1;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_host_expert_alias(ef_ctx* ctx, int32_t layer, int32_t expert, int32_t src_layer,
+                                        int32_t src_expert) {
+    EF_CHECK_CTX(ctx);
+    const ef_config& c = ctx->cfg;
+    if (layer < 0 || layer >= c.n_layers || expert < 0 || expert >= c.n_experts || src_layer < 0 ||
+        src_layer >= c.n_layers || src_expert < 0 || src_expert >= c.n_experts)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_alias: bad ids");
+    size_t g = (size_t)layer * c.n_experts + expert, sg = (size_t)src_layer * c.n_experts + src_expert;
+    if (!ctx->host_expert[sg]) return ef_fail(ctx, EF_ERR_NOT_REGISTERED, "ef_host_expert_alias: source not registered");
+    if (ctx->host_expert[g] && ctx->host_owned[g]) cudaFreeHost(ctx->host_expert[g]);
+    ctx->host_expert[g] = ctx->host_expert[sg];
+    ctx->host_owned[g] = 0;
+    return EF_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// thin wrappers around the memory-bound kernels
+// ---------------------------------------------------------------------------------------------------
+extern "C" int32_t ef_route_topk(ef_ctx* ctx, void* stream, const void* x, const void* w_router, const float* bias,
+                                 int64_t bias_token_stride, int32_t T, int32_t renorm, int32_t* topk_idx,
+                                 float* topk_w, float* logits_out) {
+    EF_CHECK_CTX(ctx);
+    if (T < 0 || (T > 0 && (!x || !w_router || !topk_idx || !topk_w)))
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_route_topk: null pointer or negative T");
+    if (T > ctx->cfg.max_tokens) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_route_topk: T > max_tokens");
+    if (bias && bias_token_stride != 0 && bias_token_stride != ctx->cfg.n_experts)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_route_topk: bias_token_stride must be 0 or E");
+    return efk_route_topk(ctx, (cudaStream_t)stream, x, w_router, bias, bias_token_stride, T, renorm ? 1 : 0,
+                          topk_idx, topk_w, logits_out);
+}
+
+extern "C" int32_t ef_permute(ef_ctx* ctx, void* stream, const int32_t* topk_idx, const void* x, int32_t T,
+                              void* x_perm, int32_t* counts, int32_t* offsets, int32_t* src, int32_t* inv,
+                              int32_t* counts_host_pinned) {
+    EF_CHECK_CTX(ctx);
+    if (T < 0 || !counts || !offsets || (T > 0 && (!topk_idx || !x || !x_perm || !src || !inv)))
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_permute: null pointer or negative T");
+    if (T > ctx->cfg.max_tokens) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_permute: T > max_tokens");
+    int32_t* mirror = counts_host_pinned ? counts_host_pinned : ctx->counts_pinned;
+    int32_t rc = efk_permute(ctx, (cudaStream_t)stream, topk_idx, x, T, x_perm, counts, offsets, src, inv, mirror);
+    if (rc != EF_OK) return rc;
+    if (!counts_host_pinned) EF_CUDA(ctx, cudaEventRecord(ctx->counts_event, (cudaStream_t)stream));
+    return EF_OK;
+}
+
+extern "C" int32_t ef_combine(ef_ctx* ctx, void* stream, const void* y_perm, const int32_t* inv, const float* topk_w,
+                              int32_t T, const void* residual, const void* y_shared, void* out) {
+    EF_CHECK_CTX(ctx);
+    if (T < 0 || (T > 0 && (!y_perm || !inv || !topk_w || !out)))
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_combine: null pointer or negative T");
+    if (y_shared && ctx->cfg.n_shared == 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_combine: y_shared given but n_shared == 0");
+    return efk_combine(ctx, (cudaStream_t)stream, y_perm, inv, topk_w, T, residual, y_shared, out);
+}
+
+extern "C" int32_t ef_rmsnorm(ef_ctx* ctx, void* stream, const void* x, int32_t T, float eps, void* out) {
+    EF_CHECK_CTX(ctx);
+    if (T < 0 || (T > 0 && (!x || !out))) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_rmsnorm: null pointer or negative T");
+    return efk_rmsnorm(ctx, (cudaStream_t)stream, x, T, eps, out);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// cache policy
+// ---------------------------------------------------------------------------------------------------
+namespace {
+
+inline bool pending(const EfSlot& s) { return s.pred_for != -1 && !s.used; }
+
+int64_t next_visit_of_layer(int L, int layer, int64_t v) {
+    const int64_t v1 = v + 1;
+    int64_t r = (layer - v1) % L;
+    if (r < 0) r += L;
+    return v1 + r;
+}
+
+// first visit > v of the expert's layer where it is predicted active; visits without a supplied
+// prediction count as "assume used"
+int64_t est_next_use(ef_ctx* ctx, int32_t g, int64_t v) {
+    const int E = ctx->cfg.n_experts, L = ctx->cfg.n_layers;
+    const int layer = g / E, e = g % E;
+    int64_t t = next_visit_of_layer(L, layer, v);
+    for (;;) {
+        auto it = ctx->pred.find(t);
+        if (it == ctx->pred.end() || it->second[e]) return t;
+        t += L;
+    }
+}
+
+// class 0 empty; 1 mis-prefetched; 2 completed & next use later than target; 3 (on demand only) the rest
+int pick_victim(ef_ctx* ctx, int64_t v_now, int64_t target, bool allow3, const std::vector<char>& locked) {
+    typedef std::tuple<int, int64_t, uint64_t, int> Key;
+    bool have = false;
+    Key best;
+    for (int s = 0; s < ctx->cfg.n_slots; ++s) {
+        const EfSlot& sl = ctx->slots[s];
+        Key key;
+        if (sl.expert < 0) {
+            key = Key(0, 0, 0, s);
+        } else if (locked[s]) {
+            continue;
+        } else if (pending(sl) && sl.pred_for <= v_now) {
+            key = Key(1, 0, sl.stamp, s);
+        } else {
+            const int64_t nu = est_next_use(ctx, sl.expert, v_now);
+            if (!pending(sl) && nu > target) key = Key(2, -nu, sl.stamp, s);
+            else if (allow3) key = Key(3, -nu, sl.stamp, s);
+            else continue;
+        }
+        if (!have || key < best) { best = key; have = true; }
+    }
+    return have ? std::get<3>(best) : -1;
+}
+
+void drain_copy_spans(ef_ctx* ctx, bool wait, float* acc_ms);
+
+// policy bookkeeping + the physical H2D for one load
+int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
+    if (!ctx->host_expert[g])
+        return ef_fail(ctx, EF_ERR_NOT_REGISTERED, "expert (layer %d, id %d) was never registered", g / ctx->cfg.n_experts,
+                       g % ctx->cfg.n_experts);
+    EfSlot& sl = ctx->slots[slot];
+    if (sl.expert >= 0) {
+        ctx->stats.evictions++;
+        if (pending(sl)) ctx->stats.prefetch_wasted++;
+        ctx->slot_of[sl.expert] = -1;
+    }
+    sl.expert = g;
+    sl.pred_for = pred_for;
+    sl.used = false;
+    sl.stamp = ++ctx->tick;
+    ctx->slot_of[g] = slot;
+    ctx->stats.bytes_h2d += (uint64_t)ctx->W;
+
+    EfPhys& ph = ctx->phys[slot];
+    EF_CUDA(ctx, ring_wait(ctx, ctx->copy_stream, ph.free_, ctx->last_compute));
+    cudaEvent_t t0, t1;
+    if (ctx->copy_spans.size() > 8192) drain_copy_spans(ctx, false, nullptr);
+    EF_CUDA(ctx, cudaEventCreate(&t0));
+    EF_CUDA(ctx, cudaEventCreate(&t1));
+    EF_CUDA(ctx, cudaEventRecord(t0, ctx->copy_stream));
+    EF_CUDA(ctx, cudaMemcpyAsync(ctx->arena + (size_t)slot * ctx->W, ctx->host_expert[g], (size_t)ctx->W,
+                                 cudaMemcpyHostToDevice, ctx->copy_stream));
+    EF_CUDA(ctx, cudaEventRecord(t1, ctx->copy_stream));
+    ctx->copy_spans.emplace_back(t0, t1);
+    cudaError_t e;
+    ph.ready = ring_record(ctx, ctx->copy_stream, &e);
+    EF_CUDA(ctx, e);
+    ph.free_ = EvHandle();
+    ph.waited = nullptr;
+    return EF_OK;
+}
+
+void drain_copy_spans(ef_ctx* ctx, bool wait, float* acc_ms) {
+    (void)acc_ms;
+    auto& v = ctx->copy_spans;
+    size_t keep = 0;
+    for (size_t i = 0; i < v.size(); ++i) {
+        bool done = wait ? (cudaEventSynchronize(v[i].second) == cudaSuccess)
+                         : (cudaEventQuery(v[i].second) == cudaSuccess);
+        if (done) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, v[i].first, v[i].second) == cudaSuccess) ctx->copy_ms += ms;
+            cudaEventDestroy(v[i].first);
+            cudaEventDestroy(v[i].second);
+        } else {
+            v[keep++] = v[i];
+        }
+    }
+    v.resize(keep);
+}
+
+// one wave: groups (expert-local id e, slot) computed by one grouped launch (chunks of EF_MAX_GROUPS)
+struct WaveItem { int32_t row0, rows, slot; };
+
+int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm, const std::vector<WaveItem>& items) {
+    if (items.empty()) return EF_OK;
+    auto& phys = ctx->phys;
+    for (const WaveItem& it : items) {
+        EfPhys& ph = phys[it.slot];
+        if (ph.ready.idx >= 0 && ph.waited != st) {
+            EF_CUDA(ctx, ring_wait(ctx, st, ph.ready, ctx->copy_stream));
+            ph.waited = st;
+        }
+    }
+    for (size_t base = 0; base < items.size(); base += EF_MAX_GROUPS) {
+        EfGroupTable tab;
+        int32_t h_row0[EF_MAX_GROUPS];
+        tab.n = (int32_t)std::min<size_t>(EF_MAX_GROUPS, items.size() - base);
+        for (int i = 0; i < tab.n; ++i) {
+            const WaveItem& it = items[base + i];
+            tab.g[i] = EfGroup{it.row0, it.row0, it.rows, it.slot};
+            h_row0[i] = it.row0;
+        }
+        int32_t rc = efk_ffn_grouped(ctx, st, x_perm, y_perm, tab, h_row0);
+        if (rc != EF_OK) return rc;
+    }
+    cudaError_t e;
+    EvHandle ev = ring_record(ctx, st, &e);
+    EF_CUDA(ctx, e);
+    for (const WaveItem& it : items) phys[it.slot].free_ = ev;
+    ctx->last_compute = st;
+    return EF_OK;
+}
+
+}  // namespace
+
+int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
+                        const int32_t* h_row0) {
+    if (ctx->debug_simt) return efk_ffn_simt(ctx, st, x, y, tab, h_row0);
+    return efk_ffn_tc(ctx, st, x, y, tab, h_row0);
+}
+
+extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visit, int32_t layer, const void* x_perm,
+                                         const int32_t* counts_host, void* y_perm) {
+    EF_CHECK_CTX(ctx);
+    const ef_config& c = ctx->cfg;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (layer < 0 || layer >= c.n_layers || !x_perm || !y_perm)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_expert_ffn_grouped: bad layer or null pointer");
+    if (visit < 0 || (int32_t)(visit % c.n_layers) != layer)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_expert_ffn_grouped: visit %% n_layers must equal layer");
+    if (!counts_host) {
+        EF_CUDA(ctx, cudaEventSynchronize(ctx->counts_event));   // the one device->host sync per visit
+        counts_host = ctx->counts_pinned;
+    }
+    const int E = c.n_experts;
+    std::vector<int32_t> off(E + 1, 0);
+    for (int e = 0; e < E; ++e) {
+        if (counts_host[e] < 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_expert_ffn_grouped: negative count");
+        off[e + 1] = off[e] + counts_host[e];
+    }
+    if ((int64_t)off[E] > (int64_t)c.max_tokens * c.top_k)
+        return ef_fail(ctx, EF_ERR_CAPACITY, "ef_expert_ffn_grouped: sum(counts) > max_tokens * top_k");
+    ctx->last_compute = st;
+
+    // lookup (R6)
+    std::vector<int> hits, misses;
+    for (int e = 0; e < E; ++e) {
+        if (counts_host[e] == 0) continue;
+        (ctx->slot_of[(size_t)layer * E + e] >= 0 ? hits : misses).push_back(e);
+    }
+    ctx->stats.lookups += hits.size() + misses.size();
+    ctx->stats.hits += hits.size();
+    ctx->stats.misses += misses.size();
+    std::vector<char> locked(c.n_slots, 0);
+    std::vector<WaveItem> wave0;
+    for (int e : hits) {
+        const int s = ctx->slot_of[(size_t)layer * E + e];
+        EfSlot& sl = ctx->slots[s];
+        if (pending(sl)) ctx->stats.prefetch_used++;
+        sl.used = true;
+        sl.stamp = ++ctx->tick;
+        locked[s] = 1;
+        wave0.push_back(WaveItem{off[e], counts_host[e], s});
+    }
+    // phase A: on-demand loads into empty / mis-prefetched / completed slots; copies start now and
+    // overlap wave 0
+    std::vector<WaveItem> wavesA;
+    std::vector<int> rest;
+    for (int e : misses) {
+        const int s = pick_victim(ctx, visit, visit, false, locked);
+        if (s < 0) { rest.push_back(e); continue; }
+        int32_t rc = issue_load(ctx, s, layer * E + e, -1);
+        if (rc != EF_OK) return rc;
+        ctx->stats.ondemand_loads++;
+        ctx->slots[s].used = true;
+        locked[s] = 1;
+        wavesA.push_back(WaveItem{off[e], counts_host[e], s});
+    }
+    int32_t rc = run_wave(ctx, st, x_perm, y_perm, wave0);
+    if (rc != EF_OK) return rc;
+    for (const WaveItem& it : wavesA) {   // one wave each: compute starts as each copy lands
+        rc = run_wave(ctx, st, x_perm, y_perm, std::vector<WaveItem>{it});
+        if (rc != EF_OK) return rc;
+    }
+    // phase B: the pool was full of this visit's own experts and useful prefetches
+    std::fill(locked.begin(), locked.end(), 0);
+    for (int e : rest) {
+        const int s = pick_victim(ctx, visit, visit, true, locked);
+        if (s < 0) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_expert_ffn_grouped: no victim slot (internal)");
+        rc = issue_load(ctx, s, layer * E + e, -1);
+        if (rc != EF_OK) return rc;
+        ctx->stats.ondemand_loads++;
+        ctx->slots[s].used = true;
+        rc = run_wave(ctx, st, x_perm, y_perm, std::vector<WaveItem>{WaveItem{off[e], counts_host[e], s}});
+        if (rc != EF_OK) return rc;
+    }
+    return EF_OK;
+}
+
+extern "C" int32_t ef_expert_ffn_grouped_resident(ef_ctx* ctx, void* stream, const void* x_perm, int32_t n_groups,
+                                                  const int32_t* row_begin, const int32_t* rows,
+                                                  const int32_t* slots, void* y_perm) {
+    EF_CHECK_CTX(ctx);
+    if (n_groups < 0 || (n_groups > 0 && (!x_perm || !y_perm || !row_begin || !rows || !slots)))
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_expert_ffn_grouped_resident: null pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<WaveItem> items;
+    for (int i = 0; i < n_groups; ++i) {
+        if (rows[i] == 0) continue;
+        if (rows[i] < 0 || row_begin[i] < 0 || slots[i] < 0 || slots[i] >= ctx->cfg.n_slots ||
+            (int64_t)row_begin[i] + rows[i] > (int64_t)ctx->cfg.max_tokens * ctx->cfg.top_k)
+            return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_expert_ffn_grouped_resident: bad group %d", i);
+        items.push_back(WaveItem{row_begin[i], rows[i], slots[i]});
+    }
+    ctx->last_compute = st;
+    return run_wave(ctx, st, x_perm, y_perm, items);
+}
+
+extern "C" int32_t ef_shared_ffn(ef_ctx* ctx, void* stream, int32_t layer, const void* x, int32_t T, void* y_shared) {
+    EF_CHECK_CTX(ctx);
+    const ef_config& c = ctx->cfg;
+    if (c.n_shared == 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_shared_ffn: n_shared == 0");
+    if (layer < 0 || layer >= c.n_layers || T < 0 || (T > 0 && (!x || !y_shared)))
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_shared_ffn: bad argument");
+    if (T > c.max_tokens) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_shared_ffn: T > max_tokens");
+    if (T == 0) return EF_OK;
+    EfGroupTable tab;
+    int32_t h_row0[EF_MAX_GROUPS];
+    if (c.n_shared > EF_MAX_GROUPS) return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_shared_ffn: too many shared experts");
+    tab.n = c.n_shared;
+    for (int s = 0; s < c.n_shared; ++s) {
+        if (!ctx->shared_registered[(size_t)layer * c.n_shared + s])
+            return ef_fail(ctx, EF_ERR_NOT_REGISTERED, "shared expert %d of layer %d not registered", s, layer);
+        tab.g[s] = EfGroup{0, s * T, T, c.n_slots + layer * c.n_shared + s};
+        h_row0[s] = c.max_tokens * c.top_k + s * c.max_tokens;   // shared region of the h workspace
+    }
+    return efk_ffn_grouped(ctx, (cudaStream_t)stream, x, y_shared, tab, h_row0);
+}
+
+extern "C" int32_t ef_cache_prefetch(ef_ctx* ctx, int64_t visit_now, const uint8_t* predicted, int32_t n_ahead) {
+    EF_CHECK_CTX(ctx);
+    const ef_config& c = ctx->cfg;
+    if (n_ahead < 0 || (n_ahead > 0 && !predicted) || visit_now < -1)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_cache_prefetch: bad argument");
+    const int E = c.n_experts, L = c.n_layers;
+    for (int i = 0; i < n_ahead; ++i)
+        ctx->pred[visit_now + 1 + i] = std::vector<uint8_t>(predicted + (size_t)i * E, predicted + (size_t)(i + 1) * E);
+    while (!ctx->pred.empty() && ctx->pred.begin()->first <= visit_now) ctx->pred.erase(ctx->pred.begin());
+    const int span = c.prefetch_horizon > 0 ? std::min(c.prefetch_horizon, n_ahead) : n_ahead;
+    std::vector<char> no_lock(c.n_slots, 0);
+    for (int64_t t = visit_now + 1; t <= visit_now + span; ++t) {
+        const int layer = (int)(t % L);
+        const std::vector<uint8_t>& p = ctx->pred[t];
+        for (int e = 0; e < E; ++e) {
+            if (!p[e]) continue;
+            const int32_t g = layer * E + e;
+            const int cur = ctx->slot_of[g];
+            if (cur >= 0) {
+                EfSlot& sl = ctx->slots[cur];
+                if (pending(sl) && sl.pred_for <= visit_now) sl.pred_for = t;   // R25: re-target a stale prefetch
+                continue;
+            }
+            const int s = pick_victim(ctx, visit_now, t, false, no_lock);
+            if (s < 0) return EF_OK;   // pool is full of useful experts
+            int32_t rc = issue_load(ctx, s, g, t);
+            if (rc != EF_OK) return rc;
+            ctx->stats.prefetch_issued++;
+        }
+    }
+    return EF_OK;
+}
+
+extern "C" int32_t ef_cache_evict(ef_ctx* ctx, int32_t layer, const int32_t* experts, int32_t n) {
+    EF_CHECK_CTX(ctx);
+    const ef_config& c = ctx->cfg;
+    if (layer < 0 || layer >= c.n_layers || n < 0 || (n > 0 && !experts))
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_cache_evict: bad argument");
+    for (int i = 0; i < n; ++i) {
+        if (experts[i] < 0 || experts[i] >= c.n_experts) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_cache_evict: bad expert id");
+        const int32_t g = layer * c.n_experts + experts[i];
+        const int s = ctx->slot_of[g];
+        if (s < 0) continue;
+        EfSlot& sl = ctx->slots[s];
+        ctx->stats.evictions++;
+        if (pending(sl)) ctx->stats.prefetch_wasted++;
+        ctx->slot_of[g] = -1;
+        sl.expert = -1; sl.pred_for = -1; sl.used = false; sl.stamp = 0;
+    }
+    return EF_OK;
+}
+
+extern "C" int32_t ef_cache_get_stats(ef_ctx* ctx, ef_cache_stats* out) {
+    EF_CHECK_CTX(ctx);
+    if (!out) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_cache_get_stats: null");
+    *out = ctx->stats;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_cache_reset_stats(ef_ctx* ctx) {
+    EF_CHECK_CTX(ctx);
+    ctx->stats = ef_cache_stats();
+    drain_copy_spans(ctx, true, nullptr);
+    ctx->copy_ms = 0.f;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_cache_snapshot(ef_ctx* ctx, int32_t* slot_to_expert) {
+    EF_CHECK_CTX(ctx);
+    if (!slot_to_expert) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_cache_snapshot: null");
+    for (int s = 0; s < ctx->cfg.n_slots; ++s) slot_to_expert[s] = ctx->slots[s].expert;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_cache_clear(ef_ctx* ctx) {
+    EF_CHECK_CTX(ctx);
+    for (auto& sl : ctx->slots) { sl.expert = -1; sl.pred_for = -1; sl.used = false; sl.stamp = 0; }
+    std::fill(ctx->slot_of.begin(), ctx->slot_of.end(), -1);
+    ctx->pred.clear();
+    ctx->tick = 0;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_copy_busy_ms(ef_ctx* ctx, float* ms_out) {
+    EF_CHECK_CTX(ctx);
+    if (!ms_out) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_copy_busy_ms: null");
+    EF_CUDA(ctx, cudaStreamSynchronize(ctx->copy_stream));
+    drain_copy_spans(ctx, true, nullptr);
+    *ms_out = ctx->copy_ms;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_sync(ef_ctx* ctx) {
+    EF_CHECK_CTX(ctx);
+    EF_CUDA(ctx, cudaStreamSynchronize(ctx->copy_stream));
+    EF_CUDA(ctx, cudaDeviceSynchronize());
+    return EF_OK;
+}
+
+extern "C" const char* ef_last_error(ef_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+extern "C" int64_t ef_launch_count(ef_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on) {
+    EF_CHECK_CTX(ctx);
+    ctx->debug_simt = on ? 1 : 0;
+    return EF_OK;
+}

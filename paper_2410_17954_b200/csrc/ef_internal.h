@@ -1,0 +1,131 @@
+// Internal declarations shared by libef's translation units.  Not part of the C ABI.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda.h>
+#include <stdint.h>
+
+#include <map>
+#include <string>
+#include <vector>
+
+#include "ef.h"
+
+#define EF_MAX_GROUPS 64   // groups per grouped-GEMM launch (table travels in kernel params)
+#define EF_W13_BLOCK 128   // gate/up interleave granularity in the packed expert layout
+
+// ---- packed expert layout (library-defined; the caller never sees it) ----------------------------
+// An expert occupies W = 3*d*f*2 bytes:
+//   [ W13 : 2f rows x d ]  row 256*j + i       = Wg[128*j + i, :]   (i < 128)
+//                          row 256*j + 128 + i = Wu[128*j + i, :]
+//   [ Wd  : d rows x f  ]  as given
+// so one 256-row B tile of GEMM1 yields 128 gate columns and the matching 128 up columns.
+
+struct EfGroup {
+    int32_t a_row0;   // first row of A (x_perm or h)
+    int32_t c_row0;   // first row of the output
+    int32_t rows;     // M of this group (>0)
+    int32_t slot;     // arena slot holding the expert
+};
+
+struct EfGroupTable {
+    int32_t n;
+    EfGroup g[EF_MAX_GROUPS];
+};
+
+// One slot's policy state (mirror of DESIGN.md §4; written independently of oracle/cache_sim.py).
+struct EfSlot {
+    int32_t expert = -1;      // global id layer*E + e, or -1
+    int64_t pred_for = -1;    // visit the expert was prefetched for; -1: loaded on demand
+    bool used = false;        // used since load
+    uint64_t stamp = 0;       // tick of last use / of the load
+};
+
+// Physical ordering of a slot.  Events come from a ring; a handle whose generation moved on has been
+// recycled, and waiting on it falls back to "everything enqueued on the origin stream so far".
+struct EvHandle {
+    int32_t idx = -1;
+    uint32_t gen = 0;
+};
+struct EfPhys {
+    EvHandle ready;                  // recorded on the copy stream after the H2D into the slot
+    EvHandle free_;                  // recorded on the compute stream after the last wave reading the slot
+    cudaStream_t waited = nullptr;   // compute stream that has already waited on `ready`
+};
+
+struct ef_ctx {
+    ef_config cfg{};
+    int64_t W = 0;                 // bytes per expert
+    int32_t n_sms = 148;
+    char* arena = nullptr;         // (S + L*n_shared) slots
+    int32_t n_arena_slots = 0;
+    void* h_ws = nullptr;          // bf16 [h_rows, f]
+    int64_t h_rows = 0;
+    int32_t* counts_pinned = nullptr;   // pinned mirror of counts[E]
+    cudaEvent_t counts_event = nullptr;
+    int32_t* permute_ws = nullptr;      // device scratch for ef_permute
+    cudaStream_t copy_stream = nullptr;
+    std::vector<cudaEvent_t> ev_ring;
+    std::vector<uint32_t> ev_gen;
+    int32_t ev_next = 0;
+    std::vector<EfPhys> phys;           // [S]
+    cudaStream_t last_compute = nullptr;
+    // host pool
+    std::vector<void*> host_expert;     // [L*E] packed pinned buffers (owned unless aliased)
+    std::vector<char> host_owned;
+    std::vector<char> shared_registered;  // [L*n_shared]
+    // policy
+    std::vector<EfSlot> slots;
+    std::vector<int32_t> slot_of;       // [L*E] -> slot or -1
+    std::map<int64_t, std::vector<uint8_t>> pred;   // visit -> predicted active flags [E]
+    uint64_t tick = 0;
+    ef_cache_stats stats{};
+    // tensor maps over the arena (3-D: k, row, slot)
+    CUtensorMap tm_w13{}, tm_wd{};
+    bool tm_ok = false;
+    // copy timing
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> copy_spans;
+    float copy_ms = 0.f;
+    // misc
+    int64_t launches = 0;
+    int32_t debug_simt = 0;
+    std::string err;
+    int32_t sticky = EF_OK;
+};
+
+int32_t ef_fail(ef_ctx* ctx, int32_t code, const char* fmt, ...);
+
+#define EF_CUDA(ctx, call)                                                                              \
+    do {                                                                                                \
+        cudaError_t e__ = (call);                                                                       \
+        if (e__ != cudaSuccess) {                                                                       \
+            (ctx)->sticky = EF_ERR_CUDA;                                                                \
+            return ef_fail((ctx), EF_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), \
+                           __FILE__, __LINE__);                                                         \
+        }                                                                                               \
+    } while (0)
+
+#define EF_CHECK_CTX(ctx)                         \
+    do {                                          \
+        if (!(ctx)) return EF_ERR_INVALID_ARG;    \
+        if ((ctx)->sticky != EF_OK) return (ctx)->sticky; \
+    } while (0)
+
+// ---- kernels (one launcher per translation unit) ---------------------------------------------------
+int32_t efk_route_topk(ef_ctx* ctx, cudaStream_t st, const void* x, const void* wr, const float* bias,
+                       int64_t bias_stride, int T, int renorm, int32_t* idx, float* w, float* logits);
+int32_t efk_permute(ef_ctx* ctx, cudaStream_t st, const int32_t* idx, const void* x, int T, void* x_perm,
+                    int32_t* counts, int32_t* offsets, int32_t* src, int32_t* inv, int32_t* counts_host);
+int32_t efk_combine(ef_ctx* ctx, cudaStream_t st, const void* y_perm, const int32_t* inv, const float* w, int T,
+                    const void* residual, const void* y_shared, void* out);
+int32_t efk_rmsnorm(ef_ctx* ctx, cudaStream_t st, const void* x, int T, float eps, void* out);
+
+// Grouped SwiGLU FFN over arena slots: x rows -> h workspace -> y rows.  tab.g[i] = {x_row0, y_row0, rows, slot};
+// h rows are placed at h_row0 + (x_row0 - tab.g[0].x_row0 is NOT assumed): h row of group i = h_row_of[i].
+int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& x_to_y,
+                        const int32_t* h_row0 /*[n]*/);
+int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
+                     const int32_t* h_row0);
+int32_t efk_ffn_tc_init(ef_ctx* ctx);   // build arena tensor maps, set smem attributes
+int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
+                   const int32_t* h_row0);

@@ -1,0 +1,415 @@
+// a4: grouped SwiGLU expert FFN over cache slots -- tcgen05 / TMEM / TMA kernels for sm_100a.
+//
+// Two launches per wave, both instances of one persistent, warp-specialised grouped GEMM
+//   C[rows_g, N] = A[rows_g, K] . B_slot(g)[N, K]^T      (bf16 x bf16 -> fp32 in TMEM)
+//   GEMM1: A = x_perm, B = packed W13 (gate/up interleaved by 128 rows), epilogue h = silu(g) * u  -> bf16
+//   GEMM2: A = h,      B = Wd,                                           epilogue y               -> bf16
+// (PAPER.md L46 leaves e_i opaque; SwiGLU is BASELINE.json's choice, R4.)
+//
+// Tile = up to 256 rows (two 128-lane accumulators "halves") x 256 B-rows, K step 64 (one 128-byte
+// swizzle span).  Per k-step each CTA pulls (128*halves + 256) rows x 128 B through TMA, so a
+// 256-row tile needs 1/3 less L2->SM traffic per flop than a 128-row one; L2 bandwidth, not the
+// tensor pipe, is what bounds a plain 128x256 tiling.
+//
+// Warp roles (256 threads, 1 CTA/SM, persistent over a static tile sequence):
+//   warp 0    TMA producer      : A boxes (64 x 128 rows, one per half) + B box (64 x 256 rows) per stage
+//   warp 1    MMA issuer        : one lane issues tcgen05.mma (M128 N256 K16), commits to mbarriers
+//   warp 2    TMEM allocator    : 512 columns = two 128x256 fp32 accumulator buffers
+//   warps 4-7 epilogue          : tcgen05.ld -> registers -> SwiGLU / cast -> 64-byte global stores
+// Ragged M: a group's last tile may be short; TMA zero-fills rows past the tensor, rows past the
+// group are computed and discarded (stores are row-predicated), so neighbours are never touched.
+#include <cuda_bf16.h>
+
+#include "ef_internal.h"
+
+namespace {
+
+constexpr int BK = 64;                 // K elements per stage (128 bytes of bf16)
+constexpr int BN = 256;                // B rows per tile
+constexpr int HALF_M = 128;            // rows per accumulator half
+constexpr int kStages = 3;
+constexpr int A_HALF_BYTES = HALF_M * BK * 2;   // 16 KB
+constexpr int B_BYTES = BN * BK * 2;            // 32 KB
+constexpr int STAGE_BYTES = 2 * A_HALF_BYTES + B_BYTES;   // 64 KB
+constexpr int kThreads = 256;
+constexpr int kTmemCols = 512;
+
+struct __align__(8) SmemCtl {
+    uint64_t full[kStages];
+    uint64_t empty[kStages];
+    uint64_t tmem_full[2];
+    uint64_t tmem_empty[2];
+    uint32_t tmem_base;
+    int32_t gstart[EF_MAX_GROUPS + 1];
+};
+
+constexpr size_t kSmemBytes = 1024 /*align slack*/ + (size_t)kStages * STAGE_BYTES + sizeof(SmemCtl);
+
+// ---- PTX wrappers ----------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// D[tmem] (+)= A[smem] . B[smem]^T, M128 N256 K16, bf16 -> fp32
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accum) : "memory");
+}
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t* v) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// K-major, 128-byte swizzle: 8-row groups 1024 B apart (SBO), LBO unused (=1), descriptor version 1
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
+}
+// kind::f16 instruction descriptor: D fp32, A/B bf16, both K-major, N=256, M=128
+constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(HALF_M >> 4) << 24);
+
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&v);
+}
+
+struct Tile {
+    int a_row, c_row, rows_valid, halves, n_tile, slot;
+};
+
+__device__ __forceinline__ int group_mtiles(int rows, int tile_rows) { return (rows + tile_rows - 1) / tile_rows; }
+
+__device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const int32_t* gstart, int tile, int n_tiles_n,
+                                            int max_halves) {
+    int g = 0;
+    while (tile >= gstart[g + 1]) ++g;
+    const int tile_rows = HALF_M * max_halves;
+    const int local = tile - gstart[g];
+    const int mt = group_mtiles(tab.g[g].rows, tile_rows);
+    const int n = local / mt, m = local % mt;
+    const int row_off = m * tile_rows;
+    const int rem = tab.g[g].rows - row_off;
+    Tile t;
+    t.halves = (max_halves == 2 && rem > HALF_M) ? 2 : 1;
+    t.rows_valid = min(rem, HALF_M * t.halves);
+    t.a_row = tab.g[g].a_row0 + row_off;
+    t.c_row = tab.g[g].c_row0 + row_off;
+    t.n_tile = n;
+    t.slot = tab.g[g].slot;
+    (void)n_tiles_n;
+    return t;
+}
+
+// kSwiglu: accumulator columns [0,128) = gate, [128,256) = up for 128 output columns; else 256 output columns
+template <bool kSwiglu>
+__global__ void __launch_bounds__(kThreads, 1)
+ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int max_halves, int total_tiles,
+                const __grid_constant__ EfGroupTable tab) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    SmemCtl* ctl = (SmemCtl*)(smem + (size_t)kStages * STAGE_BYTES);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+    }
+    if (warp == 1 && lane == 0) {
+        for (int i = 0; i < kStages; ++i) { mbar_init(&ctl->full[i], 1); mbar_init(&ctl->empty[i], 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&ctl->tmem_full[i], 1); mbar_init(&ctl->tmem_empty[i], 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&ctl->tmem_base)), "r"(kTmemCols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (warp == 3 && lane == 0) {
+        const int tile_rows = HALF_M * max_halves;
+        int acc = 0;
+        for (int g = 0; g < tab.n; ++g) {
+            ctl->gstart[g] = acc;
+            acc += group_mtiles(tab.g[g].rows, tile_rows) * n_tiles_n;
+        }
+        ctl->gstart[tab.n] = acc;
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = ctl->tmem_base;
+    const int KB = K / BK;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+                const Tile t = decode_tile(tab, ctl->gstart, tile, n_tiles_n, max_halves);
+                const uint32_t bytes = (uint32_t)(t.halves * A_HALF_BYTES + B_BYTES);
+                for (int kb = 0; kb < KB; ++kb) {
+                    mbar_wait(&ctl->empty[stage], phase ^ 1);
+                    uint8_t* sa = smem + (size_t)stage * STAGE_BYTES;
+                    mbar_expect_tx(&ctl->full[stage], bytes);
+                    tma_load_2d(sa, &tmA, &ctl->full[stage], kb * BK, t.a_row);
+                    if (t.halves == 2) tma_load_2d(sa + A_HALF_BYTES, &tmA, &ctl->full[stage], kb * BK, t.a_row + HALF_M);
+                    tma_load_3d(sa + 2 * A_HALF_BYTES, &tmB, &ctl->full[stage], kb * BK, t.n_tile * BN, t.slot);
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            int buf = 0; uint32_t bphase[2] = {0, 0};
+            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+                const Tile t = decode_tile(tab, ctl->gstart, tile, n_tiles_n, max_halves);
+                if (t.halves == 2) buf = 0;
+                const int b0 = buf;
+                for (int h = 0; h < t.halves; ++h) mbar_wait(&ctl->tmem_empty[b0 + h], bphase[b0 + h] ^ 1);
+                tc_fence_after();
+                for (int kb = 0; kb < KB; ++kb) {
+                    mbar_wait(&ctl->full[stage], phase);
+                    tc_fence_after();
+                    const uint32_t sa = smem_u32(smem + (size_t)stage * STAGE_BYTES);
+                    const uint32_t sb = sa + 2 * A_HALF_BYTES;
+#pragma unroll
+                    for (int k = 0; k < BK / 16; ++k) {
+                        const uint64_t bd = smem_desc(sb + k * 32);
+                        const uint32_t acc = (kb > 0 || k > 0) ? 1u : 0u;
+                        tc_mma(tmem_base + (uint32_t)(b0 * BN), smem_desc(sa + k * 32), bd, kIdesc, acc);
+                        if (t.halves == 2)
+                            tc_mma(tmem_base + (uint32_t)((b0 + 1) * BN), smem_desc(sa + A_HALF_BYTES + k * 32), bd, kIdesc, acc);
+                    }
+                    tc_commit(&ctl->empty[stage]);    // frees the smem stage once these MMAs have read it
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                }
+                for (int h = 0; h < t.halves; ++h) {
+                    tc_commit(&ctl->tmem_full[b0 + h]);
+                    bphase[b0 + h] ^= 1;
+                }
+                buf = (t.halves == 2) ? 0 : (b0 ^ 1);
+            }
+        }
+    } else if (warp >= 4) {
+        // ===== epilogue =====
+        const int q = warp - 4;                      // TMEM lane quarter of this warp (warp % 4)
+        int buf = 0; uint32_t bphase[2] = {0, 0};
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+            const Tile t = decode_tile(tab, ctl->gstart, tile, n_tiles_n, max_halves);
+            if (t.halves == 2) buf = 0;
+            const int b0 = buf;
+            for (int h = 0; h < t.halves; ++h) {
+                const int b = b0 + h;
+                mbar_wait(&ctl->tmem_full[b], bphase[b]);
+                bphase[b] ^= 1;
+                tc_fence_after();
+                const int r = h * HALF_M + q * 32 + lane;            // row inside the tile
+                const bool row_ok = r < t.rows_valid;
+                const bool warp_ok = (h * HALF_M + q * 32) < t.rows_valid;
+                const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b * BN);
+                if (warp_ok) {
+                    if (kSwiglu) {
+                        uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * 128;
+#pragma unroll 1
+                        for (int c = 0; c < 4; ++c) {
+                            uint32_t g[32], u[32];
+                            tc_ld32(tbase + c * 32, g);
+                            tc_ld32(tbase + 128 + c * 32, u);
+                            tc_wait_ld();
+                            uint32_t o[16];
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) {
+                                const float g0 = __uint_as_float(g[2 * i]), g1 = __uint_as_float(g[2 * i + 1]);
+                                const float u0 = __uint_as_float(u[2 * i]), u1 = __uint_as_float(u[2 * i + 1]);
+                                const float h0 = __fdividef(g0, 1.f + __expf(-g0)) * u0;
+                                const float h1 = __fdividef(g1, 1.f + __expf(-g1)) * u1;
+                                o[i] = pack_bf16(h0, h1);
+                            }
+                            if (row_ok) {
+                                uint4* dst = (uint4*)(crow + c * 32);
+#pragma unroll
+                                for (int i = 0; i < 4; ++i) dst[i] = make_uint4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
+                            }
+                        }
+                    } else {
+                        uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * BN;
+#pragma unroll 1
+                        for (int c = 0; c < 8; ++c) {
+                            if (t.n_tile * BN + c * 32 >= n_cols) break;     // N tail (n_cols % 64 == 0)
+                            uint32_t v[32];
+                            tc_ld32(tbase + c * 32, v);
+                            tc_wait_ld();
+                            uint32_t o[16];
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) o[i] = pack_bf16(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
+                            if (row_ok) {
+                                uint4* dst = (uint4*)(crow + c * 32);
+#pragma unroll
+                                for (int i = 0; i < 4; ++i) dst[i] = make_uint4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
+                            }
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&ctl->tmem_empty[b]);
+            }
+            buf = (t.halves == 2) ? 0 : (b0 ^ 1);
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+    }
+}
+
+// ---- host side -------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// 2-D bf16 [rows, K] row-major, box 64 x 128, 128-byte swizzle
+int32_t make_map_2d(ef_ctx* ctx, CUtensorMap* tm, const void* base, int64_t rows, int64_t K) {
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return ef_fail(ctx, EF_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+    cuuint64_t strides[1] = {(cuuint64_t)K * 2};
+    cuuint32_t box[2] = {BK, HALF_M};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return ef_fail(ctx, EF_ERR_CUDA, "cuTensorMapEncodeTiled(2d) failed: %d", (int)r);
+    return EF_OK;
+}
+
+// 3-D bf16 [slot, rows, K] over the arena, box 64 x 256 x 1
+int32_t make_map_arena(ef_ctx* ctx, CUtensorMap* tm, const void* base, int64_t rows, int64_t K) {
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return ef_fail(ctx, EF_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    cuuint64_t dims[3] = {(cuuint64_t)K, (cuuint64_t)rows, (cuuint64_t)ctx->n_arena_slots};
+    cuuint64_t strides[2] = {(cuuint64_t)K * 2, (cuuint64_t)ctx->W};
+    cuuint32_t box[3] = {BK, BN, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return ef_fail(ctx, EF_ERR_CUDA, "cuTensorMapEncodeTiled(arena) failed: %d", (int)r);
+    return EF_OK;
+}
+
+}  // namespace
+
+int32_t efk_ffn_tc_init(ef_ctx* ctx) {
+    const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
+    int32_t rc = make_map_arena(ctx, &ctx->tm_w13, ctx->arena, 2 * (int64_t)f, d);
+    if (rc != EF_OK) return rc;
+    rc = make_map_arena(ctx, &ctx->tm_wd, ctx->arena + (size_t)2 * f * d * 2, d, f);
+    if (rc != EF_OK) return rc;
+    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+    ctx->tm_ok = true;
+    return EF_OK;
+}
+
+int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
+                   const int32_t* h_row0) {
+    const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
+    if (tab.n == 0) return EF_OK;
+    int64_t x_rows = 0;
+    for (int i = 0; i < tab.n; ++i) x_rows = std::max<int64_t>(x_rows, (int64_t)tab.g[i].a_row0 + tab.g[i].rows);
+    CUtensorMap tmX, tmH;
+    int32_t rc = make_map_2d(ctx, &tmX, x, x_rows, d);
+    if (rc != EF_OK) return rc;
+    rc = make_map_2d(ctx, &tmH, ctx->h_ws, ctx->h_rows, f);
+    if (rc != EF_OK) return rc;
+
+    const int max_halves = 2;
+    const int tile_rows = HALF_M * max_halves;
+    int mtiles = 0;
+    EfGroupTable t1 = tab, t2 = tab;
+    for (int i = 0; i < tab.n; ++i) {
+        mtiles += (tab.g[i].rows + tile_rows - 1) / tile_rows;
+        t1.g[i].c_row0 = h_row0[i];   // GEMM1: x rows -> h rows
+        t2.g[i].a_row0 = h_row0[i];   // GEMM2: h rows -> y rows
+    }
+    {
+        const int ntn = f / 128;      // 256 packed W13 rows -> 128 h columns
+        const int total = mtiles * ntn;
+        const int grid = std::min(total, ctx->n_sms);
+        ffn_gemm_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn,
+                                                                  max_halves, total, t1);
+        ctx->launches++;
+        EF_CUDA(ctx, cudaGetLastError());
+    }
+    {
+        const int ntn = (d + BN - 1) / BN;
+        const int total = mtiles * ntn;
+        const int grid = std::min(total, ctx->n_sms);
+        ffn_gemm_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_wd, (uint16_t*)y, d, d, f, ntn,
+                                                                   max_halves, total, t2);
+        ctx->launches++;
+        EF_CUDA(ctx, cudaGetLastError());
+    }
+    return EF_OK;
+}

@@ -1,0 +1,117 @@
+// a2: permute tokens by expert (dispatch implied by PAPER.md L21, L68; R5).
+//
+// Two launches.
+//  (1) permute_index_kernel -- one CTA, 32 warps.  Stable counting sort of the R = T*k flat pairs:
+//      each warp owns a contiguous chunk of pairs; per-warp histograms in shared memory
+//      (__match_any_sync groups equal keys, one lane adds the group size: no atomics), a scan over
+//      warps then over experts, then every pair's row = offsets[e] + (pairs of e in earlier warps)
+//      + (rank inside the warp's running chunk).  Also mirrors counts into pinned host memory.
+//  (2) gather_rows_kernel -- HBM-bound row copy x[src[row]/k,:] -> x_perm[row,:], one warp per row,
+//      128-bit loads/stores (reads 2*d bytes per token once from HBM -- the k re-reads hit L2 --
+//      and writes 2*d*k bytes per token).
+#include "ef_internal.h"
+
+namespace {
+
+constexpr int kIdxWarps = 32;
+
+__global__ void __launch_bounds__(kIdxWarps * 32)
+permute_index_kernel(const int32_t* __restrict__ idx, int R, int E, int32_t* __restrict__ counts,
+                     int32_t* __restrict__ offsets, int32_t* __restrict__ src, int32_t* __restrict__ inv,
+                     int32_t* counts_host) {
+    extern __shared__ int32_t sm[];
+    int32_t* hist = sm;                       // [kIdxWarps][E]
+    int32_t* s_off = sm + kIdxWarps * E;      // [E + 1]
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < kIdxWarps * E; i += blockDim.x) hist[i] = 0;
+    __syncthreads();
+
+    // contiguous chunk per warp, multiple of 32 so that iterations are lane-aligned
+    int chunk = (R + kIdxWarps - 1) / kIdxWarps;
+    chunk = (chunk + 31) & ~31;
+    const int lo = min(R, warp * chunk), hi = min(R, lo + chunk);
+    int32_t* myh = hist + warp * E;
+
+    for (int base = lo; base < hi; base += 32) {
+        const int p = base + lane;
+        const bool valid = p < hi;
+        const int key = valid ? idx[p] : (E + lane);     // invalid lanes get unique keys
+        const unsigned mask = __match_any_sync(0xffffffffu, key);
+        if (valid && lane == (__ffs(mask) - 1)) myh[key] += __popc(mask);
+        __syncwarp();
+    }
+    __syncthreads();
+
+    // scan over warps for each expert: hist[w][e] becomes the number of e-pairs in warps < w
+    for (int e = threadIdx.x; e < E; e += blockDim.x) {
+        int run = 0;
+        for (int w = 0; w < kIdxWarps; ++w) {
+            int c = hist[w * E + e];
+            hist[w * E + e] = run;
+            run += c;
+        }
+        s_off[e + 1] = run;   // temporarily: counts, shifted by one
+        counts[e] = run;
+        if (counts_host) counts_host[e] = run;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        // E <= 256: a serial scan by one thread costs well under a microsecond
+        s_off[0] = 0;
+        for (int e = 0; e < E; ++e) s_off[e + 1] += s_off[e];
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e <= E; e += blockDim.x) offsets[e] = s_off[e];
+    if (counts_host) __threadfence_system();
+
+    for (int base = lo; base < hi; base += 32) {
+        const int p = base + lane;
+        const bool valid = p < hi;
+        const int key = valid ? idx[p] : (E + lane);
+        const unsigned mask = __match_any_sync(0xffffffffu, key);
+        const int rank = __popc(mask & ((1u << lane) - 1u));
+        if (valid) {
+            const int row = s_off[key] + myh[key] + rank;
+            inv[p] = row;
+            src[row] = p;
+        }
+        __syncwarp();
+        if (valid && lane == (__ffs(mask) - 1)) myh[key] += __popc(mask);
+        __syncwarp();
+    }
+}
+
+__global__ void __launch_bounds__(256)
+gather_rows_kernel(const uint4* __restrict__ x, const int32_t* __restrict__ src, int R, int k, int d8,
+                   uint4* __restrict__ x_perm) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (warp >= R) return;
+    const int t = src[warp] / k;
+    const uint4* in = x + (int64_t)t * d8;
+    uint4* out = x_perm + (int64_t)warp * d8;
+    int c = lane;
+    for (; c + 96 < d8; c += 128) {   // 4 independent 128-bit loads in flight per lane
+        uint4 a = in[c], b = in[c + 32], e = in[c + 64], f = in[c + 96];
+        out[c] = a; out[c + 32] = b; out[c + 64] = e; out[c + 96] = f;
+    }
+    for (; c < d8; c += 32) out[c] = in[c];
+}
+
+}  // namespace
+
+int32_t efk_permute(ef_ctx* ctx, cudaStream_t st, const int32_t* idx, const void* x, int T, void* x_perm,
+                    int32_t* counts, int32_t* offsets, int32_t* src, int32_t* inv, int32_t* counts_host) {
+    const int E = ctx->cfg.n_experts, k = ctx->cfg.top_k, d = ctx->cfg.d_model;
+    const int R = T * k;
+    size_t smem = ((size_t)kIdxWarps * E + E + 1) * sizeof(int32_t);
+    permute_index_kernel<<<1, kIdxWarps * 32, smem, st>>>(idx, R, E, counts, offsets, src, inv, counts_host);
+    ctx->launches++;
+    EF_CUDA(ctx, cudaGetLastError());
+    if (R > 0) {
+        int blocks = (R * 32 + 255) / 256;
+        gather_rows_kernel<<<blocks, 256, 0, st>>>((const uint4*)x, src, R, k, d / 8, (uint4*)x_perm);
+        ctx->launches++;
+        EF_CUDA(ctx, cudaGetLastError());
+    }
+    return EF_OK;
+}

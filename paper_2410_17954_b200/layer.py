@@ -1,0 +1,88 @@
+"""MoELayerRunner: the call a user makes -- one MoE layer visit through libef, in the order of
+SURVEY.md §3(ii): route -> permute -> (cache lookup + correction + grouped FFN) -> PLEC prefetch ->
+combine.  Sequencing and buffer ownership only; every step of the path runs in the CUDA library.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from .binding import EfContext
+
+
+def bf16_tensor_from_bits(bits: np.ndarray, device=None, pin=False) -> torch.Tensor:
+    """uint16 bit patterns -> torch.bfloat16 tensor (no value conversion)."""
+    t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16)
+    if pin:
+        t = t.pin_memory()
+    if device is not None:
+        t = t.to(device, non_blocking=pin)
+    return t
+
+
+def bits_from_bf16_tensor(t: torch.Tensor) -> np.ndarray:
+    return t.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+
+
+class MoELayerRunner:
+    def __init__(self, n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared=0, max_tokens=1,
+                 prefetch_horizon=0, renorm=1, device=0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("MoELayerRunner needs a CUDA device; there is no CPU fallback")
+        self.dev = torch.device("cuda", device)
+        torch.cuda.set_device(self.dev)
+        self.L, self.E, self.k, self.d, self.f = n_layers, n_experts, top_k, d_model, d_ff
+        self.n_shared, self.renorm, self.max_tokens = n_shared, renorm, max_tokens
+        self.ctx = EfContext(n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared, max_tokens,
+                             prefetch_horizon, device)
+        T, k, E, d = max_tokens, top_k, n_experts, d_model
+        dev = self.dev
+        self.w_router = [None] * n_layers
+        self.bias = [None] * n_layers
+        self.topk_idx = torch.empty((T, k), dtype=torch.int32, device=dev)
+        self.topk_w = torch.empty((T, k), dtype=torch.float32, device=dev)
+        self.logits = torch.empty((T, E), dtype=torch.float32, device=dev)
+        self.counts = torch.empty((E,), dtype=torch.int32, device=dev)
+        self.offsets = torch.empty((E + 1,), dtype=torch.int32, device=dev)
+        self.src = torch.empty((T * k,), dtype=torch.int32, device=dev)
+        self.inv = torch.empty((T * k,), dtype=torch.int32, device=dev)
+        self.x_perm = torch.empty((T * k, d), dtype=torch.bfloat16, device=dev)
+        self.y_perm = torch.empty((T * k, d), dtype=torch.bfloat16, device=dev)
+        self.y_shared = torch.empty((max(1, n_shared) * T, d), dtype=torch.bfloat16, device=dev) if n_shared else None
+        self.normed = torch.empty((T, d), dtype=torch.bfloat16, device=dev)
+
+    # ---- setup
+    def set_router(self, layer, w_router_bits: np.ndarray, bias: np.ndarray | None = None):
+        self.w_router[layer] = bf16_tensor_from_bits(w_router_bits, self.dev)
+        self.bias[layer] = None if bias is None else torch.from_numpy(np.ascontiguousarray(bias, np.float32)).to(self.dev)
+
+    def register_expert(self, layer, expert, wg, wu, wd):
+        self.ctx.ef_host_expert_register(layer, expert, wg, wu, wd)
+
+    # ---- one visit
+    def visit(self, visit: int, x: torch.Tensor, out: torch.Tensor, token_bias: torch.Tensor | None = None,
+              predicted_next: np.ndarray | None = None, residual: torch.Tensor | None = None,
+              want_logits: bool = False, pre_norm_eps: float | None = None):
+        """x: [T, d] bf16 device.  out: [T, d] bf16 device.  predicted_next: uint8 [n_ahead, E] for visits
+        visit+1.. (None = no prefetch call).  pre_norm_eps: apply RMSNorm to x first (cfg 5 stack)."""
+        c = self.ctx
+        T = x.shape[0]
+        layer = visit % self.L
+        inp = x
+        if pre_norm_eps is not None:
+            inp = self.normed[:T]
+            c.ef_rmsnorm(x, T, pre_norm_eps, inp)
+        bias = token_bias if token_bias is not None else self.bias[layer]
+        c.ef_route_topk(inp, self.w_router[layer], bias, T, self.renorm, self.topk_idx, self.topk_w,
+                        self.logits if want_logits else None)
+        c.ef_permute(self.topk_idx, inp, T, self.x_perm, self.counts, self.offsets, self.src, self.inv)
+        if self.n_shared:
+            c.ef_shared_ffn(layer, inp, T, self.y_shared)
+        c.ef_expert_ffn_grouped(visit, layer, self.x_perm, None, self.y_perm)
+        if predicted_next is not None:
+            c.ef_cache_prefetch(visit, predicted_next)
+        c.ef_combine(self.y_perm, self.inv, self.topk_w, T, residual, self.y_shared, out)
+        return out
+
+    def close(self):
+        self.ctx.close()

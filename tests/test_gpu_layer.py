@@ -1,0 +1,191 @@
+"""GPU parity, end to end: whole layer visits through MoELayerRunner (the public call) against the
+oracle, and the cache manager's slot table + counters against oracle/cache_sim.py bit for bit."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+from oracle.cache_sim import CacheSim, STAT_KEYS
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from test_gpu_stages import bf, check_float, dev_bf16, to_bits  # noqa: E402
+
+
+def build_runner(cfg, horizon=None, experts=None, max_tokens=None):
+    from paper_2410_17954_b200 import MoELayerRunner
+    r = MoELayerRunner(cfg.n_layers, cfg.n_experts, cfg.top_k, cfg.d_model, cfg.d_ff, cfg.n_slots, cfg.n_shared,
+                       max_tokens or cfg.T, cfg.horizon if horizon is None else horizon, cfg.renorm)
+    experts = experts or {}
+    for l in range(cfg.n_layers):
+        r.set_router(l, wl.router_weight(cfg, l), wl.static_router_bias(cfg, l))
+        for e in range(cfg.n_experts):
+            if (l, e) not in experts:
+                experts[(l, e)] = wl.expert_weights(cfg, l, e)
+            r.register_expert(l, e, *experts[(l, e)])
+        for s in range(cfg.n_shared):
+            experts[(l, -1 - s)] = wl.expert_weights(cfg, l, -1 - s)
+            r.register_expert(l, -1 - s, *experts[(l, -1 - s)])
+    return r, experts
+
+
+def assert_cache_equal(runner, sim):
+    assert runner.ctx.ef_cache_snapshot() == sim.snapshot()
+    st = runner.ctx.ef_cache_get_stats()
+    assert st == {k: sim.stats[k] for k in STAT_KEYS}
+
+
+# ------------------------------------------------------------------------------------------------
+# cfg 1 (tiny): the whole visit, predicted path 100% correct, cold cache of 4 slots
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("simt", [True, False], ids=["simt_debug", "tcgen05"])
+def test_cfg1_tiny_end_to_end(simt):
+    cfg = wl.CONFIGS["tiny"]
+    r, ex = build_runner(cfg)
+    r.ctx.ef_set_debug_simt_ffn(simt)
+    x = wl.activations(cfg)
+    ref = oracle.layer_forward(x, wl.router_weight(cfg), None, [ex[(0, e)] for e in range(cfg.n_experts)], cfg.top_k)
+    predicted = (ref.counts > 0).astype(np.uint8)[None, :]          # "a routing path that is 100% correct"
+    sim = CacheSim(1, cfg.n_experts, cfg.n_slots, cfg.expert_bytes, cfg.horizon)
+    sim.prefetch(-1, predicted); r.ctx.ef_cache_prefetch(-1, predicted)
+    assert_cache_equal(r, sim)
+    out = torch.empty((cfg.T, cfg.d_model), dtype=torch.bfloat16, device="cuda")
+    r.visit(0, dev_bf16(x), out, want_logits=True)
+    sim.visit(0, ref.counts)
+    r.ctx.ef_sync()
+    assert_cache_equal(r, sim)
+    assert sim.stats["lookups"] == int((ref.counts > 0).sum())
+    # integers bit-exact
+    assert np.array_equal(r.topk_idx.cpu().numpy(), ref.idx)
+    assert np.array_equal(r.counts.cpu().numpy(), ref.counts)
+    assert np.array_equal(r.offsets.cpu().numpy(), ref.offsets)
+    assert np.array_equal(r.src.cpu().numpy(), ref.src)
+    assert np.array_equal(r.inv.cpu().numpy(), ref.inv)
+    assert np.array_equal(to_bits(r.x_perm), ref.x_perm)
+    np.testing.assert_allclose(r.topk_w.cpu().numpy(), ref.w, rtol=2e-4)
+    check_float(bf(to_bits(r.y_perm)), ref.y_perm)
+    check_float(bf(to_bits(out)), ref.out)
+    r.close()
+
+
+def test_identical_experts_reduce_to_dense_ffn_on_gpu():
+    cfg = wl.scaled(wl.CONFIGS["tiny"], T=48, n_slots=8)
+    w3 = wl.expert_weights(cfg, 0, 0)
+    r, _ = build_runner(cfg, experts={(0, e): w3 for e in range(cfg.n_experts)})
+    x = wl.activations(cfg)
+    out = torch.empty((cfg.T, cfg.d_model), dtype=torch.bfloat16, device="cuda")
+    r.visit(0, dev_bf16(x), out)
+    r.ctx.ef_sync()
+    dense = oracle.expert_ffn(x, *w3)
+    check_float(bf(to_bits(out)), dense)
+    r.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# shared experts + skewed many-expert routing (cfg 4 shape, reduced size)
+# ------------------------------------------------------------------------------------------------
+def test_cfg4_reduced_shared_experts_and_zipf():
+    cfg = wl.scaled(wl.CONFIGS["many_expert_prefill"], T=512, d_model=256, d_ff=384)
+    r, ex = build_runner(cfg)
+    x = wl.activations(cfg)
+    ref = oracle.layer_forward(x, wl.router_weight(cfg), wl.static_router_bias(cfg),
+                               [ex[(0, e)] for e in range(cfg.n_experts)], cfg.top_k,
+                               shared=[ex[(0, -1)], ex[(0, -2)]])
+    srt = np.sort(ref.logits, axis=1)[:, ::-1]
+    assert (srt[:, cfg.top_k - 1] - srt[:, cfg.top_k]).min() > 1e-5     # routing unambiguous at fp32 (R22)
+    predicted = (ref.counts > 0).astype(np.uint8)[None, :]
+    sim = CacheSim(1, cfg.n_experts, cfg.n_slots, cfg.expert_bytes, cfg.horizon)
+    sim.prefetch(-1, predicted); r.ctx.ef_cache_prefetch(-1, predicted)
+    out = torch.empty((cfg.T, cfg.d_model), dtype=torch.bfloat16, device="cuda")
+    r.visit(0, dev_bf16(x), out)
+    sim.visit(0, ref.counts)
+    r.ctx.ef_sync()
+    assert np.array_equal(r.topk_idx.cpu().numpy(), ref.idx)
+    assert np.array_equal(r.inv.cpu().numpy(), ref.inv)
+    assert_cache_equal(r, sim)
+    assert sim.stats["misses"] > 0                                       # waves were exercised
+    check_float(bf(to_bits(out)), ref.out)
+    r.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# decode traces: cache accounting bit-exact over many visits; outputs checked on sampled visits
+# ------------------------------------------------------------------------------------------------
+def run_decode(cfg, n_steps, horizon, check_out_every):
+    L, E = cfg.n_layers, cfg.n_experts
+    r, ex = build_runner(cfg, horizon=horizon)
+    tr = wl.routing_trace(cfg, n_steps)
+    sim = CacheSim(L, E, cfg.n_slots, cfg.expert_bytes, horizon)
+    nv = n_steps * L
+    look = L if horizon <= 0 else horizon
+
+    def window(v):
+        return tr.predicted[v + 1:min(nv, v + 1 + look)]
+    w0 = window(-1)
+    sim.prefetch(-1, w0); r.ctx.ef_cache_prefetch(-1, w0)
+    out = torch.empty((cfg.T, cfg.d_model), dtype=torch.bfloat16, device="cuda")
+    wrs = [wl.router_weight(cfg, l) for l in range(L)]
+    for s in range(n_steps):
+        h = wl.activations(cfg, s)                       # fresh seeded h_0 per step
+        hd = dev_bf16(h)
+        for l in range(L):
+            v = s * L + l
+            bias = wl.trace_bias(cfg, tr, v)
+            win = window(v)
+            nxt = torch.empty_like(hd)
+            r.visit(v, hd, nxt, token_bias=torch.from_numpy(bias).cuda(), predicted_next=win if len(win) else None,
+                    residual=hd if L > 1 else None, pre_norm_eps=1e-5 if L > 1 else None)
+            counts = np.bincount(tr.sets[v].ravel(), minlength=E)
+            sim.visit(v, counts)
+            if len(win):
+                sim.prefetch(v, win)
+            assert_cache_equal(r, sim)
+            check = check_out_every and v % check_out_every == 0
+            if L > 1:
+                # the oracle runs its own chain from the seeded h_0 (nothing flows from the GPU into it);
+                # activations between layers are bf16 at the boundary, so it rounds exactly there
+                u = oracle.round_bf16(oracle.rmsnorm(h, 1e-5))
+                ref = oracle.layer_forward(u, wrs[l], bias, [ex[(l, e)] for e in range(E)], cfg.top_k, res=h)
+                h = oracle.round_bf16(ref.out)
+            elif check:
+                ref = oracle.layer_forward(h, wrs[l], bias, [ex[(l, e)] for e in range(E)], cfg.top_k)
+            if check:
+                r.ctx.ef_sync()
+                assert np.array_equal(r.counts.cpu().numpy(), counts)          # the trace bias drove the router
+                assert np.array_equal(r.topk_idx.cpu().numpy(), ref.idx)
+                check_float(bf(to_bits(nxt)), ref.out)
+            hd = nxt
+    r.ctx.ef_sync()
+    st = r.ctx.ef_cache_get_stats()
+    r.close()
+    return st, sim
+
+
+@pytest.mark.parametrize("horizon", [1, 0])
+def test_cfg3_reduced_decode_trace(horizon):
+    cfg = wl.scaled(wl.CONFIGS["mixtral_decode"], d_model=256, d_ff=512)
+    st, sim = run_decode(cfg, n_steps=48, horizon=horizon, check_out_every=7)
+    assert st["lookups"] > 0 and st["hits"] + st["misses"] == st["lookups"]
+    assert st["bytes_h2d"] == cfg.expert_bytes * (st["ondemand_loads"] + st["prefetch_issued"])
+
+
+@pytest.mark.parametrize("horizon", [0, 1])
+def test_cfg5_reduced_stack_trace(horizon):
+    cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=256, d_ff=512, T=32, n_layers=6, n_slots=12)
+    st, sim = run_decode(cfg, n_steps=10, horizon=horizon, check_out_every=5)
+    assert st["prefetch_issued"] > 0 and st["misses"] < st["lookups"]
+
+
+def test_evict_and_clear_match_simulator():
+    cfg = wl.scaled(wl.CONFIGS["tiny"], n_slots=6)
+    r, _ = build_runner(cfg)
+    sim = CacheSim(1, cfg.n_experts, cfg.n_slots, cfg.expert_bytes)
+    p = np.array([[1, 1, 0, 1, 1, 0, 1, 0]], np.uint8)
+    sim.prefetch(-1, p); r.ctx.ef_cache_prefetch(-1, p)
+    sim.evict(0, [1, 2, 4]); r.ctx.ef_cache_evict(0, [1, 2, 4])
+    assert_cache_equal(r, sim)
+    r.ctx.ef_cache_clear()
+    assert r.ctx.ef_cache_snapshot() == [-1] * cfg.n_slots
+    r.close()
