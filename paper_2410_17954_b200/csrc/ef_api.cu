@@ -43,10 +43,11 @@ static EvHandle ring_record(ef_ctx* ctx, cudaStream_t st, cudaError_t* err) {
 
 // make `waiter` wait for handle h (recorded on `origin`); if h was recycled, wait for everything
 // enqueued on `origin` so far, which is a superset.
-static cudaError_t ring_wait(ef_ctx* ctx, cudaStream_t waiter, const EvHandle& h, cudaStream_t origin) {
+static cudaError_t ring_wait(ef_ctx* ctx, cudaStream_t waiter, const EvHandle& h, cudaStream_t origin,
+                             bool origin_valid = true) {
     if (h.idx < 0) return cudaSuccess;
     if (ctx->ev_gen[h.idx] == h.gen) return cudaStreamWaitEvent(waiter, ctx->ev_ring[h.idx], 0);
-    if (!origin || origin == waiter) return cudaSuccess;
+    if (!origin_valid || origin == waiter) return cudaSuccess;
     cudaError_t e;
     EvHandle f = ring_record(ctx, origin, &e);
     if (e != cudaSuccess) return e;
@@ -305,7 +306,7 @@ int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
     ctx->stats.bytes_h2d += (uint64_t)ctx->W;
 
     EfPhys& ph = ctx->phys[slot];
-    EF_CUDA(ctx, ring_wait(ctx, ctx->copy_stream, ph.free_, ctx->last_compute));
+    EF_CUDA(ctx, ring_wait(ctx, ctx->copy_stream, ph.free_, ctx->last_compute, ctx->has_last_compute));
     cudaEvent_t t0, t1;
     if (ctx->copy_spans.size() > 8192) drain_copy_spans(ctx, false, nullptr);
     EF_CUDA(ctx, cudaEventCreate(&t0));
@@ -319,6 +320,7 @@ int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
     ph.ready = ring_record(ctx, ctx->copy_stream, &e);
     EF_CUDA(ctx, e);
     ph.free_ = EvHandle();
+    ph.has_waited = false;
     ph.waited = nullptr;
     return EF_OK;
 }
@@ -350,8 +352,9 @@ int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm,
     auto& phys = ctx->phys;
     for (const WaveItem& it : items) {
         EfPhys& ph = phys[it.slot];
-        if (ph.ready.idx >= 0 && ph.waited != st) {
+        if (ph.ready.idx >= 0 && !(ph.has_waited && ph.waited == st)) {
             EF_CUDA(ctx, ring_wait(ctx, st, ph.ready, ctx->copy_stream));
+            ph.has_waited = true;
             ph.waited = st;
         }
     }
@@ -372,6 +375,7 @@ int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm,
     EF_CUDA(ctx, e);
     for (const WaveItem& it : items) phys[it.slot].free_ = ev;
     ctx->last_compute = st;
+    ctx->has_last_compute = true;
     return EF_OK;
 }
 
@@ -405,6 +409,7 @@ extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visi
     if ((int64_t)off[E] > (int64_t)c.max_tokens * c.top_k)
         return ef_fail(ctx, EF_ERR_CAPACITY, "ef_expert_ffn_grouped: sum(counts) > max_tokens * top_k");
     ctx->last_compute = st;
+    ctx->has_last_compute = true;
 
     // lookup (R6)
     std::vector<int> hits, misses;
@@ -477,6 +482,7 @@ extern "C" int32_t ef_expert_ffn_grouped_resident(ef_ctx* ctx, void* stream, con
         items.push_back(WaveItem{row_begin[i], rows[i], slots[i]});
     }
     ctx->last_compute = st;
+    ctx->has_last_compute = true;
     return run_wave(ctx, st, x_perm, y_perm, items);
 }
 

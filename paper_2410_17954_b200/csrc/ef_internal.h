@@ -50,7 +50,8 @@ struct EvHandle {
 struct EfPhys {
     EvHandle ready;                  // recorded on the copy stream after the H2D into the slot
     EvHandle free_;                  // recorded on the compute stream after the last wave reading the slot
-    cudaStream_t waited = nullptr;   // compute stream that has already waited on `ready`
+    bool has_waited = false;         // some compute stream has waited on `ready` since the load ...
+    cudaStream_t waited = nullptr;   // ... namely this one (the legacy default stream is a valid value: 0)
 };
 
 struct ef_ctx {
@@ -70,6 +71,7 @@ struct ef_ctx {
     int32_t ev_next = 0;
     std::vector<EfPhys> phys;           // [S]
     cudaStream_t last_compute = nullptr;
+    bool has_last_compute = false;
     // host pool
     std::vector<void*> host_expert;     // [L*E] packed pinned buffers (owned unless aliased)
     std::vector<char> host_owned;
