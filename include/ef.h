@@ -174,6 +174,19 @@ int32_t ef_sync(ef_ctx* ctx);
 const char* ef_last_error(ef_ctx* ctx);
 /* Number of kernels this ctx has launched since creation (for bench.py's gpu_launches). */
 int64_t ef_launch_count(ef_ctx* ctx);
+/* Per-kernel device timing of the grouped FFN, for roofline reporting (bench.py).  When on, every
+ * grouped-GEMM launch is bracketed by CUDA events on the compute stream.  ef_get_kernel_times waits for
+ * the recorded events (synchronous), returns the totals since the last reset and optionally resets.
+ * rows = sum over launches of the routed rows they processed (algorithmic FLOPs: gemm1 4*d*f per row,
+ * gemm2 2*d*f per row; algorithmic weight bytes: groups * 3*d*f*2). */
+typedef struct {
+    double gemm1_ms, gemm2_ms;
+    int64_t gemm1_launches, gemm2_launches;
+    int64_t rows;     /* routed rows processed (each counted once per FFN, not per GEMM) */
+    int64_t groups;   /* expert groups processed */
+} ef_kernel_times;
+int32_t ef_set_kernel_timing(ef_ctx* ctx, int32_t on);
+int32_t ef_get_kernel_times(ef_ctx* ctx, ef_kernel_times* out, int32_t reset);
 /* 0 = tcgen05 kernels (default); 1 = plain-FMA debug kernels for the grouped FFN (bring-up aid, slow). */
 int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on);
 

@@ -17,7 +17,8 @@ DECLARED_SYMBOLS = [
     "ef_create", "ef_destroy", "ef_host_expert_register", "ef_host_expert_alias", "ef_route_topk", "ef_permute",
     "ef_expert_ffn_grouped", "ef_expert_ffn_grouped_resident", "ef_shared_ffn", "ef_combine", "ef_rmsnorm",
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
-    "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn",
+    "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
+    "ef_get_kernel_times",
 ]
 
 
@@ -38,6 +39,14 @@ class CacheStats(ctypes.Structure):
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+class KernelTimes(ctypes.Structure):
+    _fields_ = [("gemm1_ms", ctypes.c_double), ("gemm2_ms", ctypes.c_double), ("gemm1_launches", ctypes.c_int64),
+                ("gemm2_launches", ctypes.c_int64), ("rows", ctypes.c_int64), ("groups", ctypes.c_int64)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
 
 
 def library_path() -> str:
@@ -75,6 +84,8 @@ def load_library() -> ctypes.CDLL:
             "ef_copy_busy_ms": [vp, ctypes.POINTER(ctypes.c_float)],
             "ef_sync": [vp],
             "ef_set_debug_simt_ffn": [vp, i32],
+            "ef_set_kernel_timing": [vp, i32],
+            "ef_get_kernel_times": [vp, ctypes.POINTER(KernelTimes), i32],
         }
         for name, args in sig.items():
             fn = getattr(lib, name)
@@ -232,3 +243,11 @@ class EfContext:
 
     def ef_set_debug_simt_ffn(self, on: bool):
         self._chk(self.lib.ef_set_debug_simt_ffn(self.h, 1 if on else 0))
+
+    def ef_set_kernel_timing(self, on: bool):
+        self._chk(self.lib.ef_set_kernel_timing(self.h, 1 if on else 0))
+
+    def ef_get_kernel_times(self, reset: bool = True) -> dict:
+        kt = KernelTimes()
+        self._chk(self.lib.ef_get_kernel_times(self.h, ctypes.byref(kt), 1 if reset else 0))
+        return kt.as_dict()

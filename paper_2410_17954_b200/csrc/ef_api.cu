@@ -120,6 +120,7 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
     cudaSetDevice(ctx->cfg.device);
     cudaDeviceSynchronize();
     for (auto& sp : ctx->copy_spans) { cudaEventDestroy(sp.first); cudaEventDestroy(sp.second); }
+    for (auto& k : ctx->kspans) { cudaEventDestroy(k.e0); cudaEventDestroy(k.e1); cudaEventDestroy(k.e2); }
     for (auto ev : ctx->ev_ring) if (ev) cudaEventDestroy(ev);
     if (ctx->counts_event) cudaEventDestroy(ctx->counts_event);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
@@ -613,5 +614,31 @@ extern "C" int64_t ef_launch_count(ef_ctx* ctx) { return ctx ? ctx->launches : 0
 extern "C" int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on) {
     EF_CHECK_CTX(ctx);
     ctx->debug_simt = on ? 1 : 0;
+    return EF_OK;
+}
+
+static void drain_kernel_spans(ef_ctx* ctx) {
+    for (auto& k : ctx->kspans) {
+        cudaEventSynchronize(k.e2);
+        float a = 0.f, b = 0.f;
+        if (cudaEventElapsedTime(&a, k.e0, k.e1) == cudaSuccess) ctx->ktimes.gemm1_ms += a;
+        if (cudaEventElapsedTime(&b, k.e1, k.e2) == cudaSuccess) ctx->ktimes.gemm2_ms += b;
+        cudaEventDestroy(k.e0); cudaEventDestroy(k.e1); cudaEventDestroy(k.e2);
+    }
+    ctx->kspans.clear();
+}
+
+extern "C" int32_t ef_set_kernel_timing(ef_ctx* ctx, int32_t on) {
+    EF_CHECK_CTX(ctx);
+    ctx->time_kernels = on ? 1 : 0;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_get_kernel_times(ef_ctx* ctx, ef_kernel_times* out, int32_t reset) {
+    EF_CHECK_CTX(ctx);
+    if (!out) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_get_kernel_times: null");
+    drain_kernel_spans(ctx);
+    *out = ctx->ktimes;
+    if (reset) ctx->ktimes = ef_kernel_times();
     return EF_OK;
 }

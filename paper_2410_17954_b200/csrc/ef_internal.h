@@ -88,6 +88,11 @@ struct ef_ctx {
     // copy timing
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> copy_spans;
     float copy_ms = 0.f;
+    // optional per-kernel timing (ef_set_kernel_timing)
+    int32_t time_kernels = 0;
+    struct KSpan { cudaEvent_t e0, e1, e2; };
+    std::vector<KSpan> kspans;
+    ef_kernel_times ktimes{};
     // misc
     int64_t launches = 0;
     int32_t debug_simt = 0;

@@ -393,6 +393,15 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         t1.g[i].c_row0 = h_row0[i];   // GEMM1: x rows -> h rows
         t2.g[i].a_row0 = h_row0[i];   // GEMM2: h rows -> y rows
     }
+    ef_ctx::KSpan span{};
+    int64_t rows_total = 0;
+    for (int i = 0; i < tab.n; ++i) rows_total += tab.g[i].rows;
+    if (ctx->time_kernels) {
+        EF_CUDA(ctx, cudaEventCreate(&span.e0));
+        EF_CUDA(ctx, cudaEventCreate(&span.e1));
+        EF_CUDA(ctx, cudaEventCreate(&span.e2));
+        EF_CUDA(ctx, cudaEventRecord(span.e0, st));
+    }
     {
         const int ntn = f / 128;      // 256 packed W13 rows -> 128 h columns
         const int total = mtiles * ntn;
@@ -402,6 +411,7 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
     }
+    if (ctx->time_kernels) EF_CUDA(ctx, cudaEventRecord(span.e1, st));
     {
         const int ntn = (d + BN - 1) / BN;
         const int total = mtiles * ntn;
@@ -410,6 +420,14 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
                                                                    max_halves, total, t2);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
+    }
+    if (ctx->time_kernels) {
+        EF_CUDA(ctx, cudaEventRecord(span.e2, st));
+        ctx->kspans.push_back(span);
+        ctx->ktimes.gemm1_launches++;
+        ctx->ktimes.gemm2_launches++;
+        ctx->ktimes.rows += rows_total;
+        ctx->ktimes.groups += tab.n;
     }
     return EF_OK;
 }
