@@ -1,12 +1,14 @@
 #!/usr/bin/env python
-"""bench.py -- MoE-layer tokens/s on the BASELINE.json headline workload (Mixtral-8x7B-shaped prefill,
-configs[1]) through libef's C ABI, with the grouped-GEMM roofline and the CPU-oracle baseline.
+"""bench.py -- MoE-layer tokens/s through libef's C ABI, with the grouped-FFN roofline, the H2D link fraction and
+the CPU-oracle baseline.  Default workload = BASELINE.json configs[1] (Mixtral-8x7B-shaped prefill, the headline).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload mixtral_prefill|mixtral_decode|many_expert_prefill|stack_decode|tiny]
 
-One "step" = one pass of the whole hot path over one batch: route -> permute -> cache lookup + real-time
-correction (on-demand H2D in waves) + grouped SwiGLU FFN -> PLEC prefetch -> combine.  With cache capacity
-4 of 8 experts and all 8 active, every step streams 4 experts (1.41 GB) from pinned host memory.
+One "step" = one pass of the whole hot path over one batch: per layer visit  [rmsnorm ->] route -> permute ->
+cache lookup + real-time correction (on-demand H2D in waves) + grouped SwiGLU FFN -> PLEC prefetch -> combine
+[+ residual].  Prefill workloads: 1 visit per step; mixtral_decode: 1 visit of 16 tokens; stack_decode: 32 visits
+of 64 tokens.  The cache state carries over from step to step; expert weights stream from the pinned host pool.
 N > 1 (torchrun): independent data-parallel replicas, one per GPU, no data-path collective (weak scaling).
 """
 from __future__ import annotations
@@ -144,28 +146,81 @@ def measured_peaks():
 
 
 # ---------------------------------------------------------------------------------------------------
+# workload plumbing shared by both arms (inputs only -- no method arithmetic)
+# ---------------------------------------------------------------------------------------------------
+def trace_steps_needed(cfg, steps_total: int) -> int:
+    return max(1, min(cfg.n_steps, steps_total))
+
+
+def workload_config(cfg, world, extra=None):
+    c = {"workload": cfg.name, "tokens_per_step_per_gpu": cfg.T, "visits_per_step": cfg.n_layers,
+         "d_model": cfg.d_model, "d_ff": cfg.d_ff, "n_layers": cfg.n_layers, "n_experts": cfg.n_experts,
+         "top_k": cfg.top_k, "cache_slots": cfg.n_slots, "n_shared": cfg.n_shared, "expert_bytes": cfg.expert_bytes,
+         "prefetch_horizon": cfg.horizon, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+         "l2_policy": "inputs larger than L2: every step reads >= 0.69 GB of expert weights from HBM slots that the "
+                      "copy stream rewrites, against a 126 MB L2; no explicit flush"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+# ---------------------------------------------------------------------------------------------------
 # the reference arm / cpu_baseline: the oracle as it stands, on host cores, bounded sample
 # ---------------------------------------------------------------------------------------------------
-def oracle_sample(cfg, n_tokens: int, experts=None):
-    """Time the oracle's whole layer on the first n_tokens tokens of the workload."""
+def oracle_sample(cfg, n_tokens: int, n_layers: int, cache=None):
+    """Time the oracle on a bounded sample of one step: the first n_tokens tokens through the first n_layers
+    layers (whole layer each: route, permute, FFN, combine[, rmsnorm + residual]).  Returns tokens/s scaled to a
+    whole step (time * L / n_layers), seconds spent, threads used, and a description."""
     import oracle
-    x = wl.activations(cfg)[:n_tokens]
-    wr = wl.router_weight(cfg)
-    bias = wl.static_router_bias(cfg)
-    cache = experts if experts is not None else {}
+    L = cfg.n_layers
+    n_layers = max(1, min(L, n_layers))
+    n_tokens = max(1, min(cfg.T, n_tokens))
+    cache = cache if cache is not None else {}
+    tr = wl.routing_trace(wl.scaled(cfg, T=cfg.T), 1) if cfg.bias_kind == "trace" else None
 
-    def get(e):
-        if e not in cache:
-            cache[e] = wl.expert_weights(cfg, 0, e)
-        return cache[e]
-    # weights are materialised before the clock starts (the GPU arm's are resident in pinned memory too)
-    for e in range(cfg.n_experts):
-        get(e)
-    shared = [wl.expert_weights(cfg, 0, -1 - s) for s in range(cfg.n_shared)]
+    def get(l, e):
+        if (l, e) not in cache:
+            cache[(l, e)] = wl.expert_weights(cfg, l, e, threads=os.cpu_count() or 8)
+        return cache[(l, e)]
+    x = wl.activations(cfg, 0)[:n_tokens]
+    biases, wrs, needed = [], [], []
+    for l in range(n_layers):
+        wrs.append(wl.router_weight(cfg, l))
+        b = wl.trace_bias(cfg, tr, l)[:n_tokens] if tr is not None else wl.static_router_bias(cfg, l)
+        biases.append(b)
+        if tr is not None:
+            needed.append(sorted(set(int(e) for e in tr.sets[l, :n_tokens].ravel())))
+        else:
+            needed.append(list(range(cfg.n_experts)))
+    # weights are materialised before the clock starts (the GPU arm's sit in pinned memory before its clock too)
+    for l in range(n_layers):
+        for e in needed[l]:
+            get(l, e)
+    shared = [[get(l, -1 - s) for s in range(cfg.n_shared)] for l in range(n_layers)]
     t0 = time.perf_counter()
-    oracle.layer_forward(x, wr, bias, get, cfg.top_k, cfg.renorm, shared=shared)
+    h = x
+    for l in range(n_layers):
+        if L > 1:
+            u = oracle.round_bf16(oracle.rmsnorm(h, 1e-5))
+            ref = oracle.layer_forward(u, wrs[l], biases[l], lambda e, l=l: get(l, e), cfg.top_k, cfg.renorm,
+                                       shared=shared[l], res=h)
+            h = oracle.round_bf16(ref.out)
+        else:
+            oracle.layer_forward(h, wrs[l], biases[l], lambda e, l=l: get(l, e), cfg.top_k, cfg.renorm,
+                                 shared=shared[l])
     dt = time.perf_counter() - t0
-    return n_tokens / dt, dt, oracle.num_threads()
+    step_s = dt * L / n_layers
+    what = (f"first {n_tokens} of {cfg.T} tokens through the first {n_layers} of {L} layer visit(s) of one step of "
+            f"{cfg.name}, whole layer in fp64 ({dt:.1f} s; scaled x{L / n_layers:g} to a step), weights pre-generated, "
+            "no host<->device traffic, no cache")
+    return n_tokens / step_s, dt, oracle.num_threads(), what
+
+
+def ref_sample_size(cfg, args):
+    """Bounded oracle sample: ~10-30 s of CPU work on a 16-core host."""
+    n_tok = args.ref_tokens if args.ref_tokens > 0 else {"mixtral_prefill": 256, "many_expert_prefill": 1024}.get(cfg.name, cfg.T)
+    n_lay = args.ref_layers if args.ref_layers > 0 else (2 if cfg.n_layers > 1 else 1)
+    return n_tok, n_lay
 
 
 def run_reference(args):
@@ -173,40 +228,147 @@ def run_reference(args):
     if rank != 0:
         return
     cfg = wl.CONFIGS[args.workload]
-    n = args.ref_tokens
-    experts = {}
+    n_tok, n_lay = ref_sample_size(cfg, args)
+    cache = {}
     vals = []
     for i in range(args.warmup + args.steps):
-        v, dt, cores = oracle_sample(cfg, n, experts)
+        v, dt, cores, what = oracle_sample(cfg, n_tok, n_lay, cache)
         if i >= args.warmup:
             vals.append((v, dt))
     value = float(np.mean([v for v, _ in vals]))
     ms = float(np.mean([dt for _, dt in vals])) * 1e3
-    sample = f"first {n} of {cfg.T} tokens of {cfg.name} per step, whole layer in fp64, weights pre-generated"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
-            "config": workload_config(cfg, world),
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, world),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def workload_config(cfg, world):
-    return {"workload": cfg.name, "tokens_per_step_per_gpu": cfg.T, "d_model": cfg.d_model, "d_ff": cfg.d_ff,
-            "n_experts": cfg.n_experts, "top_k": cfg.top_k, "cache_slots": cfg.n_slots, "n_shared": cfg.n_shared,
-            "expert_bytes": cfg.expert_bytes, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-            "l2_policy": "per-step weight traffic (>= 1.4 GB) exceeds the 126 MB L2; no explicit flush"}
-
-
 # ---------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------
+class Driver:
+    """Owns one MoELayerRunner plus the step inputs of a workload; step(i) = one pass of the whole hot path
+    (n_layers visits) over batch i.  Sequencing only: every step of the path runs in libef's kernels."""
+
+    def __init__(self, cfg, dev, x_stream: str, steps_total: int, phys_experts: int = 0, log=lambda *_: None):
+        import torch
+        from paper_2410_17954_b200 import MoELayerRunner
+        from paper_2410_17954_b200.layer import bf16_tensor_from_bits
+        self.torch, self.cfg, self.dev = torch, cfg, dev
+        L, E, T, d = cfg.n_layers, cfg.n_experts, cfg.T, cfg.d_model
+        self.runner = r = MoELayerRunner(L, E, cfg.top_k, d, cfg.d_ff, cfg.n_slots, cfg.n_shared, T, cfg.horizon,
+                                         cfg.renorm, device=dev.index)
+        threads = os.cpu_count() or 8
+        n_total = L * E
+        self.phys = phys_experts if 0 < phys_experts < n_total else 0
+        gen_cfg = wl.scaled(cfg, phys_experts=self.phys)
+        t0 = time.perf_counter()
+        for l in range(L):
+            r.set_router(l, wl.router_weight(cfg, l), wl.static_router_bias(cfg, l))
+            for e in range(E):
+                g = l * E + e
+                if self.phys and g >= self.phys:
+                    src = g % self.phys
+                    r.ctx.ef_host_expert_alias(l, e, src // E, src % E)
+                else:
+                    r.register_expert(l, e, *wl.expert_weights(gen_cfg, l, e, threads=threads))
+            for s in range(cfg.n_shared):
+                r.register_expert(l, -1 - s, *wl.expert_weights(cfg, l, -1 - s, threads=threads))
+            if L > 1 and (l % 4 == 3):
+                log(f"registered layers 0..{l} ({time.perf_counter() - t0:.0f} s)")
+        # step inputs
+        self.is_trace = cfg.bias_kind == "trace"
+        self.ts = trace_steps_needed(cfg, steps_total) if self.is_trace else 1
+        xs = [wl.normal_bf16(cfg.seed, f"x.step{s}.{x_stream}", (T, d), 1.0) for s in range(self.ts)]
+        self.x_pin = bf16_tensor_from_bits(np.stack(xs), pin=True)              # [ts, T, d]
+        self.x_dev = self.x_pin.to(dev)
+        self.x_stage = torch.empty((T, d), dtype=torch.bfloat16, device=dev)    # e2e: per-step H2D target
+        self.out = torch.empty((T, d), dtype=torch.bfloat16, device=dev)
+        self.hbuf = [torch.empty((T, d), dtype=torch.bfloat16, device=dev) for _ in range(2)]
+        self.out_pin = torch.empty((T, d), dtype=torch.bfloat16).pin_memory()
+        self.nv = self.ts * L
+        if self.is_trace:
+            self.trace = wl.routing_trace(cfg, self.ts)
+            b = np.stack([wl.trace_bias(cfg, self.trace, v) for v in range(self.nv)])   # [nv, T, E] fp32
+            self.bias_pin = torch.from_numpy(b).pin_memory()
+            self.bias_dev = self.bias_pin.to(dev)
+            self.bias_stage = torch.empty((L, T, E), dtype=torch.float32, device=dev)
+            self.look = L if cfg.horizon <= 0 else cfg.horizon
+            self.pred = self.trace.predicted
+        else:
+            self.look = 1
+            self.pred = np.ones((1, E), np.uint8)      # replaced by the gate's own active set after warm-up
+        self.visit = 0
+        r.ctx.ef_cache_prefetch(-1, self.window(-1))
+
+    def window(self, v):
+        """Predicted batch-level path rows for visits v+1 .. v+look (the supplied predictor output)."""
+        if not self.is_trace:
+            return self.pred
+        idx = [(v + 1 + j) % self.nv for j in range(self.look)]
+        return np.ascontiguousarray(self.pred[idx])
+
+    def adopt_gate_prediction(self):
+        """Prefill workloads re-run the same batch every step: the predicted path of the next step is the active
+        set the gate produced on this one (read back once, after warm-up)."""
+        if not self.is_trace:
+            self.torch.cuda.synchronize()
+            self.pred = (self.runner.counts.cpu().numpy() > 0).astype(np.uint8)[None, :]
+
+    def step(self, e2e: bool):
+        torch, cfg, r = self.torch, self.cfg, self.runner
+        L = cfg.n_layers
+        s = (self.visit // L) % self.ts
+        if e2e:
+            self.x_stage.copy_(self.x_pin[s], non_blocking=True)
+            x = self.x_stage
+            if self.is_trace:
+                self.bias_stage.copy_(self.bias_pin[s * L:(s + 1) * L], non_blocking=True)
+        else:
+            x = self.x_dev[s]
+        h = x
+        for l in range(L):
+            v = self.visit
+            tb = None
+            if self.is_trace:
+                tb = self.bias_stage[l] if e2e else self.bias_dev[v % self.nv]
+            dst = self.out if l == L - 1 else self.hbuf[l & 1]
+            r.visit(v, h, dst, token_bias=tb, predicted_next=self.window(v), residual=h if L > 1 else None,
+                    pre_norm_eps=1e-5 if L > 1 else None)
+            h = dst
+            self.visit += 1
+        if e2e:
+            self.out_pin.copy_(self.out, non_blocking=True)
+            torch.cuda.current_stream().synchronize()      # the caller reads the result
+
+    def io_bytes(self):
+        cfg = self.cfg
+        h2d = cfg.T * cfg.d_model * 2 + (cfg.n_layers * cfg.T * cfg.n_experts * 4 if self.is_trace else 0)
+        return h2d, cfg.T * cfg.d_model * 2
+
+    def close(self):
+        self.runner.close()
+
+
+def measure_pinned_h2d(dev, nbytes: int, reps: int = 5) -> float:
+    """Pinned host -> device copy bandwidth of this box (GB/s), one expert-sized buffer, best of reps."""
+    import torch
+    src = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    dst = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    best = 0.0
+    for _ in range(reps + 1):
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(); dst.copy_(src, non_blocking=True); e1.record(); e1.synchronize()
+        best = max(best, nbytes / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    del src, dst
+    return best
+
+
 def run_ours(args):
     import torch
-    from paper_2410_17954_b200 import MoELayerRunner
-    from paper_2410_17954_b200.layer import bf16_tensor_from_bits
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
@@ -216,50 +378,40 @@ def run_ours(args):
     cfg = wl.CONFIGS[args.workload]
     plan = replica_plan(rank, world, cfg.T)
     peaks = measured_peaks()
+    log = (lambda m: print(f"[bench] {m}", file=sys.stderr, flush=True)) if rank == 0 else (lambda m: None)
 
-    runner = MoELayerRunner(cfg.n_layers, cfg.n_experts, cfg.top_k, cfg.d_model, cfg.d_ff, cfg.n_slots, cfg.n_shared,
-                            cfg.T, cfg.horizon, cfg.renorm, device=local)
-    runner.set_router(0, wl.router_weight(cfg), wl.static_router_bias(cfg))
-    for e in range(cfg.n_experts):
-        runner.register_expert(0, e, *wl.expert_weights(cfg, 0, e, threads=os.cpu_count() or 8))
-    for s in range(cfg.n_shared):
-        runner.register_expert(0, -1 - s, *wl.expert_weights(cfg, 0, -1 - s))
-    x_bits = wl.normal_bf16(cfg.seed, f"x.step0.{plan['x_stream']}", (cfg.T, cfg.d_model), 1.0)
-    x_pin = bf16_tensor_from_bits(x_bits, pin=True)
-    x_dev = x_pin.to(dev)
-    out = torch.empty((cfg.T, cfg.d_model), dtype=torch.bfloat16, device=dev)
-    out_pin = torch.empty((cfg.T, cfg.d_model), dtype=torch.bfloat16).pin_memory()
-    # the supplied predicted path: every expert active (true for this workload: T*k >> E); cold cache + warm-up
-    predicted = np.ones((1, cfg.n_experts), np.uint8)
-    runner.ctx.ef_cache_prefetch(-1, predicted)
+    # host memory check for the pinned pool (cfg 5: 90 GB); alias onto fewer physical buffers if it cannot fit
+    phys = args.phys_experts
+    need = cfg.n_layers * cfg.n_experts * cfg.expert_bytes
+    if phys == 0:
+        try:
+            avail = int(next(l for l in open("/proc/meminfo") if l.startswith("MemAvailable")).split()[1]) * 1024
+        except Exception:
+            avail = need * 4
+        if need * world > 0.6 * avail:
+            phys = max(cfg.n_experts, int(0.5 * avail / world / cfg.expert_bytes))
+            log(f"pinned pool of {need / 1e9:.1f} GB does not fit comfortably in {avail / 1e9:.1f} GB of host memory: "
+                f"aliasing {cfg.n_layers * cfg.n_experts} logical experts onto {phys} physical buffers")
+    steps_total = 2 * (args.steps + args.warmup) + 2
+    drv = Driver(cfg, dev, plan["x_stream"], steps_total, phys, log)
+    runner = drv.runner
+    h2d_peak = measure_pinned_h2d(dev, cfg.expert_bytes) if rank == 0 else None
 
-    visit = [0]
-
-    def step_device():
-        runner.visit(visit[0], x_dev, out, predicted_next=predicted)
-        visit[0] += 1
-
-    def step_e2e():
-        x_dev.copy_(x_pin, non_blocking=True)
-        runner.visit(visit[0], x_dev, out, predicted_next=predicted)
-        out_pin.copy_(out, non_blocking=True)
-        torch.cuda.current_stream().synchronize()      # the caller reads the result
-        visit[0] += 1
-
-    def timed(fn, steps, warmup, with_kernel_times=False):
+    def timed(e2e, steps, warmup, with_kernel_times=False):
         for _ in range(warmup):
-            fn()
+            drv.step(e2e)
+        drv.adopt_gate_prediction()
         runner.ctx.ef_sync()
+        runner.ctx.ef_cache_reset_stats()               # also clears the copy-busy accumulator
         if with_kernel_times:
             runner.ctx.ef_get_kernel_times(reset=True)
             runner.ctx.ef_set_kernel_timing(True)
         l0 = runner.ctx.ef_launch_count()
-        st0 = runner.ctx.ef_cache_get_stats()
         dist_barrier(); torch.cuda.synchronize()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
         e0.record()
         for _ in range(steps):
-            fn()
+            drv.step(e2e)
         e1.record()
         runner.ctx.ef_sync()
         torch.cuda.synchronize(); dist_barrier()
@@ -268,75 +420,104 @@ def run_ours(args):
         if with_kernel_times:
             kt = runner.ctx.ef_get_kernel_times(reset=True)
             runner.ctx.ef_set_kernel_timing(False)
-        st1 = runner.ctx.ef_cache_get_stats()
-        return ms, runner.ctx.ef_launch_count() - l0, kt, {k: st1[k] - st0[k] for k in st1}
+        st = runner.ctx.ef_cache_get_stats()
+        copy_ms = runner.ctx.ef_copy_busy_ms()
+        return ms, runner.ctx.ef_launch_count() - l0, kt, st, copy_ms
 
     sampler = ClockSampler(local)
     sampler.start()
-    ms, launches, kt, dstats = timed(step_device, args.steps, args.warmup, with_kernel_times=True)
+    ms, launches, kt, st, copy_ms = timed(False, args.steps, args.warmup, with_kernel_times=True)
     clocks = sampler.stop()
     ms_max = dist_max(ms, dev)
     value = plan["global_tokens"] * args.steps / (ms_max * 1e-3)
 
-    ms_e2e, _, _, _ = timed(step_e2e, args.steps, max(1, args.warmup // 2))
+    ms_e2e, _, _, _, _ = timed(True, args.steps, max(1, args.warmup // 2))
     ms_e2e_max = dist_max(ms_e2e, dev)
     e2e_value = plan["global_tokens"] * args.steps / (ms_e2e_max * 1e-3)
-    io_bytes = cfg.T * cfg.d_model * 2
+    io_h2d, io_d2h = drv.io_bytes()
 
-    # roofline of the dominant kernel (GEMM1: gate/up projection + SwiGLU), launches of the timed region
     d, f = cfg.d_model, cfg.d_ff
-    flops1 = 4.0 * d * f * kt["rows"]
-    flops2 = 2.0 * d * f * kt["rows"]
-    ach1 = flops1 / (kt["gemm1_ms"] * 1e-3) / 1e12 if kt["gemm1_ms"] > 0 else 0.0
-    ach2 = flops2 / (kt["gemm2_ms"] * 1e-3) / 1e12 if kt["gemm2_ms"] > 0 else 0.0
-    peak = peaks["bf16_tflops_sustained"] or peaks["bf16_tflops"]
-    roofline = {"bound": "tensor", "kernel": "ffn_gemm_kernel<swiglu> (GEMM1, streaming step: 1 wave of hits + 1 wave per miss)",
-                "achieved": ach1, "peak": peak, "unit": "TFLOP/s", "frac": ach1 / peak,
-                "peak_source": f"{peaks['source']} bf16 sustained (kernel timed inside a long step)",
-                "traffic": None, "launches": kt["gemm1_launches"], "avg_launch_ms": kt["gemm1_ms"] / max(1, kt["gemm1_launches"]),
-                "gemm2": {"achieved": ach2, "frac": ach2 / peak, "avg_launch_ms": kt["gemm2_ms"] / max(1, kt["gemm2_launches"])}}
+    decode = cfg.T * cfg.top_k / cfg.n_experts < 249 and cfg.name in ("mixtral_decode", "stack_decode")
+    roofline = ffn_roofline(kt, d, f, peaks, decode, "streaming step (one wave of hits + one wave per miss)")
 
-    # kernel-only leg: all experts resident (second context with E slots), the grouped GEMM alone
+    h2d = {"bytes_per_step": st["bytes_h2d"] / args.steps, "loads_per_step": (st["ondemand_loads"] + st["prefetch_issued"]) / args.steps,
+           "copy_busy_ms_per_step": copy_ms / args.steps,
+           "achieved_gbs": (st["bytes_h2d"] / (copy_ms * 1e-3) / 1e9) if copy_ms > 0 else None,
+           "peak_gbs": h2d_peak, "peak_source": "measured in this run: pinned->device copy of one expert, best of 5",
+           "frac": (st["bytes_h2d"] / (copy_ms * 1e-3) / 1e9 / h2d_peak) if copy_ms > 0 and h2d_peak else None,
+           "gbs_over_step": st["bytes_h2d"] / (ms * 1e-3) / 1e9,
+           "step_ms_lower_bound_from_link": (st["bytes_h2d"] / args.steps / (h2d_peak * 1e9) * 1e3) if h2d_peak else None,
+           "copy_overlap": "copies run on the library's copy stream concurrently with the grouped-FFN waves"}
+    cache = dict(st)
+    cache["hit_ratio"] = st["hits"] / max(1, st["lookups"])
+
     resident = None
     if rank == 0 and not args.no_resident:
-        resident = resident_leg(cfg, runner, peaks, dev, args)
-
-    h2d = {"bytes_per_step": dstats["bytes_h2d"] / args.steps,
-           "gbs_over_step": dstats["bytes_h2d"] / (ms * 1e-3) / 1e9}
+        counts = runner.counts.cpu().numpy()
+        drv.close()
+        resident = resident_leg(cfg, counts, peaks, dev, args, decode)
+    else:
+        drv.close()
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        n = args.ref_tokens
-        v, dt, cores = oracle_sample(cfg, n)
-        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": f"first {n} of {cfg.T} tokens, whole layer in fp64, {dt:.1f} s, weights pre-generated, "
-                                  "no host<->device traffic"}
+        n_tok, n_lay = ref_sample_size(cfg, args)
+        v, dt, cores, what = oracle_sample(cfg, n_tok, n_lay)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                "config": workload_config(cfg, world), "clocks": clocks,
-                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes + int(h2d["bytes_per_step"]),
-                        "d2h_bytes_per_step": io_bytes, "ms_per_step": ms_e2e_max / args.steps,
-                        "note": "x from pinned host and out back to pinned host every step; expert weights stream "
-                                "from the pinned host pool in both legs"},
+                "config": workload_config(cfg, world, {"phys_host_experts": drv.phys or cfg.n_layers * cfg.n_experts}),
+                "clocks": clocks,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_h2d + int(h2d["bytes_per_step"]),
+                        "d2h_bytes_per_step": io_d2h, "ms_per_step": ms_e2e_max / args.steps,
+                        "note": "step inputs (x, per-token router bias) from pinned host memory and out back to pinned "
+                                "host memory every step; expert weights stream from the pinned host pool in both legs"},
                 "gpu_launches": launches, "roofline": roofline, "roofline_resident": resident,
-                "h2d": h2d, "cache": dstats, "cpu_baseline": cpu_baseline}
+                "h2d": h2d, "cache": cache, "cpu_baseline": cpu_baseline}
         print(json.dumps(line), flush=True)
-    runner.close()
 
 
-def resident_leg(cfg, runner, peaks, dev, args):
-    """Grouped FFN alone with every needed expert resident: the prefill tensor-core roofline."""
+def ffn_roofline(kt, d, f, peaks, decode, where):
+    """Roofline of the dominant kernel (GEMM1 of the grouped FFN) from the library's per-launch CUDA events."""
+    t1, t2 = kt["gemm1_ms"] * 1e-3, kt["gemm2_ms"] * 1e-3
+    n1, n2 = max(1, kt["gemm1_launches"]), max(1, kt["gemm2_launches"])
+    if decode:
+        b1, b2 = 4.0 * d * f * kt["groups"], 2.0 * d * f * kt["groups"]      # weight bytes read once per active expert
+        peak = peaks["hbm_gbs"]
+        a1 = b1 / t1 / 1e9 if t1 > 0 else 0.0
+        a2 = b2 / t2 / 1e9 if t2 > 0 else 0.0
+        return {"bound": "hbm", "kernel": f"ffn_gemm_kernel<swiglu> (GEMM1), {where}", "achieved": a1, "peak": peak,
+                "unit": "GB/s", "frac": a1 / peak, "peak_source": f"{peaks['source']} HBM copy bandwidth", "traffic": None,
+                "launches": kt["gemm1_launches"], "avg_launch_ms": t1 * 1e3 / n1, "groups_per_launch": kt["groups"] / n1,
+                "gemm2": {"achieved": a2, "frac": a2 / peak, "avg_launch_ms": t2 * 1e3 / n2},
+                "ffn": {"achieved": (b1 + b2) / (t1 + t2) / 1e9 if t1 + t2 > 0 else 0.0,
+                        "frac": (b1 + b2) / (t1 + t2) / 1e9 / peak if t1 + t2 > 0 else 0.0}}
+    fl1, fl2 = 4.0 * d * f * kt["rows"], 2.0 * d * f * kt["rows"]
+    peak = peaks["bf16_tflops_sustained"] or peaks["bf16_tflops"]
+    a1 = fl1 / t1 / 1e12 if t1 > 0 else 0.0
+    a2 = fl2 / t2 / 1e12 if t2 > 0 else 0.0
+    return {"bound": "tensor", "kernel": f"ffn_gemm_kernel<swiglu> (GEMM1), {where}", "achieved": a1, "peak": peak,
+            "unit": "TFLOP/s", "frac": a1 / peak,
+            "peak_source": f"{peaks['source']} bf16 sustained (kernel timed inside a long step)", "traffic": None,
+            "launches": kt["gemm1_launches"], "avg_launch_ms": t1 * 1e3 / n1, "rows_per_launch": kt["rows"] / n1,
+            "gemm2": {"achieved": a2, "frac": a2 / peak, "avg_launch_ms": t2 * 1e3 / n2},
+            "ffn": {"achieved": (fl1 + fl2) / (t1 + t2) / 1e12 if t1 + t2 > 0 else 0.0,
+                    "frac": (fl1 + fl2) / (t1 + t2) / 1e12 / peak if t1 + t2 > 0 else 0.0}}
+
+
+def resident_leg(cfg, counts, peaks, dev, args, decode):
+    """The grouped FFN alone with every active expert of one visit resident (kernel-only roofline): one launch
+    pair over all groups, timed by the library's CUDA events on the compute stream, weights > L2."""
     import torch
     from paper_2410_17954_b200 import EfContext
-    counts = runner.counts.cpu().numpy()
-    runner.close()                                   # free the streaming arena before allocating E slots
     E = cfg.n_experts
     ctx = EfContext(1, E, cfg.top_k, cfg.d_model, cfg.d_ff, E, 0, cfg.T, 0, dev.index)
+    threads = os.cpu_count() or 8
     for e in range(E):
-        ctx.ef_host_expert_register(0, e, *wl.expert_weights(cfg, 0, e, threads=os.cpu_count() or 8))
+        ctx.ef_host_expert_register(0, e, *wl.expert_weights(cfg, 0, e, threads=threads))
     ctx.ef_cache_prefetch(-1, np.ones((1, E), np.uint8))
     slot_of = {g: s for s, g in enumerate(ctx.ef_cache_snapshot())}
     offs = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
@@ -345,6 +526,10 @@ def resident_leg(cfg, runner, peaks, dev, args):
     y = torch.empty((R, cfg.d_model), dtype=torch.bfloat16, device=dev)
     act = [e for e in range(E) if counts[e] > 0]
     rb, rw, sl = [int(offs[e]) for e in act], [int(counts[e]) for e in act], [slot_of[e] for e in act]
+    # when the active experts' weights fit in L2 (cfg 4: 64 x 17 MB > 126 MB still; tiny: no) flush between launches
+    flush = None
+    if len(act) * cfg.expert_bytes < 512e6:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     ctx.ef_sync()
     for _ in range(3):
         ctx.ef_expert_ffn_grouped_resident(x_perm, rb, rw, sl, y)
@@ -353,17 +538,16 @@ def resident_leg(cfg, runner, peaks, dev, args):
     ctx.ef_get_kernel_times(reset=True)
     n = max(5, args.steps)
     for _ in range(n):
+        if flush is not None:
+            flush.zero_()
         ctx.ef_expert_ffn_grouped_resident(x_perm, rb, rw, sl, y)
     kt = ctx.ef_get_kernel_times(reset=True)
-    d, f = cfg.d_model, cfg.d_ff
-    t1, t2 = kt["gemm1_ms"] / n, kt["gemm2_ms"] / n
-    fl1, fl2 = 4.0 * d * f * R, 2.0 * d * f * R
-    peak = peaks["bf16_tflops"]
-    res = {"rows": R, "rows_per_expert": [int(c) for c in counts], "gemm1_ms": t1, "gemm2_ms": t2,
-           "gemm1_tflops": fl1 / t1 / 1e9, "gemm2_tflops": fl2 / t2 / 1e9,
-           "ffn_tflops": (fl1 + fl2) / (t1 + t2) / 1e9, "peak": peak, "unit": "TFLOP/s",
-           "frac": (fl1 + fl2) / (t1 + t2) / 1e9 / peak, "peak_source": f"{peaks['source']} bf16 burst",
-           "note": "true ragged rows, padding not counted; weights (2.8 GB) exceed L2 between launches"}
+    res = ffn_roofline(kt, cfg.d_model, cfg.d_ff, dict(peaks, bf16_tflops_sustained=None), decode,
+                       "all active experts of one visit resident, one launch over all groups")
+    if not decode:
+        res["peak_source"] = f"{peaks['source']} bf16 burst (kernel timed alone)"
+    res["rows_per_expert"] = [int(c) for c in counts]
+    res["l2"] = "256 MB flush write between launches" if flush is not None else "weights exceed L2 between launches"
     ctx.close()
     return res
 
@@ -375,7 +559,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="mixtral_prefill", choices=sorted(wl.CONFIGS))
-    ap.add_argument("--ref-tokens", type=int, default=256, help="tokens in the bounded oracle sample")
+    ap.add_argument("--ref-tokens", type=int, default=0, help="tokens in the bounded oracle sample (0 = per-workload default)")
+    ap.add_argument("--ref-layers", type=int, default=0, help="layer visits in the bounded oracle sample (0 = default)")
+    ap.add_argument("--phys-experts", type=int, default=0,
+                    help="alias the logical experts onto this many physical pinned host buffers (0 = one per expert "
+                         "if host memory allows)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-resident", action="store_true")
     args = ap.parse_args()
