@@ -127,6 +127,7 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
     for (size_t i = 0; i < ctx->host_expert.size(); ++i)
         if (ctx->host_expert[i] && ctx->host_owned[i]) cudaFreeHost(ctx->host_expert[i]);
     if (ctx->counts_pinned) cudaFreeHost(ctx->counts_pinned);
+    if (ctx->sched_words) cudaFree(ctx->sched_words);
     if (ctx->h_ws) cudaFree(ctx->h_ws);
     if (ctx->arena) cudaFree(ctx->arena);
     delete ctx;

@@ -12,6 +12,7 @@
 #include "ef.h"
 
 #define EF_MAX_GROUPS 64   // groups per grouped-GEMM launch (table travels in kernel params)
+#define EF_SCHED_RING 1024 // per-launch tile-scheduler word pairs (self-resetting; ring keeps in-flight launches apart)
 #define EF_W13_BLOCK 128   // gate/up interleave granularity in the packed expert layout
 
 // ---- packed expert layout (library-defined; the caller never sees it) ----------------------------
@@ -85,6 +86,8 @@ struct ef_ctx {
     // tensor maps over the arena (3-D: k, row, slot)
     CUtensorMap tm_w13{}, tm_wd{};
     bool tm_ok = false;
+    int32_t* sched_words = nullptr;     // device, [EF_SCHED_RING][2]
+    int32_t sched_next = 0;
     // copy timing
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> copy_spans;
     float copy_ms = 0.f;

@@ -11,11 +11,18 @@
 // 256-row tile needs 1/3 less L2->SM traffic per flop than a 128-row one; L2 bandwidth, not the
 // tensor pipe, is what bounds a plain 128x256 tiling.
 //
-// Warp roles (256 threads, 1 CTA/SM, persistent over a static tile sequence):
-//   warp 0    TMA producer      : A boxes (64 x 128 rows, one per half) + B box (64 x 256 rows) per stage
-//   warp 1    MMA issuer        : one lane issues tcgen05.mma (M128 N256 K16), commits to mbarriers
-//   warp 2    TMEM allocator    : 512 columns = two 128x256 fp32 accumulator buffers
-//   warps 4-7 epilogue          : tcgen05.ld -> registers -> SwiGLU / cast -> 64-byte global stores
+// Warp roles (384 threads, 1 CTA/SM, persistent):
+//   warp 0     TMA producer + tile scheduler : claims the next tile with one atomicAdd on a per-launch counter,
+//                                broadcasts it to the other roles through a 4-deep smem ring guarded by mbarriers,
+//                                then issues A boxes (64 x 128 rows, one per half) + B box (64 x 256 rows) per stage
+//   warp 1     MMA issuer        : one lane issues tcgen05.mma (M128 N256 K16), commits to mbarriers
+//   warp 2     TMEM allocator    : 512 columns = two 128x256 fp32 accumulator buffers
+//   warps 4-11 epilogue          : tcgen05.ld -> registers -> SwiGLU / cast -> 64-byte global stores; warps w and w+4
+//                                share a TMEM lane quarter and split the columns
+// Per-expert tile scheduling over ragged token counts: tiles are numbered longest-first -- every 256-row tile of
+// every group (n-major inside a group, so the M-tiles that share a weight tile are claimed back to back and hit L2),
+// then the short (<= 128-row) tail tiles -- and claimed dynamically, i.e. greedy longest-processing-time list
+// scheduling: the makespan is within one short tile of the mean load whatever the row counts are.
 // Ragged M: a group's last tile may be short; TMA zero-fills rows past the tensor, rows past the
 // group are computed and discarded (stores are row-predicated), so neighbours are never touched.
 #include <cuda_bf16.h>
@@ -31,7 +38,9 @@ constexpr int kStages = 3;
 constexpr int A_HALF_BYTES = HALF_M * BK * 2;   // 16 KB
 constexpr int B_BYTES = BN * BK * 2;            // 32 KB
 constexpr int STAGE_BYTES = 2 * A_HALF_BYTES + B_BYTES;   // 64 KB
-constexpr int kThreads = 256;
+constexpr int kThreads = 384;
+constexpr int kEpiWarps = 8;
+constexpr int kSched = 4;               // depth of the tile-broadcast ring
 constexpr int kTmemCols = 512;
 
 struct __align__(8) SmemCtl {
@@ -39,8 +48,13 @@ struct __align__(8) SmemCtl {
     uint64_t empty[kStages];
     uint64_t tmem_full[2];
     uint64_t tmem_empty[2];
+    uint64_t sched_full[kSched];
+    uint64_t sched_empty[kSched];
+    int32_t sched_tile[kSched];
     uint32_t tmem_base;
-    int32_t gstart[EF_MAX_GROUPS + 1];
+    int32_t total_long;                   // number of 2-half tiles (they come first)
+    int32_t gstart_long[EF_MAX_GROUPS + 1];
+    int32_t gstart_short[EF_MAX_GROUPS + 1];
 };
 
 constexpr size_t kSmemBytes = 1024 /*align slack*/ + (size_t)kStages * STAGE_BYTES + sizeof(SmemCtl);
@@ -121,26 +135,31 @@ struct Tile {
     int a_row, c_row, rows_valid, halves, n_tile, slot;
 };
 
-__device__ __forceinline__ int group_mtiles(int rows, int tile_rows) { return (rows + tile_rows - 1) / tile_rows; }
+// number of 2-half ("long", 129..256 rows) tiles of a group; the remainder, if any, is one short tile per n
+__device__ __host__ __forceinline__ int group_long_tiles(int rows) { return rows / (2 * 128) + ((rows % (2 * 128)) > 128 ? 1 : 0); }
+__device__ __host__ __forceinline__ int group_has_short(int rows) { int r = rows % (2 * 128); return (r > 0 && r <= 128) ? 1 : 0; }
 
-__device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const int32_t* gstart, int tile, int n_tiles_n,
-                                            int max_halves) {
-    int g = 0;
-    while (tile >= gstart[g + 1]) ++g;
-    const int tile_rows = HALF_M * max_halves;
-    const int local = tile - gstart[g];
-    const int mt = group_mtiles(tab.g[g].rows, tile_rows);
-    const int n = local / mt, m = local % mt;
-    const int row_off = m * tile_rows;
-    const int rem = tab.g[g].rows - row_off;
+__device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemCtl* ctl, int tile) {
     Tile t;
-    t.halves = (max_halves == 2 && rem > HALF_M) ? 2 : 1;
-    t.rows_valid = min(rem, HALF_M * t.halves);
+    int g = 0, row_off;
+    if (tile < ctl->total_long) {
+        while (tile >= ctl->gstart_long[g + 1]) ++g;
+        const int local = tile - ctl->gstart_long[g];
+        const int nl = group_long_tiles(tab.g[g].rows);
+        t.n_tile = local / nl;
+        row_off = (local % nl) * (2 * HALF_M);
+        t.halves = 2;
+    } else {
+        const int ts = tile - ctl->total_long;
+        while (ts >= ctl->gstart_short[g + 1]) ++g;
+        t.n_tile = ts - ctl->gstart_short[g];
+        row_off = group_long_tiles(tab.g[g].rows) * (2 * HALF_M);
+        t.halves = 1;
+    }
+    t.rows_valid = min(tab.g[g].rows - row_off, HALF_M * t.halves);
     t.a_row = tab.g[g].a_row0 + row_off;
     t.c_row = tab.g[g].c_row0 + row_off;
-    t.n_tile = n;
     t.slot = tab.g[g].slot;
-    (void)n_tiles_n;
     return t;
 }
 
@@ -148,8 +167,8 @@ __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const int32
 template <bool kSwiglu>
 __global__ void __launch_bounds__(kThreads, 1)
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int max_halves, int total_tiles,
-                const __grid_constant__ EfGroupTable tab) {
+                uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int total_tiles,
+                int32_t* __restrict__ sched, const __grid_constant__ EfGroupTable tab) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     SmemCtl* ctl = (SmemCtl*)(smem + (size_t)kStages * STAGE_BYTES);
@@ -161,7 +180,8 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     }
     if (warp == 1 && lane == 0) {
         for (int i = 0; i < kStages; ++i) { mbar_init(&ctl->full[i], 1); mbar_init(&ctl->empty[i], 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(&ctl->tmem_full[i], 1); mbar_init(&ctl->tmem_empty[i], 4); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&ctl->tmem_full[i], 1); mbar_init(&ctl->tmem_empty[i], kEpiWarps); }
+        for (int i = 0; i < kSched; ++i) { mbar_init(&ctl->sched_full[i], 1); mbar_init(&ctl->sched_empty[i], 1 + kEpiWarps); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
@@ -169,13 +189,16 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     if (warp == 3 && lane == 0) {
-        const int tile_rows = HALF_M * max_halves;
-        int acc = 0;
+        int nl = 0, ns = 0;
         for (int g = 0; g < tab.n; ++g) {
-            ctl->gstart[g] = acc;
-            acc += group_mtiles(tab.g[g].rows, tile_rows) * n_tiles_n;
+            ctl->gstart_long[g] = nl;
+            ctl->gstart_short[g] = ns;
+            nl += group_long_tiles(tab.g[g].rows) * n_tiles_n;
+            ns += group_has_short(tab.g[g].rows) * n_tiles_n;
         }
-        ctl->gstart[tab.n] = acc;
+        ctl->gstart_long[tab.n] = nl;
+        ctl->gstart_short[tab.n] = ns;
+        ctl->total_long = nl;
     }
     tc_fence_before();
     __syncthreads();
@@ -184,11 +207,17 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const int KB = K / BK;
 
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== tile scheduler + TMA producer =====
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
-            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-                const Tile t = decode_tile(tab, ctl->gstart, tile, n_tiles_n, max_halves);
+            for (int it = 0;; ++it) {
+                const int ss = it % kSched;
+                mbar_wait(&ctl->sched_empty[ss], ((it / kSched) & 1) ^ 1);
+                const int tile = atomicAdd(sched, 1);
+                ctl->sched_tile[ss] = tile;
+                mbar_arrive(&ctl->sched_full[ss]);          // release: the tile index is visible to the waiters
+                if (tile >= total_tiles) break;
+                const Tile t = decode_tile(tab, ctl, tile);
                 const uint32_t bytes = (uint32_t)(t.halves * A_HALF_BYTES + B_BYTES);
                 for (int kb = 0; kb < KB; ++kb) {
                     mbar_wait(&ctl->empty[stage], phase ^ 1);
@@ -206,8 +235,13 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
             int buf = 0; uint32_t bphase[2] = {0, 0};
-            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-                const Tile t = decode_tile(tab, ctl->gstart, tile, n_tiles_n, max_halves);
+            for (int it = 0;; ++it) {
+                const int ss = it % kSched;
+                mbar_wait(&ctl->sched_full[ss], (it / kSched) & 1);
+                const int tile = ctl->sched_tile[ss];
+                mbar_arrive(&ctl->sched_empty[ss]);
+                if (tile >= total_tiles) break;
+                const Tile t = decode_tile(tab, ctl, tile);
                 if (t.halves == 2) buf = 0;
                 const int b0 = buf;
                 for (int h = 0; h < t.halves; ++h) mbar_wait(&ctl->tmem_empty[b0 + h], bphase[b0 + h] ^ 1);
@@ -236,11 +270,18 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             }
         }
     } else if (warp >= 4) {
-        // ===== epilogue =====
-        const int q = warp - 4;                      // TMEM lane quarter of this warp (warp % 4)
+        // ===== epilogue: warps w and w+4 share TMEM lane quarter (w % 4) and split the columns =====
+        const int q = warp & 3;
+        const int part = (warp - 4) >> 2;            // 0: first half of the column chunks, 1: second half
         int buf = 0; uint32_t bphase[2] = {0, 0};
-        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-            const Tile t = decode_tile(tab, ctl->gstart, tile, n_tiles_n, max_halves);
+        for (int it = 0;; ++it) {
+            const int ss = it % kSched;
+            mbar_wait(&ctl->sched_full[ss], (it / kSched) & 1);
+            const int tile = ctl->sched_tile[ss];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&ctl->sched_empty[ss]);
+            if (tile >= total_tiles) break;
+            const Tile t = decode_tile(tab, ctl, tile);
             if (t.halves == 2) buf = 0;
             const int b0 = buf;
             for (int h = 0; h < t.halves; ++h) {
@@ -256,7 +297,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                     if (kSwiglu) {
                         uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * 128;
 #pragma unroll 1
-                        for (int c = 0; c < 4; ++c) {
+                        for (int c = part * 2; c < part * 2 + 2; ++c) {
                             uint32_t g[32], u[32];
                             tc_ld32(tbase + c * 32, g);
                             tc_ld32(tbase + 128 + c * 32, u);
@@ -279,7 +320,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                     } else {
                         uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * BN;
 #pragma unroll 1
-                        for (int c = 0; c < 8; ++c) {
+                        for (int c = part * 4; c < part * 4 + 4; ++c) {
                             if (t.n_tile * BN + c * 32 >= n_cols) break;     // N tail (n_cols % 64 == 0)
                             uint32_t v[32];
                             tc_ld32(tbase + c * 32, v);
@@ -308,6 +349,12 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (warp == 2) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+    }
+    // the last CTA to finish re-arms the scheduler words for the launch that reuses them (every CTA's producer has
+    // drawn its terminal ticket by now, so nobody reads the counter again)
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(sched + 1, 1) == (int)gridDim.x - 1) { sched[0] = 0; sched[1] = 0; }
     }
 }
 
@@ -358,6 +405,14 @@ int32_t make_map_arena(ef_ctx* ctx, CUtensorMap* tm, const void* base, int64_t r
     return EF_OK;
 }
 
+// per-launch scheduler words {ticket counter, finished CTAs}; the kernel zeroes them again when it ends, and a
+// ring of EF_SCHED_RING pairs keeps launches that may still be in flight apart
+int32_t* next_sched(ef_ctx* ctx) {
+    int32_t* p = ctx->sched_words + 2 * (size_t)ctx->sched_next;
+    ctx->sched_next = (ctx->sched_next + 1) % EF_SCHED_RING;
+    return p;
+}
+
 }  // namespace
 
 int32_t efk_ffn_tc_init(ef_ctx* ctx) {
@@ -368,6 +423,8 @@ int32_t efk_ffn_tc_init(ef_ctx* ctx) {
     if (rc != EF_OK) return rc;
     EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
     EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+    EF_CUDA(ctx, cudaMalloc(&ctx->sched_words, sizeof(int32_t) * 2 * EF_SCHED_RING));
+    EF_CUDA(ctx, cudaMemset(ctx->sched_words, 0, sizeof(int32_t) * 2 * EF_SCHED_RING));
     ctx->tm_ok = true;
     return EF_OK;
 }
@@ -384,12 +441,10 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     rc = make_map_2d(ctx, &tmH, ctx->h_ws, ctx->h_rows, f);
     if (rc != EF_OK) return rc;
 
-    const int max_halves = 2;
-    const int tile_rows = HALF_M * max_halves;
-    int mtiles = 0;
+    int mtiles = 0;       // tiles per n column: every group's 256-row tiles plus its short tail tile
     EfGroupTable t1 = tab, t2 = tab;
     for (int i = 0; i < tab.n; ++i) {
-        mtiles += (tab.g[i].rows + tile_rows - 1) / tile_rows;
+        mtiles += group_long_tiles(tab.g[i].rows) + group_has_short(tab.g[i].rows);
         t1.g[i].c_row0 = h_row0[i];   // GEMM1: x rows -> h rows
         t2.g[i].a_row0 = h_row0[i];   // GEMM2: h rows -> y rows
     }
@@ -407,7 +462,7 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         const int total = mtiles * ntn;
         const int grid = std::min(total, ctx->n_sms);
         ffn_gemm_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn,
-                                                                  max_halves, total, t1);
+                                                                  total, next_sched(ctx), t1);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
     }
@@ -417,7 +472,7 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         const int total = mtiles * ntn;
         const int grid = std::min(total, ctx->n_sms);
         ffn_gemm_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_wd, (uint16_t*)y, d, d, f, ntn,
-                                                                   max_halves, total, t2);
+                                                                   total, next_sched(ctx), t2);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
     }
