@@ -187,6 +187,11 @@ typedef struct {
 } ef_kernel_times;
 int32_t ef_set_kernel_timing(ef_ctx* ctx, int32_t on);
 int32_t ef_get_kernel_times(ef_ctx* ctx, ef_kernel_times* out, int32_t reset);
+/* Tail split-K of the grouped GEMM: 0 = automatic (default: split the tiles of the last, partly
+ * filled round along K so that every SM stays busy), 1 = never split, 2..16 = split EVERY tile into that many
+ * K parts (test hook: exercises the partial-sum workspace on small shapes).  Results differ between modes only
+ * by fp32 summation order. */
+int32_t ef_set_splitk(ef_ctx* ctx, int32_t mode);
 /* 0 = tcgen05 kernels (default); 1 = plain-FMA debug kernels for the grouped FFN (bring-up aid, slow). */
 int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on);
 

@@ -18,7 +18,7 @@ DECLARED_SYMBOLS = [
     "ef_expert_ffn_grouped", "ef_expert_ffn_grouped_resident", "ef_shared_ffn", "ef_combine", "ef_rmsnorm",
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
     "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
-    "ef_get_kernel_times",
+    "ef_get_kernel_times", "ef_set_splitk",
 ]
 
 
@@ -85,6 +85,7 @@ def load_library() -> ctypes.CDLL:
             "ef_sync": [vp],
             "ef_set_debug_simt_ffn": [vp, i32],
             "ef_set_kernel_timing": [vp, i32],
+            "ef_set_splitk": [vp, i32],
             "ef_get_kernel_times": [vp, ctypes.POINTER(KernelTimes), i32],
         }
         for name, args in sig.items():
@@ -243,6 +244,9 @@ class EfContext:
 
     def ef_set_debug_simt_ffn(self, on: bool):
         self._chk(self.lib.ef_set_debug_simt_ffn(self.h, 1 if on else 0))
+
+    def ef_set_splitk(self, mode: int):
+        self._chk(self.lib.ef_set_splitk(self.h, int(mode)))
 
     def ef_set_kernel_timing(self, on: bool):
         self._chk(self.lib.ef_set_kernel_timing(self.h, 1 if on else 0))

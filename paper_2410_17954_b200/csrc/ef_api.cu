@@ -128,6 +128,8 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
         if (ctx->host_expert[i] && ctx->host_owned[i]) cudaFreeHost(ctx->host_expert[i]);
     if (ctx->counts_pinned) cudaFreeHost(ctx->counts_pinned);
     if (ctx->sched_words) cudaFree(ctx->sched_words);
+    if (ctx->splitk_ws) cudaFree(ctx->splitk_ws);
+    if (ctx->splitk_counters) cudaFree(ctx->splitk_counters);
     if (ctx->h_ws) cudaFree(ctx->h_ws);
     if (ctx->arena) cudaFree(ctx->arena);
     delete ctx;
@@ -615,6 +617,13 @@ extern "C" int64_t ef_launch_count(ef_ctx* ctx) { return ctx ? ctx->launches : 0
 extern "C" int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on) {
     EF_CHECK_CTX(ctx);
     ctx->debug_simt = on ? 1 : 0;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_set_splitk(ef_ctx* ctx, int32_t mode) {
+    EF_CHECK_CTX(ctx);
+    if (mode < 0 || mode > 16) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_splitk: mode must be 0 (auto), 1 (off) or 2..16");
+    ctx->splitk_mode = mode;
     return EF_OK;
 }
 

@@ -88,6 +88,11 @@ struct ef_ctx {
     bool tm_ok = false;
     int32_t* sched_words = nullptr;     // device, [EF_SCHED_RING][2]
     int32_t sched_next = 0;
+    // tail split-K of the grouped GEMM (ffn_tc.cu): fp32 partial slots + per-tile arrival counters
+    float* splitk_ws = nullptr;
+    int32_t* splitk_counters = nullptr;
+    int32_t splitk_max_units = 0;
+    int32_t splitk_mode = 0;            // 0 auto, 1 off, >= 2 force that many K parts on every tile (tests)
     // copy timing
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> copy_spans;
     float copy_ms = 0.f;
@@ -99,6 +104,7 @@ struct ef_ctx {
     // misc
     int64_t launches = 0;
     int32_t debug_simt = 0;
+    bool route_smem_set = false;        // route kernel opted in to > 48 KB dynamic smem (E > 176)
     std::string err;
     int32_t sticky = EF_OK;
 };

@@ -23,6 +23,11 @@
 // every group (n-major inside a group, so the M-tiles that share a weight tile are claimed back to back and hit L2),
 // then the short (<= 128-row) tail tiles -- and claimed dynamically, i.e. greedy longest-processing-time list
 // scheduling: the makespan is within one short tile of the mean load whatever the row counts are.
+// Tail split-K: with T tiles on G SMs the last T mod G tiles (all of them when T < G -- decode, single-expert miss
+// waves) would leave most SMs idle for a whole tile time, so the host splits each of those tiles s ways along K.
+// A split unit writes its raw fp32 accumulator to a workspace slot, then bumps the tile's arrival counter; the
+// unit that arrives last sums the s partials in split order (deterministic) and runs the normal epilogue.  No
+// CTA ever waits for another one.
 // Ragged M: a group's last tile may be short; TMA zero-fills rows past the tensor, rows past the
 // group are computed and discarded (stores are row-predicated), so neighbours are never touched.
 #include <cuda_bf16.h>
@@ -42,6 +47,7 @@ constexpr int kThreads = 384;
 constexpr int kEpiWarps = 8;
 constexpr int kSched = 4;               // depth of the tile-broadcast ring
 constexpr int kTmemCols = 512;
+constexpr int kSlotFloats = 2 * 128 * 256;   // split-K workspace slot: one 256 x 256 fp32 accumulator pair
 
 struct __align__(8) SmemCtl {
     uint64_t full[kStages];
@@ -52,6 +58,7 @@ struct __align__(8) SmemCtl {
     uint64_t sched_empty[kSched];
     int32_t sched_tile[kSched];
     uint32_t tmem_base;
+    int32_t split_last;                   // epilogue broadcast: this unit arrived last at its split tile
     int32_t total_long;                   // number of 2-half tiles (they come first)
     int32_t gstart_long[EF_MAX_GROUPS + 1];
     int32_t gstart_short[EF_MAX_GROUPS + 1];
@@ -131,17 +138,84 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     return *reinterpret_cast<uint32_t*>(&v);
 }
 
+// 32 accumulator columns of one row -> bf16, four 16-byte stores
+__device__ __forceinline__ void store_plain32(uint16_t* dst, const uint32_t (&v)[32]) {
+    uint32_t o[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) o[i] = pack_bf16(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
+    uint4* d4 = reinterpret_cast<uint4*>(dst);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) d4[i] = make_uint4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
+}
+// h = silu(g) * u for 32 columns of one row
+__device__ __forceinline__ void store_swiglu32(uint16_t* dst, const uint32_t (&g)[32], const uint32_t (&u)[32]) {
+    uint32_t o[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const float g0 = __uint_as_float(g[2 * i]), g1 = __uint_as_float(g[2 * i + 1]);
+        const float u0 = __uint_as_float(u[2 * i]), u1 = __uint_as_float(u[2 * i + 1]);
+        const float h0 = __fdividef(g0, 1.f + __expf(-g0)) * u0;
+        const float h1 = __fdividef(g1, 1.f + __expf(-g1)) * u1;
+        o[i] = pack_bf16(h0, h1);
+    }
+    uint4* d4 = reinterpret_cast<uint4*>(dst);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) d4[i] = make_uint4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
+}
+// split-K reduction: 32 columns (chunk c) of this thread's row, summed over the s partial slots in slot order.
+// rrow points at this row's float4 in slot 0; L2-only loads (the partials were written by other SMs).
+__device__ __forceinline__ void sum_partials32(const float4* rrow, int c, int s, uint32_t (&out)[32]) {
+    float4 acc[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int j = 0; j < s; ++j) {
+        const float4* p = rrow + (size_t)j * (kSlotFloats / 4) + (size_t)(c * 8) * 128;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const float4 v = __ldcg(p + (size_t)i * 128);
+            acc[i].x += v.x; acc[i].y += v.y; acc[i].z += v.z; acc[i].w += v.w;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        out[4 * i] = __float_as_uint(acc[i].x); out[4 * i + 1] = __float_as_uint(acc[i].y);
+        out[4 * i + 2] = __float_as_uint(acc[i].z); out[4 * i + 3] = __float_as_uint(acc[i].w);
+    }
+}
+// barrier among the 8 epilogue warps only
+__device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+
 struct Tile {
     int a_row, c_row, rows_valid, halves, n_tile, slot;
+    int kb0, kb1;        // k-block range of this unit
+    int tail, split_j;   // index among the split tiles (-1: whole tile) and which K part this unit is
+};
+
+struct SplitArgs {
+    int32_t n_plain;     // tickets [0, n_plain) are whole tiles; the rest are (tile, K part) pairs, part fastest
+    int32_t s;           // K parts per split tile (>= 2 when any tile is split)
+    float* ws;           // [n_split_tiles * s] slots of kSlotFloats fp32
+    int32_t* counters;   // [n_split_tiles] arrival counters, zero between launches
 };
 
 // number of 2-half ("long", 129..256 rows) tiles of a group; the remainder, if any, is one short tile per n
 __device__ __host__ __forceinline__ int group_long_tiles(int rows) { return rows / (2 * 128) + ((rows % (2 * 128)) > 128 ? 1 : 0); }
 __device__ __host__ __forceinline__ int group_has_short(int rows) { int r = rows % (2 * 128); return (r > 0 && r <= 128) ? 1 : 0; }
 
-__device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemCtl* ctl, int tile) {
+__device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemCtl* ctl, int unit, const SplitArgs& sp,
+                                            int KB) {
     Tile t;
     int g = 0, row_off;
+    int tile = unit;
+    t.kb0 = 0; t.kb1 = KB; t.tail = -1; t.split_j = 0;
+    if (unit >= sp.n_plain) {
+        const int v = unit - sp.n_plain;
+        t.tail = v / sp.s;
+        t.split_j = v - t.tail * sp.s;
+        tile = sp.n_plain + t.tail;
+        t.kb0 = (t.split_j * KB) / sp.s;
+        t.kb1 = ((t.split_j + 1) * KB) / sp.s;
+    }
     if (tile < ctl->total_long) {
         while (tile >= ctl->gstart_long[g + 1]) ++g;
         const int local = tile - ctl->gstart_long[g];
@@ -168,7 +242,7 @@ template <bool kSwiglu>
 __global__ void __launch_bounds__(kThreads, 1)
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                 uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int total_tiles,
-                int32_t* __restrict__ sched, const __grid_constant__ EfGroupTable tab) {
+                int32_t* __restrict__ sched, const SplitArgs sp, const __grid_constant__ EfGroupTable tab) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     SmemCtl* ctl = (SmemCtl*)(smem + (size_t)kStages * STAGE_BYTES);
@@ -217,9 +291,9 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 ctl->sched_tile[ss] = tile;
                 mbar_arrive(&ctl->sched_full[ss]);          // release: the tile index is visible to the waiters
                 if (tile >= total_tiles) break;
-                const Tile t = decode_tile(tab, ctl, tile);
+                const Tile t = decode_tile(tab, ctl, tile, sp, KB);
                 const uint32_t bytes = (uint32_t)(t.halves * A_HALF_BYTES + B_BYTES);
-                for (int kb = 0; kb < KB; ++kb) {
+                for (int kb = t.kb0; kb < t.kb1; ++kb) {
                     mbar_wait(&ctl->empty[stage], phase ^ 1);
                     uint8_t* sa = smem + (size_t)stage * STAGE_BYTES;
                     mbar_expect_tx(&ctl->full[stage], bytes);
@@ -234,19 +308,19 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         // ===== MMA issuer =====
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
-            int buf = 0; uint32_t bphase[2] = {0, 0};
+            int buf = 0; uint32_t bphase = 0;          // bit b = phase of accumulator buffer b
             for (int it = 0;; ++it) {
                 const int ss = it % kSched;
                 mbar_wait(&ctl->sched_full[ss], (it / kSched) & 1);
                 const int tile = ctl->sched_tile[ss];
                 mbar_arrive(&ctl->sched_empty[ss]);
                 if (tile >= total_tiles) break;
-                const Tile t = decode_tile(tab, ctl, tile);
+                const Tile t = decode_tile(tab, ctl, tile, sp, KB);
                 if (t.halves == 2) buf = 0;
                 const int b0 = buf;
-                for (int h = 0; h < t.halves; ++h) mbar_wait(&ctl->tmem_empty[b0 + h], bphase[b0 + h] ^ 1);
+                for (int h = 0; h < t.halves; ++h) mbar_wait(&ctl->tmem_empty[b0 + h], ((bphase >> (b0 + h)) & 1u) ^ 1u);
                 tc_fence_after();
-                for (int kb = 0; kb < KB; ++kb) {
+                for (int kb = t.kb0; kb < t.kb1; ++kb) {
                     mbar_wait(&ctl->full[stage], phase);
                     tc_fence_after();
                     const uint32_t sa = smem_u32(smem + (size_t)stage * STAGE_BYTES);
@@ -254,7 +328,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 #pragma unroll
                     for (int k = 0; k < BK / 16; ++k) {
                         const uint64_t bd = smem_desc(sb + k * 32);
-                        const uint32_t acc = (kb > 0 || k > 0) ? 1u : 0u;
+                        const uint32_t acc = (kb > t.kb0 || k > 0) ? 1u : 0u;
                         tc_mma(tmem_base + (uint32_t)(b0 * BN), smem_desc(sa + k * 32), bd, kIdesc, acc);
                         if (t.halves == 2)
                             tc_mma(tmem_base + (uint32_t)((b0 + 1) * BN), smem_desc(sa + A_HALF_BYTES + k * 32), bd, kIdesc, acc);
@@ -264,7 +338,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 }
                 for (int h = 0; h < t.halves; ++h) {
                     tc_commit(&ctl->tmem_full[b0 + h]);
-                    bphase[b0 + h] ^= 1;
+                    bphase ^= 1u << (b0 + h);
                 }
                 buf = (t.halves == 2) ? 0 : (b0 ^ 1);
             }
@@ -273,7 +347,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         // ===== epilogue: warps w and w+4 share TMEM lane quarter (w % 4) and split the columns =====
         const int q = warp & 3;
         const int part = (warp - 4) >> 2;            // 0: first half of the column chunks, 1: second half
-        int buf = 0; uint32_t bphase[2] = {0, 0};
+        int buf = 0; uint32_t bphase = 0;
         for (int it = 0;; ++it) {
             const int ss = it % kSched;
             mbar_wait(&ctl->sched_full[ss], (it / kSched) & 1);
@@ -281,19 +355,39 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             __syncwarp();
             if (lane == 0) mbar_arrive(&ctl->sched_empty[ss]);
             if (tile >= total_tiles) break;
-            const Tile t = decode_tile(tab, ctl, tile);
+            const Tile t = decode_tile(tab, ctl, tile, sp, KB);
             if (t.halves == 2) buf = 0;
             const int b0 = buf;
+            const bool split = t.tail >= 0;
+            // fp32 workspace of this unit: [half][col/4][row in half][4 floats] -- a warp's float4 stores are contiguous
+            float* ws_mine = split ? sp.ws + ((size_t)t.tail * sp.s + t.split_j) * kSlotFloats : nullptr;
             for (int h = 0; h < t.halves; ++h) {
                 const int b = b0 + h;
-                mbar_wait(&ctl->tmem_full[b], bphase[b]);
-                bphase[b] ^= 1;
+                mbar_wait(&ctl->tmem_full[b], (bphase >> b) & 1u);
+                bphase ^= 1u << b;
                 tc_fence_after();
                 const int r = h * HALF_M + q * 32 + lane;            // row inside the tile
                 const bool row_ok = r < t.rows_valid;
                 const bool warp_ok = (h * HALF_M + q * 32) < t.rows_valid;
                 const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b * BN);
-                if (warp_ok) {
+                if (warp_ok && split) {
+                    // raw accumulator chunks of 32 columns -> workspace (the finalising unit applies the epilogue)
+                    float4* wrow = reinterpret_cast<float4*>(ws_mine) + (size_t)h * (HALF_M * BN / 4) + (q * 32 + lane);
+#pragma unroll 1
+                    for (int cc = 0; cc < 4; ++cc) {
+                        const int c = kSwiglu ? ((cc & 1) * 4 + part * 2 + (cc >> 1)) : (part * 4 + cc);
+                        if (!kSwiglu && t.n_tile * BN + c * 32 >= n_cols) break;
+                        uint32_t v[32];
+                        tc_ld32(tbase + c * 32, v);
+                        tc_wait_ld();
+                        if (row_ok) {
+#pragma unroll
+                            for (int i = 0; i < 8; ++i)
+                                wrow[(size_t)(c * 8 + i) * HALF_M] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                                                                                 __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+                        }
+                    }
+                } else if (warp_ok) {
                     if (kSwiglu) {
                         uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * 128;
 #pragma unroll 1
@@ -302,20 +396,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                             tc_ld32(tbase + c * 32, g);
                             tc_ld32(tbase + 128 + c * 32, u);
                             tc_wait_ld();
-                            uint32_t o[16];
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) {
-                                const float g0 = __uint_as_float(g[2 * i]), g1 = __uint_as_float(g[2 * i + 1]);
-                                const float u0 = __uint_as_float(u[2 * i]), u1 = __uint_as_float(u[2 * i + 1]);
-                                const float h0 = __fdividef(g0, 1.f + __expf(-g0)) * u0;
-                                const float h1 = __fdividef(g1, 1.f + __expf(-g1)) * u1;
-                                o[i] = pack_bf16(h0, h1);
-                            }
-                            if (row_ok) {
-                                uint4* dst = (uint4*)(crow + c * 32);
-#pragma unroll
-                                for (int i = 0; i < 4; ++i) dst[i] = make_uint4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
-                            }
+                            if (row_ok) store_swiglu32(crow + c * 32, g, u);
                         }
                     } else {
                         uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * BN;
@@ -325,14 +406,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                             uint32_t v[32];
                             tc_ld32(tbase + c * 32, v);
                             tc_wait_ld();
-                            uint32_t o[16];
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) o[i] = pack_bf16(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
-                            if (row_ok) {
-                                uint4* dst = (uint4*)(crow + c * 32);
-#pragma unroll
-                                for (int i = 0; i < 4; ++i) dst[i] = make_uint4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
-                            }
+                            if (row_ok) store_plain32(crow + c * 32, v);
                         }
                     }
                 }
@@ -341,6 +415,47 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 if (lane == 0) mbar_arrive(&ctl->tmem_empty[b]);
             }
             buf = (t.halves == 2) ? 0 : (b0 ^ 1);
+            if (split) {
+                // publish the partial, count arrivals; the last unit of the tile reduces all s partials in split order
+                __threadfence();
+                epi_bar();
+                if (threadIdx.x == 4 * 32) {
+                    const int old = atomicAdd(sp.counters + t.tail, 1);
+                    const int last = (old == sp.s - 1) ? 1 : 0;
+                    if (last) sp.counters[t.tail] = 0;          // re-arm for the next launch
+                    ctl->split_last = last;
+                }
+                epi_bar();
+                const bool last = ctl->split_last != 0;          // rewritten only after the next split unit's first barrier
+                if (last) {
+                    __threadfence();
+                    const float* ws_tile = sp.ws + (size_t)t.tail * sp.s * kSlotFloats;
+                    for (int h = 0; h < t.halves; ++h) {
+                        const int r = h * HALF_M + q * 32 + lane;
+                        if (r >= t.rows_valid) continue;
+                        const float4* rrow = reinterpret_cast<const float4*>(ws_tile) + (size_t)h * (HALF_M * BN / 4) + (q * 32 + lane);
+                        if (kSwiglu) {
+                            uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * 128;
+#pragma unroll 1
+                            for (int c = part * 2; c < part * 2 + 2; ++c) {
+                                uint32_t g[32], u[32];
+                                sum_partials32(rrow, c, sp.s, g);
+                                sum_partials32(rrow, c + 4, sp.s, u);
+                                store_swiglu32(crow + c * 32, g, u);
+                            }
+                        } else {
+                            uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * BN;
+#pragma unroll 1
+                            for (int c = part * 4; c < part * 4 + 4; ++c) {
+                                if (t.n_tile * BN + c * 32 >= n_cols) break;
+                                uint32_t v[32];
+                                sum_partials32(rrow, c, sp.s, v);
+                                store_plain32(crow + c * 32, v);
+                            }
+                        }
+                    }
+                }
+            }
         }
     }
 
@@ -413,6 +528,38 @@ int32_t* next_sched(ef_ctx* ctx) {
     return p;
 }
 
+// Tail split-K plan for one launch: `tiles` tickets in scheduler order with `n_short` short ones at the end, G CTAs,
+// KB k-blocks per tile.  Costs are in k-block times of a 256-row tile (1024 tensor cycles): a whole tail tile holds
+// an SM for KB (KB/2 if short) of them; a split unit adds a partial write and the finaliser reads s partials
+// (~0.03 per valid row each, from the measured ~50 GB/s per-SM global bandwidth).
+struct SplitPlan { int n_plain, n_tail, s; };
+
+SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, double avg_rows) {
+    SplitPlan p{tiles, 0, 1};
+    if (ctx->splitk_mode == 1 || tiles == 0) return p;
+    int r = tiles % G;
+    if (tiles < G) r = tiles;
+    if (ctx->splitk_mode >= 2) {                       // forced (tests): split every tile
+        p.s = std::min(ctx->splitk_mode, std::max(1, KB));
+        if (p.s < 2) return SplitPlan{tiles, 0, 1};
+        p.n_tail = std::min(tiles, ctx->splitk_max_units / p.s);
+        p.n_plain = tiles - p.n_tail;
+        return p.n_tail ? p : SplitPlan{tiles, 0, 1};
+    }
+    if (r == 0) return p;
+    const double w = (n_short >= r) ? 0.5 : 1.0;       // the tail is the end of the list: short tiles first
+    const double ovh = 0.03 * avg_rows;
+    const int smax = std::min(16, KB / 4);
+    double best = KB * w;                              // s = 1: one more round of whole tiles
+    for (int s = 2; s <= smax; ++s) {
+        if (r * s > ctx->splitk_max_units) break;
+        const double cost = (double)((r * s + G - 1) / G) * (KB * w / s) + 1.0 + ovh * (1 + s);
+        if (cost < best * 0.9) { best = cost; p.s = s; }
+    }
+    if (p.s > 1) { p.n_tail = r; p.n_plain = tiles - r; }
+    return p;
+}
+
 }  // namespace
 
 int32_t efk_ffn_tc_init(ef_ctx* ctx) {
@@ -425,6 +572,10 @@ int32_t efk_ffn_tc_init(ef_ctx* ctx) {
     EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
     EF_CUDA(ctx, cudaMalloc(&ctx->sched_words, sizeof(int32_t) * 2 * EF_SCHED_RING));
     EF_CUDA(ctx, cudaMemset(ctx->sched_words, 0, sizeof(int32_t) * 2 * EF_SCHED_RING));
+    ctx->splitk_max_units = 2 * ctx->n_sms;
+    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_ws, sizeof(float) * kSlotFloats * (size_t)ctx->splitk_max_units));
+    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_counters, sizeof(int32_t) * ctx->splitk_max_units));
+    EF_CUDA(ctx, cudaMemset(ctx->splitk_counters, 0, sizeof(int32_t) * ctx->splitk_max_units));
     ctx->tm_ok = true;
     return EF_OK;
 }
@@ -441,16 +592,17 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     rc = make_map_2d(ctx, &tmH, ctx->h_ws, ctx->h_rows, f);
     if (rc != EF_OK) return rc;
 
-    int mtiles = 0;       // tiles per n column: every group's 256-row tiles plus its short tail tile
+    int64_t rows_total = 0;
+    for (int i = 0; i < tab.n; ++i) rows_total += tab.g[i].rows;
+    int mtiles = 0, mshort = 0;   // tiles per n column: every group's 256-row tiles plus its short tail tile
     EfGroupTable t1 = tab, t2 = tab;
     for (int i = 0; i < tab.n; ++i) {
         mtiles += group_long_tiles(tab.g[i].rows) + group_has_short(tab.g[i].rows);
+        mshort += group_has_short(tab.g[i].rows);
         t1.g[i].c_row0 = h_row0[i];   // GEMM1: x rows -> h rows
         t2.g[i].a_row0 = h_row0[i];   // GEMM2: h rows -> y rows
     }
     ef_ctx::KSpan span{};
-    int64_t rows_total = 0;
-    for (int i = 0; i < tab.n; ++i) rows_total += tab.g[i].rows;
     if (ctx->time_kernels) {
         EF_CUDA(ctx, cudaEventCreate(&span.e0));
         EF_CUDA(ctx, cudaEventCreate(&span.e1));
@@ -459,20 +611,26 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     }
     {
         const int ntn = f / 128;      // 256 packed W13 rows -> 128 h columns
-        const int total = mtiles * ntn;
+        const int tiles = mtiles * ntn;
+        const SplitPlan pl = plan_split(ctx, tiles, mshort * ntn, ctx->n_sms, d / BK, (double)rows_total / mtiles);
+        const int total = pl.n_plain + pl.n_tail * pl.s;
         const int grid = std::min(total, ctx->n_sms);
+        const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
         ffn_gemm_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn,
-                                                                  total, next_sched(ctx), t1);
+                                                                  total, next_sched(ctx), sp, t1);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
     }
     if (ctx->time_kernels) EF_CUDA(ctx, cudaEventRecord(span.e1, st));
     {
         const int ntn = (d + BN - 1) / BN;
-        const int total = mtiles * ntn;
+        const int tiles = mtiles * ntn;
+        const SplitPlan pl = plan_split(ctx, tiles, mshort * ntn, ctx->n_sms, f / BK, (double)rows_total / mtiles);
+        const int total = pl.n_plain + pl.n_tail * pl.s;
         const int grid = std::min(total, ctx->n_sms);
+        const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
         ffn_gemm_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_wd, (uint16_t*)y, d, d, f, ntn,
-                                                                   total, next_sched(ctx), t2);
+                                                                   total, next_sched(ctx), sp, t2);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
     }

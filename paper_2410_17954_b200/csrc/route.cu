@@ -1,31 +1,28 @@
 // a1: router logits + top-k + gate weights  (Eq. 1-2, L40-46; R1-R3).
 //
-// HBM-bound: reads x once (2*d bytes per token); Wr (E*d*2 bytes) stays in L1/L2.  One warp per
-// token, 128-bit loads, fp32 accumulate, warp-shuffle reductions; top-k by k rounds of warp argmax
-// (ties -> lower expert index), gate weights with expf in fp32.
+// logits[T,E] = x[T,d] . Wr[E,d]^T + b is a skinny GEMM (N = E <= 256): HBM-bound on x for E = 8, ALU-bound on
+// plain FMA for E = 64 (2*d*E flop per token), so the contraction runs on the legacy tensor path (mma.sync
+// m16n8k16, bf16 x bf16 -> fp32) -- the tile is far too small for a tcgen05 pipeline, and the kernel is
+// latency-bound, not throughput-bound.
+//
+// One CTA = 16 tokens (one MMA M tile) x all experts, 8 warps splitting K: warp w takes the 32-wide k chunks
+// w, w+8, ...  Fragments come straight from global memory with 128-bit loads: thread (g, t) of a warp loads
+// elements [8t, 8t+8) of the chunk from row g (and g+8) of x and from row g of each 8-expert tile of Wr, and
+// feeds elements (4s, 4s+1 | 4s+2, 4s+3) to MMA step s = 0, 1.  That is a permutation of k inside the chunk,
+// applied identically to both operands, so every product still meets its partner.  Per-warp partial tiles are
+// summed across the 8 warps through shared memory in a fixed order (deterministic), the bias is added, and
+// each warp then finishes two tokens: k rounds of warp arg-max (ties -> lower expert index) and the gate
+// weights with expf in fp32.
 #include <cuda_bf16.h>
 
 #include "ef_internal.h"
 
 namespace {
 
-constexpr int kWarps = 4;
-constexpr int kEGroup = 8;
-
-__device__ __forceinline__ float bf_lo(uint32_t u) { return __uint_as_float(u << 16); }
-__device__ __forceinline__ float bf_hi(uint32_t u) { return __uint_as_float(u & 0xffff0000u); }
-
-__device__ __forceinline__ float dot8(const uint4& a, const uint4& b, float acc) {
-    acc = fmaf(bf_lo(a.x), bf_lo(b.x), acc);
-    acc = fmaf(bf_hi(a.x), bf_hi(b.x), acc);
-    acc = fmaf(bf_lo(a.y), bf_lo(b.y), acc);
-    acc = fmaf(bf_hi(a.y), bf_hi(b.y), acc);
-    acc = fmaf(bf_lo(a.z), bf_lo(b.z), acc);
-    acc = fmaf(bf_hi(a.z), bf_hi(b.z), acc);
-    acc = fmaf(bf_lo(a.w), bf_lo(b.w), acc);
-    acc = fmaf(bf_hi(a.w), bf_hi(b.w), acc);
-    return acc;
-}
+constexpr int kWarps = 8;
+constexpr int kTok = 16;          // tokens per CTA
+constexpr int kEChunk = 64;       // experts per accumulation pass (8 MMA N tiles)
+constexpr int kPartLd = 72;       // padded row stride of the partial tiles (floats)
 
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
@@ -43,82 +40,116 @@ __device__ __forceinline__ void warp_argmax(float& v, int& i) {
     }
 }
 
+__device__ __forceinline__ void mma_bf16(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                         uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
 __global__ void __launch_bounds__(kWarps * 32)
 route_topk_kernel(const uint4* __restrict__ x, const uint4* __restrict__ wr, const float* __restrict__ bias,
                   int64_t bias_stride, int T, int d8, int E, int k, int renorm, int32_t* __restrict__ idx,
                   float* __restrict__ w, float* __restrict__ logits_out) {
-    extern __shared__ float s_logits[];   // [kWarps][E]
+    extern __shared__ float smem_f[];
+    float* s_part = smem_f;                                   // [kWarps][kTok][kPartLd]
+    float* s_logits = smem_f + kWarps * kTok * kPartLd;       // [kTok][E]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int t = blockIdx.x * kWarps + warp;
-    if (t >= T) return;
-    float* lg = s_logits + warp * E;
-    const uint4* xr = x + (int64_t)t * d8;
+    const int g = lane >> 2, tq = lane & 3;
+    const int t0 = blockIdx.x * kTok;
+    const int n_chunks = d8 >> 2;                             // 32-element k chunks (d % 64 == 0)
+    const uint4 zero4 = make_uint4(0, 0, 0, 0);
+    const bool r0_ok = t0 + g < T, r1_ok = t0 + g + 8 < T;
+    const uint4* xa = x + (int64_t)(t0 + g) * d8 + tq;
+    const uint4* xb = x + (int64_t)(t0 + g + 8) * d8 + tq;
 
-    for (int e0 = 0; e0 < E; e0 += kEGroup) {
-        float acc[kEGroup];
+    for (int e0 = 0; e0 < E; e0 += kEChunk) {
+        float acc[kEChunk / 8][4];
 #pragma unroll
-        for (int j = 0; j < kEGroup; ++j) acc[j] = 0.f;
-        for (int c = lane; c < d8; c += 32) {
-            const uint4 xv = xr[c];
+        for (int n = 0; n < kEChunk / 8; ++n) { acc[n][0] = acc[n][1] = acc[n][2] = acc[n][3] = 0.f; }
+        const int n_tiles = min(kEChunk / 8, (E - e0 + 7) >> 3);
+#pragma unroll 2
+        for (int c = warp; c < n_chunks; c += kWarps) {
+            const uint4 a_lo = r0_ok ? xa[c * 4] : zero4;
+            const uint4 a_hi = r1_ok ? xb[c * 4] : zero4;
 #pragma unroll
-            for (int j = 0; j < kEGroup; ++j) {
-                if (e0 + j < E) {
-                    const uint4 wv = __ldg(wr + (int64_t)(e0 + j) * d8 + c);
-                    acc[j] = dot8(xv, wv, acc[j]);
+            for (int n = 0; n < kEChunk / 8; ++n) {
+                if (n < n_tiles) {
+                    const int e = e0 + n * 8 + g;
+                    const uint4 b = (e < E) ? __ldg(wr + (int64_t)e * d8 + c * 4 + tq) : zero4;
+                    mma_bf16(acc[n], a_lo.x, a_hi.x, a_lo.y, a_hi.y, b.x, b.y);
+                    mma_bf16(acc[n], a_lo.z, a_hi.z, a_lo.w, a_hi.w, b.z, b.w);
                 }
             }
         }
+        // partial tiles -> shared memory, fixed-order sum over the 8 warps, + bias
+        float* mine = s_part + warp * kTok * kPartLd;
 #pragma unroll
-        for (int j = 0; j < kEGroup; ++j) {
-            float s = warp_sum(acc[j]);
-            if (lane == 0 && e0 + j < E) {
-                float b = bias ? bias[(int64_t)t * bias_stride + e0 + j] : 0.f;
-                lg[e0 + j] = s + b;
+        for (int n = 0; n < kEChunk / 8; ++n) {
+            *reinterpret_cast<float2*>(mine + g * kPartLd + n * 8 + 2 * tq) = make_float2(acc[n][0], acc[n][1]);
+            *reinterpret_cast<float2*>(mine + (g + 8) * kPartLd + n * 8 + 2 * tq) = make_float2(acc[n][2], acc[n][3]);
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < kTok * kEChunk; i += kWarps * 32) {
+            const int r = i / kEChunk, col = i % kEChunk;
+            if (e0 + col < E) {
+                float s = 0.f;
+#pragma unroll
+                for (int ww = 0; ww < kWarps; ++ww) s += s_part[(ww * kTok + r) * kPartLd + col];
+                const int t = t0 + r;
+                if (bias && t < T) s += bias[(int64_t)t * bias_stride + e0 + col];
+                s_logits[r * E + e0 + col] = s;
             }
         }
+        __syncthreads();
     }
-    __syncwarp();
-    if (logits_out)
-        for (int e = lane; e < E; e += 32) logits_out[(int64_t)t * E + e] = lg[e];
 
-    // candidates: lane owns experts lane, lane+32, ...
-    float v[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        int e = lane + 32 * i;
-        v[i] = (e < E) ? lg[e] : -INFINITY;
-    }
-    float zall = 0.f, m = 0.f, zsel = 0.f, my_val = 0.f;
-    int my_idx = 0;
-    for (int j = 0; j < k; ++j) {
-        float bv = -INFINITY;
-        int bi = 0x7fffffff;
+    // each warp finishes two tokens
+    for (int r = warp; r < kTok; r += kWarps) {
+        const int t = t0 + r;
+        if (t >= T) break;
+        const float* lg = s_logits + r * E;
+        if (logits_out)
+            for (int e = lane; e < E; e += 32) logits_out[(int64_t)t * E + e] = lg[e];
+        // candidates: lane owns experts lane, lane+32, ...
+        float v[8];
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             int e = lane + 32 * i;
-            if (e < E && (v[i] > bv || (v[i] == bv && e < bi))) { bv = v[i]; bi = e; }
+            v[i] = (e < E) ? lg[e] : -INFINITY;
         }
-        warp_argmax(bv, bi);
-        if (j == 0) {
-            m = bv;
-            if (!renorm) {
-                float z = 0.f;
-                for (int e = lane; e < E; e += 32) z += expf(lg[e] - m);
-                zall = warp_sum(z);
+        float zall = 0.f, m = 0.f, zsel = 0.f, my_val = 0.f;
+        int my_idx = 0;
+        for (int j = 0; j < k; ++j) {
+            float bv = -INFINITY;
+            int bi = 0x7fffffff;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                int e = lane + 32 * i;
+                if (e < E && (v[i] > bv || (v[i] == bv && e < bi))) { bv = v[i]; bi = e; }
+            }
+            warp_argmax(bv, bi);
+            if (j == 0) {
+                m = bv;
+                if (!renorm) {
+                    float z = 0.f;
+                    for (int e = lane; e < E; e += 32) z += expf(lg[e] - m);
+                    zall = warp_sum(z);
+                }
+            }
+            zsel += expf(bv - m);
+            if (lane == j) { my_val = bv; my_idx = bi; }
+            if ((bi & 31) == lane) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    if (i == (bi >> 5)) v[i] = -INFINITY;   // taken; E real logits are finite
             }
         }
-        zsel += expf(bv - m);
-        if (lane == j) { my_val = bv; my_idx = bi; }
-        if ((bi & 31) == lane) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i)
-                if (i == (bi >> 5)) v[i] = -INFINITY;   // taken; E real logits are finite
+        if (lane < k) {
+            const float Z = renorm ? zsel : zall;
+            idx[(int64_t)t * k + lane] = my_idx;
+            w[(int64_t)t * k + lane] = expf(my_val - m) / Z;
         }
-    }
-    if (lane < k) {
-        const float Z = renorm ? zsel : zall;
-        idx[(int64_t)t * k + lane] = my_idx;
-        w[(int64_t)t * k + lane] = expf(my_val - m) / Z;
     }
 }
 
@@ -128,8 +159,12 @@ int32_t efk_route_topk(ef_ctx* ctx, cudaStream_t st, const void* x, const void* 
                        int64_t bias_stride, int T, int renorm, int32_t* idx, float* w, float* logits) {
     if (T == 0) return EF_OK;
     const int E = ctx->cfg.n_experts, d = ctx->cfg.d_model, k = ctx->cfg.top_k;
-    dim3 grid((T + kWarps - 1) / kWarps), block(kWarps * 32);
-    size_t smem = (size_t)kWarps * E * sizeof(float);
+    dim3 grid((T + kTok - 1) / kTok), block(kWarps * 32);
+    const size_t smem = ((size_t)kWarps * kTok * kPartLd + (size_t)kTok * E) * sizeof(float);
+    if (smem > 48 * 1024 && !ctx->route_smem_set) {
+        EF_CUDA(ctx, cudaFuncSetAttribute(route_topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+        ctx->route_smem_set = true;
+    }
     route_topk_kernel<<<grid, block, smem, st>>>((const uint4*)x, (const uint4*)wr, bias, bias_stride, T, d / 8, E, k,
                                                  renorm, idx, w, logits);
     ctx->launches++;

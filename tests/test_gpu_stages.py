@@ -146,7 +146,7 @@ def test_permute_bit_exact(T, k, E, d):
 # ------------------------------------------------------------------------------------------------
 # a4 grouped FFN (resident experts)
 # ------------------------------------------------------------------------------------------------
-def run_resident_ffn(ctx, E, d, f, counts, seed, simt):
+def run_resident_ffn(ctx, E, d, f, counts, seed, simt, splitk=0):
     """Load experts 0..E-1 into slots via the cache, run the grouped FFN on oracle-permuted rows."""
     cfg = wl.scaled(wl.CONFIGS["tiny"], d_model=d, d_ff=f, n_experts=E, seed=seed)
     experts = [wl.expert_weights(cfg, 0, e) for e in range(E)]
@@ -161,6 +161,7 @@ def run_resident_ffn(ctx, E, d, f, counts, seed, simt):
     offs = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
     y = torch.full((R, d), float("nan"), dtype=torch.bfloat16, device="cuda")
     ctx.ef_set_debug_simt_ffn(simt)
+    ctx.ef_set_splitk(splitk)
     act = [e for e in range(E) if counts[e] > 0]
     ctx.ef_expert_ffn_grouped_resident(dev_bf16(x_perm), [offs[e] for e in act], [counts[e] for e in act],
                                        [slot_of[e] for e in act], y)
@@ -181,13 +182,33 @@ FFN_CASES = [
 ]
 
 
-@pytest.mark.parametrize("simt", [True, False], ids=["simt_debug", "tcgen05"])
+# splitk: 0 = automatic tail split-K (these launches have fewer tiles than SMs, so it engages), 1 = off,
+# 2 / 3 / 5 = every tile split into that many K parts (uneven k-block ranges, partial-sum workspace, last-arriver
+# reduction)
+@pytest.mark.parametrize("simt,splitk", [(True, 0), (False, 1), (False, 0), (False, 2), (False, 3), (False, 5)],
+                         ids=["simt_debug", "tcgen05_nosplit", "tcgen05_auto", "tcgen05_split2", "tcgen05_split3",
+                              "tcgen05_split5"])
 @pytest.mark.parametrize("E,d,f,counts", FFN_CASES)
-def test_ffn_grouped_resident(E, d, f, counts, simt):
+def test_ffn_grouped_resident(E, d, f, counts, simt, splitk):
     ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)))
-    got, ref = run_resident_ffn(ctx, E, d, f, counts, seed=13, simt=simt)
+    got, ref = run_resident_ffn(ctx, E, d, f, counts, seed=13, simt=simt, splitk=splitk)
     assert not np.isnan(got).any()          # every routed row was written
     check_float(got, ref)
+    ctx.close()
+
+
+def test_ffn_splitk_repeated_launches_rearm_counters():
+    """The arrival counters and scheduler words re-arm themselves: many launches in a row, alternating split
+    factors, all give the same answer as the unsplit kernel up to fp32 summation order."""
+    E, d, f, counts = 3, 512, 1024, [300, 17, 129]
+    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)))
+    base, ref = run_resident_ffn(ctx, E, d, f, counts, seed=21, simt=False, splitk=1)
+    check_float(base, ref)
+    for i, mode in enumerate([0, 4, 2, 0, 7, 16, 3, 0]):
+        got, _ = run_resident_ffn(ctx, E, d, f, counts, seed=21, simt=False, splitk=mode)
+        assert not np.isnan(got).any()
+        check_float(got, ref)
+        assert np.abs(got - base).max() <= 2e-2 * np.abs(ref).max(), (i, mode)
     ctx.close()
 
 
