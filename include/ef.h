@@ -192,6 +192,11 @@ int32_t ef_get_kernel_times(ef_ctx* ctx, ef_kernel_times* out, int32_t reset);
  * K parts (test hook: exercises the partial-sum workspace on small shapes).  Results differ between modes only
  * by fp32 summation order. */
 int32_t ef_set_splitk(ef_ctx* ctx, int32_t mode);
+/* Diagnostic, only in libraries built with -DEF_KPROF (EF_ERR_UNSUPPORTED otherwise): the first call arms the
+ * counters, later calls return, per CTA of the last GEMM1 (which = 1) or GEMM2 (which = 2) launch, the cycles the
+ * MMA-issuing lane spent {in total, waiting for a tile ticket, waiting for the epilogue to free TMEM, waiting for
+ * TMA to fill a stage} and the units it processed.  out: HOST int64[5 * SM count].  Synchronous. */
+int32_t ef_debug_kprof(ef_ctx* ctx, int32_t which, int64_t* out);
 /* 0 = tcgen05 kernels (default); 1 = plain-FMA debug kernels for the grouped FFN (bring-up aid, slow). */
 int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on);
 

@@ -18,7 +18,7 @@ DECLARED_SYMBOLS = [
     "ef_expert_ffn_grouped", "ef_expert_ffn_grouped_resident", "ef_shared_ffn", "ef_combine", "ef_rmsnorm",
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
     "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
-    "ef_get_kernel_times", "ef_set_splitk",
+    "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof",
 ]
 
 
@@ -86,6 +86,7 @@ def load_library() -> ctypes.CDLL:
             "ef_set_debug_simt_ffn": [vp, i32],
             "ef_set_kernel_timing": [vp, i32],
             "ef_set_splitk": [vp, i32],
+            "ef_debug_kprof": [vp, i32, vp],
             "ef_get_kernel_times": [vp, ctypes.POINTER(KernelTimes), i32],
         }
         for name, args in sig.items():
@@ -247,6 +248,11 @@ class EfContext:
 
     def ef_set_splitk(self, mode: int):
         self._chk(self.lib.ef_set_splitk(self.h, int(mode)))
+
+    def ef_debug_kprof(self, which: int, n_sms: int = 148):
+        out = np.zeros((n_sms, 5), np.int64)
+        self._chk(self.lib.ef_debug_kprof(self.h, int(which), out.ctypes.data_as(ctypes.c_void_p)))
+        return out
 
     def ef_set_kernel_timing(self, on: bool):
         self._chk(self.lib.ef_set_kernel_timing(self.h, 1 if on else 0))

@@ -30,6 +30,7 @@ def _newer(src_list, target):
 def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     os.makedirs(OBJ, exist_ok=True)
+    flags = NVCC_FLAGS + (["-DEF_KPROF"] if os.environ.get("EF_KPROF") else [])   # diagnostic build, see ef.h
     srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
     hdrs = sorted(glob.glob(os.path.join(CSRC, "*.h"))) + [os.path.join(ROOT, "include", "ef.h")]
     jobs = []
@@ -37,7 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         o = os.path.join(OBJ, os.path.basename(s)[:-3] + ".o")
         if force or _newer([s] + hdrs, o):
             extra = ["-Xptxas", "-v"] if verbose else []
-            jobs.append(([nvcc] + NVCC_FLAGS + extra + ["-c", s, "-o", o], s))
+            jobs.append(([nvcc] + flags + extra + ["-c", s, "-o", o], s))
 
     def run(job):
         cmd, s = job

@@ -129,6 +129,8 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
     if (ctx->counts_pinned) cudaFreeHost(ctx->counts_pinned);
     if (ctx->sched_words) cudaFree(ctx->sched_words);
     if (ctx->splitk_ws) cudaFree(ctx->splitk_ws);
+    if (ctx->kprof1) cudaFree(ctx->kprof1);
+    if (ctx->kprof2) cudaFree(ctx->kprof2);
     if (ctx->splitk_counters) cudaFree(ctx->splitk_counters);
     if (ctx->h_ws) cudaFree(ctx->h_ws);
     if (ctx->arena) cudaFree(ctx->arena);
@@ -625,6 +627,24 @@ extern "C" int32_t ef_set_splitk(ef_ctx* ctx, int32_t mode) {
     if (mode < 0 || mode > 16) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_splitk: mode must be 0 (auto), 1 (off) or 2..16");
     ctx->splitk_mode = mode;
     return EF_OK;
+}
+
+// Debug builds (-DEF_KPROF) only: per-CTA {total, wait ticket, wait TMEM, wait TMA, units} cycles of the MMA-issuing lane for
+// the last GEMM1 (which = 1) or GEMM2 (which = 2) launch.  out: HOST int64[n_sms * 5].  Synchronous.
+extern "C" int32_t ef_debug_kprof(ef_ctx* ctx, int32_t which, int64_t* out) {
+    EF_CHECK_CTX(ctx);
+#ifdef EF_KPROF
+    if (!out || (which != 1 && which != 2)) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_debug_kprof: bad argument");
+    const size_t bytes = sizeof(long long) * 5 * (size_t)ctx->n_sms;
+    for (long long** p : {&ctx->kprof1, &ctx->kprof2})
+        if (!*p) { EF_CUDA(ctx, cudaMalloc(p, bytes)); EF_CUDA(ctx, cudaMemset(*p, 0, bytes)); }
+    EF_CUDA(ctx, cudaDeviceSynchronize());
+    EF_CUDA(ctx, cudaMemcpy(out, which == 1 ? ctx->kprof1 : ctx->kprof2, bytes, cudaMemcpyDeviceToHost));
+    return EF_OK;
+#else
+    (void)which; (void)out;
+    return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_debug_kprof: library built without -DEF_KPROF");
+#endif
 }
 
 static void drain_kernel_spans(ef_ctx* ctx) {

@@ -92,6 +92,8 @@ struct ef_ctx {
     float* splitk_ws = nullptr;
     int32_t* splitk_counters = nullptr;
     int32_t splitk_max_units = 0;
+    long long* kprof1 = nullptr;        // -DEF_KPROF builds: per-CTA MMA-warp wait cycles of the last GEMM1 / GEMM2 launch
+    long long* kprof2 = nullptr;
     int32_t splitk_mode = 0;            // 0 auto, 1 off, >= 2 force that many K parts on every tile (tests)
     // copy timing
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> copy_spans;

@@ -49,6 +49,14 @@ constexpr int kSched = 4;               // depth of the tile-broadcast ring
 constexpr int kTmemCols = 512;
 constexpr int kSlotFloats = 2 * 128 * 256;   // split-K workspace slot: one 256 x 256 fp32 accumulator pair
 
+// -DEF_KPROF: the MMA-issuing lane of every CTA accumulates the cycles it spends waiting for a tile ticket, for the
+// epilogue to free TMEM and for TMA to fill a stage, and dumps them per CTA (ef_debug_kprof).  Off in normal builds.
+#ifdef EF_KPROF
+#define KPROF(...) __VA_ARGS__
+#else
+#define KPROF(...)
+#endif
+
 struct __align__(8) SmemCtl {
     uint64_t full[kStages];
     uint64_t empty[kStages];
@@ -242,7 +250,8 @@ template <bool kSwiglu>
 __global__ void __launch_bounds__(kThreads, 1)
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                 uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int total_tiles,
-                int32_t* __restrict__ sched, const SplitArgs sp, const __grid_constant__ EfGroupTable tab) {
+                int32_t* __restrict__ sched, const SplitArgs sp, long long* __restrict__ kprof,
+                const __grid_constant__ EfGroupTable tab) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     SmemCtl* ctl = (SmemCtl*)(smem + (size_t)kStages * STAGE_BYTES);
@@ -309,19 +318,27 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
             int buf = 0; uint32_t bphase = 0;          // bit b = phase of accumulator buffer b
+            KPROF(long long kp_t0 = clock64(); long long kp_sched = 0, kp_tmem = 0, kp_full = 0; int kp_units = 0;)
             for (int it = 0;; ++it) {
                 const int ss = it % kSched;
+                KPROF(long long kp_a = clock64();)
                 mbar_wait(&ctl->sched_full[ss], (it / kSched) & 1);
+                KPROF(kp_sched += clock64() - kp_a;)
                 const int tile = ctl->sched_tile[ss];
                 mbar_arrive(&ctl->sched_empty[ss]);
                 if (tile >= total_tiles) break;
+                KPROF(++kp_units;)
                 const Tile t = decode_tile(tab, ctl, tile, sp, KB);
                 if (t.halves == 2) buf = 0;
                 const int b0 = buf;
+                KPROF(long long kp_b = clock64();)
                 for (int h = 0; h < t.halves; ++h) mbar_wait(&ctl->tmem_empty[b0 + h], ((bphase >> (b0 + h)) & 1u) ^ 1u);
+                KPROF(kp_tmem += clock64() - kp_b;)
                 tc_fence_after();
                 for (int kb = t.kb0; kb < t.kb1; ++kb) {
+                    KPROF(long long kp_c = clock64();)
                     mbar_wait(&ctl->full[stage], phase);
+                    KPROF(kp_full += clock64() - kp_c;)
                     tc_fence_after();
                     const uint32_t sa = smem_u32(smem + (size_t)stage * STAGE_BYTES);
                     const uint32_t sb = sa + 2 * A_HALF_BYTES;
@@ -342,6 +359,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 }
                 buf = (t.halves == 2) ? 0 : (b0 ^ 1);
             }
+            KPROF(if (kprof) {
+                long long* o = kprof + (size_t)blockIdx.x * 5;
+                o[0] = clock64() - kp_t0; o[1] = kp_sched; o[2] = kp_tmem; o[3] = kp_full; o[4] = kp_units;
+            })
         }
     } else if (warp >= 4) {
         // ===== epilogue: warps w and w+4 share TMEM lane quarter (w % 4) and split the columns =====
@@ -617,7 +638,7 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         const int grid = std::min(total, ctx->n_sms);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
         ffn_gemm_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn,
-                                                                  total, next_sched(ctx), sp, t1);
+                                                                  total, next_sched(ctx), sp, ctx->kprof1, t1);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
     }
@@ -630,7 +651,7 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         const int grid = std::min(total, ctx->n_sms);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
         ffn_gemm_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_wd, (uint16_t*)y, d, d, f, ntn,
-                                                                   total, next_sched(ctx), sp, t2);
+                                                                   total, next_sched(ctx), sp, ctx->kprof2, t2);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
     }
