@@ -1,35 +1,38 @@
 // a4: grouped SwiGLU expert FFN over cache slots -- tcgen05 / TMEM / TMA kernels for sm_100a.
 //
-// Two launches per wave, both instances of one persistent, warp-specialised grouped GEMM
-//   C[rows_g, N] = A[rows_g, K] . B_slot(g)[N, K]^T      (bf16 x bf16 -> fp32 in TMEM)
-//   GEMM1: A = x_perm, B = packed W13 (gate/up interleaved by 128 rows), epilogue h = silu(g) * u  -> bf16
-//   GEMM2: A = h,      B = Wd,                                           epilogue y               -> bf16
+// Two launches per wave, both instances of one persistent, warp-specialised grouped GEMM, computed TRANSPOSED
+// ("swap-AB"): the weight rows are the MMA M side (always full 128-lane accumulators), the ragged token rows are
+// the MMA N side, whose granularity is 16 -- so an expert with M_e routed rows costs ceil16(M_e) MMA columns, not
+// a multiple of 128 rows (BASELINE.json cfg 2: 4096 routed rows occupy 4144 MMA columns instead of 4608 rows).
+//   D[w, t] = sum_k W_slot(g)[w, k] . A[t, k]          (bf16 x bf16 -> fp32 in TMEM; lanes = weight rows, columns = tokens)
+//   GEMM1: A = x_perm, W = packed W13 (gate/up interleaved by 128 rows): accumulator 0 = 128 gate rows, accumulator 1 =
+//          the matching 128 up rows, same lanes -> epilogue h = silu(g) * u -> bf16
+//   GEMM2: A = h,      W = Wd: accumulators 0 / 1 = output features [256 n, +128) / [256 n + 128, +128) -> bf16 y
 // (PAPER.md L46 leaves e_i opaque; SwiGLU is BASELINE.json's choice, R4.)
 //
-// Tile = up to 256 rows (two 128-lane accumulators "halves") x 256 B-rows, K step 64 (one 128-byte
-// swizzle span).  Per k-step each CTA pulls (128*halves + 256) rows x 128 B through TMA, so a
-// 256-row tile needs 1/3 less L2->SM traffic per flop than a 128-row one; L2 bandwidth, not the
-// tensor pipe, is what bounds a plain 128x256 tiling.
+// Tile = 256 weight rows x up to 256 tokens, K step 64 (one 128-byte swizzle span).  Per k-step a CTA pulls one
+// 64 x 256 weight box and ceil(n/64) 64 x 64 token boxes through TMA; 3 stages of 64 KB.  Tokens past the end of
+// the group are loaded and multiplied (their columns are never stored), rows past the tensor are zero-filled.
 //
 // Warp roles (384 threads, 1 CTA/SM, persistent):
-//   warp 0     TMA producer + tile scheduler : claims the next tile with one atomicAdd on a per-launch counter,
-//                                broadcasts it to the other roles through a 4-deep smem ring guarded by mbarriers,
-//                                then issues A boxes (64 x 128 rows, one per half) + B box (64 x 256 rows) per stage
-//   warp 1     MMA issuer        : one lane issues tcgen05.mma (M128 N256 K16), commits to mbarriers
-//   warp 2     TMEM allocator    : 512 columns = two 128x256 fp32 accumulator buffers
-//   warps 4-11 epilogue          : tcgen05.ld -> registers -> SwiGLU / cast -> 64-byte global stores; warps w and w+4
-//                                share a TMEM lane quarter and split the columns
-// Per-expert tile scheduling over ragged token counts: tiles are numbered longest-first -- every 256-row tile of
-// every group (n-major inside a group, so the M-tiles that share a weight tile are claimed back to back and hit L2),
-// then the short (<= 128-row) tail tiles -- and claimed dynamically, i.e. greedy longest-processing-time list
-// scheduling: the makespan is within one short tile of the mean load whatever the row counts are.
+//   warp 0     TMA producer + tile scheduler : claims the next unit with one atomicAdd on a per-launch counter,
+//                                broadcasts it to the other roles through a 4-deep smem ring guarded by mbarriers
+//   warp 1     MMA issuer        : one lane issues tcgen05.mma (M128 N<=256 K16) twice per k-step (one per
+//                                accumulator, same token operand), commits to mbarriers
+//   warp 2     TMEM allocator    : 512 columns.  A tile with > 128 tokens takes all of them (accumulators at columns
+//                                0 and 256); tiles with <= 128 tokens alternate between the two 256-column halves
+//                                (accumulators at +0 and +128), so their epilogue overlaps the next tile's MMAs
+//   warps 4-11 epilogue          : tcgen05.ld (32 lanes x 32 token columns) -> registers -> SwiGLU / cast -> one 2-byte
+//                                store per token, 64 contiguous bytes per warp; warps w and w+4 share a TMEM lane
+//                                quarter and take alternate 32-token chunks
+// Per-expert tile scheduling over ragged token counts: units are numbered longest-first -- every > 128-token tile
+// of every group (n-major inside a group, so the token tiles that share a weight tile are claimed back to back and
+// hit L2), then the <= 128-token tail tiles -- and claimed dynamically (greedy list scheduling).
 // Tail split-K: with T tiles on G SMs the last T mod G tiles (all of them when T < G -- decode, single-expert miss
 // waves) would leave most SMs idle for a whole tile time, so the host splits each of those tiles s ways along K.
-// A split unit writes its raw fp32 accumulator to a workspace slot, then bumps the tile's arrival counter; the
+// A split unit writes its raw fp32 accumulators to a workspace slot, then bumps the tile's arrival counter; the
 // unit that arrives last sums the s partials in split order (deterministic) and runs the normal epilogue.  No
 // CTA ever waits for another one.
-// Ragged M: a group's last tile may be short; TMA zero-fills rows past the tensor, rows past the
-// group are computed and discarded (stores are row-predicated), so neighbours are never touched.
 #include <cuda_bf16.h>
 
 #include "ef_internal.h"
@@ -37,17 +40,23 @@
 namespace {
 
 constexpr int BK = 64;                 // K elements per stage (128 bytes of bf16)
-constexpr int BN = 256;                // B rows per tile
-constexpr int HALF_M = 128;            // rows per accumulator half
+constexpr int BW = 256;                // weight rows per tile (two 128-lane accumulators)
+constexpr int ACC_M = 128;             // weight rows per accumulator
+constexpr int BT = 256;                // max tokens per tile
+constexpr int XBOX = 64;               // token rows per TMA box
 constexpr int kStages = 3;
-constexpr int A_HALF_BYTES = HALF_M * BK * 2;   // 16 KB
-constexpr int B_BYTES = BN * BK * 2;            // 32 KB
-constexpr int STAGE_BYTES = 2 * A_HALF_BYTES + B_BYTES;   // 64 KB
+constexpr int W_BYTES = BW * BK * 2;              // 32 KB
+constexpr int XBOX_BYTES = XBOX * BK * 2;         // 8 KB
+constexpr int STAGE_BYTES = W_BYTES + BT * BK * 2;   // 64 KB
 constexpr int kThreads = 384;
 constexpr int kEpiWarps = 8;
 constexpr int kSched = 4;               // depth of the tile-broadcast ring
 constexpr int kTmemCols = 512;
-constexpr int kSlotFloats = 2 * 128 * 256;   // split-K workspace slot: one 256 x 256 fp32 accumulator pair
+constexpr int kSlotFloats = 2 * 128 * 256;   // split-K workspace slot: two 128-lane x 256-column fp32 accumulators
+// Epilogue staging (transpose): per column-parity group of 4 warps one [32 tokens][128 features] bf16 tile, rows
+// padded by 16 B so that stmatrix rows (stride 272 B) and 16-byte read-backs are bank-conflict free
+constexpr int STG_LD = ACC_M * 2 + 16;
+constexpr int STG_BYTES = 32 * STG_LD;
 
 // -DEF_KPROF: the MMA-issuing lane of every CTA accumulates the cycles it spends waiting for a tile ticket, for the
 // epilogue to free TMEM and for TMA to fill a stage, and dumps them per CTA (ef_debug_kprof).  Off in normal builds.
@@ -67,12 +76,12 @@ struct __align__(8) SmemCtl {
     int32_t sched_tile[kSched];
     uint32_t tmem_base;
     int32_t split_last;                   // epilogue broadcast: this unit arrived last at its split tile
-    int32_t total_long;                   // number of 2-half tiles (they come first)
+    int32_t total_long;                   // number of > 128-token tiles (they come first)
     int32_t gstart_long[EF_MAX_GROUPS + 1];
     int32_t gstart_short[EF_MAX_GROUPS + 1];
 };
 
-constexpr size_t kSmemBytes = 1024 /*align slack*/ + (size_t)kStages * STAGE_BYTES + sizeof(SmemCtl);
+constexpr size_t kSmemBytes = 1024 /*align slack*/ + (size_t)kStages * STAGE_BYTES + 2 * STG_BYTES + sizeof(SmemCtl);
 
 // ---- PTX wrappers ----------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -112,7 +121,7 @@ __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::
 __device__ __forceinline__ void tc_commit(uint64_t* bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-// D[tmem] (+)= A[smem] . B[smem]^T, M128 N256 K16, bf16 -> fp32
+// D[tmem] (+)= A[smem] . B[smem]^T, M128 N(idesc) K16, bf16 -> fp32
 __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
     asm volatile(
         "{\n"
@@ -138,63 +147,101 @@ __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sy
 __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
 }
-// kind::f16 instruction descriptor: D fp32, A/B bf16, both K-major, N=256, M=128
-constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(HALF_M >> 4) << 24);
+// kind::f16 instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N = n (multiple of 16, 16..256)
+__device__ __forceinline__ uint32_t make_idesc(int n) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(ACC_M >> 4) << 24);
+}
 
+__device__ __forceinline__ uint16_t bf16_bits(float v) {
+    __nv_bfloat16 b = __float2bfloat16_rn(v);
+    return *reinterpret_cast<uint16_t*>(&b);
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
     return *reinterpret_cast<uint32_t*>(&v);
 }
+// silu(g) * u with one MUFU op: g * sigmoid(g) = 0.5 g (1 + tanh(g / 2)); tanh.approx has ~2^-11 relative error,
+// a quarter of the bf16 rounding that follows
+__device__ __forceinline__ float silu_mul(float g, float u) {
+    float th;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(0.5f * g));
+    const float hg = 0.5f * g;
+    return fmaf(hg, th, hg) * u;
+}
+// 16 TMEM lanes x 32 columns: thread T gets lane T/4 (regs 4j, 4j+1) and lane T/4 + 8 (regs 4j+2, 4j+3), columns
+// 8j + 2(T%4) + {0, 1} -- the MMA C-fragment layout, which is what stmatrix consumes
+__device__ __forceinline__ void tc_ld16x256b_x4(uint32_t taddr, uint32_t* v) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.16x256b.x4.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr));
+}
+// four 8x8 bf16 blocks, transposed on the way: smem row (16 B at the address thread 8i + r supplies for block i,
+// row r) = one token, its 8 entries = the 8 TMEM lanes (features) of the block
+__device__ __forceinline__ void stmatrix_x4_trans(uint32_t saddr, uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3) {
+    asm volatile("stmatrix.sync.aligned.m8n8.x4.trans.shared.b16 [%0], {%1, %2, %3, %4};" ::"r"(saddr), "r"(r0), "r"(r1), "r"(r2), "r"(r3)
+                 : "memory");
+}
+__device__ __forceinline__ void named_bar(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
-// 32 accumulator columns of one row -> bf16, four 16-byte stores
-__device__ __forceinline__ void store_plain32(uint16_t* dst, const uint32_t (&v)[32]) {
-    uint32_t o[16];
+// The 4 warps of one column-parity group write the staged [32 tokens][128 features] tile to C with 16-byte stores
+// (a half-warp covers the 256 contiguous bytes of one token row).  Barriers: staging complete / staging free again.
+__device__ __forceinline__ void stage_to_global(const uint8_t* stg, uint16_t* __restrict__ C, int ldc, int64_t row0, int n_rows,
+                                                int col0, int n_cols, int tid128, int bar_id) {
+    named_bar(bar_id, 128);
+    const int ch = tid128 & 15;
+    if (col0 + ch * 8 < n_cols) {
 #pragma unroll
-    for (int i = 0; i < 16; ++i) o[i] = pack_bf16(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
-    uint4* d4 = reinterpret_cast<uint4*>(dst);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) d4[i] = make_uint4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
-}
-// h = silu(g) * u for 32 columns of one row
-__device__ __forceinline__ void store_swiglu32(uint16_t* dst, const uint32_t (&g)[32], const uint32_t (&u)[32]) {
-    uint32_t o[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        const float g0 = __uint_as_float(g[2 * i]), g1 = __uint_as_float(g[2 * i + 1]);
-        const float u0 = __uint_as_float(u[2 * i]), u1 = __uint_as_float(u[2 * i + 1]);
-        const float h0 = __fdividef(g0, 1.f + __expf(-g0)) * u0;
-        const float h1 = __fdividef(g1, 1.f + __expf(-g1)) * u1;
-        o[i] = pack_bf16(h0, h1);
+        for (int p = 0; p < 4; ++p) {
+            const int row = p * 8 + (tid128 >> 4);
+            if (row < n_rows) {
+                const uint4 v = *reinterpret_cast<const uint4*>(stg + row * STG_LD + ch * 16);
+                *reinterpret_cast<uint4*>(C + (row0 + row) * ldc + col0 + ch * 8) = v;
+            }
+        }
     }
-    uint4* d4 = reinterpret_cast<uint4*>(dst);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) d4[i] = make_uint4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
+    named_bar(bar_id, 128);
 }
-// split-K reduction: 32 columns (chunk c) of this thread's row, summed over the s partial slots in slot order.
-// rrow points at this row's float4 in slot 0; L2-only loads (the partials were written by other SMs).
-__device__ __forceinline__ void sum_partials32(const float4* rrow, int c, int s, uint32_t (&out)[32]) {
-    float4 acc[8];
+
+// split-K workspace slot layout: [accumulator][column / 4][lane][4 floats] -- a warp's float4 accesses are contiguous
+__device__ __forceinline__ void ws_store32(float* slot, int acc, int c, int lane128, const uint32_t (&v)[32]) {
+    float4* p = reinterpret_cast<float4*>(slot) + (size_t)acc * (ACC_M * BT / 4) + (size_t)(c * 8) * ACC_M + lane128;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) acc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int i = 0; i < 8; ++i)
+        p[(size_t)i * ACC_M] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
+                                           __uint_as_float(v[4 * i + 3]));
+}
+// sum over the s partial slots of a tile, in slot order; L2-only loads (the partials were written by other SMs)
+__device__ __forceinline__ void ws_sum32(const float* tile_slots, int s, int acc, int c, int lane128, uint32_t (&out)[32]) {
+    float4 sum[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) sum[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4* p = reinterpret_cast<const float4*>(tile_slots) + (size_t)acc * (ACC_M * BT / 4) + (size_t)(c * 8) * ACC_M + lane128;
     for (int j = 0; j < s; ++j) {
-        const float4* p = rrow + (size_t)j * (kSlotFloats / 4) + (size_t)(c * 8) * 128;
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
-            const float4 v = __ldcg(p + (size_t)i * 128);
-            acc[i].x += v.x; acc[i].y += v.y; acc[i].z += v.z; acc[i].w += v.w;
+            const float4 v = __ldcg(p + (size_t)i * ACC_M);
+            sum[i].x += v.x; sum[i].y += v.y; sum[i].z += v.z; sum[i].w += v.w;
         }
+        p += kSlotFloats / 4;
     }
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
-        out[4 * i] = __float_as_uint(acc[i].x); out[4 * i + 1] = __float_as_uint(acc[i].y);
-        out[4 * i + 2] = __float_as_uint(acc[i].z); out[4 * i + 3] = __float_as_uint(acc[i].w);
+        out[4 * i] = __float_as_uint(sum[i].x); out[4 * i + 1] = __float_as_uint(sum[i].y);
+        out[4 * i + 2] = __float_as_uint(sum[i].z); out[4 * i + 3] = __float_as_uint(sum[i].w);
     }
 }
 // barrier among the 8 epilogue warps only
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 
 struct Tile {
-    int a_row, c_row, rows_valid, halves, n_tile, slot;
+    int a_row, c_row;    // first token row in the A tensor / in the output
+    int rows_valid;      // tokens of this tile (1..256)
+    int n_mma;           // rows_valid rounded up to the MMA N granularity (16)
+    int is_long;         // > 128 tokens: takes the whole TMEM
+    int n_tile, slot;
     int kb0, kb1;        // k-block range of this unit
     int tail, split_j;   // index among the split tiles (-1: whole tile) and which K part this unit is
 };
@@ -206,9 +253,9 @@ struct SplitArgs {
     int32_t* counters;   // [n_split_tiles] arrival counters, zero between launches
 };
 
-// number of 2-half ("long", 129..256 rows) tiles of a group; the remainder, if any, is one short tile per n
-__device__ __host__ __forceinline__ int group_long_tiles(int rows) { return rows / (2 * 128) + ((rows % (2 * 128)) > 128 ? 1 : 0); }
-__device__ __host__ __forceinline__ int group_has_short(int rows) { int r = rows % (2 * 128); return (r > 0 && r <= 128) ? 1 : 0; }
+// number of "long" (129..256-token) tiles of a group; the remainder, if any, is one short tile per n
+__device__ __host__ __forceinline__ int group_long_tiles(int rows) { return rows / BT + ((rows % BT) > 128 ? 1 : 0); }
+__device__ __host__ __forceinline__ int group_has_short(int rows) { int r = rows % BT; return (r > 0 && r <= 128) ? 1 : 0; }
 
 __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemCtl* ctl, int unit, const SplitArgs& sp,
                                             int KB) {
@@ -229,37 +276,40 @@ __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemC
         const int local = tile - ctl->gstart_long[g];
         const int nl = group_long_tiles(tab.g[g].rows);
         t.n_tile = local / nl;
-        row_off = (local % nl) * (2 * HALF_M);
-        t.halves = 2;
+        row_off = (local % nl) * BT;
+        t.is_long = 1;
     } else {
         const int ts = tile - ctl->total_long;
         while (ts >= ctl->gstart_short[g + 1]) ++g;
         t.n_tile = ts - ctl->gstart_short[g];
-        row_off = group_long_tiles(tab.g[g].rows) * (2 * HALF_M);
-        t.halves = 1;
+        row_off = group_long_tiles(tab.g[g].rows) * BT;
+        t.is_long = 0;
     }
-    t.rows_valid = min(tab.g[g].rows - row_off, HALF_M * t.halves);
+    t.rows_valid = min(tab.g[g].rows - row_off, BT);
+    t.n_mma = (t.rows_valid + 15) & ~15;
     t.a_row = tab.g[g].a_row0 + row_off;
     t.c_row = tab.g[g].c_row0 + row_off;
     t.slot = tab.g[g].slot;
     return t;
 }
 
-// kSwiglu: accumulator columns [0,128) = gate, [128,256) = up for 128 output columns; else 256 output columns
+// kSwiglu: accumulator 0 = 128 gate rows, accumulator 1 = the matching up rows -> 128 output columns per tile;
+// else accumulators 0 / 1 = output columns [256 n, +128) / [256 n + 128, +128)
 template <bool kSwiglu>
 __global__ void __launch_bounds__(kThreads, 1)
-ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmW,
                 uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int total_tiles,
                 int32_t* __restrict__ sched, const SplitArgs sp, long long* __restrict__ kprof,
                 const __grid_constant__ EfGroupTable tab) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    SmemCtl* ctl = (SmemCtl*)(smem + (size_t)kStages * STAGE_BYTES);
+    uint8_t* stg_base = smem + (size_t)kStages * STAGE_BYTES;
+    SmemCtl* ctl = (SmemCtl*)(stg_base + 2 * STG_BYTES);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     if (warp == 0 && lane == 0) {
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmX) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmW) : "memory");
     }
     if (warp == 1 && lane == 0) {
         for (int i = 0; i < kStages; ++i) { mbar_init(&ctl->full[i], 1); mbar_init(&ctl->empty[i], 1); }
@@ -301,14 +351,15 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 mbar_arrive(&ctl->sched_full[ss]);          // release: the tile index is visible to the waiters
                 if (tile >= total_tiles) break;
                 const Tile t = decode_tile(tab, ctl, tile, sp, KB);
-                const uint32_t bytes = (uint32_t)(t.halves * A_HALF_BYTES + B_BYTES);
+                const int n_box = (t.n_mma + XBOX - 1) / XBOX;
+                const uint32_t bytes = (uint32_t)(W_BYTES + n_box * XBOX_BYTES);
                 for (int kb = t.kb0; kb < t.kb1; ++kb) {
                     mbar_wait(&ctl->empty[stage], phase ^ 1);
-                    uint8_t* sa = smem + (size_t)stage * STAGE_BYTES;
+                    uint8_t* sw = smem + (size_t)stage * STAGE_BYTES;
                     mbar_expect_tx(&ctl->full[stage], bytes);
-                    tma_load_2d(sa, &tmA, &ctl->full[stage], kb * BK, t.a_row);
-                    if (t.halves == 2) tma_load_2d(sa + A_HALF_BYTES, &tmA, &ctl->full[stage], kb * BK, t.a_row + HALF_M);
-                    tma_load_3d(sa + 2 * A_HALF_BYTES, &tmB, &ctl->full[stage], kb * BK, t.n_tile * BN, t.slot);
+                    tma_load_3d(sw, &tmW, &ctl->full[stage], kb * BK, t.n_tile * BW, t.slot);
+                    for (int j = 0; j < n_box; ++j)
+                        tma_load_2d(sw + W_BYTES + j * XBOX_BYTES, &tmX, &ctl->full[stage], kb * BK, t.a_row + j * XBOX);
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
@@ -317,7 +368,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         // ===== MMA issuer =====
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
-            int buf = 0; uint32_t bphase = 0;          // bit b = phase of accumulator buffer b
+            int buf = 0; uint32_t bphase = 0;          // bit b = phase of TMEM half b
             KPROF(long long kp_t0 = clock64(); long long kp_sched = 0, kp_tmem = 0, kp_full = 0; int kp_units = 0;)
             for (int it = 0;; ++it) {
                 const int ss = it % kSched;
@@ -329,35 +380,36 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 if (tile >= total_tiles) break;
                 KPROF(++kp_units;)
                 const Tile t = decode_tile(tab, ctl, tile, sp, KB);
-                if (t.halves == 2) buf = 0;
-                const int b0 = buf;
+                const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
                 KPROF(long long kp_b = clock64();)
-                for (int h = 0; h < t.halves; ++h) mbar_wait(&ctl->tmem_empty[b0 + h], ((bphase >> (b0 + h)) & 1u) ^ 1u);
+                for (int h = 0; h < nb; ++h) mbar_wait(&ctl->tmem_empty[b0 + h], ((bphase >> (b0 + h)) & 1u) ^ 1u);
                 KPROF(kp_tmem += clock64() - kp_b;)
                 tc_fence_after();
+                const uint32_t d0 = tmem_base + (uint32_t)(b0 * 256);
+                const uint32_t d1 = d0 + (t.is_long ? 256u : 128u);
+                const uint32_t idesc = make_idesc(t.n_mma);
                 for (int kb = t.kb0; kb < t.kb1; ++kb) {
                     KPROF(long long kp_c = clock64();)
                     mbar_wait(&ctl->full[stage], phase);
                     KPROF(kp_full += clock64() - kp_c;)
                     tc_fence_after();
-                    const uint32_t sa = smem_u32(smem + (size_t)stage * STAGE_BYTES);
-                    const uint32_t sb = sa + 2 * A_HALF_BYTES;
+                    const uint32_t sw = smem_u32(smem + (size_t)stage * STAGE_BYTES);
+                    const uint32_t sx = sw + W_BYTES;
 #pragma unroll
                     for (int k = 0; k < BK / 16; ++k) {
-                        const uint64_t bd = smem_desc(sb + k * 32);
+                        const uint64_t xd = smem_desc(sx + k * 32);
                         const uint32_t acc = (kb > t.kb0 || k > 0) ? 1u : 0u;
-                        tc_mma(tmem_base + (uint32_t)(b0 * BN), smem_desc(sa + k * 32), bd, kIdesc, acc);
-                        if (t.halves == 2)
-                            tc_mma(tmem_base + (uint32_t)((b0 + 1) * BN), smem_desc(sa + A_HALF_BYTES + k * 32), bd, kIdesc, acc);
+                        tc_mma(d0, smem_desc(sw + k * 32), xd, idesc, acc);
+                        tc_mma(d1, smem_desc(sw + ACC_M * BK * 2 + k * 32), xd, idesc, acc);
                     }
                     tc_commit(&ctl->empty[stage]);    // frees the smem stage once these MMAs have read it
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
-                for (int h = 0; h < t.halves; ++h) {
+                for (int h = 0; h < nb; ++h) {
                     tc_commit(&ctl->tmem_full[b0 + h]);
                     bphase ^= 1u << (b0 + h);
                 }
-                buf = (t.halves == 2) ? 0 : (b0 ^ 1);
+                buf = t.is_long ? 0 : (b0 ^ 1);
             }
             KPROF(if (kprof) {
                 long long* o = kprof + (size_t)blockIdx.x * 5;
@@ -365,9 +417,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             })
         }
     } else if (warp >= 4) {
-        // ===== epilogue: warps w and w+4 share TMEM lane quarter (w % 4) and split the columns =====
+        // ===== epilogue: warps w and w+4 share TMEM lane quarter (w % 4) and take alternate 32-token chunks =====
         const int q = warp & 3;
-        const int part = (warp - 4) >> 2;            // 0: first half of the column chunks, 1: second half
+        const int part = (warp - 4) >> 2;
+        const int lane128 = q * 32 + lane;            // accumulator lane = weight row inside the 128-row block
         int buf = 0; uint32_t bphase = 0;
         for (int it = 0;; ++it) {
             const int ss = it % kSched;
@@ -377,65 +430,68 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             if (lane == 0) mbar_arrive(&ctl->sched_empty[ss]);
             if (tile >= total_tiles) break;
             const Tile t = decode_tile(tab, ctl, tile, sp, KB);
-            if (t.halves == 2) buf = 0;
-            const int b0 = buf;
+            const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
             const bool split = t.tail >= 0;
-            // fp32 workspace of this unit: [half][col/4][row in half][4 floats] -- a warp's float4 stores are contiguous
             float* ws_mine = split ? sp.ws + ((size_t)t.tail * sp.s + t.split_j) * kSlotFloats : nullptr;
-            for (int h = 0; h < t.halves; ++h) {
-                const int b = b0 + h;
-                mbar_wait(&ctl->tmem_full[b], (bphase >> b) & 1u);
-                bphase ^= 1u << b;
-                tc_fence_after();
-                const int r = h * HALF_M + q * 32 + lane;            // row inside the tile
-                const bool row_ok = r < t.rows_valid;
-                const bool warp_ok = (h * HALF_M + q * 32) < t.rows_valid;
-                const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b * BN);
-                if (warp_ok && split) {
-                    // raw accumulator chunks of 32 columns -> workspace (the finalising unit applies the epilogue)
-                    float4* wrow = reinterpret_cast<float4*>(ws_mine) + (size_t)h * (HALF_M * BN / 4) + (q * 32 + lane);
+            for (int h = 0; h < nb; ++h) {
+                mbar_wait(&ctl->tmem_full[b0 + h], (bphase >> (b0 + h)) & 1u);
+                bphase ^= 1u << (b0 + h);
+            }
+            tc_fence_after();
+            const uint32_t tb0 = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b0 * 256);
+            const uint32_t tb1 = tb0 + (t.is_long ? 256u : 128u);
+            const int n_chunks = (t.rows_valid + 31) >> 5;
+            const int col0 = kSwiglu ? t.n_tile * ACC_M : t.n_tile * BW;      // first output column of accumulator 0
+            uint8_t* stg = stg_base + part * STG_BYTES;
+            // stmatrix row address of this thread: block i = lane / 8 (tokens 8i..8i+7), row lane % 8, + feature offset
+            const uint32_t st_row = smem_u32(stg) + (uint32_t)(((lane >> 3) * 8 + (lane & 7)) * STG_LD + q * 64);
 #pragma unroll 1
-                    for (int cc = 0; cc < 4; ++cc) {
-                        const int c = kSwiglu ? ((cc & 1) * 4 + part * 2 + (cc >> 1)) : (part * 4 + cc);
-                        if (!kSwiglu && t.n_tile * BN + c * 32 >= n_cols) break;
-                        uint32_t v[32];
-                        tc_ld32(tbase + c * 32, v);
-                        tc_wait_ld();
-                        if (row_ok) {
+            for (int c = part; c < n_chunks; c += 2) {
+                const int n_rows = min(32, t.rows_valid - c * 32);
+                if (split) {
+                    uint32_t a0[32];
+                    tc_ld32(tb0 + c * 32, a0);
+                    tc_wait_ld();
+                    ws_store32(ws_mine, 0, c, lane128, a0);
+                    tc_ld32(tb1 + c * 32, a0);
+                    tc_wait_ld();
+                    ws_store32(ws_mine, 1, c, lane128, a0);
+                    continue;
+                }
+#pragma unroll 1
+                for (int acc = 0; acc < (kSwiglu ? 1 : 2); ++acc) {
+#pragma unroll
+                    for (int hh = 0; hh < 2; ++hh) {
+                        const uint32_t lane_off = (uint32_t)(hh * 16) << 16;
+                        uint32_t r[8];
+                        if (kSwiglu) {
+                            uint32_t g[16], u[16];
+                            tc_ld16x256b_x4(tb0 + lane_off + c * 32, g);
+                            tc_ld16x256b_x4(tb1 + lane_off + c * 32, u);
+                            tc_wait_ld();
 #pragma unroll
                             for (int i = 0; i < 8; ++i)
-                                wrow[(size_t)(c * 8 + i) * HALF_M] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
-                                                                                 __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
-                        }
-                    }
-                } else if (warp_ok) {
-                    if (kSwiglu) {
-                        uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * 128;
-#pragma unroll 1
-                        for (int c = part * 2; c < part * 2 + 2; ++c) {
-                            uint32_t g[32], u[32];
-                            tc_ld32(tbase + c * 32, g);
-                            tc_ld32(tbase + 128 + c * 32, u);
+                                r[i] = pack_bf16(silu_mul(__uint_as_float(g[2 * i]), __uint_as_float(u[2 * i])),
+                                                 silu_mul(__uint_as_float(g[2 * i + 1]), __uint_as_float(u[2 * i + 1])));
+                        } else {
+                            uint32_t v[16];
+                            tc_ld16x256b_x4((acc ? tb1 : tb0) + lane_off + c * 32, v);
                             tc_wait_ld();
-                            if (row_ok) store_swiglu32(crow + c * 32, g, u);
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) r[i] = pack_bf16(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
                         }
-                    } else {
-                        uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * BN;
-#pragma unroll 1
-                        for (int c = part * 4; c < part * 4 + 4; ++c) {
-                            if (t.n_tile * BN + c * 32 >= n_cols) break;     // N tail (n_cols % 64 == 0)
-                            uint32_t v[32];
-                            tc_ld32(tbase + c * 32, v);
-                            tc_wait_ld();
-                            if (row_ok) store_plain32(crow + c * 32, v);
-                        }
+                        // r[2j] = lanes 0-7 of this half, r[2j+1] = lanes 8-15; token block j
+                        stmatrix_x4_trans(st_row + hh * 32, r[0], r[2], r[4], r[6]);
+                        stmatrix_x4_trans(st_row + hh * 32 + 16, r[1], r[3], r[5], r[7]);
                     }
+                    stage_to_global(stg, C, ldc, (int64_t)t.c_row + c * 32, n_rows, col0 + acc * ACC_M, n_cols, lane128, 2 + part);
                 }
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&ctl->tmem_empty[b]);
             }
-            buf = (t.halves == 2) ? 0 : (b0 ^ 1);
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0)
+                for (int h = 0; h < nb; ++h) mbar_arrive(&ctl->tmem_empty[b0 + h]);
+            buf = t.is_long ? 0 : (b0 ^ 1);
             if (split) {
                 // publish the partial, count arrivals; the last unit of the tile reduces all s partials in split order
                 __threadfence();
@@ -451,28 +507,22 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 if (last) {
                     __threadfence();
                     const float* ws_tile = sp.ws + (size_t)t.tail * sp.s * kSlotFloats;
-                    for (int h = 0; h < t.halves; ++h) {
-                        const int r = h * HALF_M + q * 32 + lane;
-                        if (r >= t.rows_valid) continue;
-                        const float4* rrow = reinterpret_cast<const float4*>(ws_tile) + (size_t)h * (HALF_M * BN / 4) + (q * 32 + lane);
-                        if (kSwiglu) {
-                            uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * 128;
 #pragma unroll 1
-                            for (int c = part * 2; c < part * 2 + 2; ++c) {
-                                uint32_t g[32], u[32];
-                                sum_partials32(rrow, c, sp.s, g);
-                                sum_partials32(rrow, c + 4, sp.s, u);
-                                store_swiglu32(crow + c * 32, g, u);
-                            }
-                        } else {
-                            uint16_t* crow = C + (int64_t)(t.c_row + r) * ldc + (int64_t)t.n_tile * BN;
+                    for (int c = part; c < n_chunks; c += 2) {
+                        const int n_rows = min(32, t.rows_valid - c * 32);
+                        uint32_t a0[32], a1[32];
+                        ws_sum32(ws_tile, sp.s, 0, c, lane128, a0);
+                        ws_sum32(ws_tile, sp.s, 1, c, lane128, a1);
+                        uint16_t* srow = reinterpret_cast<uint16_t*>(stg) + lane128;       // [token][feature], 2-byte stores
 #pragma unroll 1
-                            for (int c = part * 4; c < part * 4 + 4; ++c) {
-                                if (t.n_tile * BN + c * 32 >= n_cols) break;
-                                uint32_t v[32];
-                                sum_partials32(rrow, c, sp.s, v);
-                                store_plain32(crow + c * 32, v);
+                        for (int acc = 0; acc < (kSwiglu ? 1 : 2); ++acc) {
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) {
+                                const float v = kSwiglu ? silu_mul(__uint_as_float(a0[i]), __uint_as_float(a1[i]))
+                                                        : __uint_as_float(acc ? a1[i] : a0[i]);
+                                srow[i * (STG_LD / 2)] = bf16_bits(v);
                             }
+                            stage_to_global(stg, C, ldc, (int64_t)t.c_row + c * 32, n_rows, col0 + acc * ACC_M, n_cols, lane128, 2 + part);
                         }
                     }
                 }
@@ -511,13 +561,13 @@ EncodeTiledFn get_encode() {
     return fn;
 }
 
-// 2-D bf16 [rows, K] row-major, box 64 x 128, 128-byte swizzle
+// 2-D bf16 [rows, K] row-major, box 64 x 64 token rows, 128-byte swizzle
 int32_t make_map_2d(ef_ctx* ctx, CUtensorMap* tm, const void* base, int64_t rows, int64_t K) {
     EncodeTiledFn enc = get_encode();
     if (!enc) return ef_fail(ctx, EF_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
     cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
     cuuint64_t strides[1] = {(cuuint64_t)K * 2};
-    cuuint32_t box[2] = {BK, HALF_M};
+    cuuint32_t box[2] = {BK, XBOX};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -532,7 +582,7 @@ int32_t make_map_arena(ef_ctx* ctx, CUtensorMap* tm, const void* base, int64_t r
     if (!enc) return ef_fail(ctx, EF_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
     cuuint64_t dims[3] = {(cuuint64_t)K, (cuuint64_t)rows, (cuuint64_t)ctx->n_arena_slots};
     cuuint64_t strides[2] = {(cuuint64_t)K * 2, (cuuint64_t)ctx->W};
-    cuuint32_t box[3] = {BK, BN, 1};
+    cuuint32_t box[3] = {BK, BW, 1};
     cuuint32_t estr[3] = {1, 1, 1};
     CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -644,7 +694,7 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     }
     if (ctx->time_kernels) EF_CUDA(ctx, cudaEventRecord(span.e1, st));
     {
-        const int ntn = (d + BN - 1) / BN;
+        const int ntn = (d + BW - 1) / BW;
         const int tiles = mtiles * ntn;
         const SplitPlan pl = plan_split(ctx, tiles, mshort * ntn, ctx->n_sms, f / BK, (double)rows_total / mtiles);
         const int total = pl.n_plain + pl.n_tail * pl.s;
