@@ -10,29 +10,37 @@
 //   GEMM2: A = h,      W = Wd: accumulators 0 / 1 = output features [256 n, +128) / [256 n + 128, +128) -> bf16 y
 // (PAPER.md L46 leaves e_i opaque; SwiGLU is BASELINE.json's choice, R4.)
 //
-// Tile = 256 weight rows x up to 256 tokens, K step 64 (one 128-byte swizzle span).  Per k-step a CTA pulls one
-// 64 x 256 weight box and ceil(n/64) 64 x 64 token boxes through TMA; 3 stages of 64 KB.  Tokens past the end of
-// the group are loaded and multiplied (their columns are never stored), rows past the tensor are zero-filled.
+// CTA pairs (cta_group::2): the two CTAs of a cluster work on the same token tile and on two adjacent 256-row weight
+// tiles.  Each CTA loads its own weight tile (M side, 128 + 128 rows for its two accumulators) and HALF of the token
+// tile (N side); one tcgen05.mma.cta_group::2 (M256 N<=256 K16) per accumulator, issued by the leader CTA, reads both
+// halves, so the token operand is fetched from L2 and staged in shared memory once per pair.  Per k-step (K = 64) a
+// CTA therefore pulls 32 KB of weights + <= 16 KB of tokens for 2 * n/2 * 4 tensor cycles -- 48 B/cycle at n = 256
+// against 64 for a single-CTA 256 x 256 tile -- and a stage is 48 KB, which buys a 4th pipeline stage.
+// Tokens past the end of the group are loaded and multiplied (their columns are never stored), rows past the tensor
+// are zero-filled by TMA.
 //
-// Warp roles (384 threads, 1 CTA/SM, persistent):
-//   warp 0     TMA producer + tile scheduler : claims the next unit with one atomicAdd on a per-launch counter,
-//                                broadcasts it to the other roles through a 4-deep smem ring guarded by mbarriers
-//   warp 1     MMA issuer        : one lane issues tcgen05.mma (M128 N<=256 K16) twice per k-step (one per
-//                                accumulator, same token operand), commits to mbarriers
-//   warp 2     TMEM allocator    : 512 columns.  A tile with > 128 tokens takes all of them (accumulators at columns
-//                                0 and 256); tiles with <= 128 tokens alternate between the two 256-column halves
-//                                (accumulators at +0 and +128), so their epilogue overlaps the next tile's MMAs
-//   warps 4-11 epilogue          : tcgen05.ld (32 lanes x 32 token columns) -> registers -> SwiGLU / cast -> one 2-byte
-//                                store per token, 64 contiguous bytes per warp; warps w and w+4 share a TMEM lane
-//                                quarter and take alternate 32-token chunks
+// Warp roles (384 threads, 1 CTA/SM, persistent; both CTAs unless stated):
+//   warp 0     TMA producer + tile scheduler : the LEADER claims the next unit with one atomicAdd on a per-launch
+//                                counter and hands it to both CTAs' roles through 4-deep smem rings (remote store +
+//                                remote mbarrier arrive for the peer); each CTA's producer then issues its own boxes,
+//                                all completing on the leader's "full" barrier
+//   warp 1     MMA issuer (leader only) : one lane issues the two MMAs per k-step; tcgen05.commit multicasts the
+//                                "stage free" / "accumulator ready" arrivals to both CTAs
+//   warp 2     TMEM allocator    : 512 columns per CTA.  A tile with > 128 tokens takes all of them (accumulators at
+//                                columns 0 and 256); tiles with <= 128 tokens alternate between the two 256-column
+//                                halves (accumulators at +0 and +128), so their epilogue overlaps the next tile's MMAs
+//   warps 4-11 epilogue          : tcgen05.ld 16x256b (the MMA C-fragment layout) -> SwiGLU / cast -> stmatrix.trans
+//                                into a [32 tokens][128 features] staging tile -> 16-byte global stores, 256
+//                                contiguous bytes per token row; warps w and w+4 share a TMEM lane quarter and
+//                                take alternate 32-token chunks; "accumulator free" arrives on the leader's barrier
 // Per-expert tile scheduling over ragged token counts: units are numbered longest-first -- every > 128-token tile
 // of every group (n-major inside a group, so the token tiles that share a weight tile are claimed back to back and
 // hit L2), then the <= 128-token tail tiles -- and claimed dynamically (greedy list scheduling).
-// Tail split-K: with T tiles on G SMs the last T mod G tiles (all of them when T < G -- decode, single-expert miss
-// waves) would leave most SMs idle for a whole tile time, so the host splits each of those tiles s ways along K.
+// Tail split-K: with T units on G pairs the last T mod G units (all of them when T < G -- decode, single-expert miss
+// waves) would leave most SMs idle for a whole tile time, so the host splits each of those units s ways along K.
 // A split unit writes its raw fp32 accumulators to a workspace slot, then bumps the tile's arrival counter; the
 // unit that arrives last sums the s partials in split order (deterministic) and runs the normal epilogue.  No
-// CTA ever waits for another one.
+// CTA ever waits for another cluster.
 #include <cuda_bf16.h>
 
 #include "ef_internal.h"
@@ -44,10 +52,10 @@ constexpr int BW = 256;                // weight rows per tile (two 128-lane acc
 constexpr int ACC_M = 128;             // weight rows per accumulator
 constexpr int BT = 256;                // max tokens per tile
 constexpr int XBOX = 64;               // token rows per TMA box
-constexpr int kStages = 3;
+constexpr int kStages = 4;
 constexpr int W_BYTES = BW * BK * 2;              // 32 KB
 constexpr int XBOX_BYTES = XBOX * BK * 2;         // 8 KB
-constexpr int STAGE_BYTES = W_BYTES + BT * BK * 2;   // 64 KB
+constexpr int STAGE_BYTES = W_BYTES + (BT / 2) * BK * 2;   // 48 KB: own weight tile + own half of the token tile
 constexpr int kThreads = 384;
 constexpr int kEpiWarps = 8;
 constexpr int kSched = 4;               // depth of the tile-broadcast ring
@@ -106,28 +114,64 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1) {
+// cluster-scope acquire: the data published before the arrive may come from the peer CTA
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
     asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1) : "memory");
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2) {
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+// shared::cluster address of `p` (a pointer into this CTA's shared memory) in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(const void* p, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(p)), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void st_remote_u32(uint32_t cluster_addr, uint32_t v) {
+    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void cluster_sync() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// TMA loads into this CTA's shared memory whose bytes complete on the LEADER's mbarrier (cluster address `bar`)
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1) {
     asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.cta_group::2 [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(tm), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.cta_group::2 [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// arrives, once the MMAs issued so far have completed, on the barrier at this offset in BOTH CTAs of the pair
 __device__ __forceinline__ void tc_commit(uint64_t* bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(smem_u32(bar)), "h"((uint16_t)3) : "memory");
 }
-// D[tmem] (+)= A[smem] . B[smem]^T, M128 N(idesc) K16, bf16 -> fp32
+// D[tmem, both CTAs] (+)= A[smem, 128 rows per CTA] . B[smem, n/2 rows per CTA]^T, M256 N(idesc) K16, bf16 -> fp32
 __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n"
         "}\n" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accum) : "memory");
 }
 __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t* v) {
@@ -147,9 +191,9 @@ __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sy
 __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
 }
-// kind::f16 instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N = n (multiple of 16, 16..256)
+// kind::f16 instruction descriptor: D fp32, A/B bf16, both K-major, M = 256 (128 per CTA), N = n (multiple of 16)
 __device__ __forceinline__ uint32_t make_idesc(int n) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(ACC_M >> 4) << 24);
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)((2 * ACC_M) >> 4) << 24);
 }
 
 __device__ __forceinline__ uint16_t bf16_bits(float v) {
@@ -225,7 +269,7 @@ __device__ __forceinline__ void ws_sum32(const float* tile_slots, int s, int acc
             const float4 v = __ldcg(p + (size_t)i * ACC_M);
             sum[i].x += v.x; sum[i].y += v.y; sum[i].z += v.z; sum[i].w += v.w;
         }
-        p += kSlotFloats / 4;
+        p += 2 * (kSlotFloats / 4);      // slots alternate between the two CTAs of the pair
     }
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
@@ -241,7 +285,7 @@ struct Tile {
     int rows_valid;      // tokens of this tile (1..256)
     int n_mma;           // rows_valid rounded up to the MMA N granularity (16)
     int is_long;         // > 128 tokens: takes the whole TMEM
-    int n_tile, slot;
+    int n_pair, slot;    // n_pair: the pair's two adjacent weight tiles are 2 * n_pair + cluster rank
     int kb0, kb1;        // k-block range of this unit
     int tail, split_j;   // index among the split tiles (-1: whole tile) and which K part this unit is
 };
@@ -275,13 +319,13 @@ __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemC
         while (tile >= ctl->gstart_long[g + 1]) ++g;
         const int local = tile - ctl->gstart_long[g];
         const int nl = group_long_tiles(tab.g[g].rows);
-        t.n_tile = local / nl;
+        t.n_pair = local / nl;
         row_off = (local % nl) * BT;
         t.is_long = 1;
     } else {
         const int ts = tile - ctl->total_long;
         while (ts >= ctl->gstart_short[g + 1]) ++g;
-        t.n_tile = ts - ctl->gstart_short[g];
+        t.n_pair = ts - ctl->gstart_short[g];
         row_off = group_long_tiles(tab.g[g].rows) * BT;
         t.is_long = 0;
     }
@@ -293,12 +337,13 @@ __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemC
     return t;
 }
 
-// kSwiglu: accumulator 0 = 128 gate rows, accumulator 1 = the matching up rows -> 128 output columns per tile;
-// else accumulators 0 / 1 = output columns [256 n, +128) / [256 n + 128, +128)
+// kSwiglu: accumulator 0 = 128 gate rows, accumulator 1 = the matching up rows -> 128 output columns per weight tile;
+// else accumulators 0 / 1 = output columns [256 n, +128) / [256 n + 128, +128).  n_tiles_n = weight tiles, n_pairs_n =
+// ceil(n_tiles_n / 2) (an odd last tile leaves the peer CTA multiplying zero-filled rows).
 template <bool kSwiglu>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmW,
-                uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int total_tiles,
+                uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int n_pairs_n, int total_tiles,
                 int32_t* __restrict__ sched, const SplitArgs sp, long long* __restrict__ kprof,
                 const __grid_constant__ EfGroupTable tab) {
     extern __shared__ uint8_t smem_raw[];
@@ -306,6 +351,8 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
     uint8_t* stg_base = smem + (size_t)kStages * STAGE_BYTES;
     SmemCtl* ctl = (SmemCtl*)(stg_base + 2 * STG_BYTES);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const bool leader = rank == 0;
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmX) : "memory");
@@ -313,60 +360,73 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
     }
     if (warp == 1 && lane == 0) {
         for (int i = 0; i < kStages; ++i) { mbar_init(&ctl->full[i], 1); mbar_init(&ctl->empty[i], 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(&ctl->tmem_full[i], 1); mbar_init(&ctl->tmem_empty[i], kEpiWarps); }
-        for (int i = 0; i < kSched; ++i) { mbar_init(&ctl->sched_full[i], 1); mbar_init(&ctl->sched_empty[i], 1 + kEpiWarps); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&ctl->tmem_full[i], 1); mbar_init(&ctl->tmem_empty[i], 2 * kEpiWarps); }
+        for (int i = 0; i < kSched; ++i) { mbar_init(&ctl->sched_full[i], 1); mbar_init(&ctl->sched_empty[i], 2 * (1 + kEpiWarps)); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&ctl->tmem_base)), "r"(kTmemCols) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&ctl->tmem_base)), "r"(kTmemCols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
     }
     if (warp == 3 && lane == 0) {
         int nl = 0, ns = 0;
         for (int g = 0; g < tab.n; ++g) {
             ctl->gstart_long[g] = nl;
             ctl->gstart_short[g] = ns;
-            nl += group_long_tiles(tab.g[g].rows) * n_tiles_n;
-            ns += group_has_short(tab.g[g].rows) * n_tiles_n;
+            nl += group_long_tiles(tab.g[g].rows) * n_pairs_n;
+            ns += group_has_short(tab.g[g].rows) * n_pairs_n;
         }
         ctl->gstart_long[tab.n] = nl;
         ctl->gstart_short[tab.n] = ns;
         ctl->total_long = nl;
     }
     tc_fence_before();
-    __syncthreads();
+    cluster_sync();               // barriers of both CTAs are initialised before any remote arrive / multicast commit
     tc_fence_after();
     const uint32_t tmem_base = ctl->tmem_base;
     const int KB = K / BK;
 
     if (warp == 0) {
-        // ===== tile scheduler + TMA producer =====
+        // ===== tile scheduler (leader) + TMA producer (both) =====
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
             for (int it = 0;; ++it) {
                 const int ss = it % kSched;
-                mbar_wait(&ctl->sched_empty[ss], ((it / kSched) & 1) ^ 1);
-                const int tile = atomicAdd(sched, 1);
-                ctl->sched_tile[ss] = tile;
-                mbar_arrive(&ctl->sched_full[ss]);          // release: the tile index is visible to the waiters
+                int tile;
+                if (leader) {
+                    mbar_wait_cluster(&ctl->sched_empty[ss], ((it / kSched) & 1) ^ 1);
+                    tile = atomicAdd(sched, 1);
+                    ctl->sched_tile[ss] = tile;
+                    st_remote_u32(mapa(&ctl->sched_tile[ss], 1), (uint32_t)tile);
+                    mbar_arrive(&ctl->sched_full[ss]);                       // release.cta: local waiters
+                    mbar_arrive_remote(mapa(&ctl->sched_full[ss], 1));       // release.cluster: the peer's waiters
+                } else {
+                    mbar_wait_cluster(&ctl->sched_full[ss], (it / kSched) & 1);
+                    tile = ctl->sched_tile[ss];
+                    mbar_arrive_remote(mapa(&ctl->sched_empty[ss], 0));
+                }
                 if (tile >= total_tiles) break;
                 const Tile t = decode_tile(tab, ctl, tile, sp, KB);
-                const int n_box = (t.n_mma + XBOX - 1) / XBOX;
+                const int half = t.n_mma >> 1;                               // token rows this CTA stages
+                const int n_box = (half + XBOX - 1) / XBOX;
                 const uint32_t bytes = (uint32_t)(W_BYTES + n_box * XBOX_BYTES);
+                const int w_row = (2 * t.n_pair + (int)rank) * BW;
+                const int x_row = t.a_row + (int)rank * half;
                 for (int kb = t.kb0; kb < t.kb1; ++kb) {
                     mbar_wait(&ctl->empty[stage], phase ^ 1);
                     uint8_t* sw = smem + (size_t)stage * STAGE_BYTES;
-                    mbar_expect_tx(&ctl->full[stage], bytes);
-                    tma_load_3d(sw, &tmW, &ctl->full[stage], kb * BK, t.n_tile * BW, t.slot);
+                    if (leader) mbar_expect_tx(&ctl->full[stage], 2 * bytes);  // both CTAs' boxes land on this barrier
+                    const uint32_t bar = mapa(&ctl->full[stage], 0);
+                    tma_load_3d(sw, &tmW, bar, kb * BK, w_row, t.slot);
                     for (int j = 0; j < n_box; ++j)
-                        tma_load_2d(sw + W_BYTES + j * XBOX_BYTES, &tmX, &ctl->full[stage], kb * BK, t.a_row + j * XBOX);
+                        tma_load_2d(sw + W_BYTES + j * XBOX_BYTES, &tmX, bar, kb * BK, x_row + j * XBOX);
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer =====
-        if (lane == 0) {
+        // ===== MMA issuer (leader CTA only) =====
+        if (lane == 0 && leader) {
             int stage = 0; uint32_t phase = 0;
             int buf = 0; uint32_t bphase = 0;          // bit b = phase of TMEM half b
             KPROF(long long kp_t0 = clock64(); long long kp_sched = 0, kp_tmem = 0, kp_full = 0; int kp_units = 0;)
@@ -382,7 +442,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                 const Tile t = decode_tile(tab, ctl, tile, sp, KB);
                 const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
                 KPROF(long long kp_b = clock64();)
-                for (int h = 0; h < nb; ++h) mbar_wait(&ctl->tmem_empty[b0 + h], ((bphase >> (b0 + h)) & 1u) ^ 1u);
+                for (int h = 0; h < nb; ++h) mbar_wait_cluster(&ctl->tmem_empty[b0 + h], ((bphase >> (b0 + h)) & 1u) ^ 1u);
                 KPROF(kp_tmem += clock64() - kp_b;)
                 tc_fence_after();
                 const uint32_t d0 = tmem_base + (uint32_t)(b0 * 256);
@@ -402,7 +462,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                         tc_mma(d0, smem_desc(sw + k * 32), xd, idesc, acc);
                         tc_mma(d1, smem_desc(sw + ACC_M * BK * 2 + k * 32), xd, idesc, acc);
                     }
-                    tc_commit(&ctl->empty[stage]);    // frees the smem stage once these MMAs have read it
+                    tc_commit(&ctl->empty[stage]);    // frees the smem stage in both CTAs once these MMAs have read it
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
                 for (int h = 0; h < nb; ++h) {
@@ -412,7 +472,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                 buf = t.is_long ? 0 : (b0 ^ 1);
             }
             KPROF(if (kprof) {
-                long long* o = kprof + (size_t)blockIdx.x * 5;
+                long long* o = kprof + (size_t)(blockIdx.x >> 1) * 5;
                 o[0] = clock64() - kp_t0; o[1] = kp_sched; o[2] = kp_tmem; o[3] = kp_full; o[4] = kp_units;
             })
         }
@@ -424,15 +484,17 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
         int buf = 0; uint32_t bphase = 0;
         for (int it = 0;; ++it) {
             const int ss = it % kSched;
-            mbar_wait(&ctl->sched_full[ss], (it / kSched) & 1);
+            mbar_wait_cluster(&ctl->sched_full[ss], (it / kSched) & 1);
             const int tile = ctl->sched_tile[ss];
             __syncwarp();
-            if (lane == 0) mbar_arrive(&ctl->sched_empty[ss]);
+            if (lane == 0) mbar_arrive_remote(mapa(&ctl->sched_empty[ss], 0));
             if (tile >= total_tiles) break;
             const Tile t = decode_tile(tab, ctl, tile, sp, KB);
+            const int n_tile = 2 * t.n_pair + (int)rank;
+            const bool tile_ok = n_tile < n_tiles_n;   // false: the odd last weight tile's idle partner
             const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
             const bool split = t.tail >= 0;
-            float* ws_mine = split ? sp.ws + ((size_t)t.tail * sp.s + t.split_j) * kSlotFloats : nullptr;
+            float* ws_mine = split ? sp.ws + (((size_t)t.tail * sp.s + t.split_j) * 2 + rank) * kSlotFloats : nullptr;
             for (int h = 0; h < nb; ++h) {
                 mbar_wait(&ctl->tmem_full[b0 + h], (bphase >> (b0 + h)) & 1u);
                 bphase ^= 1u << (b0 + h);
@@ -440,11 +502,11 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
             tc_fence_after();
             const uint32_t tb0 = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b0 * 256);
             const uint32_t tb1 = tb0 + (t.is_long ? 256u : 128u);
-            const int n_chunks = (t.rows_valid + 31) >> 5;
-            const int col0 = kSwiglu ? t.n_tile * ACC_M : t.n_tile * BW;      // first output column of accumulator 0
+            const int n_chunks = tile_ok ? (t.rows_valid + 31) >> 5 : 0;
+            const int col0 = kSwiglu ? n_tile * ACC_M : n_tile * BW;      // first output column of accumulator 0
             uint8_t* stg = stg_base + part * STG_BYTES;
             // stmatrix row address of this thread: block i = lane / 8 (tokens 8i..8i+7), row lane % 8, + feature offset
-            const uint32_t st_row = smem_u32(stg) + (uint32_t)(((lane >> 3) * 8 + (lane & 7)) * STG_LD + q * 64);
+            const uint32_t st_row = smem_u32(stg) + (uint32_t)(lane * STG_LD + q * 64);
 #pragma unroll 1
             for (int c = part; c < n_chunks; c += 2) {
                 const int n_rows = min(32, t.rows_valid - c * 32);
@@ -490,23 +552,24 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
             tc_fence_before();
             __syncwarp();
             if (lane == 0)
-                for (int h = 0; h < nb; ++h) mbar_arrive(&ctl->tmem_empty[b0 + h]);
+                for (int h = 0; h < nb; ++h) mbar_arrive_remote(mapa(&ctl->tmem_empty[b0 + h], 0));
             buf = t.is_long ? 0 : (b0 ^ 1);
-            if (split) {
+            if (split && tile_ok) {
                 // publish the partial, count arrivals; the last unit of the tile reduces all s partials in split order
                 __threadfence();
                 epi_bar();
                 if (threadIdx.x == 4 * 32) {
-                    const int old = atomicAdd(sp.counters + t.tail, 1);
+                    int32_t* cnt = sp.counters + t.tail * 2 + rank;
+                    const int old = atomicAdd(cnt, 1);
                     const int last = (old == sp.s - 1) ? 1 : 0;
-                    if (last) sp.counters[t.tail] = 0;          // re-arm for the next launch
+                    if (last) *cnt = 0;                          // re-arm for the next launch
                     ctl->split_last = last;
                 }
                 epi_bar();
                 const bool last = ctl->split_last != 0;          // rewritten only after the next split unit's first barrier
                 if (last) {
                     __threadfence();
-                    const float* ws_tile = sp.ws + (size_t)t.tail * sp.s * kSlotFloats;
+                    const float* ws_tile = sp.ws + ((size_t)t.tail * sp.s * 2 + rank) * kSlotFloats;
 #pragma unroll 1
                     for (int c = part; c < n_chunks; c += 2) {
                         const int n_rows = min(32, t.rows_valid - c * 32);
@@ -531,13 +594,13 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
     }
 
     tc_fence_before();
-    __syncthreads();
+    cluster_sync();               // the peer's TMEM / shared memory / barriers stay alive until both CTAs are done
     if (warp == 2) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
     }
-    // the last CTA to finish re-arms the scheduler words for the launch that reuses them (every CTA's producer has
-    // drawn its terminal ticket by now, so nobody reads the counter again)
+    // the last CTA to finish re-arms the scheduler words for the launch that reuses them (every leader has drawn its
+    // terminal ticket by now, so nobody reads the counter again)
     if (threadIdx.x == 0) {
         __threadfence();
         if (atomicAdd(sched + 1, 1) == (int)gridDim.x - 1) { sched[0] = 0; sched[1] = 0; }
@@ -643,10 +706,10 @@ int32_t efk_ffn_tc_init(ef_ctx* ctx) {
     EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
     EF_CUDA(ctx, cudaMalloc(&ctx->sched_words, sizeof(int32_t) * 2 * EF_SCHED_RING));
     EF_CUDA(ctx, cudaMemset(ctx->sched_words, 0, sizeof(int32_t) * 2 * EF_SCHED_RING));
-    ctx->splitk_max_units = 2 * ctx->n_sms;
-    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_ws, sizeof(float) * kSlotFloats * (size_t)ctx->splitk_max_units));
-    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_counters, sizeof(int32_t) * ctx->splitk_max_units));
-    EF_CUDA(ctx, cudaMemset(ctx->splitk_counters, 0, sizeof(int32_t) * ctx->splitk_max_units));
+    ctx->splitk_max_units = ctx->n_sms;      // pair units; each has one workspace slot and one counter per CTA of the pair
+    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_ws, sizeof(float) * kSlotFloats * 2 * (size_t)ctx->splitk_max_units));
+    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_counters, sizeof(int32_t) * 2 * ctx->splitk_max_units));
+    EF_CUDA(ctx, cudaMemset(ctx->splitk_counters, 0, sizeof(int32_t) * 2 * ctx->splitk_max_units));
     ctx->tm_ok = true;
     return EF_OK;
 }
@@ -673,6 +736,7 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         t1.g[i].c_row0 = h_row0[i];   // GEMM1: x rows -> h rows
         t2.g[i].a_row0 = h_row0[i];   // GEMM2: h rows -> y rows
     }
+    const int n_pairs = ctx->n_sms / 2;     // CTA pairs (clusters of 2), one CTA per SM
     ef_ctx::KSpan span{};
     if (ctx->time_kernels) {
         EF_CUDA(ctx, cudaEventCreate(&span.e0));
@@ -682,12 +746,13 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     }
     {
         const int ntn = f / 128;      // 256 packed W13 rows -> 128 h columns
-        const int tiles = mtiles * ntn;
-        const SplitPlan pl = plan_split(ctx, tiles, mshort * ntn, ctx->n_sms, d / BK, (double)rows_total / mtiles);
+        const int npn = (ntn + 1) / 2;
+        const int tiles = mtiles * npn;
+        const SplitPlan pl = plan_split(ctx, tiles, mshort * npn, n_pairs, d / BK, (double)rows_total / mtiles);
         const int total = pl.n_plain + pl.n_tail * pl.s;
-        const int grid = std::min(total, ctx->n_sms);
+        const int grid = 2 * std::min(total, n_pairs);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
-        ffn_gemm_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn,
+        ffn_gemm_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
                                                                   total, next_sched(ctx), sp, ctx->kprof1, t1);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
@@ -695,12 +760,13 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     if (ctx->time_kernels) EF_CUDA(ctx, cudaEventRecord(span.e1, st));
     {
         const int ntn = (d + BW - 1) / BW;
-        const int tiles = mtiles * ntn;
-        const SplitPlan pl = plan_split(ctx, tiles, mshort * ntn, ctx->n_sms, f / BK, (double)rows_total / mtiles);
+        const int npn = (ntn + 1) / 2;
+        const int tiles = mtiles * npn;
+        const SplitPlan pl = plan_split(ctx, tiles, mshort * npn, n_pairs, f / BK, (double)rows_total / mtiles);
         const int total = pl.n_plain + pl.n_tail * pl.s;
-        const int grid = std::min(total, ctx->n_sms);
+        const int grid = 2 * std::min(total, n_pairs);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
-        ffn_gemm_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_wd, (uint16_t*)y, d, d, f, ntn,
+        ffn_gemm_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_wd, (uint16_t*)y, d, d, f, ntn, npn,
                                                                    total, next_sched(ctx), sp, ctx->kprof2, t2);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
