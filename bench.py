@@ -32,6 +32,12 @@ import workloads as wl  # noqa: E402
 METRIC = "moe_layer_tokens_per_s"
 UNIT = "tokens/s"
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel (GEMM1), bytes per launch averaged over the
+# launches of a streaming step, from the committed `ncu --set full` captures (never measured by this script):
+#   mixtral_prefill: profiles/r1_ffn_gemm_ncu_full.md  -- one wave-0 launch (1.2833 GB) + 4 single-expert launches (0.2406 GB)
+#   mixtral_decode : profiles/r1_ffn_decode_ncu_full.md -- single-expert launches (0.2386 GB)
+NCU_TRAFFIC_BYTES = {"mixtral_prefill": (1.2833e9 + 4 * 0.24055e9) / 5, "mixtral_decode": 0.23861e9}
+
 
 # ---------------------------------------------------------------------------------------------------
 # distributed plumbing (replicas only; works on gloo for the CPU tests)
@@ -99,7 +105,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(self.idx)], stdout=subprocess.PIPE,
+                                          "-lms", "20", "-i", str(self.idx)], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -445,6 +451,10 @@ def run_ours(args):
     d, f = cfg.d_model, cfg.d_ff
     decode = cfg.T * cfg.top_k / cfg.n_experts < 249 and cfg.name in ("mixtral_decode", "stack_decode")
     roofline = ffn_roofline(kt, d, f, peaks, decode, "streaming step (one wave of hits + one wave per miss)")
+    roofline["traffic"] = NCU_TRAFFIC_BYTES.get(cfg.name)
+    roofline["traffic_source"] = ("bytes per GEMM1 launch from the committed ncu capture under profiles/ (see NCU_TRAFFIC_BYTES)"
+                                  if cfg.name in NCU_TRAFFIC_BYTES else "no ncu capture for this workload")
+    roofline["algorithmic_bytes_per_launch"] = (4.0 * d * f * kt["groups"] + 2.0 * d * kt["rows"] + 2.0 * f * kt["rows"]) / max(1, kt["gemm1_launches"])
 
     h2d = {"bytes_per_step": st["bytes_h2d"] / args.steps, "loads_per_step": (st["ondemand_loads"] + st["prefetch_issued"]) / args.steps,
            "copy_busy_ms_per_step": copy_ms / args.steps,
