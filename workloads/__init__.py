@@ -276,3 +276,32 @@ def trace_bias(cfg: MoEConfig, trace: Trace, visit: int) -> np.ndarray:
     for j in range(k):
         b[np.arange(T), trace.sets[visit, :, j]] = np.float32(cfg.trace_margin + (k - 1 - j))
     return b
+
+
+# ----------------------------------------------------------------------------
+# token-level routing paths for the Token Scheduler (§3.3)
+# ----------------------------------------------------------------------------
+def token_paths(seed: int, n_tokens: int, n_layers: int, n_experts: int, top_k: int, n_families: int = 2,
+                family_prob: float = 0.8) -> np.ndarray:
+    """Binary routing-path matrices r[N, L, E] (uint8 0/1, exactly top_k ones per layer) with the structure
+    the Token Scheduler exploits: every token belongs to one of n_families latent groups ("tokens sharing similar
+    routing paths"); per layer a token takes its family's expert set with probability family_prob, else a
+    fresh top_k draw from that layer's popularity (softmax of N(0,1) offsets, as in routing_trace).  Families are
+    interleaved at random over the token index, so the incoming batches [0, T) and [T, 2T) mix them."""
+    g = stream(seed, f"tokpaths.N{n_tokens}.L{n_layers}.E{n_experts}.k{top_k}.F{n_families}")
+    pops = []
+    for l in range(n_layers):
+        o = g.standard_normal(n_experts)
+        p = np.exp(o - o.max())
+        pops.append(p / p.sum())
+    fam_sets = np.zeros((n_families, n_layers, top_k), np.int64)
+    for f in range(n_families):
+        for l in range(n_layers):
+            fam_sets[f, l] = _draw_set(g, pops[l], top_k)
+    fam = g.integers(0, n_families, size=n_tokens)
+    r = np.zeros((n_tokens, n_layers, n_experts), np.uint8)
+    for i in range(n_tokens):
+        for l in range(n_layers):
+            es = fam_sets[fam[i], l] if g.random() < family_prob else _draw_set(g, pops[l], top_k)
+            r[i, l, es] = 1
+    return r
