@@ -167,6 +167,32 @@ int32_t ef_cache_clear(ef_ctx* ctx);
  * ef_copy_busy_ms waits for the copy stream.  Synchronous. */
 int32_t ef_copy_busy_ms(ef_ctx* ctx, float* ms_out);
 
+/* ---- f1: Token Scheduler (Sec. 3.3) ------------------
+ * N = 2T tokens (two incoming batches: tokens [0, T) and [T, 2T)), each with a binary routing-path matrix r_i of
+ * size (L, E), are split into two new batches of exactly T tokens so that fewer experts are activated
+ * (Eq. 5).  Heuristic of Sec. 3.3.3: Hamming distance d_ij between paths, similarity
+ * S_ij = 1 - d_ij / (L*E) (Eq. 6); balanced 2-means whose centroids are tokens: assign every token to the more
+ * similar centroid, rebalance to exactly T per cluster (R26: cluster 0 = the T tokens with the largest
+ * S[i,c0] - S[i,c1]; R27: ties to the lower index), move each centroid to the member with the highest average
+ * similarity to the others (R27/R29), stop when the centroids repeat (R28) or after max_iter rounds.
+ *
+ * paths     DEVICE uint8[N, LE], LE = L*E, row-major, nonzero = expert on the path (the predictor's output)
+ * c0, c1    the two distinct tokens drawn as initial centroids ("random centroid selection": the draw is
+ *           the caller's, so that results are reproducible)
+ * batch_of  DEVICE int32[N]  out: 0 or 1
+ * perm      DEVICE int32[N]  out: tokens of new batch 0 in ascending index, then those of new batch 1 -- the
+ *           gather map for activations / the KV-cache "Reindex" of P:L151
+ * info      DEVICE int32[8]  out: {rounds executed, converged (0/1), final c0, final c1, Eq. 5 objective of the
+ *           result, Eq. 5 objective of the incoming batching, 0, 0}; batch-level paths combine tokens with OR (R14)
+ * Constraints: N even, 2 <= N <= EF_TS_MAX_TOKENS, 1 <= LE <= 32767, 1 <= max_iter <= 64.  Asynchronous on
+ * `stream`; the library owns the workspace (bit-packed paths, the uint16 N x N distance matrix). */
+#define EF_TS_MAX_TOKENS 16384
+int32_t ef_token_schedule(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, int32_t c0,
+                          int32_t c1, int32_t max_iter, int32_t* batch_of, int32_t* perm, int32_t* info);
+/* The Hamming distance matrix of Eq. 6 alone: dist_out DEVICE uint16[N, N] (16-byte aligned), d_ij = number of
+ * (layer, expert) entries in which r_i and r_j differ; S_ij = 1 - d_ij / LE.  N need not be even here. */
+int32_t ef_path_hamming(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, uint16_t* dist_out);
+
 /* ---- misc ---------------------------------------------------------------------------------- */
 /* Wait for the copy stream and the device.  Synchronous. */
 int32_t ef_sync(ef_ctx* ctx);

@@ -18,7 +18,7 @@ DECLARED_SYMBOLS = [
     "ef_expert_ffn_grouped", "ef_expert_ffn_grouped_resident", "ef_shared_ffn", "ef_combine", "ef_rmsnorm",
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
     "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
-    "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof",
+    "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof", "ef_token_schedule", "ef_path_hamming",
 ]
 
 
@@ -88,6 +88,8 @@ def load_library() -> ctypes.CDLL:
             "ef_set_splitk": [vp, i32],
             "ef_debug_kprof": [vp, i32, vp],
             "ef_get_kernel_times": [vp, ctypes.POINTER(KernelTimes), i32],
+            "ef_token_schedule": [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp],
+            "ef_path_hamming": [vp, vp, vp, i32, i32, vp],
         }
         for name, args in sig.items():
             fn = getattr(lib, name)
@@ -215,6 +217,19 @@ class EfContext:
     def ef_cache_evict(self, layer, experts):
         e = np.ascontiguousarray(experts, dtype=np.int32)
         self._chk(self.lib.ef_cache_evict(self.h, layer, _hp(e), len(e)))
+
+    # -- f1: token scheduler
+    def ef_token_schedule(self, paths, c0, c1, max_iter, batch_of, perm, info):
+        """paths: uint8 device tensor [N, L, E] or [N, L*E]; outputs: int32 device tensors [N], [N], [8]."""
+        N = paths.shape[0]
+        LE = paths.numel() // max(1, N)
+        self._chk(self.lib.ef_token_schedule(self.h, _stream(), _dp(paths), N, LE, c0, c1, max_iter, _dp(batch_of),
+                                             _dp(perm), _dp(info)))
+
+    def ef_path_hamming(self, paths, dist_out):
+        N = paths.shape[0]
+        LE = paths.numel() // max(1, N)
+        self._chk(self.lib.ef_path_hamming(self.h, _stream(), _dp(paths), N, LE, _dp(dist_out)))
 
     def ef_cache_get_stats(self) -> dict:
         st = CacheStats()

@@ -132,6 +132,7 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
     if (ctx->kprof1) cudaFree(ctx->kprof1);
     if (ctx->kprof2) cudaFree(ctx->kprof2);
     if (ctx->splitk_counters) cudaFree(ctx->splitk_counters);
+    efk_token_sched_free(ctx);
     if (ctx->h_ws) cudaFree(ctx->h_ws);
     if (ctx->arena) cudaFree(ctx->arena);
     delete ctx;
@@ -563,6 +564,27 @@ extern "C" int32_t ef_cache_evict(ef_ctx* ctx, int32_t layer, const int32_t* exp
         sl.expert = -1; sl.pred_for = -1; sl.used = false; sl.stamp = 0;
     }
     return EF_OK;
+}
+
+extern "C" int32_t ef_token_schedule(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, int32_t c0,
+                                     int32_t c1, int32_t max_iter, int32_t* batch_of, int32_t* perm, int32_t* info) {
+    EF_CHECK_CTX(ctx);
+    if (!paths || !batch_of || !perm || !info) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_token_schedule: null pointer");
+    if (N < 2 || (N & 1) || c0 < 0 || c1 < 0 || c0 >= N || c1 >= N || c0 == c1 || max_iter < 1 || LE < 1)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_token_schedule: need even N >= 2, distinct centroids in [0, N), max_iter >= 1");
+    if (N > EF_TS_MAX_TOKENS || LE > 32767 || max_iter > 64)
+        return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_token_schedule: N <= %d, LE <= 32767, max_iter <= 64", EF_TS_MAX_TOKENS);
+    return efk_token_schedule(ctx, (cudaStream_t)stream, paths, N, LE, c0, c1, max_iter, batch_of, perm, info);
+}
+
+extern "C" int32_t ef_path_hamming(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE,
+                                   uint16_t* dist_out) {
+    EF_CHECK_CTX(ctx);
+    if (N < 0 || (N > 0 && (!paths || !dist_out)) || LE < 1) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_path_hamming: bad argument");
+    if (N > EF_TS_MAX_TOKENS || LE > 32767 || ((uintptr_t)dist_out & 15))
+        return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_path_hamming: N <= %d, LE <= 32767, dist_out 16-byte aligned", EF_TS_MAX_TOKENS);
+    if (N == 0) return EF_OK;
+    return efk_path_hamming(ctx, (cudaStream_t)stream, paths, N, LE, dist_out);
 }
 
 extern "C" int32_t ef_cache_get_stats(ef_ctx* ctx, ef_cache_stats* out) {

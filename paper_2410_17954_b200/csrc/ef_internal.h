@@ -103,6 +103,12 @@ struct ef_ctx {
     struct KSpan { cudaEvent_t e0, e1, e2; };
     std::vector<KSpan> kspans;
     ef_kernel_times ktimes{};
+    // token scheduler workspace (token_sched.cu): state words, packed paths + membership bits, distance matrix
+    void* ts_state = nullptr;
+    void* ts_small = nullptr;
+    size_t ts_small_bytes = 0;
+    void* ts_dist = nullptr;
+    size_t ts_dist_bytes = 0;
     // misc
     int64_t launches = 0;
     int32_t debug_simt = 0;
@@ -144,6 +150,10 @@ int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, co
                         const int32_t* h_row0 /*[n]*/);
 int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
                      const int32_t* h_row0);
+int32_t efk_token_schedule(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, int c0, int c1,
+                           int max_iter, int32_t* batch_of, int32_t* perm, int32_t* info);
+int32_t efk_path_hamming(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, uint16_t* dist_out);
+void efk_token_sched_free(ef_ctx* ctx);
 int32_t efk_ffn_tc_init(ef_ctx* ctx);   // build arena tensor maps, set smem attributes
 int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
                    const int32_t* h_row0);
