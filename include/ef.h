@@ -189,6 +189,9 @@ int32_t ef_copy_busy_ms(ef_ctx* ctx, float* ms_out);
 #define EF_TS_MAX_TOKENS 16384
 int32_t ef_token_schedule(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, int32_t c0,
                           int32_t c1, int32_t max_iter, int32_t* batch_of, int32_t* perm, int32_t* info);
+/* Problems with N <= 256 (decode batches) run in one single-CTA kernel with the distance matrix in shared memory;
+ * larger ones in the multi-kernel path.  Test hook: 1 = always take the multi-kernel path.  Results are identical. */
+int32_t ef_set_token_sched_path(ef_ctx* ctx, int32_t force_multi_kernel);
 /* The Hamming distance matrix of Eq. 6 alone: dist_out DEVICE uint16[N, N] (16-byte aligned), d_ij = number of
  * (layer, expert) entries in which r_i and r_j differ; S_ij = 1 - d_ij / LE.  N need not be even here. */
 int32_t ef_path_hamming(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, uint16_t* dist_out);

@@ -18,7 +18,7 @@ DECLARED_SYMBOLS = [
     "ef_expert_ffn_grouped", "ef_expert_ffn_grouped_resident", "ef_shared_ffn", "ef_combine", "ef_rmsnorm",
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
     "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
-    "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof", "ef_token_schedule", "ef_path_hamming",
+    "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof", "ef_token_schedule", "ef_path_hamming", "ef_set_token_sched_path",
 ]
 
 
@@ -90,6 +90,7 @@ def load_library() -> ctypes.CDLL:
             "ef_get_kernel_times": [vp, ctypes.POINTER(KernelTimes), i32],
             "ef_token_schedule": [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp],
             "ef_path_hamming": [vp, vp, vp, i32, i32, vp],
+            "ef_set_token_sched_path": [vp, i32],
         }
         for name, args in sig.items():
             fn = getattr(lib, name)
@@ -225,6 +226,9 @@ class EfContext:
         LE = paths.numel() // max(1, N)
         self._chk(self.lib.ef_token_schedule(self.h, _stream(), _dp(paths), N, LE, c0, c1, max_iter, _dp(batch_of),
                                              _dp(perm), _dp(info)))
+
+    def ef_set_token_sched_path(self, force_multi_kernel: bool):
+        self._chk(self.lib.ef_set_token_sched_path(self.h, 1 if force_multi_kernel else 0))
 
     def ef_path_hamming(self, paths, dist_out):
         N = paths.shape[0]

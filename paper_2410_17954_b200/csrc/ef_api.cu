@@ -577,6 +577,12 @@ extern "C" int32_t ef_token_schedule(ef_ctx* ctx, void* stream, const uint8_t* p
     return efk_token_schedule(ctx, (cudaStream_t)stream, paths, N, LE, c0, c1, max_iter, batch_of, perm, info);
 }
 
+extern "C" int32_t ef_set_token_sched_path(ef_ctx* ctx, int32_t force_multi_kernel) {
+    EF_CHECK_CTX(ctx);
+    ctx->ts_force_multi = force_multi_kernel ? 1 : 0;
+    return EF_OK;
+}
+
 extern "C" int32_t ef_path_hamming(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE,
                                    uint16_t* dist_out) {
     EF_CHECK_CTX(ctx);

@@ -109,6 +109,8 @@ struct ef_ctx {
     size_t ts_small_bytes = 0;
     void* ts_dist = nullptr;
     size_t ts_dist_bytes = 0;
+    bool ts_small_attr = false;         // ts_small_kernel opted in to > 48 KB dynamic smem
+    int32_t ts_force_multi = 0;         // test hook (ef_set_token_sched_path): 1 = never take the single-CTA path
     // misc
     int64_t launches = 0;
     int32_t debug_simt = 0;

@@ -287,6 +287,112 @@ ts_finalize_kernel(const uint32_t* __restrict__ P, int N, int Wd, TsState* st, c
     }
 }
 
+// ---- decode-sized problems (N <= 256): the whole schedule in ONE CTA, distance matrix in shared memory ------------
+// Same arithmetic as the multi-kernel path (same margins, same tie rules), but one launch instead of 3 + 2 * max_iter:
+// at N = 2 x 16 .. 2 x 64 decode tokens the multi-kernel path is all launch latency.
+constexpr int TS_SMALL_N = 256;
+
+__global__ void __launch_bounds__(TS_BLOCK)
+ts_small_kernel(const uint8_t* __restrict__ r, int N, int LE, int Wd, int c0, int c1, int max_iter,
+                int32_t* __restrict__ batch_of, int32_t* __restrict__ perm, int32_t* __restrict__ info) {
+    extern __shared__ __align__(16) uint8_t ts_smem[];
+    const int ldp = Wd | 1;                                   // odd word stride: conflict-free column walks
+    const int ldd = N + 2;
+    uint32_t* sP = reinterpret_cast<uint32_t*>(ts_smem);      // [N][ldp]
+    uint32_t* sOr = sP + (size_t)N * ldp;                     // [4][Wd]
+    int* sM = reinterpret_cast<int*>(sOr + 4 * Wd);           // [N] margins
+    int* sB = sM + N;                                         // [N] batch_of
+    uint16_t* sD = reinterpret_cast<uint16_t*>(sB + N);       // [N][ldd]
+    __shared__ unsigned long long s_best[2];
+    __shared__ int s_st[5];                                   // c0, c1, done, converged, iters
+    __shared__ int s_red[TS_BLOCK / 32];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, T = N >> 1;
+
+    for (int i = warp; i < N; i += TS_BLOCK / 32) {
+        const uint8_t* row = r + (size_t)i * LE;
+        for (int w = 0; w < Wd; ++w) {
+            const int c = w * 32 + lane;
+            const unsigned bits = __ballot_sync(0xffffffffu, c < LE && row[c] != 0);
+            if (lane == 0) sP[i * ldp + w] = bits;
+        }
+    }
+    if (tid == 0) { s_st[0] = c0; s_st[1] = c1; s_st[2] = 0; s_st[3] = 0; s_st[4] = 0; }
+    __syncthreads();
+    for (int t = tid; t < N * N; t += TS_BLOCK) {
+        const int i = t / N, j = t - i * N;
+        uint32_t d = 0;
+        for (int w = 0; w < Wd; ++w) d += __popc(sP[i * ldp + w] ^ sP[j * ldp + w]);
+        sD[i * ldd + j] = (uint16_t)d;
+    }
+    __syncthreads();
+
+    for (int round = 0; round < max_iter; ++round) {
+        const int a0 = s_st[0], a1 = s_st[1];
+        if (tid < N) sM[tid] = (int)sD[a1 * ldd + tid] - (int)sD[a0 * ldd + tid];
+        if (tid == 0) { s_best[0] = ~0ull; s_best[1] = ~0ull; s_st[4] = round + 1; }
+        __syncthreads();
+        if (tid < N) {
+            // rank in the order (margin descending, index ascending): cluster 0 = ranks [0, T)   (R26, R27)
+            const int mi = sM[tid];
+            int rank = 0;
+            for (int j = 0; j < N; ++j) {
+                const int mj = sM[j];
+                rank += (mj > mi || (mj == mi && j < tid)) ? 1 : 0;
+            }
+            sB[tid] = rank < T ? 0 : 1;
+        }
+        __syncthreads();
+        if (tid < N) {
+            const int b = sB[tid];
+            uint32_t sum = 0;
+            for (int j = 0; j < N; ++j) sum += (sB[j] == b) ? (uint32_t)sD[j * ldd + tid] : 0u;   // D is symmetric
+            atomicMin(&s_best[b], ((unsigned long long)sum << 32) | (unsigned long long)(uint32_t)tid);
+        }
+        __syncthreads();
+        if (tid == 0) {
+            const int n0 = (int)(s_best[0] & 0xffffffffull), n1 = (int)(s_best[1] & 0xffffffffull);
+            if (n0 == s_st[0] && n1 == s_st[1]) { s_st[2] = 1; s_st[3] = 1; }
+            else { s_st[0] = n0; s_st[1] = n1; }
+        }
+        __syncthreads();
+        if (s_st[2]) break;
+    }
+
+    for (int t = tid; t < 4 * Wd; t += TS_BLOCK) sOr[t] = 0;
+    __syncthreads();
+    if (tid < N) {
+        const int b = sB[tid];
+        int r0 = 0;
+        for (int j = 0; j < tid; ++j) r0 += (sB[j] == 0) ? 1 : 0;
+        batch_of[tid] = b;
+        perm[b == 0 ? r0 : T + (tid - r0)] = tid;
+    }
+    for (int t = tid; t < N * Wd; t += TS_BLOCK) {
+        const int i = t / Wd, w = t - i * Wd;
+        const uint32_t v = sP[i * ldp + w];
+        if (v) {
+            atomicOr(&sOr[sB[i] * Wd + w], v);
+            atomicOr(&sOr[(2 + (i >= T ? 1 : 0)) * Wd + w], v);
+        }
+    }
+    __syncthreads();
+    int after = 0, before = 0;
+    for (int t = tid; t < 2 * Wd; t += TS_BLOCK) {
+        after += __popc(sOr[t]);
+        before += __popc(sOr[2 * Wd + t]);
+    }
+    after = block_sum(after, s_red);
+    before = block_sum(before, s_red);
+    if (tid == 0) {
+        info[0] = s_st[4]; info[1] = s_st[3]; info[2] = s_st[0]; info[3] = s_st[1];
+        info[4] = after; info[5] = before; info[6] = 0; info[7] = 0;
+    }
+}
+
+size_t ts_small_smem(int N, int Wd) {
+    return (size_t)N * (Wd | 1) * 4 + (size_t)4 * Wd * 4 + (size_t)2 * N * 4 + (size_t)N * (N + 2) * 2;
+}
+
 __global__ void ts_init_kernel(TsState* st, int c0, int c1, int max_iter) {
     st->c0 = c0; st->c1 = c1; st->done = 0; st->converged = 0; st->iters = 0; st->max_iter = max_iter;
     st->best[0] = ~0ull; st->best[1] = ~0ull;
@@ -342,6 +448,17 @@ int32_t efk_path_hamming(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int
 int32_t efk_token_schedule(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, int c0, int c1,
                            int max_iter, int32_t* batch_of, int32_t* perm, int32_t* info) {
     const int Wd = (LE + 31) / 32;
+    if (N <= TS_SMALL_N && ts_small_smem(N, Wd) <= 200 * 1024 && !ctx->ts_force_multi) {
+        const size_t smem = ts_small_smem(N, Wd);
+        if (!ctx->ts_small_attr) {
+            EF_CUDA(ctx, cudaFuncSetAttribute(ts_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            ctx->ts_small_attr = true;
+        }
+        ts_small_kernel<<<1, TS_BLOCK, smem, st>>>(paths, N, LE, Wd, c0, c1, max_iter, batch_of, perm, info);
+        ctx->launches++;
+        EF_CUDA(ctx, cudaGetLastError());
+        return EF_OK;
+    }
     int32_t rc = ts_reserve(ctx, N, Wd, true);
     if (rc != EF_OK) return rc;
     uint16_t* D = (uint16_t*)ctx->ts_dist;

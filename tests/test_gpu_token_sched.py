@@ -37,12 +37,16 @@ def run_schedule(ctx, r, c0, c1, max_iter=16):
 
 
 def check_against_oracle(ctx, r, c0, c1, max_iter=16):
+    """Both device paths (single-CTA for N <= 256, multi-kernel) against the oracle."""
     ref = ots.schedule(r, c0, c1, max_iter)
-    b, p, info = run_schedule(ctx, r, c0, c1, max_iter)
-    assert np.array_equal(b, ref.batch_of)
-    assert np.array_equal(p, ref.perm)
-    assert info[:6].tolist() == [ref.iters, int(ref.converged), ref.centroids[0], ref.centroids[1], ref.objective,
-                                 ref.objective_before]
+    for force_multi in (False, True):
+        ctx.ef_set_token_sched_path(force_multi)
+        b, p, info = run_schedule(ctx, r, c0, c1, max_iter)
+        assert np.array_equal(b, ref.batch_of), force_multi
+        assert np.array_equal(p, ref.perm), force_multi
+        assert info[:6].tolist() == [ref.iters, int(ref.converged), ref.centroids[0], ref.centroids[1], ref.objective,
+                                     ref.objective_before], force_multi
+    ctx.ef_set_token_sched_path(False)
     return ref
 
 
@@ -80,7 +84,7 @@ def test_fig4_example_on_gpu(ctx):
 
 @pytest.mark.parametrize("N,L,E,k,fam,prob", [
     (2, 1, 4, 1, 2, 1.0), (8, 2, 4, 2, 2, 0.9), (32, 1, 8, 2, 2, 0.8),        # cfg 3: 2 x 16 decode tokens, one layer
-    (128, 32, 8, 2, 2, 0.6), (128, 32, 8, 2, 4, 0.5),                         # cfg 5: 2 x 64 tokens, 32 x 8 paths
+    (128, 32, 8, 2, 2, 0.6), (128, 32, 8, 2, 4, 0.5), (256, 32, 8, 2, 3, 0.5), (254, 26, 64, 6, 2, 0.5), (258, 4, 8, 2, 2, 0.5),                      # cfg 5: 2 x 64 tokens, 32 x 8 paths
     (1000, 8, 16, 2, 3, 0.7), (1002, 8, 16, 2, 3, 0.7), (1030, 5, 7, 1, 2, 0.5),   # vector / scalar row paths, ragged tiles
     (2048, 26, 64, 6, 2, 0.5),                                                # many-expert paths: 52 words per token
 ])
