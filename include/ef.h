@@ -92,7 +92,8 @@ int32_t ef_host_expert_alias(ef_ctx* ctx, int32_t layer, int32_t expert, int32_t
  * topk_idx[t,:] = the k largest logits' experts, descending, ties -> lower index (R2)
  * topk_w[t,j]   = exp(l_j - max) / Z,  Z over the k selected (renorm=1) or over all E (renorm=0, Eq. 1)
  * x: [T, d] bf16 device.  w_router: [E, d] bf16 device.  bias: fp32 device, nullable;
- * bias_token_stride 0 (per expert, [E]) or E (per token, [T,E]).  topk_idx: [T,k] int32, topk_w: [T,k]
+ * bias_token_stride 0 (per expert, [E]) or >= E floats (per token; E for a dense [T,E], larger to select one layer of a
+ * [T,L,E] tensor).  topk_idx: [T,k] int32, topk_w: [T,k]
  * fp32, logits_out: [T,E] fp32 nullable -- all device.  T may be 0. */
 int32_t ef_route_topk(ef_ctx* ctx, void* stream, const void* x, const void* w_router, const float* bias,
                       int64_t bias_token_stride, int32_t T, int32_t renorm, int32_t* topk_idx, float* topk_w,
@@ -184,11 +185,19 @@ int32_t ef_copy_busy_ms(ef_ctx* ctx, float* ms_out);
  *           gather map for activations / the KV-cache "Reindex" of P:L151
  * info      DEVICE int32[8]  out: {rounds executed, converged (0/1), final c0, final c1, Eq. 5 objective of the
  *           result, Eq. 5 objective of the incoming batching, 0, 0}; batch-level paths combine tokens with OR (R14)
+ * batch_paths DEVICE uint8[2, LE] out, nullable: the batch-level routing paths R_1, R_2 of Eq. 4 (0/1) of the new
+ *           batches -- what ef_cache_prefetch wants as the predicted path of each batch's visits
  * Constraints: N even, 2 <= N <= EF_TS_MAX_TOKENS, 1 <= LE <= 32767, 1 <= max_iter <= 64.  Asynchronous on
  * `stream`; the library owns the workspace (bit-packed paths, the uint16 N x N distance matrix). */
 #define EF_TS_MAX_TOKENS 16384
 int32_t ef_token_schedule(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, int32_t c0,
-                          int32_t c1, int32_t max_iter, int32_t* batch_of, int32_t* perm, int32_t* info);
+                          int32_t c1, int32_t max_iter, int32_t* batch_of, int32_t* perm, int32_t* info,
+                          uint8_t* batch_paths);
+/* "Reindex": dst row i = src row perm[i] for i < n_rows -- moves activations (and any other per-token rows:
+ * router bias, KV entries) into the order of the new batches.  src, dst DEVICE, rows of row_bytes bytes (multiple of
+ * 16, 16-byte aligned), out of place; perm DEVICE int32[n_rows] (need not be a permutation).  Asynchronous. */
+int32_t ef_reindex_rows(ef_ctx* ctx, void* stream, const void* src, const int32_t* perm, int32_t n_rows,
+                        int64_t row_bytes, void* dst);
 /* Problems with N <= 256 (decode batches) run in one single-CTA kernel with the distance matrix in shared memory;
  * larger ones in the multi-kernel path.  Test hook: 1 = always take the multi-kernel path.  Results are identical. */
 int32_t ef_set_token_sched_path(ef_ctx* ctx, int32_t force_multi_kernel);

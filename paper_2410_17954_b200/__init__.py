@@ -5,4 +5,4 @@ arguments.  There is no CPU fallback: if the library is missing or no CUDA devic
 """
 from .binding import (EfError, EfContext, EfConfig, CacheStats, load_library, library_path,  # noqa: F401
                       exported_symbols, DECLARED_SYMBOLS)
-from .layer import MoELayerRunner  # noqa: F401
+from .layer import MoELayerRunner, DualBatchRunner  # noqa: F401

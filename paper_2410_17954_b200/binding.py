@@ -18,7 +18,7 @@ DECLARED_SYMBOLS = [
     "ef_expert_ffn_grouped", "ef_expert_ffn_grouped_resident", "ef_shared_ffn", "ef_combine", "ef_rmsnorm",
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
     "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
-    "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof", "ef_token_schedule", "ef_path_hamming", "ef_set_token_sched_path",
+    "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof", "ef_token_schedule", "ef_path_hamming", "ef_set_token_sched_path", "ef_reindex_rows",
 ]
 
 
@@ -88,7 +88,8 @@ def load_library() -> ctypes.CDLL:
             "ef_set_splitk": [vp, i32],
             "ef_debug_kprof": [vp, i32, vp],
             "ef_get_kernel_times": [vp, ctypes.POINTER(KernelTimes), i32],
-            "ef_token_schedule": [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp],
+            "ef_token_schedule": [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp],
+            "ef_reindex_rows": [vp, vp, vp, vp, i32, i64, vp],
             "ef_path_hamming": [vp, vp, vp, i32, i32, vp],
             "ef_set_token_sched_path": [vp, i32],
         }
@@ -170,10 +171,14 @@ class EfContext:
 
     # -- a1
     def ef_route_topk(self, x, w_router, bias, T, renorm, topk_idx, topk_w, logits_out=None):
-        stride = 0
-        if bias is not None and bias.dim() == 2:
-            stride = bias.shape[1]
-        self._chk(self.lib.ef_route_topk(self.h, _stream(), _dp(x), _dp(w_router), _dp(bias), stride, T, renorm,
+        stride, bp = 0, None
+        if bias is not None:
+            if bias.dim() == 2:      # per-token rows; a row stride above E selects one layer of a [T, L, E] tensor
+                assert bias.is_cuda and bias.stride(1) == 1
+                stride, bp = bias.stride(0), ctypes.c_void_p(bias.data_ptr())
+            else:
+                bp = _dp(bias)
+        self._chk(self.lib.ef_route_topk(self.h, _stream(), _dp(x), _dp(w_router), bp, stride, T, renorm,
                                          _dp(topk_idx), _dp(topk_w), _dp(logits_out)))
 
     # -- a2
@@ -220,12 +225,18 @@ class EfContext:
         self._chk(self.lib.ef_cache_evict(self.h, layer, _hp(e), len(e)))
 
     # -- f1: token scheduler
-    def ef_token_schedule(self, paths, c0, c1, max_iter, batch_of, perm, info):
-        """paths: uint8 device tensor [N, L, E] or [N, L*E]; outputs: int32 device tensors [N], [N], [8]."""
+    def ef_token_schedule(self, paths, c0, c1, max_iter, batch_of, perm, info, batch_paths=None):
+        """paths: uint8 device tensor [N, L, E] or [N, L*E]; outputs: int32 device tensors [N], [N], [8] and
+        optionally uint8 [2, L*E]."""
         N = paths.shape[0]
         LE = paths.numel() // max(1, N)
         self._chk(self.lib.ef_token_schedule(self.h, _stream(), _dp(paths), N, LE, c0, c1, max_iter, _dp(batch_of),
-                                             _dp(perm), _dp(info)))
+                                             _dp(perm), _dp(info), _dp(batch_paths)))
+
+    def ef_reindex_rows(self, src, perm, dst):
+        n = perm.shape[0]
+        row_bytes = src.element_size() * (src.numel() // max(1, src.shape[0]))
+        self._chk(self.lib.ef_reindex_rows(self.h, _stream(), _dp(src), _dp(perm), n, row_bytes, _dp(dst)))
 
     def ef_set_token_sched_path(self, force_multi_kernel: bool):
         self._chk(self.lib.ef_set_token_sched_path(self.h, 1 if force_multi_kernel else 0))

@@ -205,8 +205,8 @@ extern "C" int32_t ef_route_topk(ef_ctx* ctx, void* stream, const void* x, const
     if (T < 0 || (T > 0 && (!x || !w_router || !topk_idx || !topk_w)))
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_route_topk: null pointer or negative T");
     if (T > ctx->cfg.max_tokens) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_route_topk: T > max_tokens");
-    if (bias && bias_token_stride != 0 && bias_token_stride != ctx->cfg.n_experts)
-        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_route_topk: bias_token_stride must be 0 or E");
+    if (bias && bias_token_stride != 0 && bias_token_stride < ctx->cfg.n_experts)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_route_topk: bias_token_stride must be 0 or >= E");
     return efk_route_topk(ctx, (cudaStream_t)stream, x, w_router, bias, bias_token_stride, T, renorm ? 1 : 0,
                           topk_idx, topk_w, logits_out);
 }
@@ -567,14 +567,26 @@ extern "C" int32_t ef_cache_evict(ef_ctx* ctx, int32_t layer, const int32_t* exp
 }
 
 extern "C" int32_t ef_token_schedule(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, int32_t c0,
-                                     int32_t c1, int32_t max_iter, int32_t* batch_of, int32_t* perm, int32_t* info) {
+                                     int32_t c1, int32_t max_iter, int32_t* batch_of, int32_t* perm, int32_t* info,
+                                     uint8_t* batch_paths) {
     EF_CHECK_CTX(ctx);
     if (!paths || !batch_of || !perm || !info) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_token_schedule: null pointer");
     if (N < 2 || (N & 1) || c0 < 0 || c1 < 0 || c0 >= N || c1 >= N || c0 == c1 || max_iter < 1 || LE < 1)
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_token_schedule: need even N >= 2, distinct centroids in [0, N), max_iter >= 1");
     if (N > EF_TS_MAX_TOKENS || LE > 32767 || max_iter > 64)
         return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_token_schedule: N <= %d, LE <= 32767, max_iter <= 64", EF_TS_MAX_TOKENS);
-    return efk_token_schedule(ctx, (cudaStream_t)stream, paths, N, LE, c0, c1, max_iter, batch_of, perm, info);
+    return efk_token_schedule(ctx, (cudaStream_t)stream, paths, N, LE, c0, c1, max_iter, batch_of, perm, info, batch_paths);
+}
+
+extern "C" int32_t ef_reindex_rows(ef_ctx* ctx, void* stream, const void* src, const int32_t* perm, int32_t n_rows,
+                                   int64_t row_bytes, void* dst) {
+    EF_CHECK_CTX(ctx);
+    if (n_rows < 0 || row_bytes < 0 || (n_rows > 0 && row_bytes > 0 && (!src || !perm || !dst)) || src == dst)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_reindex_rows: bad argument (out of place only)");
+    if ((row_bytes & 15) || ((uintptr_t)src & 15) || ((uintptr_t)dst & 15) || row_bytes / 16 > INT32_MAX)
+        return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_reindex_rows: rows must be multiples of 16 bytes, 16-byte aligned");
+    if (n_rows == 0 || row_bytes == 0) return EF_OK;
+    return efk_reindex_rows(ctx, (cudaStream_t)stream, src, perm, n_rows, row_bytes, dst);
 }
 
 extern "C" int32_t ef_set_token_sched_path(ef_ctx* ctx, int32_t force_multi_kernel) {

@@ -153,7 +153,9 @@ int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, co
 int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
                      const int32_t* h_row0);
 int32_t efk_token_schedule(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, int c0, int c1,
-                           int max_iter, int32_t* batch_of, int32_t* perm, int32_t* info);
+                           int max_iter, int32_t* batch_of, int32_t* perm, int32_t* info, uint8_t* batch_paths);
+int32_t efk_reindex_rows(ef_ctx* ctx, cudaStream_t st, const void* src, const int32_t* perm, int n_rows, int64_t row_bytes,
+                         void* dst);
 int32_t efk_path_hamming(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, uint16_t* dist_out);
 void efk_token_sched_free(ef_ctx* ctx);
 int32_t efk_ffn_tc_init(ef_ctx* ctx);   // build arena tensor maps, set smem attributes

@@ -115,3 +115,15 @@ int32_t efk_permute(ef_ctx* ctx, cudaStream_t st, const int32_t* idx, const void
     }
     return EF_OK;
 }
+
+// "Reindex" of the Token Scheduler (PAPER.md 3.3.1): dst row i = src row perm[i]; the same HBM-bound row copy
+// as the dispatch gather, with one source row per destination row.
+int32_t efk_reindex_rows(ef_ctx* ctx, cudaStream_t st, const void* src, const int32_t* perm, int n_rows, int64_t row_bytes,
+                         void* dst) {
+    if (n_rows == 0) return EF_OK;
+    const int blocks = (n_rows * 32 + 255) / 256;
+    gather_rows_kernel<<<blocks, 256, 0, st>>>((const uint4*)src, perm, n_rows, 1, (int)(row_bytes / 16), (uint4*)dst);
+    ctx->launches++;
+    EF_CUDA(ctx, cudaGetLastError());
+    return EF_OK;
+}

@@ -246,8 +246,8 @@ ts_medoid_kernel(const uint16_t* __restrict__ D, int N, const int32_t* __restric
 }
 
 __global__ void __launch_bounds__(TS_BLOCK)
-ts_finalize_kernel(const uint32_t* __restrict__ P, int N, int Wd, TsState* st, const int32_t* __restrict__ batch_of,
-                   int32_t* __restrict__ perm, int32_t* __restrict__ info) {
+ts_finalize_kernel(const uint32_t* __restrict__ P, int N, int LE, int Wd, TsState* st, const int32_t* __restrict__ batch_of,
+                   int32_t* __restrict__ perm, int32_t* __restrict__ info, uint8_t* __restrict__ batch_paths) {
     extern __shared__ uint32_t s_or[];        // [4][Wd]: new batch 0, new batch 1, incoming batch 0, incoming batch 1
     __shared__ int s_red[TS_BLOCK / 32];
     if (threadIdx.x == 0 && !st->done) { ts_apply_update(st); st->done = 1; }
@@ -274,6 +274,11 @@ ts_finalize_kernel(const uint32_t* __restrict__ P, int N, int Wd, TsState* st, c
         }
     }
     __syncthreads();
+    if (batch_paths)
+        for (int t = threadIdx.x; t < 2 * LE; t += TS_BLOCK) {
+            const int b = t / LE, c = t - b * LE;
+            batch_paths[t] = (uint8_t)((s_or[b * Wd + (c >> 5)] >> (c & 31)) & 1u);
+        }
     int after = 0, before = 0;
     for (int t = threadIdx.x; t < 2 * Wd; t += TS_BLOCK) {
         after += __popc(s_or[t]);
@@ -294,7 +299,8 @@ constexpr int TS_SMALL_N = 256;
 
 __global__ void __launch_bounds__(TS_BLOCK)
 ts_small_kernel(const uint8_t* __restrict__ r, int N, int LE, int Wd, int c0, int c1, int max_iter,
-                int32_t* __restrict__ batch_of, int32_t* __restrict__ perm, int32_t* __restrict__ info) {
+                int32_t* __restrict__ batch_of, int32_t* __restrict__ perm, int32_t* __restrict__ info,
+                uint8_t* __restrict__ batch_paths) {
     extern __shared__ __align__(16) uint8_t ts_smem[];
     const int ldp = Wd | 1;                                   // odd word stride: conflict-free column walks
     const int ldd = N + 2;
@@ -376,6 +382,11 @@ ts_small_kernel(const uint8_t* __restrict__ r, int N, int LE, int Wd, int c0, in
         }
     }
     __syncthreads();
+    if (batch_paths)
+        for (int t = tid; t < 2 * LE; t += TS_BLOCK) {
+            const int b = t / LE, c = t - b * LE;
+            batch_paths[t] = (uint8_t)((sOr[b * Wd + (c >> 5)] >> (c & 31)) & 1u);
+        }
     int after = 0, before = 0;
     for (int t = tid; t < 2 * Wd; t += TS_BLOCK) {
         after += __popc(sOr[t]);
@@ -446,7 +457,7 @@ int32_t efk_path_hamming(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int
 }
 
 int32_t efk_token_schedule(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, int c0, int c1,
-                           int max_iter, int32_t* batch_of, int32_t* perm, int32_t* info) {
+                           int max_iter, int32_t* batch_of, int32_t* perm, int32_t* info, uint8_t* batch_paths) {
     const int Wd = (LE + 31) / 32;
     if (N <= TS_SMALL_N && ts_small_smem(N, Wd) <= 200 * 1024 && !ctx->ts_force_multi) {
         const size_t smem = ts_small_smem(N, Wd);
@@ -454,7 +465,7 @@ int32_t efk_token_schedule(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, i
             EF_CUDA(ctx, cudaFuncSetAttribute(ts_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
             ctx->ts_small_attr = true;
         }
-        ts_small_kernel<<<1, TS_BLOCK, smem, st>>>(paths, N, LE, Wd, c0, c1, max_iter, batch_of, perm, info);
+        ts_small_kernel<<<1, TS_BLOCK, smem, st>>>(paths, N, LE, Wd, c0, c1, max_iter, batch_of, perm, info, batch_paths);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
         return EF_OK;
@@ -475,7 +486,7 @@ int32_t efk_token_schedule(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, i
         ts_medoid_kernel<<<(N + TS_ROWS_PER_CTA - 1) / TS_ROWS_PER_CTA, 256, bits_smem, st>>>(D, N, batch_of, bits, state);
         ctx->launches += 2;
     }
-    ts_finalize_kernel<<<1, TS_BLOCK, (size_t)4 * Wd * sizeof(uint32_t), st>>>(P, N, Wd, state, batch_of, perm, info);
+    ts_finalize_kernel<<<1, TS_BLOCK, (size_t)4 * Wd * sizeof(uint32_t), st>>>(P, N, LE, Wd, state, batch_of, perm, info, batch_paths);
     ctx->launches++;
     EF_CUDA(ctx, cudaGetLastError());
     return EF_OK;

@@ -86,3 +86,57 @@ class MoELayerRunner:
 
     def close(self):
         self.ctx.close()
+
+
+class DualBatchRunner:
+    """Two incoming batches of T tokens per step through the Token Scheduler (§3.3, §4.2): schedule on the
+    predicted routing paths -> Reindex activations and per-token rows into the new batches -> the new batches'
+    batch-level predicted paths drive the cache prefetch -> 2 x L layer visits.  Sequencing and buffers only."""
+
+    def __init__(self, runner: MoELayerRunner, max_iter: int = 8):
+        self.r = r = runner
+        T, L, E, d, dev = r.max_tokens, r.L, r.E, r.d, r.dev
+        self.T, self.N, self.max_iter = T, 2 * T, max_iter
+        N = self.N
+        self.batch_of = torch.empty((N,), dtype=torch.int32, device=dev)
+        self.perm = torch.empty((N,), dtype=torch.int32, device=dev)
+        self.info = torch.empty((8,), dtype=torch.int32, device=dev)
+        self.batch_paths = torch.empty((2, L * E), dtype=torch.uint8, device=dev)
+        self.batch_paths_host = torch.empty((2, L * E), dtype=torch.uint8).pin_memory()
+        self.x_re = torch.empty((N, d), dtype=torch.bfloat16, device=dev)
+        self.bias_re = torch.empty((N, L, E), dtype=torch.float32, device=dev)
+        self.hbuf = [torch.empty((T, d), dtype=torch.bfloat16, device=dev) for _ in range(2)]
+
+    def schedule(self, pred_paths: torch.Tensor, c0: int, c1: int, x: torch.Tensor, token_bias: torch.Tensor | None):
+        """pred_paths uint8 [N, L, E], x bf16 [N, d], token_bias fp32 [N, L, E] (all device).  Returns the predicted
+        batch-level rows uint8 [2L, E] (host) of the 2L visits of this step, and leaves x / bias reindexed in
+        self.x_re / self.bias_re.  The one host wait is on the 2*L*E bytes of batch paths the prefetch call needs."""
+        c = self.r.ctx
+        c.ef_token_schedule(pred_paths, c0, c1, self.max_iter, self.batch_of, self.perm, self.info, self.batch_paths)
+        c.ef_reindex_rows(x, self.perm, self.x_re)
+        if token_bias is not None:
+            c.ef_reindex_rows(token_bias, self.perm, self.bias_re)
+        self.batch_paths_host.copy_(self.batch_paths, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        return self.batch_paths_host.numpy().reshape(2 * self.r.L, self.r.E)
+
+    def run_step(self, step: int, rows: np.ndarray, x: torch.Tensor, token_bias: torch.Tensor | None, out: torch.Tensor,
+                 on_visit=None):
+        """x [N, d] / token_bias [N, L, E] in batch order (self.x_re / self.bias_re after schedule(), or the incoming
+        order for the unscheduled arm); rows uint8 [2L, E] host.  out [N, d]: row i = final hidden state of x row i."""
+        r, L, T = self.r, self.r.L, self.T
+        v0 = step * 2 * L
+        r.ctx.ef_cache_prefetch(v0 - 1, rows)
+        for b in range(2):
+            h = x[b * T:(b + 1) * T]
+            for l in range(L):
+                v = v0 + b * L + l
+                dst = out[b * T:(b + 1) * T] if l == L - 1 else self.hbuf[l & 1]
+                nxt = rows[b * L + l + 1:]
+                r.visit(v, h, dst, token_bias=None if token_bias is None else token_bias[b * T:(b + 1) * T, l],
+                        predicted_next=nxt if len(nxt) else None, residual=h if L > 1 else None,
+                        pre_norm_eps=1e-5 if L > 1 else None)
+                if on_visit is not None:
+                    on_visit(v, b, l, dst)
+                h = dst
+        return out

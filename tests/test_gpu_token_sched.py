@@ -31,9 +31,10 @@ def run_schedule(ctx, r, c0, c1, max_iter=16):
     batch_of = torch.full((N,), -7, dtype=torch.int32, device=dev)
     perm = torch.full((N,), -7, dtype=torch.int32, device=dev)
     info = torch.full((8,), -7, dtype=torch.int32, device=dev)
-    ctx.ef_token_schedule(p, c0, c1, max_iter, batch_of, perm, info)
+    bp = torch.full((2, r[0].size), 9, dtype=torch.uint8, device=dev)
+    ctx.ef_token_schedule(p, c0, c1, max_iter, batch_of, perm, info, bp)
     torch.cuda.synchronize()
-    return batch_of.cpu().numpy(), perm.cpu().numpy(), info.cpu().numpy()
+    return batch_of.cpu().numpy(), perm.cpu().numpy(), info.cpu().numpy(), bp.cpu().numpy()
 
 
 def check_against_oracle(ctx, r, c0, c1, max_iter=16):
@@ -41,8 +42,10 @@ def check_against_oracle(ctx, r, c0, c1, max_iter=16):
     ref = ots.schedule(r, c0, c1, max_iter)
     for force_multi in (False, True):
         ctx.ef_set_token_sched_path(force_multi)
-        b, p, info = run_schedule(ctx, r, c0, c1, max_iter)
+        b, p, info, bp = run_schedule(ctx, r, c0, c1, max_iter)
         assert np.array_equal(b, ref.batch_of), force_multi
+        for c in (0, 1):
+            assert np.array_equal(bp[c], ots.batch_path(r, np.flatnonzero(ref.batch_of == c))), force_multi
         assert np.array_equal(p, ref.perm), force_multi
         assert info[:6].tolist() == [ref.iters, int(ref.converged), ref.centroids[0], ref.centroids[1], ref.objective,
                                      ref.objective_before], force_multi
@@ -122,6 +125,23 @@ def test_repeated_calls_reuse_workspace(ctx):
         check_against_oracle(ctx, r, 0, N - 1)
 
 
+@pytest.mark.parametrize("n_src,n,row_elems,dtype", [(64, 64, 256, "bf16"), (100, 37, 8, "f32"), (5, 9, 4096, "bf16"), (3, 0, 8, "f32")])
+def test_reindex_rows(ctx, n_src, n, row_elems, dtype):
+    """Reindex: a pure row gather, bit-exact."""
+    dev = torch.device("cuda", 0)
+    g = np.random.default_rng(n_src + n)
+    if dtype == "bf16":
+        src = torch.from_numpy(g.integers(0, 1 << 15, (n_src, row_elems)).astype(np.int16)).to(dev)
+    else:
+        src = torch.from_numpy(g.standard_normal((n_src, row_elems)).astype(np.float32)).to(dev)
+    perm_np = g.integers(0, n_src, n).astype(np.int32)
+    perm = torch.from_numpy(perm_np).to(dev)
+    dst = torch.zeros((max(n, 1), row_elems), dtype=src.dtype, device=dev)
+    ctx.ef_reindex_rows(src, perm, dst)
+    torch.cuda.synchronize()
+    assert np.array_equal(dst.cpu().numpy()[:n], src.cpu().numpy()[perm_np])
+
+
 def test_bad_arguments_are_codes(ctx):
     from paper_2410_17954_b200.binding import EfError
     dev = torch.device("cuda", 0)
@@ -132,3 +152,71 @@ def test_bad_arguments_are_codes(ctx):
             ctx.ef_token_schedule(p[:N], c0, c1, it, *out)
     with pytest.raises(EfError):
         ctx.ef_token_schedule(p, 0, 1, 65, *out)
+
+
+# ------------------------------------------------------------------------------------------------
+# the scheduler in the path: two incoming batches per step -> schedule -> Reindex -> 2 x L visits (§4.2)
+# ------------------------------------------------------------------------------------------------
+def test_dual_batch_pipeline_matches_oracle_chain():
+    """Reduced dual_batch_stack: assignment, batch paths, slot table and counters bit-exact at every visit; the final
+    hidden state of every token within the float bar, in the ORIGINAL token order after undoing the permutation."""
+    import oracle
+    from oracle.cache_sim import CacheSim
+    from paper_2410_17954_b200 import DualBatchRunner
+    from test_gpu_layer import assert_cache_equal, build_runner
+    from test_gpu_stages import bf, check_float, dev_bf16, to_bits
+
+    cfg = wl.scaled(wl.CONFIGS["dual_batch_stack"], d_model=256, d_ff=512, T=8, n_layers=4, n_slots=10)
+    L, E, T, N = cfg.n_layers, cfg.n_experts, cfg.T, 2 * cfg.T
+    n_steps = 5
+    tr = wl.dual_batch_trace(cfg, n_steps, n_families=2, family_prob=0.85)
+    r, ex = build_runner(cfg, horizon=0)
+    db = DualBatchRunner(r, max_iter=8)
+    sim = CacheSim(L, E, cfg.n_slots, cfg.expert_bytes, 0)
+    wrs = [wl.router_weight(cfg, l) for l in range(L)]
+    dev = torch.device("cuda", 0)
+    g = np.random.default_rng(1)
+    improved = 0
+    for s in range(n_steps):
+        pred_paths = wl.sets_to_paths(tr.pred_sets[s], E)
+        bias = wl.bias_from_sets(cfg, tr.sets[s])
+        x = wl.normal_bf16(cfg.seed, f"x.dual.step{s}", (N, cfg.d_model), 1.0)
+        c0, c1 = (int(v) for v in g.choice(N, 2, replace=False))
+        # oracle side: schedule, Reindex, batch-level predicted paths (Eq. 4 with OR)
+        sc = ots.schedule(pred_paths, c0, c1, 8)
+        rows_ref = np.concatenate([ots.batch_path(pred_paths, sc.perm[b * T:(b + 1) * T]).reshape(L, E) for b in (0, 1)])
+        improved += sc.objective < sc.objective_before
+        # device side
+        rows = db.schedule(torch.from_numpy(pred_paths).to(dev), c0, c1, dev_bf16(x), torch.from_numpy(bias).to(dev))
+        assert np.array_equal(db.perm.cpu().numpy(), sc.perm)
+        assert np.array_equal(rows, rows_ref)
+        assert np.array_equal(to_bits(db.x_re), x[sc.perm])
+        v0 = s * 2 * L
+        sim.prefetch(v0 - 1, rows_ref)
+
+        def on_visit(v, b, l, dst):
+            members = sc.perm[b * T:(b + 1) * T]
+            counts = np.bincount(tr.sets[s][members, l].ravel(), minlength=E)
+            sim.visit(v, counts)
+            nxt = rows_ref[b * L + l + 1:]
+            if len(nxt):
+                sim.prefetch(v, nxt)
+            assert_cache_equal(r, sim)
+
+        out = torch.empty((N, cfg.d_model), dtype=torch.bfloat16, device=dev)
+        db.run_step(s, rows, db.x_re, db.bias_re, out, on_visit=on_visit)
+        r.ctx.ef_sync()
+        got = bf(to_bits(out))
+        # oracle chain per token in the ORIGINAL order: the result must not depend on the batching
+        ref_all = np.zeros((N, cfg.d_model))
+        for b in (0, 1):
+            members = np.arange(b * T, (b + 1) * T)
+            h = x[members]
+            for l in range(L):
+                u = oracle.round_bf16(oracle.rmsnorm(h, 1e-5))
+                ref = oracle.layer_forward(u, wrs[l], bias[members, l], [ex[(l, e)] for e in range(E)], cfg.top_k, res=h)
+                h = oracle.round_bf16(ref.out)
+            ref_all[members] = bf(h)
+        check_float(got, ref_all[sc.perm])
+    assert improved >= 1
+    r.close()

@@ -157,6 +157,11 @@ CONFIGS = {
     "stack_decode": MoEConfig("stack_decode", T=64, d_model=4096, d_ff=14336, n_experts=8, top_k=2,
                               n_slots=64, n_layers=32, n_steps=128, seed=5, bias_kind="trace",
                               layer_corr=0.5, pred_acc=0.8, horizon=0),
+    # f1: the cfg 5 stack fed by TWO incoming batches of 16 decode tokens per step, rebatched by the Token Scheduler
+    # (PAPER.md 3.3 / 4.2); same shapes, cache and predictor accuracy as cfg 5
+    "dual_batch_stack": MoEConfig("dual_batch_stack", T=16, d_model=4096, d_ff=14336, n_experts=8, top_k=2,
+                                  n_slots=64, n_layers=32, n_steps=64, seed=6, bias_kind="trace",
+                                  pred_acc=0.8, horizon=0),
 }
 
 
@@ -305,3 +310,61 @@ def token_paths(seed: int, n_tokens: int, n_layers: int, n_experts: int, top_k: 
             es = fam_sets[fam[i], l] if g.random() < family_prob else _draw_set(g, pops[l], top_k)
             r[i, l, es] = 1
     return r
+
+
+# ----------------------------------------------------------------------------
+# dual-batch decode traces (Token Scheduler end to end; §3.3, §4.2)
+# ----------------------------------------------------------------------------
+@dataclass
+class DualBatchTrace:
+    """Two incoming batches of cfg.T tokens per step (global token index i < N = 2T: batch i // T, P:L153).
+    sets[s, i, l] is the ordered k-tuple of experts token i is driven to in layer l at step s; pred_sets is the
+    routing-path predictor's output for the same token (R17: equal to sets with prob pred_acc, else a uniform
+    random k-subset, drawn per token and layer)."""
+    sets: np.ndarray         # int32 [n_steps, N, L, k]
+    pred_sets: np.ndarray    # int32 [n_steps, N, L, k]
+    family: np.ndarray       # int32 [N] latent group of every sequence slot (kept over the steps)
+
+
+def dual_batch_trace(cfg: MoEConfig, n_steps: int, n_families: int = 2, family_prob: float = 0.8) -> DualBatchTrace:
+    """Sequence slots belong to latent families ("tokens sharing similar routing paths") that are mixed at
+    random over the two incoming batches.  Per step and layer a token takes its family's expert set with
+    probability family_prob, else a fresh draw from the layer's popularity."""
+    L, T, k, E = cfg.n_layers, cfg.T, cfg.top_k, cfg.n_experts
+    N = 2 * T
+    g = stream(cfg.seed, f"dualtrace.F{n_families}")
+    pops = []
+    for l in range(L):
+        o = g.standard_normal(E)
+        p = np.exp(o - o.max())
+        pops.append(p / p.sum())
+    fam_sets = np.zeros((n_families, L, k), np.int32)
+    for f in range(n_families):
+        for l in range(L):
+            fam_sets[f, l] = _draw_set(g, pops[l], k)
+    family = g.integers(0, n_families, size=N).astype(np.int32)
+    sets = np.zeros((n_steps, N, L, k), np.int32)
+    pred = np.zeros_like(sets)
+    for s in range(n_steps):
+        for i in range(N):
+            for l in range(L):
+                sets[s, i, l] = fam_sets[family[i], l] if g.random() < family_prob else _draw_set(g, pops[l], k)
+                pred[s, i, l] = sets[s, i, l] if g.random() < cfg.pred_acc else g.choice(E, size=k, replace=False)
+    return DualBatchTrace(sets=sets, pred_sets=pred, family=family)
+
+
+def sets_to_paths(sets: np.ndarray, n_experts: int) -> np.ndarray:
+    """[N, L, k] expert ids -> binary routing-path matrices uint8 [N, L, E]."""
+    N, L, _ = sets.shape
+    r = np.zeros((N, L, n_experts), np.uint8)
+    r[np.arange(N)[:, None, None], np.arange(L)[None, :, None], sets] = 1
+    return r
+
+
+def bias_from_sets(cfg: MoEConfig, sets: np.ndarray) -> np.ndarray:
+    """fp32 [N, L, E] router bias that drives token i in layer l to sets[i, l] in order (as trace_bias does)."""
+    N, L, k = sets.shape
+    b = np.zeros((N, L, cfg.n_experts), np.float32)
+    for j in range(k):
+        b[np.arange(N)[:, None], np.arange(L)[None, :], sets[:, :, j]] = np.float32(cfg.trace_margin + (k - 1 - j))
+    return b
