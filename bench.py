@@ -29,6 +29,8 @@ if ROOT not in sys.path:
 
 import workloads as wl  # noqa: E402
 
+DUAL_FAMILIES, DUAL_FAMILY_PROB = 2, 0.9     # dual_batch_stack: latent token groups
+
 METRIC = "moe_layer_tokens_per_s"
 UNIT = "tokens/s"
 
@@ -222,6 +224,39 @@ def oracle_sample(cfg, n_tokens: int, n_layers: int, cache=None):
     return n_tokens / step_s, dt, oracle.num_threads(), what
 
 
+def oracle_sample_dual(cfg, n_tokens: int, n_layers: int, cache=None):
+    """dual_batch_stack: the oracle on the first n_tokens tokens of incoming batch 0 of step 0 through the first
+    n_layers layers (unscheduled order: the layer result does not depend on the batching)."""
+    import oracle
+    L = cfg.n_layers
+    n_layers = max(1, min(L, n_layers))
+    n_tokens = max(1, min(cfg.T, n_tokens))
+    cache = cache if cache is not None else {}
+    tr = wl.dual_batch_trace(cfg, 1, DUAL_FAMILIES, DUAL_FAMILY_PROB)
+    bias = wl.bias_from_sets(cfg, tr.sets[0])[:n_tokens]
+    x = wl.normal_bf16(cfg.seed, "x.dual.step0.rank0", (2 * cfg.T, cfg.d_model), 1.0)[:n_tokens]
+
+    def get(l, e):
+        if (l, e) not in cache:
+            cache[(l, e)] = wl.expert_weights(cfg, l, e, threads=os.cpu_count() or 8)
+        return cache[(l, e)]
+    wrs = [wl.router_weight(cfg, l) for l in range(n_layers)]
+    for l in range(n_layers):
+        for e in sorted(set(int(v) for v in tr.sets[0][:n_tokens, l].ravel())):
+            get(l, e)
+    t0 = time.perf_counter()
+    h = x
+    for l in range(n_layers):
+        u = oracle.round_bf16(oracle.rmsnorm(h, 1e-5))
+        ref = oracle.layer_forward(u, wrs[l], bias[:, l], lambda e, l=l: get(l, e), cfg.top_k, cfg.renorm, res=h)
+        h = oracle.round_bf16(ref.out)
+    dt = time.perf_counter() - t0
+    step_s = dt * L / n_layers
+    what = (f"first {n_tokens} tokens of incoming batch 0 of step 0 of {cfg.name} through the first {n_layers} of {L} "
+            f"layers, whole layer in fp64 ({dt:.1f} s; scaled x{L / n_layers:g}), weights pre-generated, no cache, no scheduler")
+    return n_tokens / step_s, dt, oracle.num_threads(), what
+
+
 def ref_sample_size(cfg, args):
     """Bounded oracle sample: ~10-30 s of CPU work on a 16-core host."""
     n_tok = args.ref_tokens if args.ref_tokens > 0 else {"mixtral_prefill": 256, "many_expert_prefill": 1024}.get(cfg.name, cfg.T)
@@ -237,8 +272,9 @@ def run_reference(args):
     n_tok, n_lay = ref_sample_size(cfg, args)
     cache = {}
     vals = []
+    sample = oracle_sample_dual if cfg.name == "dual_batch_stack" else oracle_sample
     for i in range(args.warmup + args.steps):
-        v, dt, cores, what = oracle_sample(cfg, n_tok, n_lay, cache)
+        v, dt, cores, what = sample(cfg, n_tok, n_lay, cache)
         if i >= args.warmup:
             vals.append((v, dt))
     value = float(np.mean([v for v, _ in vals]))
@@ -497,6 +533,157 @@ def run_ours(args):
         print(json.dumps(line), flush=True)
 
 
+def run_dual_batch(args):
+    """dual_batch_stack: per step TWO incoming batches of T decode tokens go through the Token Scheduler (on the
+    predicted routing paths), Reindex, and 2 x L layer visits; the same steps are also run unscheduled (incoming
+    batches as they are).  value = tokens/s with the scheduler on."""
+    import torch
+    from paper_2410_17954_b200 import DualBatchRunner, MoELayerRunner
+    from paper_2410_17954_b200.layer import bf16_tensor_from_bits
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    rank, local, world = dist_init("nccl")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    cfg = wl.CONFIGS["dual_batch_stack"]
+    L, E, T, d, f = cfg.n_layers, cfg.n_experts, cfg.T, cfg.d_model, cfg.d_ff
+    N = 2 * T
+    peaks = measured_peaks()
+    log = (lambda m: print(f"[bench] {m}", file=sys.stderr, flush=True)) if rank == 0 else (lambda m: None)
+    phys = args.phys_experts if args.phys_experts > 0 else 32       # 32 physical host buffers (11 GB) behind 256 logical experts
+    runner = MoELayerRunner(L, E, cfg.top_k, d, f, cfg.n_slots, 0, T, cfg.horizon, cfg.renorm, device=dev.index)
+    gen_cfg = wl.scaled(cfg, phys_experts=phys)
+    threads = os.cpu_count() or 8
+    for l in range(L):
+        runner.set_router(l, wl.router_weight(cfg, l), None)
+        for e in range(E):
+            g = l * E + e
+            if g >= phys:
+                runner.ctx.ef_host_expert_alias(l, e, (g % phys) // E, (g % phys) % E)
+            else:
+                runner.register_expert(l, e, *wl.expert_weights(gen_cfg, l, e, threads=threads))
+    log(f"registered {phys} physical / {L * E} logical experts")
+    db = DualBatchRunner(runner, max_iter=8)
+    ts = max(1, min(cfg.n_steps, 2 * (args.steps + args.warmup) + 2))
+    tr = wl.dual_batch_trace(cfg, ts, DUAL_FAMILIES, DUAL_FAMILY_PROB)
+    pred_paths = np.stack([wl.sets_to_paths(tr.pred_sets[s], E) for s in range(ts)])             # [ts, N, L, E] uint8
+    bias = np.stack([wl.bias_from_sets(cfg, tr.sets[s]) for s in range(ts)])                     # [ts, N, L, E] fp32
+    xs = np.stack([wl.normal_bf16(cfg.seed, f"x.dual.step{s}.rank{rank}", (N, d), 1.0) for s in range(ts)])
+    paths_pin = torch.from_numpy(pred_paths).pin_memory(); paths_dev = paths_pin.to(dev)
+    bias_pin = torch.from_numpy(bias).pin_memory(); bias_dev = bias_pin.to(dev)
+    x_pin = bf16_tensor_from_bits(xs, pin=True); x_dev = x_pin.to(dev)
+    paths_stage, bias_stage, x_stage = torch.empty_like(paths_dev[0]), torch.empty_like(bias_dev[0]), torch.empty_like(x_dev[0])
+    out = torch.empty((N, d), dtype=torch.bfloat16, device=dev)
+    out_pin = torch.empty((N, d), dtype=torch.bfloat16).pin_memory()
+    # unscheduled arm: the predicted batch-level rows of the incoming batches [0, T) and [T, 2T) (the baseline's own
+    # plumbing, on the host); initial centroids: one seeded draw per step (P:L173 "random centroid selection")
+    rows_off = [np.concatenate([pred_paths[s][b * T:(b + 1) * T].max(axis=0) for b in (0, 1)]) for s in range(ts)]
+    cg = wl.stream(cfg.seed, "dual.centroids")
+    cents = [tuple(int(v) for v in cg.choice(N, 2, replace=False)) for _ in range(ts)]
+    state = {"step": 0}
+
+    def step(sched: bool, e2e: bool):
+        s = state["step"] % ts
+        if e2e:
+            paths_stage.copy_(paths_pin[s], non_blocking=True); bias_stage.copy_(bias_pin[s], non_blocking=True)
+            x_stage.copy_(x_pin[s], non_blocking=True)
+            p, b, x = paths_stage, bias_stage, x_stage
+        else:
+            p, b, x = paths_dev[s], bias_dev[s], x_dev[s]
+        if sched:
+            rows = db.schedule(p, cents[s][0], cents[s][1], x, b)
+            x, b = db.x_re, db.bias_re
+        else:
+            rows = rows_off[s]
+        db.run_step(state["step"], rows, x, b, out)
+        state["step"] += 1
+        if e2e:
+            out_pin.copy_(out, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+
+    def timed(sched, e2e, steps, warmup, with_kernel_times=False):
+        runner.ctx.ef_sync(); runner.ctx.ef_cache_clear()
+        state["step"] = 0
+        for _ in range(warmup):
+            step(sched, e2e)
+        runner.ctx.ef_sync(); runner.ctx.ef_cache_reset_stats()
+        if with_kernel_times:
+            runner.ctx.ef_get_kernel_times(reset=True); runner.ctx.ef_set_kernel_timing(True)
+        l0 = runner.ctx.ef_launch_count()
+        dist_barrier(); torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            step(sched, e2e)
+        e1.record()
+        runner.ctx.ef_sync(); torch.cuda.synchronize(); dist_barrier()
+        ms = dist_max(e0.elapsed_time(e1), dev)
+        kt = None
+        if with_kernel_times:
+            kt = runner.ctx.ef_get_kernel_times(reset=True); runner.ctx.ef_set_kernel_timing(False)
+        st = runner.ctx.ef_cache_get_stats()
+        copy_ms = runner.ctx.ef_copy_busy_ms()
+        return {"ms": ms, "launches": runner.ctx.ef_launch_count() - l0, "kt": kt, "st": st, "copy_ms": copy_ms}
+
+    def arm_summary(res, steps):
+        st = res["st"]
+        return {"tokens_per_s": world * N * steps / (res["ms"] * 1e-3), "ms_per_step": res["ms"] / steps,
+                "loads_per_step": (st["ondemand_loads"] + st["prefetch_issued"]) / steps,
+                "active_experts_per_visit": st["lookups"] / (steps * 2 * L), "hit_ratio": st["hits"] / max(1, st["lookups"]),
+                "bytes_h2d_per_step": st["bytes_h2d"] / steps, "ondemand_loads_per_step": st["ondemand_loads"] / steps}
+
+    runner.ctx.ef_sync()
+    h2d_peak = measure_pinned_h2d(dev, cfg.expert_bytes) if rank == 0 else None
+    off = timed(False, False, args.steps, args.warmup)
+    sampler = ClockSampler(local); sampler.start()
+    on = timed(True, False, args.steps, args.warmup, with_kernel_times=True)
+    clocks = sampler.stop()
+    e2e = timed(True, True, args.steps, max(1, args.warmup // 2))
+    # the scheduler call alone (schedule + Reindex + batch-path read-back), CUDA events around 20 calls
+    torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    objs = []
+    e0.record()
+    for i in range(20):
+        db.schedule(paths_dev[i % ts], cents[i % ts][0], cents[i % ts][1], x_dev[i % ts], bias_dev[i % ts])
+        objs.append(db.info.cpu().numpy().copy())
+    e1.record(); e1.synchronize()
+    sched_us = e0.elapsed_time(e1) / 20 * 1e3
+    objs = np.array(objs)
+    roofline = ffn_roofline(on["kt"], d, f, peaks, True, "streaming steps with the Token Scheduler on")
+    st = on["st"]
+    h2d = {"bytes_per_step": st["bytes_h2d"] / args.steps, "copy_busy_ms_per_step": on["copy_ms"] / args.steps,
+           "achieved_gbs": st["bytes_h2d"] / (on["copy_ms"] * 1e-3) / 1e9 if on["copy_ms"] > 0 else None, "peak_gbs": h2d_peak,
+           "frac": (st["bytes_h2d"] / (on["copy_ms"] * 1e-3) / 1e9 / h2d_peak) if on["copy_ms"] > 0 and h2d_peak else None}
+    runner.close()
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n_tok, n_lay = ref_sample_size(cfg, args)
+        v, dt, cores, what = oracle_sample_dual(cfg, n_tok, n_lay)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}
+    if rank == 0:
+        a_on, a_off = arm_summary(on, args.steps), arm_summary(off, args.steps)
+        io_h2d = N * d * 2 + N * L * E * 4 + N * L * E
+        line = {"metric": METRIC, "value": a_on["tokens_per_s"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": a_on["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "config": workload_config(cfg, world, {"tokens_per_step_per_gpu": N, "visits_per_step": 2 * L,
+                                                       "phys_host_experts": phys, "token_families": DUAL_FAMILIES,
+                                                       "family_prob": DUAL_FAMILY_PROB, "scheduler_max_iter": 8}),
+                "clocks": clocks,
+                "e2e": {"value": world * N * args.steps / (e2e["ms"] * 1e-3), "unit": UNIT,
+                        "h2d_bytes_per_step": io_h2d + int(e2e["st"]["bytes_h2d"] / args.steps), "d2h_bytes_per_step": N * d * 2 + 2 * L * E,
+                        "ms_per_step": e2e["ms"] / args.steps,
+                        "note": "predicted paths, router bias and x from pinned host memory, out back to pinned host memory every step"},
+                "gpu_launches": on["launches"], "roofline": roofline, "h2d": h2d,
+                "token_scheduler": {"on": a_on, "off": a_off, "speedup": a_on["tokens_per_s"] / a_off["tokens_per_s"],
+                                    "schedule_call_us": sched_us,
+                                    "eq5_objective_predicted_paths": {"incoming": float(objs[:, 5].mean()), "scheduled": float(objs[:, 4].mean())},
+                                    "kmeans_rounds_mean": float(objs[:, 0].mean()), "converged_frac": float(objs[:, 1].mean())},
+                "cache": dict(st, hit_ratio=st["hits"] / max(1, st["lookups"])), "cpu_baseline": cpu_baseline}
+        print(json.dumps(line), flush=True)
+
+
 def ffn_roofline(kt, d, f, peaks, decode, where):
     """Roofline of the dominant kernel (GEMM1 of the grouped FFN) from the library's per-launch CUDA events."""
     t1, t2 = kt["gemm1_ms"] * 1e-3, kt["gemm2_ms"] * 1e-3
@@ -586,6 +773,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "dual_batch_stack":
+        run_dual_batch(args)
     else:
         run_ours(args)
 
