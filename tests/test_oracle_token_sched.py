@@ -242,3 +242,35 @@ def test_generated_token_paths_have_topk_ones_per_layer():
     assert r.shape == (64, 4, 8) and r.dtype == np.uint8
     assert (r.sum(axis=2) == 2).all()
     assert np.array_equal(r, wl.token_paths(seed=7, n_tokens=64, n_layers=4, n_experts=8, top_k=2, n_families=2, family_prob=0.8))
+
+
+def test_scheduled_batches_need_fewer_loads_in_the_cache_simulator():
+    """The paper's claim for the scheduler ('reduces I/O overhead by decreasing expert loads'), checked on
+    the policy simulator: a perfect predictor, two families, 2 x 8 tokens through a 6-layer stack."""
+    from oracle.cache_sim import CacheSim
+    cfg = wl.scaled(wl.CONFIGS["dual_batch_stack"], T=8, n_layers=6, n_slots=12, pred_acc=1.0)
+    L, E, T = cfg.n_layers, cfg.n_experts, cfg.T
+    tr = wl.dual_batch_trace(cfg, 12, n_families=2, family_prob=0.9)
+    loads, active = {}, {}
+    for sched in (False, True):
+        sim = CacheSim(L, E, cfg.n_slots, 1000, 0)
+        n_active = 0
+        for s in range(12):
+            paths = wl.sets_to_paths(tr.pred_sets[s], E)
+            perm = ts.schedule(paths, 0, 2 * T - 1, 8).perm if sched else np.arange(2 * T)
+            rows = np.concatenate([ts.batch_path(paths, perm[b * T:(b + 1) * T]).reshape(L, E) for b in (0, 1)])
+            v0 = s * 2 * L
+            sim.prefetch(v0 - 1, rows)
+            for b in (0, 1):
+                for l in range(L):
+                    v = v0 + b * L + l
+                    counts = np.bincount(tr.sets[s][perm[b * T:(b + 1) * T], l].ravel(), minlength=E)
+                    n_active += int((counts > 0).sum())
+                    sim.visit(v, counts)
+                    if len(rows[b * L + l + 1:]):
+                        sim.prefetch(v, rows[b * L + l + 1:])
+        loads[sched] = sim.stats["ondemand_loads"] + sim.stats["prefetch_issued"]
+        active[sched] = n_active
+        assert sim.stats["misses"] == 0                      # perfect prediction, pool >= two visits' active sets
+    assert active[True] < active[False]
+    assert loads[True] < loads[False]
