@@ -452,8 +452,29 @@ extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visi
         locked[s] = 1;
         wavesA.push_back(WaveItem{off[e], counts_host[e], s});
     }
-    int32_t rc = run_wave(ctx, st, x_perm, y_perm, wave0);
-    if (rc != EF_OK) return rc;
+    // Wave 0 = the hits.  A pending phase-B load may be about to overwrite the slot of one of these very hits, and its
+    // copy waits for the "free" event of the wave that read the slot.  Copies are far slower than waves, so only the
+    // FIRST victim matters: it is known already (phase B's first pick depends on the table, not on execution), and
+    // when it is a hit that hit runs as its own wave first, so the copy starts after one expert's FFN instead of
+    // after the whole wave (physical ordering only: the policy and its accounting are unchanged).
+    int32_t rc = EF_OK;
+    int first_victim = -1;
+    if (!rest.empty() && wave0.size() > 1) first_victim = pick_victim(ctx, visit, visit, true, std::vector<char>(c.n_slots, 0));
+    size_t split_at = wave0.size();
+    for (size_t i = 0; i < wave0.size(); ++i)
+        if (wave0[i].slot == first_victim) split_at = i;
+    if (split_at == wave0.size()) {
+        rc = run_wave(ctx, st, x_perm, y_perm, wave0);
+        if (rc != EF_OK) return rc;
+    } else {
+        std::vector<WaveItem> others;
+        for (size_t i = 0; i < wave0.size(); ++i)
+            if (i != split_at) others.push_back(wave0[i]);
+        rc = run_wave(ctx, st, x_perm, y_perm, std::vector<WaveItem>{wave0[split_at]});
+        if (rc != EF_OK) return rc;
+        rc = run_wave(ctx, st, x_perm, y_perm, others);
+        if (rc != EF_OK) return rc;
+    }
     for (const WaveItem& it : wavesA) {   // one wave each: compute starts as each copy lands
         rc = run_wave(ctx, st, x_perm, y_perm, std::vector<WaveItem>{it});
         if (rc != EF_OK) return rc;
