@@ -5,6 +5,7 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 never imports ``paper_2410_17954_b200``.
 
 * ``moe_oracle.c``  -- layer math, the plain definition (Eq. 1-2).
+* ``token_sched.py`` -- the Token Scheduler of PAPER.md §3.3, step by step (integers only).
 * ``cache_sim.py``  -- the expert-cache policy, step by step, integers only (§8(c) O2;
   PAPER.md §3.2.1, §3.2.2, §4.1).
 * this file        -- builds the C file with gcc for the host it runs on and wraps it with ctypes;
@@ -129,13 +130,19 @@ def gather_rows(x, src, k):
 
 
 def expert_ffn(xrows, wg, wu, wd, want_h=False, real="double"):
-    """SwiGLU expert on M rows.  Returns y [M,d] (and h [M,f] if want_h)."""
-    xrows = _c(xrows, np.uint16); wg = _c(wg, np.uint16); wu = _c(wu, np.uint16); wd = _c(wd, np.uint16)
+    """One expert on M rows.  wu given: SwiGLU (wg, wu, wd).  wu None: the Switch-style non-gated ReLU FFN with
+    W1 = wg, W2 = wd (R30).  Returns y [M,d] (and h [M,f] if want_h)."""
+    xrows = _c(xrows, np.uint16); wg = _c(wg, np.uint16); wd = _c(wd, np.uint16)
     M, d = xrows.shape; f = wg.shape[0]
-    assert wg.shape == (f, d) and wu.shape == (f, d) and wd.shape == (d, f)
+    assert wg.shape == (f, d) and wd.shape == (d, f)
     y = np.empty((M, d), dtype=_rdt(real))
     h = np.empty((M, f), dtype=_rdt(real)) if want_h else None
-    _lib(real).orc_expert_ffn(_p(xrows), ctypes.c_int64(M), d, f, _p(wg), _p(wu), _p(wd), _p(y), _p(h))
+    if wu is None:
+        _lib(real).orc_expert_ffn_relu(_p(xrows), ctypes.c_int64(M), d, f, _p(wg), _p(wd), _p(y), _p(h))
+    else:
+        wu = _c(wu, np.uint16)
+        assert wu.shape == (f, d)
+        _lib(real).orc_expert_ffn(_p(xrows), ctypes.c_int64(M), d, f, _p(wg), _p(wu), _p(wd), _p(y), _p(h))
     return (y, h) if want_h else y
 
 

@@ -158,6 +158,28 @@ void orc_expert_ffn(const uint16_t* xrows, int64_t M, int d, int f, const uint16
     }
 }
 
+/* Switch-style expert (R30): the non-gated ReLU FFN of the Switch / T5 models the paper evaluates,
+ * without biases:  h_n = max(0, sum_d x[r,d] W1[n,d]);  y[r,c] = sum_n h_n W2[c,n].
+ * xrows: [M, d] bf16; w1: [f, d] bf16; w2: [d, f] bf16; y: [M, d] real; h_out (nullable): [M, f]. */
+void orc_expert_ffn_relu(const uint16_t* xrows, int64_t M, int d, int f, const uint16_t* w1, const uint16_t* w2,
+                         real* y, real* h_out) {
+#pragma omp parallel
+    {
+        real* h = (real*)malloc((size_t)f * sizeof(real));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t r = 0; r < M; ++r) {
+            const uint16_t* xr = xrows + r * d;
+            for (int n = 0; n < f; ++n) {
+                real a = dot_bf16(xr, w1 + (int64_t)n * d, d);
+                h[n] = a > (real)0 ? a : (real)0;
+            }
+            if (h_out) memcpy(h_out + r * f, h, (size_t)f * sizeof(real));
+            for (int c = 0; c < d; ++c) y[r * d + c] = dot_real_bf16(h, w2 + (int64_t)c * f, f);
+        }
+        free(h);
+    }
+}
+
 /* Combine (Eq. 2 summed over the k selected experts):
  *   out[t,c] = res[t,c] + sum_j w[t,j] * y_perm[inv[t*k+j], c] + y_shared[t,c]
  * res (bf16, nullable), y_shared (real, nullable). */

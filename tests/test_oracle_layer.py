@@ -313,3 +313,66 @@ def test_configs_min_routing_margin():
     l = oracle.router_logits(wl.activations(cfg), wl.router_weight(cfg), wl.static_router_bias(cfg))
     srt = np.sort(l, axis=1)[:, ::-1]
     assert (srt[:, cfg.top_k - 1] - srt[:, cfg.top_k]).min() > 1e-4
+
+
+# ------------------------------------------------------------------------------------------------
+# Switch-style non-gated ReLU experts (R30; the paper's Switch-32/64/128 models)
+# ------------------------------------------------------------------------------------------------
+def _relu_case(seed=0, T=24, d=64, f=96, E=4):
+    cfg = wl.MoEConfig("relu_case", T=T, d_model=d, d_ff=f, n_experts=E, top_k=1, n_slots=2, seed=seed, renorm=0,
+                       expert_kind="relu")
+    x = wl.activations(cfg)
+    wr = wl.router_weight(cfg)
+    experts = [wl.expert_weights(cfg, 0, e) for e in range(E)]
+    return cfg, x, wr, experts
+
+
+def test_relu_expert_matches_numpy_and_is_not_swiglu():
+    cfg, x, wr, experts = _relu_case()
+    w1, none, w2 = experts[0]
+    assert none is None
+    X = wl.bf16_bits_to_f32(x).astype(np.float64)
+    W1 = wl.bf16_bits_to_f32(w1).astype(np.float64)
+    W2 = wl.bf16_bits_to_f32(w2).astype(np.float64)
+    y, h = oracle.expert_ffn(x, w1, None, w2, want_h=True)
+    pre = X @ W1.T
+    assert np.allclose(h, np.maximum(pre, 0.0), rtol=1e-12, atol=1e-15)
+    assert (h >= 0).all() and (h[pre < 0] == 0).all() and (pre < 0).any()
+    assert np.allclose(y, np.maximum(pre, 0.0) @ W2.T, rtol=1e-11, atol=1e-14)
+    # not the gated expert with the same first matrix
+    y_gated = oracle.expert_ffn(x, w1, w1, w2)
+    assert not np.allclose(y, y_gated, rtol=1e-3)
+
+
+def test_relu_expert_is_positively_homogeneous_but_not_odd():
+    """A bias-free ReLU FFN satisfies FFN(a x) = a FFN(x) for a > 0 (exactly, for a power of two in bf16) and
+    FFN(-x) != -FFN(x): catches a missing / misplaced nonlinearity."""
+    cfg, x, wr, experts = _relu_case(seed=3)
+    w1, _, w2 = experts[1]
+    xf = wl.bf16_bits_to_f32(x)
+    x4 = wl.f32_to_bf16_bits(xf * 4.0)
+    xn = wl.f32_to_bf16_bits(-xf)
+    y = oracle.expert_ffn(x, w1, None, w2)
+    assert np.allclose(oracle.expert_ffn(x4, w1, None, w2), 4.0 * y, rtol=1e-12)
+    yn = oracle.expert_ffn(xn, w1, None, w2)
+    assert not np.allclose(yn, -y, rtol=1e-2)
+    # relu(-a) + relu(a) = |a|: FFN(x) + FFN(-x) = |x W1^T| W2^T
+    W1 = wl.bf16_bits_to_f32(w1).astype(np.float64); W2 = wl.bf16_bits_to_f32(w2).astype(np.float64)
+    assert np.allclose(y + yn, np.abs(xf.astype(np.float64) @ W1.T) @ W2.T, rtol=1e-10, atol=1e-13)
+
+
+def test_switch_layer_top1_full_softmax_weight_and_identical_experts():
+    """Eq. 2 as printed: top-1 and the gate weight is the full softmax probability (renorm=0); with
+    identical experts the layer is p_max(x) * dense ReLU FFN(x)."""
+    cfg, x, wr, experts = _relu_case(seed=5)
+    same = [experts[2]] * cfg.n_experts
+    ref = oracle.layer_forward(x, wr, None, same, 1, renorm=0)
+    X = wl.bf16_bits_to_f32(x).astype(np.float64)
+    logits = X @ wl.bf16_bits_to_f32(wr).astype(np.float64).T
+    p = np.exp(logits - logits.max(axis=1, keepdims=True))
+    p /= p.sum(axis=1, keepdims=True)
+    assert np.array_equal(ref.idx[:, 0], logits.argmax(axis=1))
+    assert np.allclose(ref.w[:, 0], p.max(axis=1), rtol=1e-12)
+    W1 = wl.bf16_bits_to_f32(same[0][0]).astype(np.float64); W2 = wl.bf16_bits_to_f32(same[0][2]).astype(np.float64)
+    dense = np.maximum(X @ W1.T, 0.0) @ W2.T
+    assert np.allclose(ref.out, p.max(axis=1, keepdims=True) * dense, rtol=1e-10, atol=1e-14)

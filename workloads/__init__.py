@@ -126,6 +126,7 @@ class MoEConfig:
     horizon: int = 0           # prefetch horizon in visits; <=0 = fill
     trace_margin: float = 12.0
     phys_experts: int = 0      # >0: alias logical experts onto this many physical host buffers
+    expert_kind: str = "swiglu"  # swiglu (BASELINE.json) | relu: Switch-style non-gated FFN (R30)
 
     @property
     def R(self) -> int:
@@ -133,7 +134,7 @@ class MoEConfig:
 
     @property
     def expert_bytes(self) -> int:
-        return 3 * self.d_model * self.d_ff * 2
+        return (3 if self.expert_kind == "swiglu" else 2) * self.d_model * self.d_ff * 2
 
     @property
     def n_visits(self) -> int:
@@ -157,6 +158,10 @@ CONFIGS = {
     "stack_decode": MoEConfig("stack_decode", T=64, d_model=4096, d_ff=14336, n_experts=8, top_k=2,
                               n_slots=64, n_layers=32, n_steps=128, seed=5, bias_kind="trace",
                               layer_corr=0.5, pred_acc=0.8, horizon=0),
+    # f4: Switch-style layer (the paper's own model family: Switch-32/64/128): top-1, gate weight = full
+    # softmax probability (Eq. 2, renorm=0), non-gated ReLU experts of Switch-base size, cache of 16 of 64 experts
+    "switch_prefill": MoEConfig("switch_prefill", T=4096, d_model=768, d_ff=3072, n_experts=64, top_k=1, n_slots=16,
+                                seed=7, renorm=0, bias_kind="zipf", zipf_s=1.1, expert_kind="relu"),
     # f1: the cfg 5 stack fed by TWO incoming batches of 16 decode tokens per step, rebatched by the Token Scheduler
     # (PAPER.md 3.3 / 4.2); same shapes, cache and predictor accuracy as cfg 5
     "dual_batch_stack": MoEConfig("dual_batch_stack", T=16, d_model=4096, d_ff=14336, n_experts=8, top_k=2,
@@ -197,7 +202,7 @@ def expert_weights(cfg: MoEConfig, layer: int, expert: int, threads: int = 8):
         tag = f"l{layer}.shared{-1 - expert}"
     f, d = cfg.d_ff, cfg.d_model
     wg = normal_bf16(cfg.seed, f"wg.{tag}", (f, d), cfg.w_std, threads)
-    wu = normal_bf16(cfg.seed, f"wu.{tag}", (f, d), cfg.w_std, threads)
+    wu = normal_bf16(cfg.seed, f"wu.{tag}", (f, d), cfg.w_std, threads) if cfg.expert_kind == "swiglu" else None
     wd = normal_bf16(cfg.seed, f"wd.{tag}", (d, f), cfg.w_std, threads)
     return wg, wu, wd
 
