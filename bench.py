@@ -259,7 +259,7 @@ def oracle_sample_dual(cfg, n_tokens: int, n_layers: int, cache=None):
 
 def ref_sample_size(cfg, args):
     """Bounded oracle sample: ~10-30 s of CPU work on a 16-core host."""
-    n_tok = args.ref_tokens if args.ref_tokens > 0 else {"mixtral_prefill": 256, "many_expert_prefill": 1024}.get(cfg.name, cfg.T)
+    n_tok = args.ref_tokens if args.ref_tokens > 0 else {"mixtral_prefill": 256, "many_expert_prefill": 1024, "switch_prefill": 4096}.get(cfg.name, cfg.T)
     n_lay = args.ref_layers if args.ref_layers > 0 else (2 if cfg.n_layers > 1 else 1)
     return n_tok, n_lay
 
@@ -302,7 +302,7 @@ class Driver:
         self.torch, self.cfg, self.dev = torch, cfg, dev
         L, E, T, d = cfg.n_layers, cfg.n_experts, cfg.T, cfg.d_model
         self.runner = r = MoELayerRunner(L, E, cfg.top_k, d, cfg.d_ff, cfg.n_slots, cfg.n_shared, T, cfg.horizon,
-                                         cfg.renorm, device=dev.index)
+                                         cfg.renorm, device=dev.index, expert_kind=1 if cfg.expert_kind == "relu" else 0)
         threads = os.cpu_count() or 8
         n_total = L * E
         self.phys = phys_experts if 0 < phys_experts < n_total else 0
@@ -486,11 +486,13 @@ def run_ours(args):
 
     d, f = cfg.d_model, cfg.d_ff
     decode = cfg.T * cfg.top_k / cfg.n_experts < 249 and cfg.name in ("mixtral_decode", "stack_decode")
-    roofline = ffn_roofline(kt, d, f, peaks, decode, "streaming step (one wave of hits + one wave per miss)")
+    roofline = ffn_roofline(kt, d, f, peaks, decode, "streaming step (one wave of hits + one wave per miss)",
+                            gated=cfg.expert_kind == "swiglu")
     roofline["traffic"] = NCU_TRAFFIC_BYTES.get(cfg.name)
     roofline["traffic_source"] = ("bytes per GEMM1 launch from the committed ncu capture under profiles/ (see NCU_TRAFFIC_BYTES)"
                                   if cfg.name in NCU_TRAFFIC_BYTES else "no ncu capture for this workload")
-    roofline["algorithmic_bytes_per_launch"] = (4.0 * d * f * kt["groups"] + 2.0 * d * kt["rows"] + 2.0 * f * kt["rows"]) / max(1, kt["gemm1_launches"])
+    roofline["algorithmic_bytes_per_launch"] = ((4.0 if cfg.expert_kind == "swiglu" else 2.0) * d * f * kt["groups"]
+                                                + 2.0 * d * kt["rows"] + 2.0 * f * kt["rows"]) / max(1, kt["gemm1_launches"])
 
     h2d = {"bytes_per_step": st["bytes_h2d"] / args.steps, "loads_per_step": (st["ondemand_loads"] + st["prefetch_issued"]) / args.steps,
            "copy_busy_ms_per_step": copy_ms / args.steps,
@@ -684,12 +686,14 @@ def run_dual_batch(args):
         print(json.dumps(line), flush=True)
 
 
-def ffn_roofline(kt, d, f, peaks, decode, where):
-    """Roofline of the dominant kernel (GEMM1 of the grouped FFN) from the library's per-launch CUDA events."""
+def ffn_roofline(kt, d, f, peaks, decode, where, gated=True):
+    """Roofline of the dominant kernel (GEMM1 of the grouped FFN) from the library's per-launch CUDA events.
+    gated: SwiGLU experts (GEMM1 contracts against gate AND up: 4 d f FLOP per row); else ReLU experts (2 d f)."""
     t1, t2 = kt["gemm1_ms"] * 1e-3, kt["gemm2_ms"] * 1e-3
     n1, n2 = max(1, kt["gemm1_launches"]), max(1, kt["gemm2_launches"])
+    g1 = 4.0 if gated else 2.0
     if decode:
-        b1, b2 = 4.0 * d * f * kt["groups"], 2.0 * d * f * kt["groups"]      # weight bytes read once per active expert
+        b1, b2 = g1 * d * f * kt["groups"], 2.0 * d * f * kt["groups"]      # weight bytes read once per active expert
         peak = peaks["hbm_gbs"]
         a1 = b1 / t1 / 1e9 if t1 > 0 else 0.0
         a2 = b2 / t2 / 1e9 if t2 > 0 else 0.0
@@ -699,7 +703,7 @@ def ffn_roofline(kt, d, f, peaks, decode, where):
                 "gemm2": {"achieved": a2, "frac": a2 / peak, "avg_launch_ms": t2 * 1e3 / n2},
                 "ffn": {"achieved": (b1 + b2) / (t1 + t2) / 1e9 if t1 + t2 > 0 else 0.0,
                         "frac": (b1 + b2) / (t1 + t2) / 1e9 / peak if t1 + t2 > 0 else 0.0}}
-    fl1, fl2 = 4.0 * d * f * kt["rows"], 2.0 * d * f * kt["rows"]
+    fl1, fl2 = g1 * d * f * kt["rows"], 2.0 * d * f * kt["rows"]
     peak = peaks["bf16_tflops_sustained"] or peaks["bf16_tflops"]
     a1 = fl1 / t1 / 1e12 if t1 > 0 else 0.0
     a2 = fl2 / t2 / 1e12 if t2 > 0 else 0.0
@@ -718,7 +722,8 @@ def resident_leg(cfg, counts, peaks, dev, args, decode):
     import torch
     from paper_2410_17954_b200 import EfContext
     E = cfg.n_experts
-    ctx = EfContext(1, E, cfg.top_k, cfg.d_model, cfg.d_ff, E, 0, cfg.T, 0, dev.index)
+    ctx = EfContext(1, E, cfg.top_k, cfg.d_model, cfg.d_ff, E, 0, cfg.T, 0, dev.index,
+                    1 if cfg.expert_kind == "relu" else 0)
     threads = os.cpu_count() or 8
     for e in range(E):
         ctx.ef_host_expert_register(0, e, *wl.expert_weights(cfg, 0, e, threads=threads))
@@ -747,7 +752,8 @@ def resident_leg(cfg, counts, peaks, dev, args, decode):
         ctx.ef_expert_ffn_grouped_resident(x_perm, rb, rw, sl, y)
     kt = ctx.ef_get_kernel_times(reset=True)
     res = ffn_roofline(kt, cfg.d_model, cfg.d_ff, dict(peaks, bf16_tflops_sustained=None), decode,
-                       "all active experts of one visit resident, one launch over all groups")
+                       "all active experts of one visit resident, one launch over all groups",
+                       gated=cfg.expert_kind == "swiglu")
     if not decode:
         res["peak_source"] = f"{peaks['source']} bf16 burst (kernel timed alone)"
     res["rows_per_expert"] = [int(c) for c in counts]

@@ -54,6 +54,9 @@ typedef struct {
     int32_t max_tokens;        /* largest T of any call */
     int32_t prefetch_horizon;  /* H: visits ahead ef_cache_prefetch may load for; <= 0: as far as supplied (R10) */
     int32_t device;            /* CUDA device ordinal */
+    int32_t expert_kind;       /* 0: SwiGLU expert (w_gate, w_up, w_down), 3*d*f*2 bytes (BASELINE.json; R4);
+                                  1: Switch-style non-gated ReLU expert y = relu(x W1^T) W2^T (w_gate = W1, w_up = NULL,
+                                  w_down = W2), 2*d*f*2 bytes (R30; the paper's Switch-32/64/128 models) */
 } ef_config;
 
 typedef struct {
@@ -77,7 +80,8 @@ int32_t ef_destroy(ef_ctx* ctx);
 
 /* Register expert `expert` of `layer` (expert < 0: shared expert -1-expert, which is also copied to
  * its resident device slot).  w_gate, w_up: [f, d] bf16; w_down: [d, f] bf16; HOST pointers, read
- * during the call only (the library packs them into its pinned pool).  Synchronous. */
+ * during the call only (the library packs them into its pinned pool).  With expert_kind = 1 (non-gated
+ * ReLU expert, R30) w_gate is W1, w_down is W2 and w_up must be NULL.  Synchronous. */
 int32_t ef_host_expert_register(ef_ctx* ctx, int32_t layer, int32_t expert, const void* w_gate,
                                 const void* w_up, const void* w_down);
 

@@ -30,7 +30,7 @@ class EfError(RuntimeError):
 
 class EfConfig(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in ("n_layers", "n_experts", "top_k", "d_model", "d_ff", "n_slots",
-                                               "n_shared", "max_tokens", "prefetch_horizon", "device")]
+                                               "n_shared", "max_tokens", "prefetch_horizon", "device", "expert_kind")]
 
 
 class CacheStats(ctypes.Structure):
@@ -134,10 +134,10 @@ class EfContext:
     """One ef_ctx.  Method names and argument order follow include/ef.h."""
 
     def __init__(self, n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared=0, max_tokens=1,
-                 prefetch_horizon=0, device=0):
+                 prefetch_horizon=0, device=0, expert_kind=0):
         self.lib = load_library()
         self.cfg = EfConfig(n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared, max_tokens,
-                            prefetch_horizon, device)
+                            prefetch_horizon, device, expert_kind)
         h = ctypes.c_void_p()
         rc = self.lib.ef_create(ctypes.byref(self.cfg), ctypes.byref(h))
         if rc != 0:
@@ -163,7 +163,7 @@ class EfContext:
     # -- registration
     def ef_host_expert_register(self, layer, expert, w_gate, w_up, w_down):
         for a in (w_gate, w_up, w_down):
-            assert a.dtype == np.uint16 and a.flags["C_CONTIGUOUS"]
+            assert a is None or (a.dtype == np.uint16 and a.flags["C_CONTIGUOUS"])
         self._chk(self.lib.ef_host_expert_register(self.h, layer, expert, _hp(w_gate), _hp(w_up), _hp(w_down)))
 
     def ef_host_expert_alias(self, layer, expert, src_layer, src_expert):

@@ -64,12 +64,14 @@ extern "C" int32_t ef_create(const ef_config* cfg, ef_ctx** out) {
     if (c.n_layers < 1 || c.n_experts < 1 || c.top_k < 1 || c.d_model < 1 || c.d_ff < 1 || c.n_slots < 1 ||
         c.n_shared < 0 || c.max_tokens < 1 || c.device < 0)
         return ef_fail(nullptr, EF_ERR_INVALID_ARG, "ef_create: non-positive field in ef_config");
+    if (c.expert_kind != 0 && c.expert_kind != 1)
+        return ef_fail(nullptr, EF_ERR_INVALID_ARG, "ef_create: expert_kind must be 0 (SwiGLU) or 1 (ReLU)");
     if (c.d_model % 64 || c.d_ff % 128 || c.top_k > 8 || c.top_k > c.n_experts || c.n_experts > 256)
         return ef_fail(nullptr, EF_ERR_UNSUPPORTED,
                        "ef_create: need d_model%%64==0, d_ff%%128==0, top_k<=8, top_k<=n_experts<=256");
     ef_ctx* ctx = new ef_ctx();
     ctx->cfg = c;
-    ctx->W = (int64_t)3 * c.d_model * c.d_ff * 2;
+    ctx->W = (int64_t)(c.expert_kind == 1 ? 2 : 3) * c.d_model * c.d_ff * 2;
     auto bail = [&](int32_t code, const char* what, cudaError_t e) {
         ef_fail(nullptr, code, "ef_create: %s: %s", what, cudaGetErrorString(e));
         ef_destroy(ctx);
@@ -142,6 +144,11 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
 // pack (Wg, Wu, Wd) into the library layout (ef_internal.h)
 static void pack_expert(const ef_config& c, const void* wg, const void* wu, const void* wd, char* dst) {
     const size_t row = (size_t)c.d_model * 2;
+    if (c.expert_kind == 1) {              // non-gated: W1[f, d] then W2[d, f], both as given
+        memcpy(dst, wg, (size_t)c.d_ff * row);
+        memcpy(dst + (size_t)c.d_ff * row, wd, (size_t)c.d_model * c.d_ff * 2);
+        return;
+    }
     const size_t blk = (size_t)EF_W13_BLOCK * row;
     const char* g = (const char*)wg;
     const char* u = (const char*)wu;
@@ -156,7 +163,9 @@ extern "C" int32_t ef_host_expert_register(ef_ctx* ctx, int32_t layer, int32_t e
                                            const void* w_up, const void* w_down) {
     EF_CHECK_CTX(ctx);
     const ef_config& c = ctx->cfg;
-    if (!w_gate || !w_up || !w_down || layer < 0 || layer >= c.n_layers || expert >= c.n_experts ||
+    if (c.expert_kind == 1 && w_up)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_register: w_up must be NULL for non-gated (ReLU) experts");
+    if (!w_gate || (!w_up && c.expert_kind == 0) || !w_down || layer < 0 || layer >= c.n_layers || expert >= c.n_experts ||
         expert < -c.n_shared)
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_register: bad layer/expert/pointer");
     EF_CUDA(ctx, cudaSetDevice(c.device));

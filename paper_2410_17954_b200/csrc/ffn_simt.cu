@@ -21,10 +21,11 @@ __device__ __forceinline__ bool find_tile(const EfGroupTable& tab, int tile, int
 }
 
 // C[m, n] for 64x64 tile; A rows from `a` (ld = K), B rows given by functor rowptr(n) (K-major).
-template <bool kSwiglu>
+template <int kEpi>     // 0 plain, 1 SwiGLU (packed gate/up rows), 2 ReLU
 __global__ void __launch_bounds__(256)
 simt_gemm_kernel(const uint16_t* __restrict__ a, uint16_t* __restrict__ c, const char* __restrict__ arena, int64_t W,
                  int64_t b_off_bytes, int K, int N, EfGroupTable tab, EfGroupTable ctab) {
+    constexpr bool kSwiglu = kEpi == 1;
     __shared__ float As[TK][TM + 1];
     __shared__ float B0[TK][TN + 1];
     __shared__ float B1[kSwiglu ? TK : 1][TN + 1];
@@ -84,6 +85,7 @@ simt_gemm_kernel(const uint16_t* __restrict__ a, uint16_t* __restrict__ c, const
             if (n >= N) continue;
             float v = acc0[i][j];
             if (kSwiglu) v = v / (1.f + expf(-v)) * acc1[i][j];
+            if (kEpi == 2) v = fmaxf(v, 0.f);
             __nv_bfloat16 o = __float2bfloat16_rn(v);
             C[(int64_t)m * N + n] = *reinterpret_cast<uint16_t*>(&o);
         }
@@ -104,10 +106,15 @@ int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const
         c2.g[i].c_row0 = tab.g[i].c_row0;    // ... and writes y rows
     }
     if (tiles == 0) return EF_OK;
-    simt_gemm_kernel<true><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
-        (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, t1, c1);
-    simt_gemm_kernel<false><<<dim3((d + TN - 1) / TN, tiles), 256, 0, st>>>(
-        (const uint16_t*)ctx->h_ws, (uint16_t*)y, ctx->arena, ctx->W, (int64_t)2 * f * d * 2, f, d, t2, c2);
+    const bool relu = ctx->cfg.expert_kind == 1;
+    if (relu)
+        simt_gemm_kernel<2><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
+            (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, t1, c1);
+    else
+        simt_gemm_kernel<1><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
+            (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, t1, c1);
+    simt_gemm_kernel<0><<<dim3((d + TN - 1) / TN, tiles), 256, 0, st>>>(
+        (const uint16_t*)ctx->h_ws, (uint16_t*)y, ctx->arena, ctx->W, (int64_t)(relu ? 1 : 2) * f * d * 2, f, d, t2, c2);
     ctx->launches += 2;
     EF_CUDA(ctx, cudaGetLastError());
     return EF_OK;

@@ -340,12 +340,14 @@ __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemC
 // kSwiglu: accumulator 0 = 128 gate rows, accumulator 1 = the matching up rows -> 128 output columns per weight tile;
 // else accumulators 0 / 1 = output columns [256 n, +128) / [256 n + 128, +128).  n_tiles_n = weight tiles, n_pairs_n =
 // ceil(n_tiles_n / 2) (an odd last tile leaves the peer CTA multiplying zero-filled rows).
-template <bool kSwiglu>
+template <int kEpi>     // 0: plain (GEMM2), 1: SwiGLU (gated GEMM1), 2: ReLU (non-gated GEMM1 of Switch-style experts, R30)
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmW,
                 uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int n_pairs_n, int total_tiles,
                 int32_t* __restrict__ sched, const SplitArgs sp, long long* __restrict__ kprof,
                 const __grid_constant__ EfGroupTable tab) {
+    constexpr bool kSwiglu = kEpi == 1;
+    constexpr bool kRelu = kEpi == 2;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t* stg_base = smem + (size_t)kStages * STAGE_BYTES;
@@ -540,7 +542,11 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                             tc_ld16x256b_x4((acc ? tb1 : tb0) + lane_off + c * 32, v);
                             tc_wait_ld();
 #pragma unroll
-                            for (int i = 0; i < 8; ++i) r[i] = pack_bf16(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
+                            for (int i = 0; i < 8; ++i) {
+                                float lo = __uint_as_float(v[2 * i]), hi = __uint_as_float(v[2 * i + 1]);
+                                if (kRelu) { lo = fmaxf(lo, 0.f); hi = fmaxf(hi, 0.f); }
+                                r[i] = pack_bf16(lo, hi);
+                            }
                         }
                         // r[2j] = lanes 0-7 of this half, r[2j+1] = lanes 8-15; token block j
                         stmatrix_x4_trans(st_row + hh * 32, r[0], r[2], r[4], r[6]);
@@ -581,8 +587,9 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                         for (int acc = 0; acc < (kSwiglu ? 1 : 2); ++acc) {
 #pragma unroll
                             for (int i = 0; i < 32; ++i) {
-                                const float v = kSwiglu ? silu_mul(__uint_as_float(a0[i]), __uint_as_float(a1[i]))
-                                                        : __uint_as_float(acc ? a1[i] : a0[i]);
+                                float v = kSwiglu ? silu_mul(__uint_as_float(a0[i]), __uint_as_float(a1[i]))
+                                                  : __uint_as_float(acc ? a1[i] : a0[i]);
+                                if (kRelu) v = fmaxf(v, 0.f);
                                 srow[i * (STG_LD / 2)] = bf16_bits(v);
                             }
                             stage_to_global(stg, C, ldc, (int64_t)t.c_row + c * 32, n_rows, col0 + acc * ACC_M, n_cols, lane128, 2 + part);
@@ -698,12 +705,14 @@ SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, d
 
 int32_t efk_ffn_tc_init(ef_ctx* ctx) {
     const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
-    int32_t rc = make_map_arena(ctx, &ctx->tm_w13, ctx->arena, 2 * (int64_t)f, d);
+    const int64_t w1_rows = ctx->cfg.expert_kind == 1 ? f : 2 * (int64_t)f;      // packed W13, or W1 of a non-gated expert
+    int32_t rc = make_map_arena(ctx, &ctx->tm_w13, ctx->arena, w1_rows, d);
     if (rc != EF_OK) return rc;
-    rc = make_map_arena(ctx, &ctx->tm_wd, ctx->arena + (size_t)2 * f * d * 2, d, f);
+    rc = make_map_arena(ctx, &ctx->tm_wd, ctx->arena + (size_t)w1_rows * d * 2, d, f);
     if (rc != EF_OK) return rc;
-    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
-    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
     EF_CUDA(ctx, cudaMalloc(&ctx->sched_words, sizeof(int32_t) * 2 * EF_SCHED_RING));
     EF_CUDA(ctx, cudaMemset(ctx->sched_words, 0, sizeof(int32_t) * 2 * EF_SCHED_RING));
     ctx->splitk_max_units = ctx->n_sms;      // pair units; each has one workspace slot and one counter per CTA of the pair
@@ -744,16 +753,21 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         EF_CUDA(ctx, cudaEventCreate(&span.e2));
         EF_CUDA(ctx, cudaEventRecord(span.e0, st));
     }
+    const bool relu = ctx->cfg.expert_kind == 1;
     {
-        const int ntn = f / 128;      // 256 packed W13 rows -> 128 h columns
+        const int ntn = relu ? (f + BW - 1) / BW : f / 128;      // 256 packed W13 rows -> 128 h columns; 256 W1 rows -> 256
         const int npn = (ntn + 1) / 2;
         const int tiles = mtiles * npn;
         const SplitPlan pl = plan_split(ctx, tiles, mshort * npn, n_pairs, d / BK, (double)rows_total / mtiles);
         const int total = pl.n_plain + pl.n_tail * pl.s;
         const int grid = 2 * std::min(total, n_pairs);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
-        ffn_gemm_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
-                                                                  total, next_sched(ctx), sp, ctx->kprof1, t1);
+        if (relu)
+            ffn_gemm_kernel<2><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
+                                                                   total, next_sched(ctx), sp, ctx->kprof1, t1);
+        else
+            ffn_gemm_kernel<1><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
+                                                                   total, next_sched(ctx), sp, ctx->kprof1, t1);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
     }
@@ -766,7 +780,7 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         const int total = pl.n_plain + pl.n_tail * pl.s;
         const int grid = 2 * std::min(total, n_pairs);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
-        ffn_gemm_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_wd, (uint16_t*)y, d, d, f, ntn, npn,
+        ffn_gemm_kernel<0><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_wd, (uint16_t*)y, d, d, f, ntn, npn,
                                                                    total, next_sched(ctx), sp, ctx->kprof2, t2);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());

@@ -17,7 +17,8 @@ from test_gpu_stages import bf, check_float, dev_bf16, to_bits  # noqa: E402
 def build_runner(cfg, horizon=None, experts=None, max_tokens=None):
     from paper_2410_17954_b200 import MoELayerRunner
     r = MoELayerRunner(cfg.n_layers, cfg.n_experts, cfg.top_k, cfg.d_model, cfg.d_ff, cfg.n_slots, cfg.n_shared,
-                       max_tokens or cfg.T, cfg.horizon if horizon is None else horizon, cfg.renorm)
+                       max_tokens or cfg.T, cfg.horizon if horizon is None else horizon, cfg.renorm,
+                       expert_kind=1 if cfg.expert_kind == "relu" else 0)
     experts = experts or {}
     for l in range(cfg.n_layers):
         r.set_router(l, wl.router_weight(cfg, l), wl.static_router_bias(cfg, l))
@@ -107,6 +108,42 @@ def test_cfg4_reduced_shared_experts_and_zipf():
     assert_cache_equal(r, sim)
     assert sim.stats["misses"] > 0                                       # waves were exercised
     check_float(bf(to_bits(out)), ref.out)
+    r.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# Switch-style layer (f4, R30): top-1, full-softmax gate weight (Eq. 2), ReLU experts, Zipf skew, 16 of 64 slots
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("T", [512, 4096], ids=["reduced", "full_size_switch_prefill"])
+def test_switch_prefill_relu_top1(T):
+    cfg = wl.scaled(wl.CONFIGS["switch_prefill"], T=T)
+    r, ex = build_runner(cfg)
+    x = wl.activations(cfg)
+    wr, bias = wl.router_weight(cfg), wl.static_router_bias(cfg)
+    g = np.random.default_rng(T)
+    rows = None if T <= 512 else np.sort(g.choice(T, 96, replace=False))
+    ref = oracle.layer_forward(x, wr, bias, [ex[(0, e)] for e in range(cfg.n_experts)], 1, renorm=0, rows=rows)
+    predicted = (ref.counts > 0).astype(np.uint8)[None, :]
+    sim = CacheSim(1, cfg.n_experts, cfg.n_slots, cfg.expert_bytes)
+    assert cfg.expert_bytes == 2 * cfg.d_model * cfg.d_ff * 2
+    sim.prefetch(-1, predicted); r.ctx.ef_cache_prefetch(-1, predicted)
+    out = torch.empty((cfg.T, cfg.d_model), dtype=torch.bfloat16, device="cuda")
+    r.visit(0, dev_bf16(x), out, want_logits=True)
+    sim.visit(0, ref.counts)
+    r.ctx.ef_sync()
+    # top-1 decided on identical logits (R22): the oracle's argmax applied to the GPU's own logits
+    gl = r.logits.cpu().numpy()[:T].astype(np.float64)
+    idx_ref, w_ref = oracle.topk_gate(gl, 1, renorm=0)
+    assert np.array_equal(r.topk_idx.cpu().numpy()[:T], idx_ref)
+    assert np.array_equal(r.topk_idx.cpu().numpy()[:T], ref.idx)          # and the generator's logit gap holds
+    assert np.allclose(r.topk_w.cpu().numpy()[:T], w_ref, rtol=1e-5)
+    assert np.array_equal(r.inv.cpu().numpy()[:T], ref.inv)
+    assert_cache_equal(r, sim)
+    assert sim.stats["bytes_h2d"] == cfg.expert_bytes * (sim.stats["ondemand_loads"] + sim.stats["prefetch_issued"])
+    if T == wl.CONFIGS["switch_prefill"].T:
+        assert sim.stats["misses"] > 0                                    # more active experts than slots: waves ran
+    got = bf(to_bits(out))
+    check_float(got if rows is None else got[rows], ref.out)
     r.close()
 
 

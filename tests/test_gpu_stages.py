@@ -146,9 +146,9 @@ def test_permute_bit_exact(T, k, E, d):
 # ------------------------------------------------------------------------------------------------
 # a4 grouped FFN (resident experts)
 # ------------------------------------------------------------------------------------------------
-def run_resident_ffn(ctx, E, d, f, counts, seed, simt, splitk=0):
+def run_resident_ffn(ctx, E, d, f, counts, seed, simt, splitk=0, expert_kind="swiglu"):
     """Load experts 0..E-1 into slots via the cache, run the grouped FFN on oracle-permuted rows."""
-    cfg = wl.scaled(wl.CONFIGS["tiny"], d_model=d, d_ff=f, n_experts=E, seed=seed)
+    cfg = wl.scaled(wl.CONFIGS["tiny"], d_model=d, d_ff=f, n_experts=E, seed=seed, expert_kind=expert_kind)
     experts = [wl.expert_weights(cfg, 0, e) for e in range(E)]
     for e in range(E):
         ctx.ef_host_expert_register(0, e, *experts[e])
@@ -193,6 +193,20 @@ def test_ffn_grouped_resident(E, d, f, counts, simt, splitk):
     ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)))
     got, ref = run_resident_ffn(ctx, E, d, f, counts, seed=13, simt=simt, splitk=splitk)
     assert not np.isnan(got).any()          # every routed row was written
+    check_float(got, ref)
+    ctx.close()
+
+
+# Switch-style non-gated ReLU experts (expert_kind = 1, R30): W1 tiles of 256 rows (f = 384: a ragged last
+# weight tile, an odd tile count for the CTA pair), all kernel variants
+@pytest.mark.parametrize("simt,splitk", [(True, 0), (False, 1), (False, 0), (False, 3)],
+                         ids=["simt_debug", "tcgen05_nosplit", "tcgen05_auto", "tcgen05_split3"])
+@pytest.mark.parametrize("E,d,f,counts", [(4, 256, 512, [40, 0, 1, 87]), (3, 768, 3072, [300, 129, 16]),
+                                          (2, 1024, 384, [257, 255]), (2, 64, 128, [1, 1])])
+def test_ffn_grouped_resident_relu_experts(E, d, f, counts, simt, splitk):
+    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)), expert_kind=1)
+    got, ref = run_resident_ffn(ctx, E, d, f, counts, seed=29, simt=simt, splitk=splitk, expert_kind="relu")
+    assert not np.isnan(got).any()
     check_float(got, ref)
     ctx.close()
 
