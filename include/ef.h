@@ -234,6 +234,15 @@ int32_t ef_get_kernel_times(ef_ctx* ctx, ef_kernel_times* out, int32_t reset);
  * K parts (test hook: exercises the partial-sum workspace on small shapes).  Results differ between modes only
  * by fp32 summation order. */
 int32_t ef_set_splitk(ef_ctx* ctx, int32_t mode);
+/* Physical scheduling of on-demand loads (never part of the policy or its counters):
+ * ef_set_wave_bytes: consecutive on-demand experts of a visit are computed by one grouped launch per `bytes` of
+ *   expert weights on the link (default 128 MiB; an expert larger than that, and always the last miss of a visit, is
+ *   its own launch; 0 = one launch pair per miss).
+ * ef_set_chunk_min_bytes: experts of at least `bytes` (default 32 MiB) are copied as two chunks -- first-GEMM weights,
+ *   then the down projection -- each with its own "ready" event, so GEMM1 overlaps the second chunk's transfer
+ *   (0 = always one copy per expert).  Results are identical in every setting. */
+int32_t ef_set_wave_bytes(ef_ctx* ctx, int64_t bytes);
+int32_t ef_set_chunk_min_bytes(ef_ctx* ctx, int64_t bytes);
 /* Diagnostic, only in libraries built with -DEF_KPROF (EF_ERR_UNSUPPORTED otherwise): the first call arms the
  * counters, later calls return, per CTA of the last GEMM1 (which = 1) or GEMM2 (which = 2) launch, the cycles the
  * MMA-issuing lane spent {in total, waiting for a tile ticket, waiting for the epilogue to free TMEM, waiting for

@@ -19,6 +19,7 @@ DECLARED_SYMBOLS = [
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
     "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
     "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof", "ef_token_schedule", "ef_path_hamming", "ef_set_token_sched_path", "ef_reindex_rows",
+    "ef_set_wave_bytes", "ef_set_chunk_min_bytes",
 ]
 
 
@@ -92,6 +93,8 @@ def load_library() -> ctypes.CDLL:
             "ef_reindex_rows": [vp, vp, vp, vp, i32, i64, vp],
             "ef_path_hamming": [vp, vp, vp, i32, i32, vp],
             "ef_set_token_sched_path": [vp, i32],
+            "ef_set_wave_bytes": [vp, i64],
+            "ef_set_chunk_min_bytes": [vp, i64],
         }
         for name, args in sig.items():
             fn = getattr(lib, name)
@@ -278,6 +281,12 @@ class EfContext:
 
     def ef_set_splitk(self, mode: int):
         self._chk(self.lib.ef_set_splitk(self.h, int(mode)))
+
+    def ef_set_wave_bytes(self, nbytes: int):
+        self._chk(self.lib.ef_set_wave_bytes(self.h, int(nbytes)))
+
+    def ef_set_chunk_min_bytes(self, nbytes: int):
+        self._chk(self.lib.ef_set_chunk_min_bytes(self.h, int(nbytes)))
 
     def ef_debug_kprof(self, which: int, n_sms: int = 148):
         out = np.zeros((n_sms, 5), np.int64)

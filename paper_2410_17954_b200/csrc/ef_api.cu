@@ -122,7 +122,7 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
     cudaSetDevice(ctx->cfg.device);
     cudaDeviceSynchronize();
     for (auto& sp : ctx->copy_spans) { cudaEventDestroy(sp.first); cudaEventDestroy(sp.second); }
-    for (auto& k : ctx->kspans) { cudaEventDestroy(k.e0); cudaEventDestroy(k.e1); cudaEventDestroy(k.e2); }
+    for (auto& k : ctx->kspans) { cudaEventDestroy(k.e0); cudaEventDestroy(k.e1); }
     for (auto ev : ctx->ev_ring) if (ev) cudaEventDestroy(ev);
     if (ctx->counts_event) cudaEventDestroy(ctx->counts_event);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
@@ -328,15 +328,30 @@ int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
     EF_CUDA(ctx, cudaEventCreate(&t0));
     EF_CUDA(ctx, cudaEventCreate(&t1));
     EF_CUDA(ctx, cudaEventRecord(t0, ctx->copy_stream));
-    EF_CUDA(ctx, cudaMemcpyAsync(ctx->arena + (size_t)slot * ctx->W, ctx->host_expert[g], (size_t)ctx->W,
-                                 cudaMemcpyHostToDevice, ctx->copy_stream));
+    // Finer-grained streaming: a large expert travels as two copies -- the first-GEMM weights
+    // (packed W13, or W1), then Wd -- with a "ready" event after each, so GEMM1 of the wave that waits for this
+    // expert runs while Wd is still on the link.  Small experts travel whole (the gap between two copies would cost
+    // more link time than the overlap wins).
+    char* dst = ctx->arena + (size_t)slot * ctx->W;
+    const char* srcp = (const char*)ctx->host_expert[g];
+    const size_t w1_bytes = (size_t)(ctx->cfg.expert_kind == 1 ? 1 : 2) * ctx->cfg.d_model * ctx->cfg.d_ff * 2;
+    cudaError_t e;
+    ph.ready1 = EvHandle();
+    if (ctx->chunk_min_bytes > 0 && ctx->W >= ctx->chunk_min_bytes) {
+        EF_CUDA(ctx, cudaMemcpyAsync(dst, srcp, w1_bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+        ph.ready1 = ring_record(ctx, ctx->copy_stream, &e);
+        EF_CUDA(ctx, e);
+        EF_CUDA(ctx, cudaMemcpyAsync(dst + w1_bytes, srcp + w1_bytes, (size_t)ctx->W - w1_bytes, cudaMemcpyHostToDevice,
+                                     ctx->copy_stream));
+    } else {
+        EF_CUDA(ctx, cudaMemcpyAsync(dst, srcp, (size_t)ctx->W, cudaMemcpyHostToDevice, ctx->copy_stream));
+    }
     EF_CUDA(ctx, cudaEventRecord(t1, ctx->copy_stream));
     ctx->copy_spans.emplace_back(t0, t1);
-    cudaError_t e;
     ph.ready = ring_record(ctx, ctx->copy_stream, &e);
     EF_CUDA(ctx, e);
     ph.free_ = EvHandle();
-    ph.has_waited = false;
+    ph.waited_mask = 0;
     ph.waited = nullptr;
     return EF_OK;
 }
@@ -363,28 +378,41 @@ void drain_copy_spans(ef_ctx* ctx, bool wait, float* acc_ms) {
 // one wave: groups (expert-local id e, slot) computed by one grouped launch (chunks of EF_MAX_GROUPS)
 struct WaveItem { int32_t row0, rows, slot; };
 
+// make `st` wait for the parts of the slot's expert that GEMM `which` (1 or 2) reads
+int32_t wait_slot_ready(ef_ctx* ctx, cudaStream_t st, EfPhys& ph, int which) {
+    if (ph.waited != st) { ph.waited = st; ph.waited_mask = 0; }
+    if (which == 1 && ph.ready1.idx >= 0) {
+        if (!(ph.waited_mask & 1)) {
+            EF_CUDA(ctx, ring_wait(ctx, st, ph.ready1, ctx->copy_stream));
+            ph.waited_mask |= 1;
+        }
+        return EF_OK;
+    }
+    if (ph.ready.idx >= 0 && !(ph.waited_mask & 2)) {
+        EF_CUDA(ctx, ring_wait(ctx, st, ph.ready, ctx->copy_stream));
+        ph.waited_mask |= 3;      // the whole-expert event is recorded after the first-chunk event
+    }
+    return EF_OK;
+}
+
 int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm, const std::vector<WaveItem>& items) {
     if (items.empty()) return EF_OK;
     auto& phys = ctx->phys;
-    for (const WaveItem& it : items) {
-        EfPhys& ph = phys[it.slot];
-        if (ph.ready.idx >= 0 && !(ph.has_waited && ph.waited == st)) {
-            EF_CUDA(ctx, ring_wait(ctx, st, ph.ready, ctx->copy_stream));
-            ph.has_waited = true;
-            ph.waited = st;
+    int32_t rc;
+    for (int which = 1; which <= 2; ++which) {
+        for (const WaveItem& it : items)
+            if ((rc = wait_slot_ready(ctx, st, phys[it.slot], which)) != EF_OK) return rc;
+        for (size_t base = 0; base < items.size(); base += EF_MAX_GROUPS) {
+            EfGroupTable tab;
+            int32_t h_row0[EF_MAX_GROUPS];
+            tab.n = (int32_t)std::min<size_t>(EF_MAX_GROUPS, items.size() - base);
+            for (int i = 0; i < tab.n; ++i) {
+                const WaveItem& it = items[base + i];
+                tab.g[i] = EfGroup{it.row0, it.row0, it.rows, it.slot};
+                h_row0[i] = it.row0;
+            }
+            if ((rc = efk_ffn_grouped(ctx, st, x_perm, y_perm, tab, h_row0, which)) != EF_OK) return rc;
         }
-    }
-    for (size_t base = 0; base < items.size(); base += EF_MAX_GROUPS) {
-        EfGroupTable tab;
-        int32_t h_row0[EF_MAX_GROUPS];
-        tab.n = (int32_t)std::min<size_t>(EF_MAX_GROUPS, items.size() - base);
-        for (int i = 0; i < tab.n; ++i) {
-            const WaveItem& it = items[base + i];
-            tab.g[i] = EfGroup{it.row0, it.row0, it.rows, it.slot};
-            h_row0[i] = it.row0;
-        }
-        int32_t rc = efk_ffn_grouped(ctx, st, x_perm, y_perm, tab, h_row0);
-        if (rc != EF_OK) return rc;
     }
     cudaError_t e;
     EvHandle ev = ring_record(ctx, st, &e);
@@ -395,12 +423,43 @@ int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm,
     return EF_OK;
 }
 
+// Miss waves.  Every on-demand expert could be its own wave (compute starts the moment its copy lands), but for small
+// experts that is one launch pair per ~0.3 ms copy, each too short to fill the GPU.  The batcher groups consecutive
+// misses into one grouped launch per ~wave_bytes of link traffic; the last miss of a visit stays alone so that the
+// tail after the final copy is one expert's FFN.  Physical scheduling only: which slot a miss takes and every counter
+// were decided before the item got here.
+struct MissBatcher {
+    ef_ctx* ctx; cudaStream_t st; const void* x_perm; void* y_perm;
+    std::vector<WaveItem> open;
+    int per_wave;
+    MissBatcher(ef_ctx* c, cudaStream_t s, const void* x, void* y) : ctx(c), st(s), x_perm(x), y_perm(y) {
+        per_wave = (int)std::max<int64_t>(1, std::min<int64_t>(EF_MAX_GROUPS, ctx->wave_bytes / ctx->W));
+    }
+    bool holds_slot(int slot) const {
+        for (const WaveItem& it : open) if (it.slot == slot) return true;
+        return false;
+    }
+    int32_t flush() {
+        if (open.empty()) return EF_OK;
+        int32_t rc = run_wave(ctx, st, x_perm, y_perm, open);
+        open.clear();
+        return rc;
+    }
+    int32_t push(const WaveItem& it, bool last_of_visit) {
+        int32_t rc = EF_OK;
+        if (last_of_visit && !open.empty() && (rc = flush()) != EF_OK) return rc;
+        open.push_back(it);
+        if ((int)open.size() >= per_wave || last_of_visit) rc = flush();
+        return rc;
+    }
+};
+
 }  // namespace
 
 int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                        const int32_t* h_row0) {
-    if (ctx->debug_simt) return efk_ffn_simt(ctx, st, x, y, tab, h_row0);
-    return efk_ffn_tc(ctx, st, x, y, tab, h_row0);
+                        const int32_t* h_row0, int phase) {
+    if (ctx->debug_simt) return efk_ffn_simt(ctx, st, x, y, tab, h_row0, phase);
+    return efk_ffn_tc(ctx, st, x, y, tab, h_row0, phase);
 }
 
 extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visit, int32_t layer, const void* x_perm,
@@ -484,23 +543,24 @@ extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visi
         rc = run_wave(ctx, st, x_perm, y_perm, others);
         if (rc != EF_OK) return rc;
     }
-    for (const WaveItem& it : wavesA) {   // one wave each: compute starts as each copy lands
-        rc = run_wave(ctx, st, x_perm, y_perm, std::vector<WaveItem>{it});
-        if (rc != EF_OK) return rc;
-    }
+    MissBatcher mb(ctx, st, x_perm, y_perm);
+    for (size_t i = 0; i < wavesA.size(); ++i)   // compute starts as the copies land, one grouped launch per batch
+        if ((rc = mb.push(wavesA[i], rest.empty() && i + 1 == wavesA.size())) != EF_OK) return rc;
     // phase B: the pool was full of this visit's own experts and useful prefetches
     std::fill(locked.begin(), locked.end(), 0);
-    for (int e : rest) {
+    for (size_t i = 0; i < rest.size(); ++i) {
+        const int e = rest[i];
         const int s = pick_victim(ctx, visit, visit, true, locked);
         if (s < 0) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_expert_ffn_grouped: no victim slot (internal)");
+        // the copy into s waits for the "free" event of the wave that read s: that wave must be enqueued first
+        if (mb.holds_slot(s) && (rc = mb.flush()) != EF_OK) return rc;
         rc = issue_load(ctx, s, layer * E + e, -1);
         if (rc != EF_OK) return rc;
         ctx->stats.ondemand_loads++;
         ctx->slots[s].used = true;
-        rc = run_wave(ctx, st, x_perm, y_perm, std::vector<WaveItem>{WaveItem{off[e], counts_host[e], s}});
-        if (rc != EF_OK) return rc;
+        if ((rc = mb.push(WaveItem{off[e], counts_host[e], s}, i + 1 == rest.size())) != EF_OK) return rc;
     }
-    return EF_OK;
+    return mb.flush();
 }
 
 extern "C" int32_t ef_expert_ffn_grouped_resident(ef_ctx* ctx, void* stream, const void* x_perm, int32_t n_groups,
@@ -541,7 +601,7 @@ extern "C" int32_t ef_shared_ffn(ef_ctx* ctx, void* stream, int32_t layer, const
         tab.g[s] = EfGroup{0, s * T, T, c.n_slots + layer * c.n_shared + s};
         h_row0[s] = c.max_tokens * c.top_k + s * c.max_tokens;   // shared region of the h workspace
     }
-    return efk_ffn_grouped(ctx, (cudaStream_t)stream, x, y_shared, tab, h_row0);
+    return efk_ffn_grouped(ctx, (cudaStream_t)stream, x, y_shared, tab, h_row0, 3);
 }
 
 extern "C" int32_t ef_cache_prefetch(ef_ctx* ctx, int64_t visit_now, const uint8_t* predicted, int32_t n_ahead) {
@@ -692,6 +752,20 @@ extern "C" int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on) {
     return EF_OK;
 }
 
+extern "C" int32_t ef_set_wave_bytes(ef_ctx* ctx, int64_t bytes) {
+    EF_CHECK_CTX(ctx);
+    if (bytes < 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_wave_bytes: negative");
+    ctx->wave_bytes = bytes;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_set_chunk_min_bytes(ef_ctx* ctx, int64_t bytes) {
+    EF_CHECK_CTX(ctx);
+    if (bytes < 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_chunk_min_bytes: negative");
+    ctx->chunk_min_bytes = bytes;
+    return EF_OK;
+}
+
 extern "C" int32_t ef_set_splitk(ef_ctx* ctx, int32_t mode) {
     EF_CHECK_CTX(ctx);
     if (mode < 0 || mode > 16) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_splitk: mode must be 0 (auto), 1 (off) or 2..16");
@@ -719,11 +793,10 @@ extern "C" int32_t ef_debug_kprof(ef_ctx* ctx, int32_t which, int64_t* out) {
 
 static void drain_kernel_spans(ef_ctx* ctx) {
     for (auto& k : ctx->kspans) {
-        cudaEventSynchronize(k.e2);
-        float a = 0.f, b = 0.f;
-        if (cudaEventElapsedTime(&a, k.e0, k.e1) == cudaSuccess) ctx->ktimes.gemm1_ms += a;
-        if (cudaEventElapsedTime(&b, k.e1, k.e2) == cudaSuccess) ctx->ktimes.gemm2_ms += b;
-        cudaEventDestroy(k.e0); cudaEventDestroy(k.e1); cudaEventDestroy(k.e2);
+        cudaEventSynchronize(k.e1);
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, k.e0, k.e1) == cudaSuccess) (k.which == 1 ? ctx->ktimes.gemm1_ms : ctx->ktimes.gemm2_ms) += ms;
+        cudaEventDestroy(k.e0); cudaEventDestroy(k.e1);
     }
     ctx->kspans.clear();
 }

@@ -49,10 +49,12 @@ struct EvHandle {
     uint32_t gen = 0;
 };
 struct EfPhys {
-    EvHandle ready;                  // recorded on the copy stream after the H2D into the slot
+    EvHandle ready1;                 // chunked load only: recorded on the copy stream once the first-GEMM weights
+                                     // (W13 / W1) have landed, before the copy of Wd starts
+    EvHandle ready;                  // recorded on the copy stream after the whole H2D into the slot
     EvHandle free_;                  // recorded on the compute stream after the last wave reading the slot
-    bool has_waited = false;         // some compute stream has waited on `ready` since the load ...
-    cudaStream_t waited = nullptr;   // ... namely this one (the legacy default stream is a valid value: 0)
+    uint8_t waited_mask = 0;         // bit 0 / bit 1: stream `waited` has waited on ready1 / ready since the load
+    cudaStream_t waited = nullptr;   // (the legacy default stream is a valid value: 0)
 };
 
 struct ef_ctx {
@@ -100,7 +102,7 @@ struct ef_ctx {
     float copy_ms = 0.f;
     // optional per-kernel timing (ef_set_kernel_timing)
     int32_t time_kernels = 0;
-    struct KSpan { cudaEvent_t e0, e1, e2; };
+    struct KSpan { cudaEvent_t e0, e1; int which; };   // one grouped-GEMM launch (which = 1: GEMM1, 2: GEMM2)
     std::vector<KSpan> kspans;
     ef_kernel_times ktimes{};
     // token scheduler workspace (token_sched.cu): state words, packed paths + membership bits, distance matrix
@@ -111,6 +113,9 @@ struct ef_ctx {
     size_t ts_dist_bytes = 0;
     bool ts_small_attr = false;         // ts_small_kernel opted in to > 48 KB dynamic smem
     int32_t ts_force_multi = 0;         // test hook (ef_set_token_sched_path): 1 = never take the single-CTA path
+    // physical scheduling knobs (never part of the policy): see ef_set_wave_bytes / ef_set_chunk_min_bytes
+    int64_t wave_bytes = (int64_t)128 << 20;
+    int64_t chunk_min_bytes = (int64_t)32 << 20;
     // misc
     int64_t launches = 0;
     int32_t debug_simt = 0;
@@ -148,10 +153,11 @@ int32_t efk_rmsnorm(ef_ctx* ctx, cudaStream_t st, const void* x, int T, float ep
 
 // Grouped SwiGLU FFN over arena slots: x rows -> h workspace -> y rows.  tab.g[i] = {x_row0, y_row0, rows, slot};
 // h rows are placed at h_row0 + (x_row0 - tab.g[0].x_row0 is NOT assumed): h row of group i = h_row_of[i].
+// phase: bit 0 = launch GEMM1 (x -> h), bit 1 = launch GEMM2 (h -> y); 3 = both, back to back.
 int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& x_to_y,
-                        const int32_t* h_row0 /*[n]*/);
+                        const int32_t* h_row0 /*[n]*/, int phase);
 int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                     const int32_t* h_row0);
+                     const int32_t* h_row0, int phase);
 int32_t efk_token_schedule(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, int c0, int c1,
                            int max_iter, int32_t* batch_of, int32_t* perm, int32_t* info, uint8_t* batch_paths);
 int32_t efk_reindex_rows(ef_ctx* ctx, cudaStream_t st, const void* src, const int32_t* perm, int n_rows, int64_t row_bytes,
@@ -160,4 +166,4 @@ int32_t efk_path_hamming(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int
 void efk_token_sched_free(ef_ctx* ctx);
 int32_t efk_ffn_tc_init(ef_ctx* ctx);   // build arena tensor maps, set smem attributes
 int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                   const int32_t* h_row0);
+                   const int32_t* h_row0, int phase);

@@ -95,7 +95,7 @@ simt_gemm_kernel(const uint16_t* __restrict__ a, uint16_t* __restrict__ c, const
 }  // namespace
 
 int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                     const int32_t* h_row0) {
+                     const int32_t* h_row0, int phase) {
     const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
     int tiles = 0;
     EfGroupTable t1 = tab, c1 = tab, t2 = tab, c2 = tab;
@@ -107,15 +107,20 @@ int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const
     }
     if (tiles == 0) return EF_OK;
     const bool relu = ctx->cfg.expert_kind == 1;
-    if (relu)
-        simt_gemm_kernel<2><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
-            (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, t1, c1);
-    else
-        simt_gemm_kernel<1><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
-            (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, t1, c1);
-    simt_gemm_kernel<0><<<dim3((d + TN - 1) / TN, tiles), 256, 0, st>>>(
-        (const uint16_t*)ctx->h_ws, (uint16_t*)y, ctx->arena, ctx->W, (int64_t)(relu ? 1 : 2) * f * d * 2, f, d, t2, c2);
-    ctx->launches += 2;
+    if (phase & 1) {
+        if (relu)
+            simt_gemm_kernel<2><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
+                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, t1, c1);
+        else
+            simt_gemm_kernel<1><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
+                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, t1, c1);
+        ctx->launches++;
+    }
+    if (phase & 2) {
+        simt_gemm_kernel<0><<<dim3((d + TN - 1) / TN, tiles), 256, 0, st>>>(
+            (const uint16_t*)ctx->h_ws, (uint16_t*)y, ctx->arena, ctx->W, (int64_t)(relu ? 1 : 2) * f * d * 2, f, d, t2, c2);
+        ctx->launches++;
+    }
     EF_CUDA(ctx, cudaGetLastError());
     return EF_OK;
 }

@@ -724,37 +724,37 @@ int32_t efk_ffn_tc_init(ef_ctx* ctx) {
 }
 
 int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                   const int32_t* h_row0) {
+                   const int32_t* h_row0, int phase) {
     const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
     if (tab.n == 0) return EF_OK;
-    int64_t x_rows = 0;
-    for (int i = 0; i < tab.n; ++i) x_rows = std::max<int64_t>(x_rows, (int64_t)tab.g[i].a_row0 + tab.g[i].rows);
-    CUtensorMap tmX, tmH;
-    int32_t rc = make_map_2d(ctx, &tmX, x, x_rows, d);
-    if (rc != EF_OK) return rc;
-    rc = make_map_2d(ctx, &tmH, ctx->h_ws, ctx->h_rows, f);
-    if (rc != EF_OK) return rc;
-
     int64_t rows_total = 0;
-    for (int i = 0; i < tab.n; ++i) rows_total += tab.g[i].rows;
     int mtiles = 0, mshort = 0;   // tiles per n column: every group's 256-row tiles plus its short tail tile
     EfGroupTable t1 = tab, t2 = tab;
     for (int i = 0; i < tab.n; ++i) {
+        rows_total += tab.g[i].rows;
         mtiles += group_long_tiles(tab.g[i].rows) + group_has_short(tab.g[i].rows);
         mshort += group_has_short(tab.g[i].rows);
         t1.g[i].c_row0 = h_row0[i];   // GEMM1: x rows -> h rows
         t2.g[i].a_row0 = h_row0[i];   // GEMM2: h rows -> y rows
     }
     const int n_pairs = ctx->n_sms / 2;     // CTA pairs (clusters of 2), one CTA per SM
-    ef_ctx::KSpan span{};
-    if (ctx->time_kernels) {
-        EF_CUDA(ctx, cudaEventCreate(&span.e0));
-        EF_CUDA(ctx, cudaEventCreate(&span.e1));
-        EF_CUDA(ctx, cudaEventCreate(&span.e2));
-        EF_CUDA(ctx, cudaEventRecord(span.e0, st));
-    }
     const bool relu = ctx->cfg.expert_kind == 1;
-    {
+    // optional per-launch timing (ef_set_kernel_timing): one event pair per GEMM launch
+    auto span_begin = [&](ef_ctx::KSpan& sp, int which) -> cudaError_t {
+        sp.which = which;
+        cudaError_t e = cudaEventCreate(&sp.e0);
+        if (e == cudaSuccess) e = cudaEventCreate(&sp.e1);
+        if (e == cudaSuccess) e = cudaEventRecord(sp.e0, st);
+        return e;
+    };
+    if (phase & 1) {
+        int64_t x_rows = 0;
+        for (int i = 0; i < tab.n; ++i) x_rows = std::max<int64_t>(x_rows, (int64_t)tab.g[i].a_row0 + tab.g[i].rows);
+        CUtensorMap tmX;
+        int32_t rc = make_map_2d(ctx, &tmX, x, x_rows, d);
+        if (rc != EF_OK) return rc;
+        ef_ctx::KSpan span{};
+        if (ctx->time_kernels) EF_CUDA(ctx, span_begin(span, 1));
         const int ntn = relu ? (f + BW - 1) / BW : f / 128;      // 256 packed W13 rows -> 128 h columns; 256 W1 rows -> 256
         const int npn = (ntn + 1) / 2;
         const int tiles = mtiles * npn;
@@ -770,9 +770,20 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
                                                                    total, next_sched(ctx), sp, ctx->kprof1, t1);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
+        if (ctx->time_kernels) {
+            EF_CUDA(ctx, cudaEventRecord(span.e1, st));
+            ctx->kspans.push_back(span);
+            ctx->ktimes.gemm1_launches++;
+            ctx->ktimes.rows += rows_total;
+            ctx->ktimes.groups += tab.n;
+        }
     }
-    if (ctx->time_kernels) EF_CUDA(ctx, cudaEventRecord(span.e1, st));
-    {
+    if (phase & 2) {
+        CUtensorMap tmH;
+        int32_t rc = make_map_2d(ctx, &tmH, ctx->h_ws, ctx->h_rows, f);
+        if (rc != EF_OK) return rc;
+        ef_ctx::KSpan span{};
+        if (ctx->time_kernels) EF_CUDA(ctx, span_begin(span, 2));
         const int ntn = (d + BW - 1) / BW;
         const int npn = (ntn + 1) / 2;
         const int tiles = mtiles * npn;
@@ -784,14 +795,11 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
                                                                    total, next_sched(ctx), sp, ctx->kprof2, t2);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
-    }
-    if (ctx->time_kernels) {
-        EF_CUDA(ctx, cudaEventRecord(span.e2, st));
-        ctx->kspans.push_back(span);
-        ctx->ktimes.gemm1_launches++;
-        ctx->ktimes.gemm2_launches++;
-        ctx->ktimes.rows += rows_total;
-        ctx->ktimes.groups += tab.n;
+        if (ctx->time_kernels) {
+            EF_CUDA(ctx, cudaEventRecord(span.e1, st));
+            ctx->kspans.push_back(span);
+            ctx->ktimes.gemm2_launches++;
+        }
     }
     return EF_OK;
 }

@@ -112,6 +112,38 @@ def test_cfg4_reduced_shared_experts_and_zipf():
 
 
 # ------------------------------------------------------------------------------------------------
+# physical scheduling of on-demand loads: batched miss waves and two-chunk expert copies change
+# neither the result nor the accounting -- down to pools so small that a miss takes the slot of a miss of the same visit
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_slots", [1, 2, 5, 24])
+@pytest.mark.parametrize("wave_bytes,chunk_min", [(0, 0), (1 << 40, 0), (0, 1), (1 << 40, 1), (None, None)],
+                         ids=["single_waves", "batched", "chunked", "batched_chunked", "defaults"])
+def test_miss_wave_batching_and_chunked_copies(n_slots, wave_bytes, chunk_min):
+    cfg = wl.scaled(wl.CONFIGS["many_expert_prefill"], T=256, d_model=256, d_ff=384, n_slots=n_slots)
+    r, ex = build_runner(cfg)
+    if wave_bytes is not None:
+        r.ctx.ef_set_wave_bytes(wave_bytes)
+        r.ctx.ef_set_chunk_min_bytes(chunk_min)
+    x = wl.activations(cfg)
+    ref = oracle.layer_forward(x, wl.router_weight(cfg), wl.static_router_bias(cfg),
+                               [ex[(0, e)] for e in range(cfg.n_experts)], cfg.top_k,
+                               shared=[ex[(0, -1)], ex[(0, -2)]])
+    predicted = (ref.counts > 0).astype(np.uint8)[None, :]
+    sim = CacheSim(1, cfg.n_experts, cfg.n_slots, cfg.expert_bytes, cfg.horizon)
+    sim.prefetch(-1, predicted); r.ctx.ef_cache_prefetch(-1, predicted)
+    out = torch.empty((cfg.T, cfg.d_model), dtype=torch.bfloat16, device="cuda")
+    for v in range(2):                                   # the second visit starts from a full pool
+        r.visit(v, dev_bf16(x), out)
+        sim.visit(v, ref.counts)
+        r.ctx.ef_sync()
+        assert_cache_equal(r, sim)
+        assert np.array_equal(r.inv.cpu().numpy(), ref.inv)
+        check_float(bf(to_bits(out)), ref.out)
+    assert sim.stats["misses"] > n_slots
+    r.close()
+
+
+# ------------------------------------------------------------------------------------------------
 # Switch-style layer (f4, R30): top-1, full-softmax gate weight (Eq. 2), ReLU experts, Zipf skew, 16 of 64 slots
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("T", [512, 4096], ids=["reduced", "full_size_switch_prefill"])
