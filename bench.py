@@ -486,8 +486,12 @@ def run_ours(args):
 
     d, f = cfg.d_model, cfg.d_ff
     decode = cfg.T * cfg.top_k / cfg.n_experts < 249 and cfg.name in ("mixtral_decode", "stack_decode")
-    roofline = ffn_roofline(kt, d, f, peaks, decode, "streaming step (one wave of hits + one wave per miss)",
-                            gated=cfg.expert_kind == "swiglu")
+    fill_peak = None
+    if rank == 0 and not decode:
+        runner.ctx.ef_sync()
+        fill_peak = runner.ctx.ef_debug_tma_fill_gbs(64 << 20, 2000)
+    roofline = ffn_roofline(kt, d, f, peaks, decode, "streaming step (one wave of hits + batched waves of misses)",
+                            gated=cfg.expert_kind == "swiglu", fill_peak=fill_peak)
     roofline["traffic"] = NCU_TRAFFIC_BYTES.get(cfg.name)
     roofline["traffic_source"] = ("bytes per GEMM1 launch from the committed ncu capture under profiles/ (see NCU_TRAFFIC_BYTES)"
                                   if cfg.name in NCU_TRAFFIC_BYTES else "no ncu capture for this workload")
@@ -510,7 +514,7 @@ def run_ours(args):
     if rank == 0 and not args.no_resident:
         counts = runner.counts.cpu().numpy()
         drv.close()
-        resident = resident_leg(cfg, counts, peaks, dev, args, decode)
+        resident = resident_leg(cfg, counts, peaks, dev, args, decode, fill_peak)
     else:
         drv.close()
 
@@ -686,7 +690,7 @@ def run_dual_batch(args):
         print(json.dumps(line), flush=True)
 
 
-def ffn_roofline(kt, d, f, peaks, decode, where, gated=True):
+def ffn_roofline(kt, d, f, peaks, decode, where, gated=True, fill_peak=None):
     """Roofline of the dominant kernel (GEMM1 of the grouped FFN) from the library's per-launch CUDA events.
     gated: SwiGLU experts (GEMM1 contracts against gate AND up: 4 d f FLOP per row); else ReLU experts (2 d f)."""
     t1, t2 = kt["gemm1_ms"] * 1e-3, kt["gemm2_ms"] * 1e-3
@@ -707,7 +711,19 @@ def ffn_roofline(kt, d, f, peaks, decode, where, gated=True):
     peak = peaks["bf16_tflops_sustained"] or peaks["bf16_tflops"]
     a1 = fl1 / t1 / 1e12 if t1 > 0 else 0.0
     a2 = fl2 / t2 / 1e12 if t2 > 0 else 0.0
-    return {"bound": "tensor", "kernel": f"ffn_gemm_kernel<swiglu> (GEMM1), {where}", "achieved": a1, "peak": peak,
+    # second ceiling: the operand bytes TMA stages into shared memory (from the tile plan) against the measured TMA fill
+    # rate of the device -- the L2 -> SM fabric, which is what the prefill GEMM actually runs into
+    fab = None
+    if fill_peak and kt.get("gemm1_fill_bytes"):
+        f1 = kt["gemm1_fill_bytes"] / t1 / 1e9 if t1 > 0 else 0.0
+        f2 = kt["gemm2_fill_bytes"] / t2 / 1e9 if t2 > 0 else 0.0
+        fab = {"bound": "l2_to_sm", "achieved": f1, "peak": fill_peak, "unit": "GB/s", "frac": f1 / fill_peak,
+               "bytes_per_launch": kt["gemm1_fill_bytes"] / n1, "flop_per_fill_byte": fl1 / max(1, kt["gemm1_fill_bytes"]),
+               "tflops_at_fill_peak": fl1 / max(1, kt["gemm1_fill_bytes"]) * fill_peak / 1e3,
+               "gemm2": {"achieved": f2, "frac": f2 / fill_peak, "flop_per_fill_byte": fl2 / max(1, kt["gemm2_fill_bytes"])},
+               "peak_source": "measured in this run: ef_debug_tma_fill_gbs, every SM streaming 32 KB TMA boxes out of a "
+                              "64 MB L2-resident region"}
+    return {"bound": "tensor", "l2_to_sm": fab, "kernel": f"ffn_gemm_kernel<swiglu> (GEMM1), {where}", "achieved": a1, "peak": peak,
             "unit": "TFLOP/s", "frac": a1 / peak,
             "peak_source": f"{peaks['source']} bf16 sustained (kernel timed inside a long step)", "traffic": None,
             "launches": kt["gemm1_launches"], "avg_launch_ms": t1 * 1e3 / n1, "rows_per_launch": kt["rows"] / n1,
@@ -716,7 +732,7 @@ def ffn_roofline(kt, d, f, peaks, decode, where, gated=True):
                     "frac": (fl1 + fl2) / (t1 + t2) / 1e12 / peak if t1 + t2 > 0 else 0.0}}
 
 
-def resident_leg(cfg, counts, peaks, dev, args, decode):
+def resident_leg(cfg, counts, peaks, dev, args, decode, fill_peak=None):
     """The grouped FFN alone with every active expert of one visit resident (kernel-only roofline): one launch
     pair over all groups, timed by the library's CUDA events on the compute stream, weights > L2."""
     import torch
@@ -753,7 +769,7 @@ def resident_leg(cfg, counts, peaks, dev, args, decode):
     kt = ctx.ef_get_kernel_times(reset=True)
     res = ffn_roofline(kt, cfg.d_model, cfg.d_ff, dict(peaks, bf16_tflops_sustained=None), decode,
                        "all active experts of one visit resident, one launch over all groups",
-                       gated=cfg.expert_kind == "swiglu")
+                       gated=cfg.expert_kind == "swiglu", fill_peak=fill_peak)
     if not decode:
         res["peak_source"] = f"{peaks['source']} bf16 burst (kernel timed alone)"
     res["rows_per_expert"] = [int(c) for c in counts]
@@ -774,9 +790,13 @@ def main():
     ap.add_argument("--phys-experts", type=int, default=0,
                     help="alias the logical experts onto this many physical pinned host buffers (0 = one per expert "
                          "if host memory allows)")
+    ap.add_argument("--horizon", type=int, default=None,
+                    help="override the workload's prefetch horizon H in visits (<= 0: as far as the supplied path reaches; R10)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-resident", action="store_true")
     args = ap.parse_args()
+    if args.horizon is not None:
+        wl.CONFIGS[args.workload] = wl.scaled(wl.CONFIGS[args.workload], horizon=args.horizon)
     if args.impl == "reference":
         run_reference(args)
     elif args.workload == "dual_batch_stack":

@@ -226,6 +226,8 @@ typedef struct {
     int64_t gemm1_launches, gemm2_launches;
     int64_t rows;     /* routed rows processed (each counted once per FFN, not per GEMM) */
     int64_t groups;   /* expert groups processed */
+    int64_t gemm1_fill_bytes, gemm2_fill_bytes;   /* bytes the launches' TMA loads staged into shared memory (weight
+                         boxes + token boxes over every tile and k-block, from the tile plan): the L2 -> SM traffic */
 } ef_kernel_times;
 int32_t ef_set_kernel_timing(ef_ctx* ctx, int32_t on);
 int32_t ef_get_kernel_times(ef_ctx* ctx, ef_kernel_times* out, int32_t reset);
@@ -243,6 +245,12 @@ int32_t ef_set_splitk(ef_ctx* ctx, int32_t mode);
  *   (0 = always one copy per expert).  Results are identical in every setting. */
 int32_t ef_set_wave_bytes(ef_ctx* ctx, int64_t bytes);
 int32_t ef_set_chunk_min_bytes(ef_ctx* ctx, int64_t bytes);
+/* Diagnostic: the rate at which TMA can fill shared memory on this device, i.e. the L2 -> SM fabric ceiling that bounds
+ * the grouped GEMM's operand traffic.  One persistent CTA per SM streams 32 KB boxes (64 x 256 bf16, the
+ * GEMM's weight box) through a 4-stage ring, `iters` boxes per CTA, out of a scratch region of region_bytes (<= 126 MB
+ * stays in L2; larger streams from HBM).  gbs_out: HOST double, delivered GB/s.  Synchronous; allocates and frees the
+ * region. */
+int32_t ef_debug_tma_fill_gbs(ef_ctx* ctx, int64_t region_bytes, int32_t iters, double* gbs_out);
 /* Diagnostic, only in libraries built with -DEF_KPROF (EF_ERR_UNSUPPORTED otherwise): the first call arms the
  * counters, later calls return, per CTA of the last GEMM1 (which = 1) or GEMM2 (which = 2) launch, the cycles the
  * MMA-issuing lane spent {in total, waiting for a tile ticket, waiting for the epilogue to free TMEM, waiting for

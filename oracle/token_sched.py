@@ -60,6 +60,30 @@ def batch_path(r: np.ndarray, members) -> np.ndarray:
     return out
 
 
+def batch_accuracy(r_batch: np.ndarray, r_batch_hat: np.ndarray) -> float:
+    """B_acc of Eq. 7: the mean over the L layers of
+        #{j : R_batch[i,j] = 1 and R^_batch[i,j] = 1} / #{j : R_batch[i,j] = 1},
+    R_batch the true and R^_batch the predicted batch-level routing path, both binary (L, E) (each the OR of its
+    tokens' paths, P:L239 -- `batch_path`).  Plain loops in the paper's index order.  A layer in which the true path
+    activates no expert has no defined ratio; it is left out of the mean (cannot happen with top-k >= 1 routing)."""
+    R = np.asarray(r_batch) != 0
+    Rh = np.asarray(r_batch_hat) != 0
+    assert R.shape == Rh.shape and R.ndim == 2
+    L, E = R.shape
+    total, layers = 0.0, 0
+    for i in range(L):
+        num = den = 0
+        for j in range(E):
+            if R[i, j]:
+                den += 1
+                if Rh[i, j]:
+                    num += 1
+        if den:
+            total += num / den
+            layers += 1
+    return total / layers if layers else float("nan")
+
+
 def objective(r: np.ndarray, batch_of) -> int:
     """Eq. 5: activated experts summed over layers, experts and the two batches."""
     batch_of = np.asarray(batch_of)

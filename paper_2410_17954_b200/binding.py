@@ -19,7 +19,7 @@ DECLARED_SYMBOLS = [
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
     "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
     "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof", "ef_token_schedule", "ef_path_hamming", "ef_set_token_sched_path", "ef_reindex_rows",
-    "ef_set_wave_bytes", "ef_set_chunk_min_bytes",
+    "ef_set_wave_bytes", "ef_set_chunk_min_bytes", "ef_debug_tma_fill_gbs",
 ]
 
 
@@ -44,7 +44,8 @@ class CacheStats(ctypes.Structure):
 
 class KernelTimes(ctypes.Structure):
     _fields_ = [("gemm1_ms", ctypes.c_double), ("gemm2_ms", ctypes.c_double), ("gemm1_launches", ctypes.c_int64),
-                ("gemm2_launches", ctypes.c_int64), ("rows", ctypes.c_int64), ("groups", ctypes.c_int64)]
+                ("gemm2_launches", ctypes.c_int64), ("rows", ctypes.c_int64), ("groups", ctypes.c_int64),
+                ("gemm1_fill_bytes", ctypes.c_int64), ("gemm2_fill_bytes", ctypes.c_int64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -93,6 +94,7 @@ def load_library() -> ctypes.CDLL:
             "ef_reindex_rows": [vp, vp, vp, vp, i32, i64, vp],
             "ef_path_hamming": [vp, vp, vp, i32, i32, vp],
             "ef_set_token_sched_path": [vp, i32],
+            "ef_debug_tma_fill_gbs": [vp, i64, i32, ctypes.POINTER(ctypes.c_double)],
             "ef_set_wave_bytes": [vp, i64],
             "ef_set_chunk_min_bytes": [vp, i64],
         }
@@ -287,6 +289,11 @@ class EfContext:
 
     def ef_set_chunk_min_bytes(self, nbytes: int):
         self._chk(self.lib.ef_set_chunk_min_bytes(self.h, int(nbytes)))
+
+    def ef_debug_tma_fill_gbs(self, region_bytes: int, iters: int = 2000) -> float:
+        out = ctypes.c_double()
+        self._chk(self.lib.ef_debug_tma_fill_gbs(self.h, int(region_bytes), int(iters), ctypes.byref(out)))
+        return float(out.value)
 
     def ef_debug_kprof(self, which: int, n_sms: int = 148):
         out = np.zeros((n_sms, 5), np.int64)

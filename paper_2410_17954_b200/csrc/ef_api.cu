@@ -141,22 +141,42 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
     return EF_OK;
 }
 
-// pack (Wg, Wu, Wd) into the library layout (ef_internal.h)
+// pack (Wg, Wu, Wd) into the library layout (ef_internal.h): W13 rows interleaved by 128, every matrix tiled
+static void pack_tiled(char* dst, int64_t rows, int64_t K, const char* (*src_row)(const void*, int64_t), const void* cookie) {
+    const int64_t chunk = EF_ROWLET * 2;                     // one rowlet: 128 bytes
+    for (int64_t r = 0; r < rows; ++r) {
+        const char* src = src_row(cookie, r);
+        char* d0 = dst + ef_tiled_index(r, 0, rows, K) * 2;
+        const int64_t t = r / EF_TILE_ROWS;
+        const int64_t h = std::min<int64_t>(EF_TILE_ROWS, rows - t * EF_TILE_ROWS);
+        for (int64_t kb = 0; kb < K / EF_ROWLET; ++kb) memcpy(d0 + kb * h * chunk, src + kb * chunk, chunk);
+    }
+}
+
+struct PackSrc { const char* a; const char* b; int64_t row_bytes; };
+
 static void pack_expert(const ef_config& c, const void* wg, const void* wu, const void* wd, char* dst) {
-    const size_t row = (size_t)c.d_model * 2;
-    if (c.expert_kind == 1) {              // non-gated: W1[f, d] then W2[d, f], both as given
-        memcpy(dst, wg, (size_t)c.d_ff * row);
-        memcpy(dst + (size_t)c.d_ff * row, wd, (size_t)c.d_model * c.d_ff * 2);
+    const int64_t d = c.d_model, f = c.d_ff;
+    PackSrc down{(const char*)wd, nullptr, f * 2};
+    auto plain = [](const void* ck, int64_t r) -> const char* {
+        const PackSrc* p = (const PackSrc*)ck;
+        return p->a + r * p->row_bytes;
+    };
+    if (c.expert_kind == 1) {              // non-gated: W1[f, d] then W2[d, f]
+        PackSrc w1{(const char*)wg, nullptr, d * 2};
+        pack_tiled(dst, f, d, plain, &w1);
+        pack_tiled(dst + f * d * 2, d, f, plain, &down);
         return;
     }
-    const size_t blk = (size_t)EF_W13_BLOCK * row;
-    const char* g = (const char*)wg;
-    const char* u = (const char*)wu;
-    for (int j = 0; j < c.d_ff / EF_W13_BLOCK; ++j) {
-        memcpy(dst + (size_t)(2 * j) * blk, g + (size_t)j * blk, blk);
-        memcpy(dst + (size_t)(2 * j + 1) * blk, u + (size_t)j * blk, blk);
-    }
-    memcpy(dst + (size_t)2 * c.d_ff * row, wd, (size_t)c.d_model * c.d_ff * 2);
+    PackSrc w13{(const char*)wg, (const char*)wu, d * 2};
+    auto interleaved = [](const void* ck, int64_t r) -> const char* {   // packed row r of W13
+        const PackSrc* p = (const PackSrc*)ck;
+        const int64_t j = r / (2 * EF_W13_BLOCK), i = r % (2 * EF_W13_BLOCK);
+        return (i < EF_W13_BLOCK ? p->a + (j * EF_W13_BLOCK + i) * p->row_bytes
+                                 : p->b + (j * EF_W13_BLOCK + i - EF_W13_BLOCK) * p->row_bytes);
+    };
+    pack_tiled(dst, 2 * f, d, interleaved, &w13);
+    pack_tiled(dst + 2 * f * d * 2, d, f, plain, &down);
 }
 
 extern "C" int32_t ef_host_expert_register(ef_ctx* ctx, int32_t layer, int32_t expert, const void* w_gate,

@@ -16,11 +16,24 @@
 #define EF_W13_BLOCK 128   // gate/up interleave granularity in the packed expert layout
 
 // ---- packed expert layout (library-defined; the caller never sees it) ----------------------------
-// An expert occupies W = 3*d*f*2 bytes:
-//   [ W13 : 2f rows x d ]  row 256*j + i       = Wg[128*j + i, :]   (i < 128)
+// An expert occupies W = 3*d*f*2 bytes: the first-GEMM matrix, then the down projection.
+//   W13 : 2f rows x d      row 256*j + i       = Wg[128*j + i, :]   (i < 128)
 //                          row 256*j + 128 + i = Wu[128*j + i, :]
-//   [ Wd  : d rows x f  ]  as given
-// so one 256-row B tile of GEMM1 yields 128 gate columns and the matching 128 up columns.
+//         (non-gated experts: W1, f rows x d, rows as given)
+//   Wd  : d rows x f       rows as given
+// so one 256-row weight tile of GEMM1 yields 128 gate columns and the matching 128 up columns.
+// Each matrix M[rows, K] is stored TILED, in the order the grouped GEMM streams it: 256-row tiles, and inside a
+// tile one block per 64-column k-block, a block being h x 64 elements row-major (h = 256, or what is left in the
+// last tile).  A k-block of a weight tile is therefore 32 KB of CONTIGUOUS memory = one TMA box of 256 "rowlets"
+// (a rowlet = 64 bf16 = 128 bytes), instead of 256 rows 2*K bytes apart.  No padding: rows * K elements in all.
+#define EF_TILE_ROWS 256
+#define EF_ROWLET 64
+// element index of M[r, c] inside the tiled matrix
+__host__ __device__ inline int64_t ef_tiled_index(int64_t r, int64_t c, int64_t rows, int64_t K) {
+    const int64_t t = r / EF_TILE_ROWS, rr = r % EF_TILE_ROWS, kb = c / EF_ROWLET, cc = c % EF_ROWLET;
+    const int64_t h = (rows - t * EF_TILE_ROWS < EF_TILE_ROWS) ? rows - t * EF_TILE_ROWS : EF_TILE_ROWS;
+    return t * EF_TILE_ROWS * K + kb * h * EF_ROWLET + rr * EF_ROWLET + cc;
+}
 
 struct EfGroup {
     int32_t a_row0;   // first row of A (x_perm or h)
@@ -85,8 +98,8 @@ struct ef_ctx {
     std::map<int64_t, std::vector<uint8_t>> pred;   // visit -> predicted active flags [E]
     uint64_t tick = 0;
     ef_cache_stats stats{};
-    // tensor maps over the arena (3-D: k, row, slot)
-    CUtensorMap tm_w13{}, tm_wd{};
+    // tensor map over the whole arena as rowlets (2-D: 64 elements x total rowlets); both GEMMs use it
+    CUtensorMap tm_w{};
     bool tm_ok = false;
     int32_t* sched_words = nullptr;     // device, [EF_SCHED_RING][2]
     int32_t sched_next = 0;

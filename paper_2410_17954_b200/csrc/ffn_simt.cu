@@ -24,7 +24,7 @@ __device__ __forceinline__ bool find_tile(const EfGroupTable& tab, int tile, int
 template <int kEpi>     // 0 plain, 1 SwiGLU (packed gate/up rows), 2 ReLU
 __global__ void __launch_bounds__(256)
 simt_gemm_kernel(const uint16_t* __restrict__ a, uint16_t* __restrict__ c, const char* __restrict__ arena, int64_t W,
-                 int64_t b_off_bytes, int K, int N, EfGroupTable tab, EfGroupTable ctab) {
+                 int64_t b_off_bytes, int K, int N, int b_rows, EfGroupTable tab, EfGroupTable ctab) {
     constexpr bool kSwiglu = kEpi == 1;
     __shared__ float As[TK][TM + 1];
     __shared__ float B0[TK][TN + 1];
@@ -48,10 +48,10 @@ simt_gemm_kernel(const uint16_t* __restrict__ a, uint16_t* __restrict__ c, const
             if (kSwiglu) {
                 // h column n -> gate row 256*(n/128) + n%128, up row = gate row + 128
                 int64_t gr = (int64_t)(n / EF_W13_BLOCK) * (2 * EF_W13_BLOCK) + (n % EF_W13_BLOCK);
-                B0[kk][r] = (n < N) ? bf2f(Bbase[gr * K + k0 + kk]) : 0.f;
-                B1[kk][r] = (n < N) ? bf2f(Bbase[(gr + EF_W13_BLOCK) * K + k0 + kk]) : 0.f;
+                B0[kk][r] = (n < N) ? bf2f(Bbase[ef_tiled_index(gr, k0 + kk, b_rows, K)]) : 0.f;
+                B1[kk][r] = (n < N) ? bf2f(Bbase[ef_tiled_index(gr + EF_W13_BLOCK, k0 + kk, b_rows, K)]) : 0.f;
             } else {
-                B0[kk][r] = (n < N) ? bf2f(Bbase[(int64_t)n * K + k0 + kk]) : 0.f;
+                B0[kk][r] = (n < N) ? bf2f(Bbase[ef_tiled_index(n, k0 + kk, b_rows, K)]) : 0.f;
             }
         }
         __syncthreads();
@@ -110,15 +110,15 @@ int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const
     if (phase & 1) {
         if (relu)
             simt_gemm_kernel<2><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
-                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, t1, c1);
+                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, f, t1, c1);
         else
             simt_gemm_kernel<1><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
-                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, t1, c1);
+                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, 2 * f, t1, c1);
         ctx->launches++;
     }
     if (phase & 2) {
         simt_gemm_kernel<0><<<dim3((d + TN - 1) / TN, tiles), 256, 0, st>>>(
-            (const uint16_t*)ctx->h_ws, (uint16_t*)y, ctx->arena, ctx->W, (int64_t)(relu ? 1 : 2) * f * d * 2, f, d, t2, c2);
+            (const uint16_t*)ctx->h_ws, (uint16_t*)y, ctx->arena, ctx->W, (int64_t)(relu ? 1 : 2) * f * d * 2, f, d, d, t2, c2);
         ctx->launches++;
     }
     EF_CUDA(ctx, cudaGetLastError());

@@ -153,11 +153,6 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, ui
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.cta_group::2 [%0], [%1, {%3, %4}], [%2];"
         ::"r"(smem_u32(dst)), "l"(tm), "r"(bar), "r"(c0), "r"(c1) : "memory");
 }
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.cta_group::2 [%0], [%1, {%3, %4, %5}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
-}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 // arrives, once the MMAs issued so far have completed, on the barrier at this offset in BOTH CTAs of the pair
@@ -344,6 +339,7 @@ template <int kEpi>     // 0: plain (GEMM2), 1: SwiGLU (gated GEMM1), 2: ReLU (n
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmW,
                 uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int n_pairs_n, int total_tiles,
+                int w_rows, int slot_rowlets, int base_rowlet,
                 int32_t* __restrict__ sched, const SplitArgs sp, long long* __restrict__ kprof,
                 const __grid_constant__ EfGroupTable tab) {
     constexpr bool kSwiglu = kEpi == 1;
@@ -412,14 +408,19 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                 const int half = t.n_mma >> 1;                               // token rows this CTA stages
                 const int n_box = (half + XBOX - 1) / XBOX;
                 const uint32_t bytes = (uint32_t)(W_BYTES + n_box * XBOX_BYTES);
-                const int w_row = (2 * t.n_pair + (int)rank) * BW;
+                // weight tile -> rowlet coordinates in the arena (tiled layout, ef_internal.h): a k-block of the tile is
+                // h_t contiguous rowlets.  The odd last pair's idle partner re-reads tile 0 (its lanes are never stored);
+                // a short last tile's box runs on into the next k-block's rowlets (lanes >= h_t, never stored either)
+                const int w_tile = (2 * t.n_pair + (int)rank) < n_tiles_n ? 2 * t.n_pair + (int)rank : 0;
+                const int h_t = min(BW, w_rows - w_tile * BW);
+                const int w_rowlet0 = t.slot * slot_rowlets + base_rowlet + w_tile * BW * KB;
                 const int x_row = t.a_row + (int)rank * half;
                 for (int kb = t.kb0; kb < t.kb1; ++kb) {
                     mbar_wait(&ctl->empty[stage], phase ^ 1);
                     uint8_t* sw = smem + (size_t)stage * STAGE_BYTES;
                     if (leader) mbar_expect_tx(&ctl->full[stage], 2 * bytes);  // both CTAs' boxes land on this barrier
                     const uint32_t bar = mapa(&ctl->full[stage], 0);
-                    tma_load_3d(sw, &tmW, bar, kb * BK, w_row, t.slot);
+                    tma_load_2d(sw, &tmW, bar, 0, w_rowlet0 + kb * h_t);
                     for (int j = 0; j < n_box; ++j)
                         tma_load_2d(sw + W_BYTES + j * XBOX_BYTES, &tmX, bar, kb * BK, x_row + j * XBOX);
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
@@ -646,15 +647,17 @@ int32_t make_map_2d(ef_ctx* ctx, CUtensorMap* tm, const void* base, int64_t rows
     return EF_OK;
 }
 
-// 3-D bf16 [slot, rows, K] over the arena, box 64 x 256 x 1
-int32_t make_map_arena(ef_ctx* ctx, CUtensorMap* tm, const void* base, int64_t rows, int64_t K) {
+// the whole arena as rowlets: 2-D bf16 [total rowlets, 64], box 64 x 256 = one k-block of one weight tile (32 KB, contiguous)
+int32_t make_map_arena(ef_ctx* ctx, CUtensorMap* tm, const void* base) {
     EncodeTiledFn enc = get_encode();
     if (!enc) return ef_fail(ctx, EF_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
-    cuuint64_t dims[3] = {(cuuint64_t)K, (cuuint64_t)rows, (cuuint64_t)ctx->n_arena_slots};
-    cuuint64_t strides[2] = {(cuuint64_t)K * 2, (cuuint64_t)ctx->W};
-    cuuint32_t box[3] = {BK, BW, 1};
-    cuuint32_t estr[3] = {1, 1, 1};
-    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+    const int64_t rowlets = (int64_t)ctx->n_arena_slots * (ctx->W / (EF_ROWLET * 2));
+    if (rowlets + BW > INT32_MAX) return ef_fail(ctx, EF_ERR_UNSUPPORTED, "slot arena too large for 32-bit rowlet coordinates");
+    cuuint64_t dims[2] = {(cuuint64_t)EF_ROWLET, (cuuint64_t)rowlets};
+    cuuint64_t strides[1] = {(cuuint64_t)EF_ROWLET * 2};
+    cuuint32_t box[2] = {BK, BW};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return ef_fail(ctx, EF_ERR_CUDA, "cuTensorMapEncodeTiled(arena) failed: %d", (int)r);
@@ -701,14 +704,24 @@ SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, d
     return p;
 }
 
+// bytes one launch's TMA loads stage into shared memory (what crosses the L2 -> SM fabric): per token tile and weight-tile
+// pair, per k-block, each CTA of the pair pulls its 32 KB weight box plus the 8 KB token boxes covering its half tile
+int64_t launch_fill_bytes(const EfGroupTable& tab, int npn, int KB) {
+    int64_t per_kb = 0;
+    for (int i = 0; i < tab.n; ++i)
+        for (int off = 0; off < tab.g[i].rows; off += BT) {
+            const int n_mma = (std::min(tab.g[i].rows - off, BT) + 15) & ~15;
+            const int n_box = (n_mma / 2 + XBOX - 1) / XBOX;
+            per_kb += 2 * (int64_t)(W_BYTES + n_box * XBOX_BYTES);
+        }
+    return per_kb * npn * KB;
+}
+
 }  // namespace
 
 int32_t efk_ffn_tc_init(ef_ctx* ctx) {
-    const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
-    const int64_t w1_rows = ctx->cfg.expert_kind == 1 ? f : 2 * (int64_t)f;      // packed W13, or W1 of a non-gated expert
-    int32_t rc = make_map_arena(ctx, &ctx->tm_w13, ctx->arena, w1_rows, d);
-    if (rc != EF_OK) return rc;
-    rc = make_map_arena(ctx, &ctx->tm_wd, ctx->arena + (size_t)w1_rows * d * 2, d, f);
+    static_assert(BK == EF_ROWLET && BW == EF_TILE_ROWS, "the packed layout is tiled for this kernel's stage shape");
+    int32_t rc = make_map_arena(ctx, &ctx->tm_w, ctx->arena);
     if (rc != EF_OK) return rc;
     EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
     EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
@@ -739,6 +752,8 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     }
     const int n_pairs = ctx->n_sms / 2;     // CTA pairs (clusters of 2), one CTA per SM
     const bool relu = ctx->cfg.expert_kind == 1;
+    const int w1_rows = relu ? f : 2 * f;                             // W1 of a non-gated expert, or packed W13
+    const int slot_rowlets = (int)(ctx->W / (EF_ROWLET * 2));
     // optional per-launch timing (ef_set_kernel_timing): one event pair per GEMM launch
     auto span_begin = [&](ef_ctx::KSpan& sp, int which) -> cudaError_t {
         sp.which = which;
@@ -763,17 +778,18 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         const int grid = 2 * std::min(total, n_pairs);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
         if (relu)
-            ffn_gemm_kernel<2><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
-                                                                   total, next_sched(ctx), sp, ctx->kprof1, t1);
+            ffn_gemm_kernel<2><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
+                                                                   total, w1_rows, slot_rowlets, 0, next_sched(ctx), sp, ctx->kprof1, t1);
         else
-            ffn_gemm_kernel<1><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w13, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
-                                                                   total, next_sched(ctx), sp, ctx->kprof1, t1);
+            ffn_gemm_kernel<1><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
+                                                                   total, w1_rows, slot_rowlets, 0, next_sched(ctx), sp, ctx->kprof1, t1);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
         if (ctx->time_kernels) {
             EF_CUDA(ctx, cudaEventRecord(span.e1, st));
             ctx->kspans.push_back(span);
             ctx->ktimes.gemm1_launches++;
+            ctx->ktimes.gemm1_fill_bytes += launch_fill_bytes(tab, npn, d / BK);
             ctx->ktimes.rows += rows_total;
             ctx->ktimes.groups += tab.n;
         }
@@ -791,14 +807,16 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         const int total = pl.n_plain + pl.n_tail * pl.s;
         const int grid = 2 * std::min(total, n_pairs);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
-        ffn_gemm_kernel<0><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_wd, (uint16_t*)y, d, d, f, ntn, npn,
-                                                                   total, next_sched(ctx), sp, ctx->kprof2, t2);
+        ffn_gemm_kernel<0><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_w, (uint16_t*)y, d, d, f, ntn, npn,
+                                                                   total, d, slot_rowlets, (int)((int64_t)w1_rows * d / EF_ROWLET),
+                                                                   next_sched(ctx), sp, ctx->kprof2, t2);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
         if (ctx->time_kernels) {
             EF_CUDA(ctx, cudaEventRecord(span.e1, st));
             ctx->kspans.push_back(span);
             ctx->ktimes.gemm2_launches++;
+            ctx->ktimes.gemm2_fill_bytes += launch_fill_bytes(tab, npn, f / BK);
         }
     }
     return EF_OK;

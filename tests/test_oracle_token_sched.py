@@ -274,3 +274,44 @@ def test_scheduled_batches_need_fewer_loads_in_the_cache_simulator():
         assert sim.stats["misses"] == 0                      # perfect prediction, pool >= two visits' active sets
     assert active[True] < active[False]
     assert loads[True] < loads[False]
+
+
+# ------------------------------------------------------------------------------------------------
+# Eq. 7: batch-level accuracy of a predicted routing path
+# ------------------------------------------------------------------------------------------------
+def test_batch_accuracy_hand_counted_and_special_cases():
+    R = np.array([[1, 1, 0, 0], [0, 1, 1, 1]], np.uint8)          # true: 2 and 3 active experts
+    Rh = np.array([[1, 0, 1, 0], [0, 1, 1, 0]], np.uint8)         # predicted: hits 1 of 2 and 2 of 3
+    assert ts.batch_accuracy(R, Rh) == pytest.approx((1 / 2 + 2 / 3) / 2)
+    assert ts.batch_accuracy(R, R) == 1.0                          # a perfect prediction
+    assert ts.batch_accuracy(R, np.ones_like(R)) == 1.0            # Eq. 7 is a recall: over-prediction is not penalised
+    assert ts.batch_accuracy(R, np.zeros_like(R)) == 0.0
+    assert ts.batch_accuracy(R, 1 - R) == 0.0                      # the complement never hits
+    # not symmetric: swapping the roles divides by the predicted counts instead
+    assert ts.batch_accuracy(Rh, R) == pytest.approx((1 / 2 + 2 / 2) / 2)
+
+
+def test_batch_accuracy_is_the_mean_of_per_layer_recalls_vectorised():
+    g = np.random.default_rng(11)
+    R = (g.random((7, 16)) < 0.4).astype(np.uint8)
+    R[:, 0] = 1                                                    # every layer activates something
+    Rh = (g.random((7, 16)) < 0.5).astype(np.uint8)
+    want = np.mean((R & Rh).sum(1) / R.sum(1))
+    assert ts.batch_accuracy(R, Rh) == pytest.approx(want, rel=1e-12)
+
+
+def test_synthetic_traces_sit_in_the_papers_accuracy_range():
+    """the R17 error model at p = 0.85 / 0.8 gives batch-level accuracies like Table 1's
+    (73-87 %) or above -- the synthetic predicted paths are no easier than a plausible predictor's."""
+    import workloads as wl
+    for name, lo in (("mixtral_decode", 0.85), ("stack_decode", 0.95)):
+        cfg = wl.CONFIGS[name]
+        L = cfg.n_layers
+        tr = wl.routing_trace(cfg, 8)
+        accs = []
+        for s in range(8):
+            true = np.zeros((L, cfg.n_experts), np.uint8)
+            for l in range(L):
+                true[l, np.unique(tr.sets[s * L + l])] = 1
+            accs.append(ts.batch_accuracy(true, tr.predicted[s * L:(s + 1) * L]))
+        assert lo <= np.mean(accs) <= 1.0, (name, np.mean(accs))
