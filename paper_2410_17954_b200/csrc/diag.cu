@@ -1,10 +1,12 @@
 // Diagnostics that are not on the hot path.
 //
 // ef_debug_tma_fill_gbs: how fast TMA can fill shared memory on this device.  The grouped GEMM (ffn_tc.cu) stages
-// 48 KB of operands per CTA per k-block; ncu shows its l1tex__m_xbar2l1tex_read_bytes rate sitting at the L2 -> SM
-// fabric ceiling, so that ceiling -- not the tensor pipe -- is what bounds the prefill GEMM.  This
-// kernel measures the ceiling directly: one persistent CTA per SM, one producer lane streaming 32 KB boxes (the
-// GEMM's weight box: 256 rows x 64 bf16, 128-byte swizzle) through a 4-stage ring, one consumer lane freeing them.
+// 48 KB of operands per CTA per k-block (1024 tensor cycles at full rate), i.e. it asks the L2 -> SM path for 48 bytes
+// per clock and SM; how close that is to what the device can deliver decides whether the tensor pipe can be kept fed
+// (contiguous 32 KB boxes fill at 18-21 TB/s, the same box gathered from 256 strided rows at
+// 14 TB/s -- the reason the packed expert layout is tiled).  This kernel measures the ceiling directly: one persistent
+// CTA per SM, one producer lane streaming 32 KB boxes (the GEMM's weight box: 256 rowlets x 64 bf16, 128-byte
+// swizzle) through a 4-stage ring, one consumer lane freeing them; CTA-scope barriers only.
 #include <algorithm>
 
 #include "ef_internal.h"

@@ -16,8 +16,9 @@
 // halves, so the token operand is fetched from L2 and staged in shared memory once per pair.  Per k-step (K = 64) a
 // CTA therefore pulls 32 KB of weights + <= 16 KB of tokens for 2 * n/2 * 4 tensor cycles -- 48 B/cycle at n = 256
 // against 64 for a single-CTA 256 x 256 tile -- and a stage is 48 KB, which buys a 4th pipeline stage.
-// Tokens past the end of the group are loaded and multiplied (their columns are never stored), rows past the tensor
-// are zero-filled by TMA.
+// Tokens past the end of the group are loaded and multiplied (their columns are never stored), token rows past the
+// tensor are zero-filled by TMA.  The weight operand of a stage is ONE contiguous 32 KB box: the packed expert layout
+// is tiled in streaming order (ef_internal.h), and the whole slot arena is one 2-D tensor map of 128-byte rowlets.
 //
 // Warp roles (384 threads, 1 CTA/SM, persistent; both CTAs unless stated):
 //   warp 0     TMA producer + tile scheduler : the LEADER claims the next unit with one atomicAdd on a per-launch
