@@ -34,11 +34,14 @@ DUAL_FAMILIES, DUAL_FAMILY_PROB = 2, 0.9     # dual_batch_stack: latent token gr
 METRIC = "moe_layer_tokens_per_s"
 UNIT = "tokens/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel (GEMM1), bytes per launch averaged over the
-# launches of a streaming step, from the committed `ncu --set full` captures (never measured by this script):
-#   mixtral_prefill: profiles/r1_ffn_gemm_ncu_full.md  -- one wave-0 launch (1.2833 GB) + 4 single-expert launches (0.2406 GB)
-#   mixtral_decode : profiles/r1_ffn_decode_ncu_full.md -- single-expert launches (0.2386 GB)
-NCU_TRAFFIC_BYTES = {"mixtral_prefill": (1.2833e9 + 4 * 0.24055e9) / 5, "mixtral_decode": 0.23861e9}
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel (GEMM1) per launch, from the
+# committed `ncu --set full` captures (never measured by this script, which never runs under a profiler):
+#   mixtral_prefill: profiles/r1f_ffn_prefill_ncu_full.md -- the 6 GEMM1 launches of one steady-state streaming step
+#                    (2.5196 GB in all); resident leg: the one launch over all 8 experts (2.5485 GB)
+#   mixtral_decode : profiles/r1f_ffn_decode_ncu_full.md  -- 4 GEMM1 launches of a streaming step (three single-expert
+#                    waves and one 5-expert wave, 1.8973 GB in all); resident leg: one launch over 7 experts (1.6498 GB)
+NCU_TRAFFIC_BYTES = {"mixtral_prefill": 2.5196e9 / 6, "mixtral_decode": 1.8973e9 / 4}
+NCU_TRAFFIC_BYTES_RESIDENT = {"mixtral_prefill": 2.5485e9, "mixtral_decode": 1.6498e9}
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -596,7 +599,18 @@ def run_dual_batch(args):
             p, b, x = paths_stage, bias_stage, x_stage
         else:
             p, b, x = paths_dev[s], bias_dev[s], x_dev[s]
-        if sched:
+        if sched and not e2e:
+            # dual-batch pipeline: this unit's schedule was enqueued on the side stream before the previous
+            # unit's decode; pick it up, then enqueue the next unit's before decoding this one
+            slot = state["step"] & 1
+            if state.get("pending") != state["step"]:
+                db.schedule_async(p, cents[s][0], cents[s][1], x, b, slot)
+            rows = db.wait_schedule(slot)
+            x, b = db.x_re, db.bias_re
+            s1 = (state["step"] + 1) % ts
+            db.schedule_async(paths_dev[s1], cents[s1][0], cents[s1][1], x_dev[s1], bias_dev[s1], slot ^ 1)
+            state["pending"] = state["step"] + 1
+        elif sched:
             rows = db.schedule(p, cents[s][0], cents[s][1], x, b)
             x, b = db.x_re, db.bias_re
         else:
@@ -609,7 +623,9 @@ def run_dual_batch(args):
 
     def timed(sched, e2e, steps, warmup, with_kernel_times=False):
         runner.ctx.ef_sync(); runner.ctx.ef_cache_clear()
+        torch.cuda.synchronize()
         state["step"] = 0
+        state["pending"] = None
         for _ in range(warmup):
             step(sched, e2e)
         runner.ctx.ef_sync(); runner.ctx.ef_cache_reset_stats()
@@ -684,6 +700,9 @@ def run_dual_batch(args):
                 "gpu_launches": on["launches"], "roofline": roofline, "h2d": h2d,
                 "token_scheduler": {"on": a_on, "off": a_off, "speedup": a_on["tokens_per_s"] / a_off["tokens_per_s"],
                                     "schedule_call_us": sched_us,
+                                    "pipeline": "dual-batch (P:L189-199): unit n+1 is scheduled on a side stream while unit n "
+                                                "decodes (DualBatchRunner.schedule_async / wait_schedule); the e2e leg schedules "
+                                                "sequentially because its inputs are staged per step",
                                     "eq5_objective_predicted_paths": {"incoming": float(objs[:, 5].mean()), "scheduled": float(objs[:, 4].mean())},
                                     "kmeans_rounds_mean": float(objs[:, 0].mean()), "converged_frac": float(objs[:, 1].mean())},
                 "cache": dict(st, hit_ratio=st["hits"] / max(1, st["lookups"])), "cpu_baseline": cpu_baseline}
@@ -772,6 +791,7 @@ def resident_leg(cfg, counts, peaks, dev, args, decode, fill_peak=None):
                        gated=cfg.expert_kind == "swiglu", fill_peak=fill_peak)
     if not decode:
         res["peak_source"] = f"{peaks['source']} bf16 burst (kernel timed alone)"
+    res["traffic"] = NCU_TRAFFIC_BYTES_RESIDENT.get(cfg.name)
     res["rows_per_expert"] = [int(c) for c in counts]
     res["l2"] = "256 MB flush write between launches" if flush is not None else "weights exceed L2 between launches"
     ctx.close()

@@ -91,34 +91,60 @@ class MoELayerRunner:
 class DualBatchRunner:
     """Two incoming batches of T tokens per step through the Token Scheduler (§3.3, §4.2): schedule on the
     predicted routing paths -> Reindex activations and per-token rows into the new batches -> the new batches'
-    batch-level predicted paths drive the cache prefetch -> 2 x L layer visits.  Sequencing and buffers only."""
+    batch-level predicted paths drive the cache prefetch -> 2 x L layer visits.  Sequencing and buffers only.
+
+    Dual-batch pipeline (§4.2, Fig. 6): the scheduling of unit n+1 is interleaved with the decoding of
+    unit n -- `schedule_async` enqueues it on a side stream into the other half of double-buffered outputs and
+    `wait_schedule` picks the result up when unit n+1 starts, so its cost (kernels, Reindex, the read-back of the
+    batch paths) never sits between two decode steps.  `schedule` is the sequential form of the same two calls."""
 
     def __init__(self, runner: MoELayerRunner, max_iter: int = 8):
         self.r = r = runner
         T, L, E, d, dev = r.max_tokens, r.L, r.E, r.d, r.dev
         self.T, self.N, self.max_iter = T, 2 * T, max_iter
         N = self.N
+        self.side = torch.cuda.Stream(device=dev)
         self.batch_of = torch.empty((N,), dtype=torch.int32, device=dev)
         self.perm = torch.empty((N,), dtype=torch.int32, device=dev)
         self.info = torch.empty((8,), dtype=torch.int32, device=dev)
         self.batch_paths = torch.empty((2, L * E), dtype=torch.uint8, device=dev)
-        self.batch_paths_host = torch.empty((2, L * E), dtype=torch.uint8).pin_memory()
-        self.x_re = torch.empty((N, d), dtype=torch.bfloat16, device=dev)
-        self.bias_re = torch.empty((N, L, E), dtype=torch.float32, device=dev)
+        # double-buffered results of a schedule call (slot = unit parity)
+        self.batch_paths_host = [torch.empty((2, L * E), dtype=torch.uint8).pin_memory() for _ in range(2)]
+        self.x_re_buf = [torch.empty((N, d), dtype=torch.bfloat16, device=dev) for _ in range(2)]
+        self.bias_re_buf = [torch.empty((N, L, E), dtype=torch.float32, device=dev) for _ in range(2)]
+        self.done = [torch.cuda.Event() for _ in range(2)]
+        self.x_re, self.bias_re = self.x_re_buf[0], self.bias_re_buf[0]
         self.hbuf = [torch.empty((T, d), dtype=torch.bfloat16, device=dev) for _ in range(2)]
 
-    def schedule(self, pred_paths: torch.Tensor, c0: int, c1: int, x: torch.Tensor, token_bias: torch.Tensor | None):
-        """pred_paths uint8 [N, L, E], x bf16 [N, d], token_bias fp32 [N, L, E] (all device).  Returns the predicted
-        batch-level rows uint8 [2L, E] (host) of the 2L visits of this step, and leaves x / bias reindexed in
-        self.x_re / self.bias_re.  The one host wait is on the 2*L*E bytes of batch paths the prefetch call needs."""
+    def schedule_async(self, pred_paths: torch.Tensor, c0: int, c1: int, x: torch.Tensor, token_bias: torch.Tensor | None,
+                       slot: int = 0):
+        """Enqueue Token Scheduler + Reindex + batch-path read-back for one dual-batch unit on the side stream, into
+        buffer `slot`.  The side stream first waits for everything enqueued on the current stream so far (the inputs'
+        producers, and the decode step that last read this slot's buffers).  Returns at once."""
         c = self.r.ctx
-        c.ef_token_schedule(pred_paths, c0, c1, self.max_iter, self.batch_of, self.perm, self.info, self.batch_paths)
-        c.ef_reindex_rows(x, self.perm, self.x_re)
-        if token_bias is not None:
-            c.ef_reindex_rows(token_bias, self.perm, self.bias_re)
-        self.batch_paths_host.copy_(self.batch_paths, non_blocking=True)
-        torch.cuda.current_stream().synchronize()
-        return self.batch_paths_host.numpy().reshape(2 * self.r.L, self.r.E)
+        self.side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(self.side):
+            c.ef_token_schedule(pred_paths, c0, c1, self.max_iter, self.batch_of, self.perm, self.info, self.batch_paths)
+            c.ef_reindex_rows(x, self.perm, self.x_re_buf[slot])
+            if token_bias is not None:
+                c.ef_reindex_rows(token_bias, self.perm, self.bias_re_buf[slot])
+            self.batch_paths_host[slot].copy_(self.batch_paths, non_blocking=True)
+            self.done[slot].record(self.side)
+
+    def wait_schedule(self, slot: int = 0):
+        """Pick up the result of schedule_async(slot): the current stream waits for the reindexed rows, the host for
+        the 2*L*E bytes of batch paths that the (host-side) prefetch call consumes.  Returns the predicted batch-level
+        rows uint8 [2L, E] (host) of the unit's 2L visits; x / bias in new-batch order are self.x_re / self.bias_re."""
+        torch.cuda.current_stream().wait_event(self.done[slot])
+        self.done[slot].synchronize()
+        self.x_re, self.bias_re = self.x_re_buf[slot], self.bias_re_buf[slot]
+        return self.batch_paths_host[slot].numpy().reshape(2 * self.r.L, self.r.E)
+
+    def schedule(self, pred_paths: torch.Tensor, c0: int, c1: int, x: torch.Tensor, token_bias: torch.Tensor | None):
+        """pred_paths uint8 [N, L, E], x bf16 [N, d], token_bias fp32 [N, L, E] (all device).  Sequential form:
+        schedule now, wait for it.  Returns what wait_schedule returns."""
+        self.schedule_async(pred_paths, c0, c1, x, token_bias, 0)
+        return self.wait_schedule(0)
 
     def run_step(self, step: int, rows: np.ndarray, x: torch.Tensor, token_bias: torch.Tensor | None, out: torch.Tensor,
                  on_visit=None):

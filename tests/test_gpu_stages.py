@@ -310,3 +310,31 @@ def test_errors_are_codes_not_crashes():
                           torch.zeros((100, 2), device="cuda"))
     assert e.value.code == -6
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# diagnostics used by bench.py's second roofline
+# ------------------------------------------------------------------------------------------------
+def test_tma_fill_rate_and_fill_byte_accounting():
+    E, d, f, counts = 2, 512, 1024, [300, 17]
+    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)))
+    gbs = ctx.ef_debug_tma_fill_gbs(32 << 20, 500)
+    assert 2000.0 < gbs < 40000.0                     # an L2-resident region: several TB/s on a B200
+    with pytest.raises(Exception):
+        ctx.ef_debug_tma_fill_gbs(16, 500)            # smaller than one box
+    ctx.ef_set_kernel_timing(True)
+    ctx.ef_get_kernel_times(reset=True)
+    run_resident_ffn(ctx, E, d, f, counts, seed=3, simt=False, splitk=1)
+    kt = ctx.ef_get_kernel_times(reset=True)
+    ctx.ef_set_kernel_timing(False)
+    # tile plan: expert 0 = tiles of 256 and 44 rows, expert 1 = one tile of 17 rows.  Per k-block a CTA pair stages
+    # 2 x 32 KB of weights and, per CTA, the 8 KB token boxes covering half of the tile rounded up to 16 rows
+    def per_kb(rows):
+        n_mma = (rows + 15) // 16 * 16
+        return 2 * (32768 + -(-(n_mma // 2) // 64) * 8192)
+    tiles = per_kb(256) + per_kb(44) + per_kb(17)
+    npn1, npn2 = (f // 128 + 1) // 2, ((d + 255) // 256 + 1) // 2
+    assert kt["gemm1_fill_bytes"] == tiles * npn1 * (d // 64)
+    assert kt["gemm2_fill_bytes"] == tiles * npn2 * (f // 64)
+    assert kt["rows"] == sum(counts) and kt["groups"] == 2
+    ctx.close()

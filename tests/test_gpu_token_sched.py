@@ -220,3 +220,53 @@ def test_dual_batch_pipeline_matches_oracle_chain():
         check_float(got, ref_all[sc.perm])
     assert improved >= 1
     r.close()
+
+
+def test_dual_batch_overlapped_schedule_equals_sequential():
+    """§4.2: scheduling unit n+1 on the side stream while unit n decodes changes nothing -- permutation,
+    batch paths, reindexed rows, cache counters and final hidden states equal those of the sequential pipeline."""
+    from paper_2410_17954_b200 import DualBatchRunner
+    from test_gpu_layer import build_runner
+    from test_gpu_stages import dev_bf16, to_bits
+
+    cfg = wl.scaled(wl.CONFIGS["dual_batch_stack"], d_model=256, d_ff=512, T=8, n_layers=3, n_slots=9)
+    L, E, T, N = cfg.n_layers, cfg.n_experts, cfg.T, 2 * cfg.T
+    n_steps = 6
+    tr = wl.dual_batch_trace(cfg, n_steps, n_families=2, family_prob=0.85)
+    dev = torch.device("cuda", 0)
+    g = np.random.default_rng(5)
+    cents = [tuple(int(v) for v in g.choice(N, 2, replace=False)) for _ in range(n_steps)]
+    paths = [torch.from_numpy(wl.sets_to_paths(tr.pred_sets[s], E)).to(dev) for s in range(n_steps)]
+    biases = [torch.from_numpy(wl.bias_from_sets(cfg, tr.sets[s])).to(dev) for s in range(n_steps)]
+    xs = [dev_bf16(wl.normal_bf16(cfg.seed, f"x.dual.step{s}", (N, cfg.d_model), 1.0)) for s in range(n_steps)]
+
+    def run(overlapped):
+        r, _ = build_runner(cfg, horizon=0)
+        db = DualBatchRunner(r, max_iter=8)
+        outs, perms, rows_all = [], [], []
+        if overlapped:
+            db.schedule_async(paths[0], *cents[0], xs[0], biases[0], 0)
+        for s in range(n_steps):
+            if overlapped:
+                rows = db.wait_schedule(s & 1).copy()
+                perms.append(db.perm.cpu().numpy().copy())          # before the next call overwrites it
+                if s + 1 < n_steps:
+                    db.schedule_async(paths[s + 1], *cents[s + 1], xs[s + 1], biases[s + 1], (s + 1) & 1)
+            else:
+                rows = db.schedule(paths[s], *cents[s], xs[s], biases[s]).copy()
+                perms.append(db.perm.cpu().numpy().copy())
+            out = torch.empty((N, cfg.d_model), dtype=torch.bfloat16, device=dev)
+            db.run_step(s, rows, db.x_re, db.bias_re, out)
+            outs.append(out)
+            rows_all.append(rows)
+        r.ctx.ef_sync()
+        st, snap = r.ctx.ef_cache_get_stats(), r.ctx.ef_cache_snapshot()
+        res = [to_bits(o) for o in outs]
+        r.close()
+        return res, perms, rows_all, st, snap
+
+    a, b = run(False), run(True)
+    for s in range(n_steps):
+        assert np.array_equal(a[1][s], b[1][s]) and np.array_equal(a[2][s], b[2][s])
+        assert np.array_equal(a[0][s], b[0][s])                      # same kernels on the same inputs: same bits
+    assert a[3] == b[3] and a[4] == b[4]
