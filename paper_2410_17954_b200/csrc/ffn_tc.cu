@@ -311,7 +311,23 @@ __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemC
         t.kb0 = (t.split_j * KB) / sp.s;
         t.kb1 = ((t.split_j + 1) * KB) / sp.s;
     }
-    if (tile < ctl->total_long) {
+    // Ticket order: long (129..256-token) tiles are tensor-bound, short ones are bound by streaming their weight tile,
+    // so a launch with many short tiles (many-expert prefill) spreads them evenly among the long ones -- both kinds
+    // are then in flight on different SMs at the same time -- and keeps only the last `tail_short` short tiles for the
+    // end of the list, where small units even out the finish (and where the split-K tail lives).
+    const int total_short = ctl->gstart_short[tab.n];
+    const int tail_short = min(total_short, (int)gridDim.x);
+    const int spread = total_short - tail_short, first = ctl->total_long + spread;
+    bool is_short;
+    if (tile >= first) {
+        is_short = true;
+        tile = spread + (tile - first);
+    } else {
+        const int sb = (int)(((long long)tile * spread) / first), sb1 = (int)(((long long)(tile + 1) * spread) / first);
+        is_short = sb1 > sb;
+        tile = is_short ? sb : tile - sb;
+    }
+    if (!is_short) {
         while (tile >= ctl->gstart_long[g + 1]) ++g;
         const int local = tile - ctl->gstart_long[g];
         const int nl = group_long_tiles(tab.g[g].rows);
@@ -319,7 +335,7 @@ __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemC
         row_off = (local % nl) * BT;
         t.is_long = 1;
     } else {
-        const int ts = tile - ctl->total_long;
+        const int ts = tile;
         while (ts >= ctl->gstart_short[g + 1]) ++g;
         t.n_pair = ts - ctl->gstart_short[g];
         row_off = group_long_tiles(tab.g[g].rows) * BT;
