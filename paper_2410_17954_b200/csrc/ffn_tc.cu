@@ -88,6 +88,8 @@ struct __align__(8) SmemCtl {
     int32_t total_long;                   // number of > 128-token tiles (they come first)
     int32_t gstart_long[EF_MAX_GROUPS + 1];
     int32_t gstart_short[EF_MAX_GROUPS + 1];
+    int16_t g_tile_rows[EF_MAX_GROUPS];   // token tiling of each group (prologue): rows per tile ...
+    int16_t g_long[EF_MAX_GROUPS];        // ... and number of > 128-token tiles
 };
 
 constexpr size_t kSmemBytes = 1024 /*align slack*/ + (size_t)kStages * STAGE_BYTES + 2 * STG_BYTES + sizeof(SmemCtl);
@@ -294,8 +296,31 @@ struct SplitArgs {
 };
 
 // number of "long" (129..256-token) tiles of a group; the remainder, if any, is one short tile per n
-__device__ __host__ __forceinline__ int group_long_tiles(int rows) { return rows / BT + ((rows % BT) > 128 ? 1 : 0); }
-__device__ __host__ __forceinline__ int group_has_short(int rows) { int r = rows % BT; return (r > 0 && r <= 128) ? 1 : 0; }
+// Token tiling of a group.  A tile narrower than ~170 tokens costs as much per k-block as a 170-token one (its 32 KB
+// weight stage has to be filled either way), so with a long K loop a group of 257..4096 rows is cut into
+// ceil(rows / 256) BALANCED tiles of b = ceil16(rows / tiles) rows instead of full 256-row tiles plus a small remainder
+// (593 rows: 208 + 208 + 177, not 256 + 256 + 81): measured +5 % / +3 % on GEMM1 / GEMM2 of the Mixtral shape.  With a
+// short K loop (K < 3072: the many-expert shapes) the fixed cost of one more 129..256-token tile -- its epilogue is not
+// overlapped, it owns all of TMEM -- outweighs that (measured -2 % / -6 %), so those keep 256-row tiles + remainder.
+// Tiles 0 .. n-2 hold b rows, the last one what is left; it is "short" (<= 128 tokens, half of TMEM) or "long".
+constexpr int kBalancedMinK = 3072;
+__device__ __host__ __forceinline__ int group_tile_rows(int rows, bool balanced) {
+    const int n = (rows + BT - 1) / BT;
+    if (!balanced || n < 2 || n > 16) return BT;
+    const int b = (((rows + n - 1) / n) + 15) & ~15;
+    return ((n - 1) * b < rows) ? b : BT;
+}
+// (the b == BT paths are shifts and masks: the kernel prologue walks up to 64 groups in one thread)
+__device__ __host__ __forceinline__ int group_long_tiles(int rows, bool balanced) {
+    const int b = group_tile_rows(rows, balanced);
+    if (b == BT) return rows / BT + ((rows % BT) > 128 ? 1 : 0);
+    return rows / b + ((rows % b) > 128 ? 1 : 0);
+}
+__device__ __host__ __forceinline__ int group_has_short(int rows, bool balanced) {
+    const int b = group_tile_rows(rows, balanced);
+    const int r = (b == BT) ? rows % BT : rows % b;
+    return (r > 0 && r <= 128) ? 1 : 0;
+}
 
 __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemCtl* ctl, int unit, const SplitArgs& sp,
                                             int KB) {
@@ -330,18 +355,18 @@ __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemC
     if (!is_short) {
         while (tile >= ctl->gstart_long[g + 1]) ++g;
         const int local = tile - ctl->gstart_long[g];
-        const int nl = group_long_tiles(tab.g[g].rows);
+        const int nl = ctl->g_long[g];
         t.n_pair = local / nl;
-        row_off = (local % nl) * BT;
+        row_off = (local - t.n_pair * nl) * ctl->g_tile_rows[g];
         t.is_long = 1;
     } else {
         const int ts = tile;
         while (ts >= ctl->gstart_short[g + 1]) ++g;
         t.n_pair = ts - ctl->gstart_short[g];
-        row_off = group_long_tiles(tab.g[g].rows) * BT;
+        row_off = ctl->g_long[g] * ctl->g_tile_rows[g];
         t.is_long = 0;
     }
-    t.rows_valid = min(tab.g[g].rows - row_off, BT);
+    t.rows_valid = min(tab.g[g].rows - row_off, (int)ctl->g_tile_rows[g]);
     t.n_mma = (t.rows_valid + 15) & ~15;
     t.a_row = tab.g[g].a_row0 + row_off;
     t.c_row = tab.g[g].c_row0 + row_off;
@@ -383,17 +408,28 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
         asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&ctl->tmem_base)), "r"(kTmemCols) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
     }
-    if (warp == 3 && lane == 0) {
-        int nl = 0, ns = 0;
-        for (int g = 0; g < tab.n; ++g) {
-            ctl->gstart_long[g] = nl;
-            ctl->gstart_short[g] = ns;
-            nl += group_long_tiles(tab.g[g].rows) * n_pairs_n;
-            ns += group_has_short(tab.g[g].rows) * n_pairs_n;
+    if (warp == 3) {
+        // per-group token tiling (lanes in parallel), then the exclusive scans of the tile counts (one lane)
+        for (int g = lane; g < tab.n; g += 32) {
+            const int rows = tab.g[g].rows;
+            const bool bal = K >= kBalancedMinK;
+            const int nlg = group_long_tiles(rows, bal);
+            ctl->g_tile_rows[g] = (int16_t)group_tile_rows(rows, bal);
+            ctl->g_long[g] = (int16_t)nlg;
+            ctl->gstart_long[g + 1] = nlg * n_pairs_n;
+            ctl->gstart_short[g + 1] = group_has_short(rows, bal) * n_pairs_n;
         }
-        ctl->gstart_long[tab.n] = nl;
-        ctl->gstart_short[tab.n] = ns;
-        ctl->total_long = nl;
+        __syncwarp();
+        if (lane == 0) {
+            int nl = 0, ns = 0;
+            ctl->gstart_long[0] = 0;
+            ctl->gstart_short[0] = 0;
+            for (int g = 1; g <= tab.n; ++g) {
+                nl += ctl->gstart_long[g];  ctl->gstart_long[g] = nl;
+                ns += ctl->gstart_short[g]; ctl->gstart_short[g] = ns;
+            }
+            ctl->total_long = nl;
+        }
     }
     tc_fence_before();
     cluster_sync();               // barriers of both CTAs are initialised before any remote arrive / multicast commit
@@ -726,8 +762,8 @@ SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, d
 int64_t launch_fill_bytes(const EfGroupTable& tab, int npn, int KB) {
     int64_t per_kb = 0;
     for (int i = 0; i < tab.n; ++i)
-        for (int off = 0; off < tab.g[i].rows; off += BT) {
-            const int n_mma = (std::min(tab.g[i].rows - off, BT) + 15) & ~15;
+        for (int off = 0, b = group_tile_rows(tab.g[i].rows, KB * BK >= kBalancedMinK); off < tab.g[i].rows; off += b) {
+            const int n_mma = (std::min(tab.g[i].rows - off, b) + 15) & ~15;
             const int n_box = (n_mma / 2 + XBOX - 1) / XBOX;
             per_kb += 2 * (int64_t)(W_BYTES + n_box * XBOX_BYTES);
         }
@@ -758,12 +794,16 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
     if (tab.n == 0) return EF_OK;
     int64_t rows_total = 0;
-    int mtiles = 0, mshort = 0;   // tiles per n column: every group's 256-row tiles plus its short tail tile
+    // tiles per n column (every group's long tiles plus its short tail tile) under the tiling GEMM1 / GEMM2 will use
+    int mtiles1 = 0, mshort1 = 0, mtiles2 = 0, mshort2 = 0;
+    const bool bal1 = d >= kBalancedMinK, bal2 = f >= kBalancedMinK;
     EfGroupTable t1 = tab, t2 = tab;
     for (int i = 0; i < tab.n; ++i) {
         rows_total += tab.g[i].rows;
-        mtiles += group_long_tiles(tab.g[i].rows) + group_has_short(tab.g[i].rows);
-        mshort += group_has_short(tab.g[i].rows);
+        mtiles1 += group_long_tiles(tab.g[i].rows, bal1) + group_has_short(tab.g[i].rows, bal1);
+        mshort1 += group_has_short(tab.g[i].rows, bal1);
+        mtiles2 += group_long_tiles(tab.g[i].rows, bal2) + group_has_short(tab.g[i].rows, bal2);
+        mshort2 += group_has_short(tab.g[i].rows, bal2);
         t1.g[i].c_row0 = h_row0[i];   // GEMM1: x rows -> h rows
         t2.g[i].a_row0 = h_row0[i];   // GEMM2: h rows -> y rows
     }
@@ -789,8 +829,8 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         if (ctx->time_kernels) EF_CUDA(ctx, span_begin(span, 1));
         const int ntn = relu ? (f + BW - 1) / BW : f / 128;      // 256 packed W13 rows -> 128 h columns; 256 W1 rows -> 256
         const int npn = (ntn + 1) / 2;
-        const int tiles = mtiles * npn;
-        const SplitPlan pl = plan_split(ctx, tiles, mshort * npn, n_pairs, d / BK, (double)rows_total / mtiles);
+        const int tiles = mtiles1 * npn;
+        const SplitPlan pl = plan_split(ctx, tiles, mshort1 * npn, n_pairs, d / BK, (double)rows_total / mtiles1);
         const int total = pl.n_plain + pl.n_tail * pl.s;
         const int grid = 2 * std::min(total, n_pairs);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
@@ -819,8 +859,8 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         if (ctx->time_kernels) EF_CUDA(ctx, span_begin(span, 2));
         const int ntn = (d + BW - 1) / BW;
         const int npn = (ntn + 1) / 2;
-        const int tiles = mtiles * npn;
-        const SplitPlan pl = plan_split(ctx, tiles, mshort * npn, n_pairs, f / BK, (double)rows_total / mtiles);
+        const int tiles = mtiles2 * npn;
+        const SplitPlan pl = plan_split(ctx, tiles, mshort2 * npn, n_pairs, f / BK, (double)rows_total / mtiles2);
         const int total = pl.n_plain + pl.n_tail * pl.s;
         const int grid = 2 * std::min(total, n_pairs);
         const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};

@@ -179,6 +179,9 @@ FFN_CASES = [
     (5, 512, 1408 - 1408 % 128, [300, 7, 0, 513, 64]),
     (2, 64, 128, [1, 1]),
     (2, 1024, 384, [257, 255]),
+    # K >= 3072 switches the token tiling to balanced tiles (593 -> 208 + 208 + 177): GEMM1 (K = d), then GEMM2 (K = f)
+    (2, 3072, 256, [300, 593]),
+    (3, 256, 3072, [513, 257, 130]),
 ]
 
 
@@ -327,7 +330,7 @@ def test_tma_fill_rate_and_fill_byte_accounting():
     run_resident_ffn(ctx, E, d, f, counts, seed=3, simt=False, splitk=1)
     kt = ctx.ef_get_kernel_times(reset=True)
     ctx.ef_set_kernel_timing(False)
-    # tile plan: expert 0 = tiles of 256 and 44 rows, expert 1 = one tile of 17 rows.  Per k-block a CTA pair stages
+    # tile plan (K < 3072: 256-row tiles + remainder): expert 0 = tiles of 256 and 44 rows, expert 1 = one tile of 17 rows.  Per k-block a CTA pair stages
     # 2 x 32 KB of weights and, per CTA, the 8 KB token boxes covering half of the tile rounded up to 16 rows
     def per_kb(rows):
         n_mma = (rows + 15) // 16 * 16
