@@ -298,7 +298,8 @@ class Driver:
     """Owns one MoELayerRunner plus the step inputs of a workload; step(i) = one pass of the whole hot path
     (n_layers visits) over batch i.  Sequencing only: every step of the path runs in libef's kernels."""
 
-    def __init__(self, cfg, dev, x_stream: str, steps_total: int, phys_experts: int = 0, log=lambda *_: None):
+    def __init__(self, cfg, dev, x_stream: str, steps_total: int, phys_experts: int = 0, log=lambda *_: None,
+                 policy: str = "plec"):
         import torch
         from paper_2410_17954_b200 import MoELayerRunner
         from paper_2410_17954_b200.layer import bf16_tensor_from_bits
@@ -306,6 +307,9 @@ class Driver:
         L, E, T, d = cfg.n_layers, cfg.n_experts, cfg.T, cfg.d_model
         self.runner = r = MoELayerRunner(L, E, cfg.top_k, d, cfg.d_ff, cfg.n_slots, cfg.n_shared, T, cfg.horizon,
                                          cfg.renorm, device=dev.index, expert_kind=1 if cfg.expert_kind == "relu" else 0)
+        # cache policy arm: the paper's PLEC, the two LRU baselines, or "prefetch every expert of the
+        # next layer" = PLEC fed an all-ones predicted path one visit ahead
+        r.ctx.ef_set_cache_policy("plec" if policy == "next_layer_all" else policy)
         threads = os.cpu_count() or 8
         n_total = L * E
         self.phys = phys_experts if 0 < phys_experts < n_total else 0
@@ -343,6 +347,8 @@ class Driver:
             self.bias_stage = torch.empty((L, T, E), dtype=torch.float32, device=dev)
             self.look = L if cfg.horizon <= 0 else cfg.horizon
             self.pred = self.trace.predicted
+            if policy == "next_layer_all":
+                self.pred = np.ones_like(self.pred)
         else:
             self.look = 1
             self.pred = np.ones((1, E), np.uint8)      # replaced by the gate's own active set after warm-up
@@ -443,7 +449,7 @@ def run_ours(args):
             log(f"pinned pool of {need / 1e9:.1f} GB does not fit comfortably in {avail / 1e9:.1f} GB of host memory: "
                 f"aliasing {cfg.n_layers * cfg.n_experts} logical experts onto {phys} physical buffers")
     steps_total = 2 * (args.steps + args.warmup) + 2
-    drv = Driver(cfg, dev, plan["x_stream"], steps_total, phys, log)
+    drv = Driver(cfg, dev, plan["x_stream"], steps_total, phys, log, args.policy)
     runner = drv.runner
     runner.ctx.ef_sync()                 # the warm-up prefetch must not share the link with the peak measurement
     h2d_peak = measure_pinned_h2d(dev, cfg.expert_bytes) if rank == 0 else None
@@ -531,7 +537,8 @@ def run_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                "config": workload_config(cfg, world, {"phys_host_experts": drv.phys or cfg.n_layers * cfg.n_experts}),
+                "config": workload_config(cfg, world, {"phys_host_experts": drv.phys or cfg.n_layers * cfg.n_experts,
+                                                       "cache_policy": args.policy}),
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_h2d + int(h2d["bytes_per_step"]),
                         "d2h_bytes_per_step": io_d2h, "ms_per_step": ms_e2e_max / args.steps,
@@ -812,11 +819,16 @@ def main():
                          "if host memory allows)")
     ap.add_argument("--horizon", type=int, default=None,
                     help="override the workload's prefetch horizon H in visits (<= 0: as far as the supplied path reaches; R10)")
+    ap.add_argument("--policy", default="plec", choices=["plec", "lru", "layer_lru", "next_layer_all"],
+                    help="cache policy arm: the paper's PLEC (default), on-demand LRU over the pool, LRU inside a per-layer "
+                         "share, or PLEC prefetching every expert of the next layer (the baselines of P:L230 as policy sketches)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-resident", action="store_true")
     args = ap.parse_args()
     if args.horizon is not None:
         wl.CONFIGS[args.workload] = wl.scaled(wl.CONFIGS[args.workload], horizon=args.horizon)
+    if args.policy == "next_layer_all":
+        wl.CONFIGS[args.workload] = wl.scaled(wl.CONFIGS[args.workload], horizon=1)
     if args.impl == "reference":
         run_reference(args)
     elif args.workload == "dual_batch_stack":

@@ -167,6 +167,18 @@ int32_t ef_cache_snapshot(ef_ctx* ctx, int32_t* slot_to_expert);
 /* Empty the slot table and forget supplied predictions (counters untouched). */
 int32_t ef_cache_clear(ef_ctx* ctx);
 
+/* Replacement policy of the slot table.  EF_POLICY_PLEC (default) is the paper's Expert Cache Engine as read
+ * in DESIGN.md section 4.  The other two are the baselines the paper compares against, as policy sketches on the same
+ * machinery: on-demand loading with least-recently-used replacement over the whole
+ * pool (EF_POLICY_LRU) or inside a fixed share of n_slots / n_layers slots per layer (EF_POLICY_LAYER_LRU, "fixed-size
+ * cache per layer"); under both, ef_cache_prefetch accepts its arguments and does nothing.  (The third baseline of
+ * P:L230, prefetching ALL experts of the next layer, needs no policy: it is EF_POLICY_PLEC with an all-ones predicted path
+ * and prefetch_horizon = 1.)  Only allowed while the slot table is empty. */
+#define EF_POLICY_PLEC 0
+#define EF_POLICY_LRU 1
+#define EF_POLICY_LAYER_LRU 2
+int32_t ef_set_cache_policy(ef_ctx* ctx, int32_t policy);
+
 /* Device time the copy stream spent on expert loads since the last reset, from events (milliseconds),
  * and the wall time of the window in which the copy queue was non-empty are not part of parity;
  * ef_copy_busy_ms waits for the copy stream.  Synchronous. */

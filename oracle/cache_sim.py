@@ -16,6 +16,13 @@ What the paper fixes (and what pins this file, tests/test_oracle_cache.py):
 What the paper leaves open (tie-breaks, horizon, "completed" under asynchrony) is a DESIGN.md
 reading; fidelity of those readings to the authors' code is unpinned (no code exists).
 
+Baseline policies (the paper's comparison points as policy sketches, "Cache-MoE ... a fixed-size
+cache per layer, using a Least-Recently-Used strategy"): `policy="lru"` -- on-demand loading, the victim is an
+empty slot, else the least recently used slot of the whole pool; `policy="layer_lru"` -- the same inside the requesting
+layer's own S // L slots.  Neither consults predictions; `prefetch` does nothing.  (SE-MoE-like "prefetch all experts of
+the next layer", is `policy="plec"` fed an all-ones predicted path with horizon 1.)  Pins: textbook LRU on a
+hand-worked reference string and an independent OrderedDict LRU (tests/test_oracle_cache.py).
+
 Vocabulary: visit v = step * L + layer (logical clock).  g = layer * E + e (global expert id).
 A slot is *pending* while it holds a prefetched expert that has not been used since its load.
 """
@@ -36,8 +43,11 @@ class VisitPlan:
 
 
 class CacheSim:
-    def __init__(self, n_layers: int, n_experts: int, n_slots: int, expert_bytes: int, horizon: int = 0):
-        assert n_slots >= 1
+    def __init__(self, n_layers: int, n_experts: int, n_slots: int, expert_bytes: int, horizon: int = 0,
+                 policy: str = "plec"):
+        assert n_slots >= 1 and policy in ("plec", "lru", "layer_lru")
+        assert policy != "layer_lru" or n_slots >= n_layers
+        self.policy = policy
         self.L, self.E, self.S, self.W, self.H = n_layers, n_experts, n_slots, expert_bytes, horizon
         self.slot_expert = [-1] * n_slots     # g or -1
         self.slot_pred_for = [-1] * n_slots   # visit the expert was prefetched for; -1 = loaded on demand
@@ -68,6 +78,8 @@ class CacheSim:
     def _victim(self, v_now: int, target: int, allow3: bool, locked: set):
         """Smallest key wins.  class 0 empty; 1 mis-prefetched (P:L130 'first'); 2 completed with next
         use later than the target (P:L130 'then'); 3 (on-demand last resort) anything else."""
+        if self.policy != "plec":
+            return self._victim_lru(target % self.L, locked)
         best_key, best_slot = None, None
         for s in range(self.S):
             g = self.slot_expert[s]
@@ -88,6 +100,24 @@ class CacheSim:
             if best_key is None or key < best_key:
                 best_key, best_slot = key, s
         return best_slot
+
+    def _victim_lru(self, layer: int, locked: set):
+        """Baselines: the first empty slot, else the least recently used unlocked slot -- of the whole pool ("lru") or
+        of the layer's own share of S // L slots ("layer_lru")."""
+        lo, hi = 0, self.S
+        if self.policy == "layer_lru":
+            share = self.S // self.L
+            lo, hi = layer * share, (layer + 1) * share
+        best = None
+        for s in range(lo, hi):
+            g = self.slot_expert[s]
+            if g < 0:
+                return s
+            if g in locked:
+                continue
+            if best is None or self.slot_stamp[s] < self.slot_stamp[best]:
+                best = s
+        return best
 
     def _load(self, s: int, g: int, pred_for: int, v_now: int, kind: str):
         old = self.slot_expert[s]
@@ -153,6 +183,8 @@ class CacheSim:
     def prefetch(self, v_now: int, predicted) -> int:
         """PLEC refill after visit v_now.  predicted[i] (iterable of 0/1 of length E) is the batch-level
         predicted path of visit v_now+1+i.  Returns the number of loads issued."""
+        if self.policy != "plec":
+            return 0                            # the LRU baselines neither predict nor prefetch
         n_ahead = len(predicted)
         for i in range(n_ahead):
             self.pred[v_now + 1 + i] = frozenset(e for e in range(self.E) if predicted[i][e])

@@ -19,7 +19,7 @@ DECLARED_SYMBOLS = [
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
     "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
     "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof", "ef_token_schedule", "ef_path_hamming", "ef_set_token_sched_path", "ef_reindex_rows",
-    "ef_set_wave_bytes", "ef_set_chunk_min_bytes", "ef_debug_tma_fill_gbs",
+    "ef_set_wave_bytes", "ef_set_chunk_min_bytes", "ef_debug_tma_fill_gbs", "ef_set_cache_policy",
 ]
 
 
@@ -95,6 +95,7 @@ def load_library() -> ctypes.CDLL:
             "ef_path_hamming": [vp, vp, vp, i32, i32, vp],
             "ef_set_token_sched_path": [vp, i32],
             "ef_debug_tma_fill_gbs": [vp, i64, i32, ctypes.POINTER(ctypes.c_double)],
+            "ef_set_cache_policy": [vp, i32],
             "ef_set_wave_bytes": [vp, i64],
             "ef_set_chunk_min_bytes": [vp, i64],
         }
@@ -283,6 +284,11 @@ class EfContext:
 
     def ef_set_splitk(self, mode: int):
         self._chk(self.lib.ef_set_splitk(self.h, int(mode)))
+
+    POLICIES = {"plec": 0, "lru": 1, "layer_lru": 2}
+
+    def ef_set_cache_policy(self, policy):
+        self._chk(self.lib.ef_set_cache_policy(self.h, self.POLICIES.get(policy, policy)))
 
     def ef_set_wave_bytes(self, nbytes: int):
         self._chk(self.lib.ef_set_wave_bytes(self.h, int(nbytes)))

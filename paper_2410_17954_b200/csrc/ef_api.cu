@@ -297,7 +297,28 @@ int64_t est_next_use(ef_ctx* ctx, int32_t g, int64_t v) {
 }
 
 // class 0 empty; 1 mis-prefetched; 2 completed & next use later than target; 3 (on demand only) the rest
+// Baseline policies (ef_set_cache_policy): least-recently-used over the whole pool, or over the
+// requesting layer's own share of it (slots [layer * S / L, (layer + 1) * S / L)).  Empty slots first, then the smallest
+// stamp; locked slots (this visit's experts) are skipped.  No predictions are consulted.
+int pick_victim_lru(ef_ctx* ctx, int layer, const std::vector<char>& locked) {
+    int s0 = 0, s1 = ctx->cfg.n_slots;
+    if (ctx->policy == EF_POLICY_LAYER_LRU) {
+        const int share = ctx->cfg.n_slots / ctx->cfg.n_layers;
+        s0 = layer * share;
+        s1 = s0 + share;
+    }
+    int best = -1;
+    for (int s = s0; s < s1; ++s) {
+        const EfSlot& sl = ctx->slots[s];
+        if (sl.expert < 0) return s;
+        if (locked[s]) continue;
+        if (best < 0 || sl.stamp < ctx->slots[best].stamp) best = s;
+    }
+    return best;
+}
+
 int pick_victim(ef_ctx* ctx, int64_t v_now, int64_t target, bool allow3, const std::vector<char>& locked) {
+    if (ctx->policy != EF_POLICY_PLEC) return pick_victim_lru(ctx, (int)(target % ctx->cfg.n_layers), locked);
     typedef std::tuple<int, int64_t, uint64_t, int> Key;
     bool have = false;
     Key best;
@@ -630,6 +651,7 @@ extern "C" int32_t ef_cache_prefetch(ef_ctx* ctx, int64_t visit_now, const uint8
     if (n_ahead < 0 || (n_ahead > 0 && !predicted) || visit_now < -1)
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_cache_prefetch: bad argument");
     const int E = c.n_experts, L = c.n_layers;
+    if (ctx->policy != EF_POLICY_PLEC) return EF_OK;      // the LRU baselines neither predict nor prefetch
     for (int i = 0; i < n_ahead; ++i)
         ctx->pred[visit_now + 1 + i] = std::vector<uint8_t>(predicted + (size_t)i * E, predicted + (size_t)(i + 1) * E);
     while (!ctx->pred.empty() && ctx->pred.begin()->first <= visit_now) ctx->pred.erase(ctx->pred.begin());
@@ -769,6 +791,18 @@ extern "C" int64_t ef_launch_count(ef_ctx* ctx) { return ctx ? ctx->launches : 0
 extern "C" int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on) {
     EF_CHECK_CTX(ctx);
     ctx->debug_simt = on ? 1 : 0;
+    return EF_OK;
+}
+
+extern "C" int32_t ef_set_cache_policy(ef_ctx* ctx, int32_t policy) {
+    EF_CHECK_CTX(ctx);
+    if (policy != EF_POLICY_PLEC && policy != EF_POLICY_LRU && policy != EF_POLICY_LAYER_LRU)
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_cache_policy: unknown policy %d", policy);
+    if (policy == EF_POLICY_LAYER_LRU && ctx->cfg.n_slots < ctx->cfg.n_layers)
+        return ef_fail(ctx, EF_ERR_CAPACITY, "ef_set_cache_policy: per-layer LRU needs at least one slot per layer");
+    for (const EfSlot& sl : ctx->slots)
+        if (sl.expert >= 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_cache_policy: the slot table must be empty (ef_cache_clear)");
+    ctx->policy = policy;
     return EF_OK;
 }
 

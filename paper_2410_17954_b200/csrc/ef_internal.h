@@ -97,6 +97,7 @@ struct ef_ctx {
     std::vector<int32_t> slot_of;       // [L*E] -> slot or -1
     std::map<int64_t, std::vector<uint8_t>> pred;   // visit -> predicted active flags [E]
     uint64_t tick = 0;
+    int32_t policy = EF_POLICY_PLEC;    // ef_set_cache_policy
     ef_cache_stats stats{};
     // tensor map over the whole arena as rowlets (2-D: 64 elements x total rowlets); both GEMMs use it
     CUtensorMap tm_w{};

@@ -182,11 +182,12 @@ def test_switch_prefill_relu_top1(T):
 # ------------------------------------------------------------------------------------------------
 # decode traces: cache accounting bit-exact over many visits; outputs checked on sampled visits
 # ------------------------------------------------------------------------------------------------
-def run_decode(cfg, n_steps, horizon, check_out_every):
+def run_decode(cfg, n_steps, horizon, check_out_every, policy="plec"):
     L, E = cfg.n_layers, cfg.n_experts
     r, ex = build_runner(cfg, horizon=horizon)
+    r.ctx.ef_set_cache_policy(policy)
     tr = wl.routing_trace(cfg, n_steps)
-    sim = CacheSim(L, E, cfg.n_slots, cfg.expert_bytes, horizon)
+    sim = CacheSim(L, E, cfg.n_slots, cfg.expert_bytes, horizon, policy=policy)
     nv = n_steps * L
     look = L if horizon <= 0 else horizon
 
@@ -245,6 +246,30 @@ def test_cfg5_reduced_stack_trace(horizon):
     cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=256, d_ff=512, T=32, n_layers=6, n_slots=12)
     st, sim = run_decode(cfg, n_steps=10, horizon=horizon, check_out_every=5)
     assert st["prefetch_issued"] > 0 and st["misses"] < st["lookups"]
+
+
+@pytest.mark.parametrize("policy", ["lru", "layer_lru"])
+def test_baseline_policies_match_simulator(policy):
+    """the LRU baselines in the library against the simulator, slot table and counters bit-exact at
+    every visit, outputs on sampled visits; predictions are supplied and ignored."""
+    cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=256, d_ff=512, T=32, n_layers=6, n_slots=12)
+    st, sim = run_decode(cfg, n_steps=8, horizon=1, check_out_every=5, policy=policy)
+    assert st["prefetch_issued"] == 0 and st["misses"] == st["ondemand_loads"] > 0
+    assert st["bytes_h2d"] == cfg.expert_bytes * st["ondemand_loads"]
+
+
+def test_cache_policy_can_only_change_on_an_empty_table():
+    from paper_2410_17954_b200 import EfError
+    cfg = wl.scaled(wl.CONFIGS["tiny"], n_slots=6)
+    r, _ = build_runner(cfg)
+    r.ctx.ef_cache_prefetch(-1, np.ones((1, cfg.n_experts), np.uint8))
+    with pytest.raises(EfError):
+        r.ctx.ef_set_cache_policy("lru")
+    r.ctx.ef_cache_clear()
+    r.ctx.ef_set_cache_policy("lru")
+    with pytest.raises(EfError):
+        r.ctx.ef_set_cache_policy(7)
+    r.close()
 
 
 def test_evict_and_clear_match_simulator():

@@ -240,3 +240,79 @@ def test_stale_prefetch_is_retargeted_not_reloaded():
     assert sim.stats["bytes_h2d"] == b
     plan = sim.visit(1, row(4, [0, 1]))
     assert plan.misses == [] and sim.stats["prefetch_used"] == 2
+
+
+# ------------------------------------------------------------------------------------------------
+# baseline policies: LRU over the pool, LRU inside a per-layer share
+# ------------------------------------------------------------------------------------------------
+def one_hot_counts(E, e):
+    c = [0] * E
+    c[e] = 1
+    return c
+
+
+def test_lru_matches_the_textbook_reference_string():
+    """The classic page-replacement reference string (20 references, 3 frames): LRU takes 12 faults -- one access
+    per visit, so the batch semantics (hits before misses) play no part."""
+    ref = [7, 0, 1, 2, 0, 3, 0, 4, 2, 3, 0, 3, 2, 1, 2, 0, 1, 7, 0, 1]
+    sim = CacheSim(1, 8, 3, W, policy="lru")
+    for v, e in enumerate(ref):
+        sim.visit(v, one_hot_counts(8, e))
+    assert sim.stats["misses"] == 12 and sim.stats["hits"] == 8
+    assert sim.stats["ondemand_loads"] == 12 and sim.stats["evictions"] == 9       # 3 cold loads evict nothing
+    assert sim.stats["bytes_h2d"] == 12 * W and sim.stats["prefetch_issued"] == 0
+    assert sorted(sim.snapshot()) == [0, 1, 7]
+
+
+@pytest.mark.parametrize("policy,L", [("lru", 1), ("lru", 3), ("layer_lru", 3)])
+def test_lru_against_an_independent_ordered_dict(policy, L):
+    from collections import OrderedDict
+    E, S, n = 12, 6, 400
+    g = np.random.default_rng(3)
+    seq = g.integers(0, E, size=n)
+    sim = CacheSim(L, E, S, W, policy=policy)
+    sim.prefetch(-1, ones(4, E))                                   # ignored by the baselines
+    caches = [OrderedDict() for _ in range(L if policy == "layer_lru" else 1)]
+    cap = S // L if policy == "layer_lru" else S
+    misses = 0
+    for v, e in enumerate(seq):
+        layer = v % L
+        sim.visit(v, one_hot_counts(E, int(e)))
+        c = caches[layer if policy == "layer_lru" else 0]
+        key = layer * E + int(e)
+        if key in c:
+            c.move_to_end(key)
+        else:
+            misses += 1
+            if len(c) >= cap:
+                c.popitem(last=False)
+            c[key] = True
+    assert sim.stats["misses"] == misses and sim.stats["prefetch_issued"] == 0
+    assert sorted(x for x in sim.snapshot() if x >= 0) == sorted(k for c in caches for k in c)
+    if policy == "layer_lru":                                      # every layer stays inside its own share
+        snap = sim.snapshot()
+        for s, gid in enumerate(snap):
+            assert gid < 0 or gid // E == s // (S // L)
+
+
+def test_lru_batch_visit_never_evicts_its_own_experts_while_others_remain():
+    sim = CacheSim(1, 8, 4, W, policy="lru")
+    sim.visit(0, row(8, [0, 1, 2, 3]))
+    plan = sim.visit(1, row(8, [2, 3, 4, 5]))                      # hits 2, 3 are locked: 4, 5 replace 0, 1
+    assert plan.hits == [2, 3] and plan.misses == [4, 5]
+    assert sorted(sim.snapshot()) == [2, 3, 4, 5]
+    plan = sim.visit(2, row(8, [0, 1, 2, 3, 4, 5]))                # more active experts than slots: phase B reuses
+    assert sim.stats["lookups"] == sim.stats["hits"] + sim.stats["misses"] == 4 + 4 + 6
+    assert len(set(x for x in sim.snapshot())) == 4
+
+
+def test_plec_beats_both_lru_baselines_on_the_stack_trace():
+    """The paper's claim in kind (Fig. 9): with a predicted path, PLEC's hit ratio is far above on-demand LRU's."""
+    cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=64, d_ff=128, T=16, n_layers=8, n_slots=16)
+    plec = run_trace(cfg, H=1, n_steps=10)
+    tr = wl.routing_trace(cfg, 10)
+    for policy in ("lru", "layer_lru"):
+        sim = CacheSim(cfg.n_layers, cfg.n_experts, cfg.n_slots, W, policy=policy)
+        for v in range(10 * cfg.n_layers):
+            sim.visit(v, np.bincount(tr.sets[v].ravel(), minlength=cfg.n_experts))
+        assert plec.hit_ratio() > sim.hit_ratio() + 0.2, policy
