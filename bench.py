@@ -37,11 +37,11 @@ UNIT = "tokens/s"
 # roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel (GEMM1) per launch, from the
 # committed `ncu --set full` captures (never measured by this script, which never runs under a profiler):
 #   mixtral_prefill: profiles/r1f_ffn_prefill_ncu_full.md -- the 6 GEMM1 launches of one steady-state streaming step
-#                    (2.5196 GB in all); resident leg: the one launch over all 8 experts (2.5485 GB)
+#                    (2.0711 GB in all); resident leg: the one launch over all 8 experts (2.0716 GB)
 #   mixtral_decode : profiles/r1f_ffn_decode_ncu_full.md  -- 4 GEMM1 launches of a streaming step (three single-expert
-#                    waves and one 5-expert wave, 1.8973 GB in all); resident leg: one launch over 7 experts (1.6498 GB)
-NCU_TRAFFIC_BYTES = {"mixtral_prefill": 2.5196e9 / 6, "mixtral_decode": 1.8973e9 / 4}
-NCU_TRAFFIC_BYTES_RESIDENT = {"mixtral_prefill": 2.5485e9, "mixtral_decode": 1.6498e9}
+#                    waves and one 5-expert wave, 1.8975 GB in all); resident leg: one launch over 7 experts (1.6523 GB)
+NCU_TRAFFIC_BYTES = {"mixtral_prefill": 2.0711e9 / 6, "mixtral_decode": 1.8975e9 / 4}
+NCU_TRAFFIC_BYTES_RESIDENT = {"mixtral_prefill": 2.0716e9, "mixtral_decode": 1.6523e9}
 
 
 # ---------------------------------------------------------------------------------------------------
