@@ -488,7 +488,7 @@ def run_ours(args):
     ms_max = dist_max(ms, dev)
     value = plan["global_tokens"] * args.steps / (ms_max * 1e-3)
 
-    ms_e2e, _, _, _, _ = timed(True, args.steps, max(1, args.warmup // 2))
+    ms_e2e, _, _, st_e2e, _ = timed(True, args.steps, max(1, args.warmup // 2))
     ms_e2e_max = dist_max(ms_e2e, dev)
     e2e_value = plan["global_tokens"] * args.steps / (ms_e2e_max * 1e-3)
     io_h2d, io_d2h = drv.io_bytes()
@@ -540,10 +540,14 @@ def run_ours(args):
                 "config": workload_config(cfg, world, {"phys_host_experts": drv.phys or cfg.n_layers * cfg.n_experts,
                                                        "cache_policy": args.policy}),
                 "clocks": clocks,
-                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_h2d + int(h2d["bytes_per_step"]),
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_h2d + int(st_e2e["bytes_h2d"] / args.steps),
                         "d2h_bytes_per_step": io_d2h, "ms_per_step": ms_e2e_max / args.steps,
+                        "expert_loads_per_step": (st_e2e["ondemand_loads"] + st_e2e["prefetch_issued"]) / args.steps,
                         "note": "step inputs (x, per-token router bias) from pinned host memory and out back to pinned "
-                                "host memory every step; expert weights stream from the pinned host pool in both legs"},
+                                "host memory every step; expert weights stream from the pinned host pool in both legs. "
+                                "Trace workloads: this leg continues the routing trace after the device-resident leg, so "
+                                "its steps move a different number of experts over the link (expert_loads_per_step here "
+                                "against h2d.loads_per_step) and, the step being link-bound, take proportionally long"},
                 "gpu_launches": launches, "roofline": roofline, "roofline_resident": resident,
                 "h2d": h2d, "cache": cache, "cpu_baseline": cpu_baseline}
         print(json.dumps(line), flush=True)
