@@ -248,6 +248,50 @@ def test_cfg5_reduced_stack_trace(horizon):
     assert st["prefetch_issued"] > 0 and st["misses"] < st["lookups"]
 
 
+def test_long_trace_wraps_the_event_ring():
+    """More loads and waves than the library's ring of 2048 sync events holds (handles are recycled, a stale handle
+    degrades to 'wait for everything enqueued so far'): accounting bit-exact at every visit and outputs on sampled
+    visits stay right over ~1000 visits with chunked copies forced on."""
+    cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=256, d_ff=512, T=32, n_layers=6, n_slots=12)
+    L, E = cfg.n_layers, cfg.n_experts
+    n_steps = 170
+    r, ex = build_runner(cfg, horizon=0)
+    r.ctx.ef_set_chunk_min_bytes(1)                      # two copies + two ready events per load
+    r.ctx.ef_set_wave_bytes(0)                           # one wave (and one free event) per miss
+    tr = wl.routing_trace(cfg, n_steps)
+    sim = CacheSim(L, E, cfg.n_slots, cfg.expert_bytes, 0)
+    nv = n_steps * L
+    window = lambda v: tr.predicted[v + 1:min(nv, v + 1 + L)]
+    sim.prefetch(-1, window(-1)); r.ctx.ef_cache_prefetch(-1, window(-1))
+    wrs = [wl.router_weight(cfg, l) for l in range(L)]
+    for s in range(n_steps):
+        h = wl.activations(cfg, s)
+        hd = dev_bf16(h)
+        check = s % 40 == 39
+        for l in range(L):
+            v = s * L + l
+            bias = wl.trace_bias(cfg, tr, v)
+            win = window(v)
+            nxt = torch.empty_like(hd)
+            r.visit(v, hd, nxt, token_bias=torch.from_numpy(bias).cuda(), predicted_next=win if len(win) else None,
+                    residual=hd, pre_norm_eps=1e-5)
+            sim.visit(v, np.bincount(tr.sets[v].ravel(), minlength=E))
+            if len(win):
+                sim.prefetch(v, win)
+            if check:
+                u = oracle.round_bf16(oracle.rmsnorm(h, 1e-5))
+                ref = oracle.layer_forward(u, wrs[l], bias, [ex[(l, e)] for e in range(E)], cfg.top_k, res=h)
+                h = oracle.round_bf16(ref.out)
+            hd = nxt
+        assert_cache_equal(r, sim)
+        if check:
+            r.ctx.ef_sync()
+            check_float(bf(to_bits(hd)), bf(h))
+    st = r.ctx.ef_cache_get_stats()
+    assert 2 * (st["ondemand_loads"] + st["prefetch_issued"]) > 2 * 2048      # the ring went round at least twice
+    r.close()
+
+
 @pytest.mark.parametrize("policy", ["lru", "layer_lru"])
 def test_baseline_policies_match_simulator(policy):
     """the LRU baselines in the library against the simulator, slot table and counters bit-exact at
