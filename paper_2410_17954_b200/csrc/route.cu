@@ -47,6 +47,9 @@ __device__ __forceinline__ void mma_bf16(float (&c)[4], uint32_t a0, uint32_t a1
                  : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 
+// kUnroll: k chunks whose x fragments are in flight per warp before the MMAs consume them (the kernel is bound by load
+// latency: more independent 128-bit loads per thread, as far as the registers of the 8-expert-tile loop allow)
+template <int kUnroll>
 __global__ void __launch_bounds__(kWarps * 32)
 route_topk_kernel(const uint4* __restrict__ x, const uint4* __restrict__ wr, const float* __restrict__ bias,
                   int64_t bias_stride, int T, int d8, int E, int k, int renorm, int32_t* __restrict__ idx,
@@ -68,17 +71,29 @@ route_topk_kernel(const uint4* __restrict__ x, const uint4* __restrict__ wr, con
 #pragma unroll
         for (int n = 0; n < kEChunk / 8; ++n) { acc[n][0] = acc[n][1] = acc[n][2] = acc[n][3] = 0.f; }
         const int n_tiles = min(kEChunk / 8, (E - e0 + 7) >> 3);
-#pragma unroll 2
-        for (int c = warp; c < n_chunks; c += kWarps) {
-            const uint4 a_lo = r0_ok ? xa[c * 4] : zero4;
-            const uint4 a_hi = r1_ok ? xb[c * 4] : zero4;
+        for (int c0 = warp; c0 < n_chunks; c0 += kWarps * kUnroll) {
+            uint4 a_lo[kUnroll], a_hi[kUnroll];
+#pragma unroll
+            for (int u = 0; u < kUnroll; ++u) {
+                const int c = c0 + u * kWarps;
+                a_lo[u] = (r0_ok && c < n_chunks) ? xa[c * 4] : zero4;
+                a_hi[u] = (r1_ok && c < n_chunks) ? xb[c * 4] : zero4;
+            }
 #pragma unroll
             for (int n = 0; n < kEChunk / 8; ++n) {
                 if (n < n_tiles) {
                     const int e = e0 + n * 8 + g;
-                    const uint4 b = (e < E) ? __ldg(wr + (int64_t)e * d8 + c * 4 + tq) : zero4;
-                    mma_bf16(acc[n], a_lo.x, a_hi.x, a_lo.y, a_hi.y, b.x, b.y);
-                    mma_bf16(acc[n], a_lo.z, a_hi.z, a_lo.w, a_hi.w, b.z, b.w);
+                    uint4 b[kUnroll];
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) {
+                        const int c = c0 + u * kWarps;
+                        b[u] = (e < E && c < n_chunks) ? __ldg(wr + (int64_t)e * d8 + c * 4 + tq) : zero4;
+                    }
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) {
+                        mma_bf16(acc[n], a_lo[u].x, a_hi[u].x, a_lo[u].y, a_hi[u].y, b[u].x, b[u].y);
+                        mma_bf16(acc[n], a_lo[u].z, a_hi[u].z, a_lo[u].w, a_hi[u].w, b[u].z, b[u].w);
+                    }
                 }
             }
         }
@@ -162,11 +177,16 @@ int32_t efk_route_topk(ef_ctx* ctx, cudaStream_t st, const void* x, const void* 
     dim3 grid((T + kTok - 1) / kTok), block(kWarps * 32);
     const size_t smem = ((size_t)kWarps * kTok * kPartLd + (size_t)kTok * E) * sizeof(float);
     if (smem > 48 * 1024 && !ctx->route_smem_set) {
-        EF_CUDA(ctx, cudaFuncSetAttribute(route_topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+        EF_CUDA(ctx, cudaFuncSetAttribute(route_topk_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+        EF_CUDA(ctx, cudaFuncSetAttribute(route_topk_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
         ctx->route_smem_set = true;
     }
-    route_topk_kernel<<<grid, block, smem, st>>>((const uint4*)x, (const uint4*)wr, bias, bias_stride, T, d / 8, E, k,
-                                                 renorm, idx, w, logits);
+    if (E <= 16)
+        route_topk_kernel<8><<<grid, block, smem, st>>>((const uint4*)x, (const uint4*)wr, bias, bias_stride, T, d / 8, E, k,
+                                                        renorm, idx, w, logits);
+    else
+        route_topk_kernel<4><<<grid, block, smem, st>>>((const uint4*)x, (const uint4*)wr, bias, bias_stride, T, d / 8, E, k,
+                                                        renorm, idx, w, logits);
     ctx->launches++;
     EF_CUDA(ctx, cudaGetLastError());
     return EF_OK;
