@@ -2,7 +2,7 @@
 
 Integers only.  It steps the Expert Cache Engine's policy (§3.2; §4.1,
 P:L183-187) exactly as DESIGN.md §4 ("cache policy, readings R6-R13, R25") words it, one decision
-at a time.  The CUDA library's cache manager (csrc/cache.cpp) must reproduce its slot table and
+at a time.  The CUDA library's cache manager (csrc/ef_api.cu) must reproduce its slot table and
 counters bit for bit; the two share no code.
 
 What the paper fixes (and what pins this file, tests/test_oracle_cache.py):
@@ -14,7 +14,11 @@ What the paper fixes (and what pins this file, tests/test_oracle_cache.py):
     worked example P:L187 ([5,6,7,8] -> [2,3,4,5]: 3 loads, expert 5 retained).
   * Every expert is backed up on the host, so eviction needs no write-back -- P:L338.
 What the paper leaves open (tie-breaks, horizon, "completed" under asynchrony) is a DESIGN.md
-reading; fidelity of those readings to the authors' code is unpinned (no code exists).
+reading (R8-R13, R25).  Each reading is pinned to a hand-worked scenario whose expected slot table and
+counters are literals derived from DESIGN.md section 4's wording (tests/test_oracle_cache.py, "Hand-worked
+scenarios"), and a mutation test there demands that every one-line change of the decision logic below
+turns one of the pins red.  What stays unpinned is only whether the authors' unpublished code breaks
+these ties the same way (there is nothing to compare with).
 
 Baseline policies (the paper's comparison points as policy sketches, "Cache-MoE ... a fixed-size
 cache per layer, using a Least-Recently-Used strategy"): `policy="lru"` -- on-demand loading, the victim is an

@@ -27,11 +27,11 @@ def row(E, active):
 # ------------------------------------------------------------------------------------------------
 # PLEC worked example
 # ------------------------------------------------------------------------------------------------
-def test_plec_worked_example():
+def test_plec_worked_example(Sim=CacheSim):
     gld = json.load(open(os.path.join(GOLD, "plec_example.json")))
     L, E, S = gld["n_layers"], gld["n_experts"], gld["n_slots"]
     exp = gld["expected"]
-    sim = CacheSim(L, E, S, W, horizon=0)
+    sim = Sim(L, E, S, W, horizon=0)
     n = sim.prefetch(-1, ones(L, E))                     # predicted path of the whole pass: all active
     assert n == exp["warmup_prefetches"] == sim.stats["prefetch_issued"]
     assert sorted({g // E for g in sim.snapshot()}) == exp["warmup_resident_layers"]
@@ -55,10 +55,10 @@ def test_plec_worked_example():
     assert sim.stats["hits"] == sim.stats["lookups"] == L * E
 
 
-def test_plec_example_second_pass_also_missless():
+def test_plec_example_second_pass_also_missless(Sim=CacheSim):
     # steady state over several passes: every load is a prefetch, none on demand
     L, E, S = 4, 4, 8
-    sim = CacheSim(L, E, S, W)
+    sim = Sim(L, E, S, W)
     sim.prefetch(-1, ones(L, E))
     for v in range(5 * L):
         assert sim.visit(v, [1] * E).misses == []
@@ -70,13 +70,13 @@ def test_plec_example_second_pass_also_missless():
 # ------------------------------------------------------------------------------------------------
 # step transition example
 # ------------------------------------------------------------------------------------------------
-def test_step_transition_example():
+def test_step_transition_example(Sim=CacheSim):
     gld = json.load(open(os.path.join(GOLD, "step_transition_example.json")))
     E, S = gld["n_experts"], gld["n_slots"]
     prev = [e - 1 for e in gld["prev_step_active"]]      # ids in the paper are one-based
     nxt = [e - 1 for e in gld["next_step_active"]]
     exp = gld["expected"]
-    sim = CacheSim(1, E, S, W, horizon=1)
+    sim = Sim(1, E, S, W, horizon=1)
     sim.prefetch(-1, [row(E, prev)])
     plan = sim.visit(0, row(E, prev))
     assert plan.misses == [] and sorted(sim.snapshot()) == prev
@@ -93,10 +93,10 @@ def test_step_transition_example():
 # ------------------------------------------------------------------------------------------------
 # correction victim order
 # ------------------------------------------------------------------------------------------------
-def test_correction_prefers_misprefetched():
+def test_correction_prefers_misprefetched(Sim=CacheSim):
     json.load(open(os.path.join(GOLD, "correction_example.json")))   # citation + scenario description
     L, E, S = 2, 4, 4
-    sim = CacheSim(L, E, S, W)
+    sim = Sim(L, E, S, W)
     # layer 0 predicted {0,1}, actual {0,1}; layer 1 predicted {0,3} but actual {0,2}
     sim.prefetch(-1, [row(E, [0, 1]), row(E, [0, 3])])
     assert sorted(sim.snapshot()) == [0, 1, 4, 7]
@@ -111,9 +111,9 @@ def test_correction_prefers_misprefetched():
     assert sim.stats["prefetch_wasted"] == 1 and sim.stats["ondemand_loads"] == 1
 
 
-def test_correction_falls_back_to_completed():
+def test_correction_falls_back_to_completed(Sim=CacheSim):
     L, E, S = 2, 4, 3
-    sim = CacheSim(L, E, S, W)
+    sim = Sim(L, E, S, W)
     sim.prefetch(-1, [row(E, [0, 1]), row(E, [0])])       # all three slots: (0,0) (0,1) (1,0)
     sim.visit(0, row(E, [0, 1]))
     plan = sim.visit(1, row(E, [0, 2]))                   # (1,2) missed, no mis-prefetched expert anywhere
@@ -123,9 +123,9 @@ def test_correction_falls_back_to_completed():
     assert (1 * E + 0) in sim.slot_of and len([g for g in sim.snapshot() if g // E == 0]) == 1
 
 
-def test_phase_b_when_pool_is_all_hits():
+def test_phase_b_when_pool_is_all_hits(Sim=CacheSim):
     # S = 2, four active experts, two resident: the other two each wait for a completed slot (waves)
-    sim = CacheSim(1, 4, 2, W)
+    sim = Sim(1, 4, 2, W)
     sim.prefetch(-1, [row(4, [0, 1, 2, 3])])
     assert sorted(sim.snapshot()) == [0, 1]
     plan = sim.visit(0, [1, 1, 1, 1])
@@ -135,8 +135,8 @@ def test_phase_b_when_pool_is_all_hits():
     assert sim.stats["ondemand_loads"] == 2 and sim.stats["evictions"] == 2
 
 
-def test_single_slot_never_deadlocks():
-    sim = CacheSim(2, 3, 1, W)
+def test_single_slot_never_deadlocks(Sim=CacheSim):
+    sim = Sim(2, 3, 1, W)
     g = wl.stream(0, "s1")
     for v in range(40):
         counts = (g.random(3) < 0.6).astype(int)
@@ -149,10 +149,10 @@ def test_single_slot_never_deadlocks():
 # ------------------------------------------------------------------------------------------------
 # invariants on seeded traces shaped like the decode configs
 # ------------------------------------------------------------------------------------------------
-def run_trace(cfg, H, n_steps, S=None, perfect=False):
+def run_trace(cfg, H, n_steps, S=None, perfect=False, Sim=CacheSim):
     tr = wl.routing_trace(cfg, n_steps)
     L, E = cfg.n_layers, cfg.n_experts
-    sim = CacheSim(L, E, S or cfg.n_slots, W, horizon=H)
+    sim = Sim(L, E, S or cfg.n_slots, W, horizon=H)
     nv = n_steps * L
     pred = tr.actual if perfect else tr.predicted
     look = L if H <= 0 else H
@@ -180,22 +180,22 @@ def run_trace(cfg, H, n_steps, S=None, perfect=False):
 
 
 @pytest.mark.parametrize("H", [0, 1, 3])
-def test_invariants_decode_single_layer(H):
+def test_invariants_decode_single_layer(H, Sim=CacheSim):
     cfg = wl.scaled(wl.CONFIGS["mixtral_decode"], d_model=64, d_ff=128)
-    run_trace(cfg, H, n_steps=60)
+    run_trace(cfg, H, n_steps=60, Sim=Sim)
 
 
 @pytest.mark.parametrize("H", [0, 1])
-def test_invariants_stack(H):
+def test_invariants_stack(H, Sim=CacheSim):
     cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=64, d_ff=128, T=16, n_layers=6, n_slots=12)
-    run_trace(cfg, H, n_steps=12)
+    run_trace(cfg, H, n_steps=12, Sim=Sim)
 
 
-def test_all_resident_means_no_loads_after_warmup():
+def test_all_resident_means_no_loads_after_warmup(Sim=CacheSim):
     # S >= L*E: the paper's All-In-GPU case -- after warm-up nothing moves
     cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=64, d_ff=128, T=8, n_layers=3, n_slots=24)
     L, E = cfg.n_layers, cfg.n_experts
-    sim = CacheSim(L, E, L * E, W)
+    sim = Sim(L, E, L * E, W)
     sim.prefetch(-1, ones(L, E))
     assert sim.stats["prefetch_issued"] == L * E
     tr = wl.routing_trace(cfg, 10)
@@ -205,24 +205,24 @@ def test_all_resident_means_no_loads_after_warmup():
     assert sim.stats["misses"] == 0 and sim.stats["bytes_h2d"] == W * L * E and sim.stats["evictions"] == 0
 
 
-def test_perfect_prediction_two_visits_fit_means_no_misses():
+def test_perfect_prediction_two_visits_fit_means_no_misses(Sim=CacheSim):
     cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=64, d_ff=128, T=4, n_layers=4, n_slots=16)
-    sim = run_trace(cfg, H=0, n_steps=15, perfect=True)    # S = 16 >= two visits' active sets (<= 8 each)
+    sim = run_trace(cfg, H=0, n_steps=15, perfect=True, Sim=Sim)    # S = 16 >= two visits' active sets (<= 8 each)
     assert sim.stats["misses"] == 0 and sim.stats["prefetch_wasted"] == 0
 
 
-def test_prediction_beats_on_demand_only():
+def test_prediction_beats_on_demand_only(Sim=CacheSim):
     cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=64, d_ff=128, T=16, n_layers=8, n_slots=16)
-    with_pred = run_trace(cfg, H=0, n_steps=10)
+    with_pred = run_trace(cfg, H=0, n_steps=10, Sim=Sim)
     tr = wl.routing_trace(cfg, 10)
-    od = CacheSim(cfg.n_layers, cfg.n_experts, cfg.n_slots, W)
+    od = Sim(cfg.n_layers, cfg.n_experts, cfg.n_slots, W)
     for v in range(10 * cfg.n_layers):
         od.visit(v, np.bincount(tr.sets[v].ravel(), minlength=cfg.n_experts))
     assert with_pred.hit_ratio() > od.hit_ratio() + 0.2
 
 
-def test_evict_removes_and_counts():
-    sim = CacheSim(1, 4, 4, W)
+def test_evict_removes_and_counts(Sim=CacheSim):
+    sim = Sim(1, 4, 4, W)
     sim.prefetch(-1, [row(4, [0, 1, 2])])
     sim.visit(0, row(4, [0]))
     sim.evict(0, [0, 1, 3])            # 0 used, 1 never-used prefetch, 3 not resident
@@ -230,9 +230,9 @@ def test_evict_removes_and_counts():
     assert sim.stats["evictions"] == 2 and sim.stats["prefetch_wasted"] == 1
 
 
-def test_stale_prefetch_is_retargeted_not_reloaded():
+def test_stale_prefetch_is_retargeted_not_reloaded(Sim=CacheSim):
     # R25: a mis-prefetched expert predicted again keeps its slot and moves no bytes
-    sim = CacheSim(1, 4, 2, W, horizon=1)
+    sim = Sim(1, 4, 2, W, horizon=1)
     sim.prefetch(-1, [row(4, [0, 1])])
     sim.visit(0, row(4, [0]))                      # expert 1 was mis-prefetched
     b = sim.stats["bytes_h2d"]
@@ -240,6 +240,173 @@ def test_stale_prefetch_is_retargeted_not_reloaded():
     assert sim.stats["bytes_h2d"] == b
     plan = sim.visit(1, row(4, [0, 1]))
     assert plan.misses == [] and sim.stats["prefetch_used"] == 2
+
+
+# ------------------------------------------------------------------------------------------------
+# Hand-worked scenarios for the readings the paper leaves open (R8, R10, R11, R12, R25; section 4:
+# the strict "next use later than the target", hits locked during phase A).  Every expected slot table, wave list and
+# counter below is a LITERAL worked out by hand from DESIGN.md section 4's wording -- the steps are in the comments --
+# never a value the simulator produced.  Global expert id g = layer * E + e; tables are slot -> g.
+# tests/test_oracle_cache.py::test_every_mutation_of_the_simulator_fails_a_pin keeps them sharp.
+# ------------------------------------------------------------------------------------------------
+def test_r8_completed_victims_farthest_next_use_first(Sim=CacheSim):
+    """R8 first key.  3 layers x 1 expert, 2 slots, no predictions (a visit without a supplied prediction counts as
+    'assume used', so an expert's next use is its layer's next visit).
+    v0: (0,0) missed -> empty slot 0.  v1: (1,0) missed -> empty slot 1.  v2: (2,0) missed, both residents completed:
+    (0,0) is next used at v3, (1,0) at v4 -> the JUST-FINISHED layer 1 is the farthest and goes, although layer 0's
+    expert is the least recently used (layer 1's slots are reused for layer 3 as layer 1 completes)."""
+    sim = Sim(3, 1, 2, W)
+    sim.visit(0, [1]); sim.visit(1, [1])
+    assert sim.snapshot() == [0, 1]
+    plan = sim.visit(2, [1])
+    assert plan.misses == [0] and plan.waves == [(0, 1, True)]
+    assert sim.snapshot() == [0, 2]
+    plan = sim.visit(3, [1])                       # layer 0 again: still resident
+    assert plan.hits == [0] and sim.snapshot() == [0, 2]
+    assert sim.stats == dict(lookups=4, hits=1, misses=3, prefetch_issued=0, prefetch_used=0, prefetch_wasted=0,
+                             ondemand_loads=3, evictions=1, bytes_h2d=3 * W)
+
+
+def test_r8_equal_next_use_falls_back_to_least_recently_used(Sim=CacheSim):
+    """R8 second key.  One layer, so every completed expert has the same next use (the next visit) and the LRU stamp
+    decides; a HIT refreshes the stamp.  v0: 0 -> slot 0, 1 -> slot 1.  v1: 0 hits (now the most recent).  v2: 2 missed
+    -> the victim is expert 1 (older use), not expert 0 (older load)."""
+    sim = Sim(1, 4, 2, W)
+    sim.visit(0, row(4, [0, 1]))
+    sim.visit(1, row(4, [0]))
+    sim.visit(2, row(4, [2]))
+    assert sim.snapshot() == [0, 2]
+
+
+def test_r11_last_resort_takes_the_prefetch_needed_latest(Sim=CacheSim):
+    """R11 (class 3).  3 layers x 2 experts, 2 slots, horizon = fill.  Warm-up prefetch with predicted sets v0: {},
+    v1: {0}, v2: {0} loads (1,0) -> slot 0 for v1 and (2,0) -> slot 1 for v2.  At v0 the gate selects (0,0): a miss,
+    and the pool holds nothing but prefetches whose visits are still to come (not mis-prefetched, not completed), so
+    phase A finds no victim and phase B takes class 3: the one needed LATEST, (2,0) at v2, not (1,0) at v1 -- although
+    (1,0) is the older load."""
+    sim = Sim(3, 2, 2, W)
+    assert sim.prefetch(-1, [row(2, []), row(2, [0]), row(2, [0])]) == 2
+    assert sim.snapshot() == [2, 4]
+    plan = sim.visit(0, row(2, [0]))
+    assert plan.misses == [0] and plan.waves == [(0, 1, True)]
+    assert sim.snapshot() == [2, 0]
+    assert sim.stats["prefetch_wasted"] == 1 and sim.stats["evictions"] == 1 and sim.stats["ondemand_loads"] == 1
+    plan = sim.visit(1, row(2, [0]))               # the prefetch for v1 survived and is used
+    assert plan.hits == [0] and sim.stats["prefetch_used"] == 1
+
+
+def test_prefetch_never_evicts_an_expert_needed_at_the_target_visit(Sim=CacheSim):
+    """Class 2 wants a next use strictly LATER than the target.  One layer x 3 experts, 2 slots, H = 1.  v0: {0, 1}
+    loaded on demand.  Predicted for v1: {0, 1, 2}: 0 and 1 are resident; for 2 the only candidates are 0 and 1, whose
+    next use IS the target visit -> no victim, nothing moves ("the cache is full of useful experts")."""
+    sim = Sim(1, 3, 2, W, horizon=1)
+    sim.visit(0, row(3, [0, 1]))
+    assert sim.prefetch(0, [row(3, [0, 1, 2])]) == 0
+    assert sim.snapshot() == [0, 1]
+    assert sim.stats["bytes_h2d"] == 2 * W and sim.stats["evictions"] == 0 and sim.stats["prefetch_issued"] == 0
+
+
+def test_r12_misses_are_served_in_ascending_expert_order(Sim=CacheSim):
+    """R12.  (a) two misses, two empty slots: the lower expert id is served first and takes the lower slot.
+    (b) one layer x 4 experts, 2 slots holding {0, 1}; v1 selects {0, 2, 3}: 0 hits and is locked; phase A serves 2
+    first -> the completed expert 1's slot 1; 3 finds every slot locked and waits for phase B, where both residents
+    are completed with the same next use and expert 0 (used at tick 3) is older than expert 2 (loaded at tick 4)
+    -> slot 0.  Served in descending order the table would end as [2, 3]."""
+    sim = Sim(1, 4, 2, W)
+    plan = sim.visit(0, row(4, [2, 3]))
+    assert plan.misses == [2, 3] and plan.waves == [(2, 0, True), (3, 1, True)] and sim.snapshot() == [2, 3]
+    sim = Sim(1, 4, 2, W)
+    sim.visit(0, row(4, [0, 1]))
+    plan = sim.visit(1, row(4, [0, 2, 3]))
+    assert plan.hits == [0] and plan.misses == [2, 3]
+    assert plan.waves == [(0, 0, False), (2, 1, True), (3, 0, True)]
+    assert sim.snapshot() == [3, 2]
+
+
+def test_r12_prefetches_are_issued_in_ascending_expert_order(Sim=CacheSim):
+    sim = Sim(2, 4, 4, W)
+    assert sim.prefetch(-1, [row(4, [1, 3]), row(4, [0, 2])]) == 4
+    assert sim.snapshot() == [1, 3, 4, 6]          # visit order first, then expert id; lowest empty slot each time
+
+
+def test_r10_horizon_limits_how_far_ahead_prefetch_loads(Sim=CacheSim):
+    """R10.  H = 1 with two visits' predictions supplied: only the next visit's expert is loaded; the second row is
+    kept as knowledge (it still feeds the next-use estimate)."""
+    sim = Sim(2, 2, 4, W, horizon=1)
+    assert sim.prefetch(-1, [row(2, [0]), row(2, [1])]) == 1
+    assert sim.snapshot() == [0, -1, -1, -1]
+    sim = Sim(2, 2, 4, W, horizon=0)
+    assert sim.prefetch(-1, [row(2, [0]), row(2, [1])]) == 2
+    assert sim.snapshot() == [0, 3, -1, -1]
+
+
+def test_r25_retargeted_prefetch_is_no_longer_a_misprefetch_victim(Sim=CacheSim):
+    """R25.  2 layers x 4 experts, 2 slots, horizon = fill.  Warm-up: predicted v0 = {0, 1}, v1 = {} -> (0,0) -> slot 0,
+    (0,1) -> slot 1, both for v0.  v0 selects only (0,0): (0,1) is now a stale prefetch.  After v0 the predictor says
+    v1 = {}, v2 = {0, 1}: both are resident, nothing is loaded, and the stale (0,1) is RE-TARGETED to v2.
+    v1 selects (1,3), a miss: (0,1) is a prefetch whose visit (v2) is still to come -- not mis-prefetched -- so the victim
+    is the completed (0,0) (next use v2 > v1).  Without the re-target (0,1) would count as mis-prefetched (its visit v0 has
+    passed) and be the first victim, and prefetch_wasted would be 1."""
+    sim = Sim(2, 4, 2, W)
+    assert sim.prefetch(-1, [row(4, [0, 1]), row(4, [])]) == 2
+    assert sim.snapshot() == [0, 1]
+    sim.visit(0, row(4, [0]))
+    assert sim.prefetch(0, [row(4, []), row(4, [0, 1])]) == 0
+    plan = sim.visit(1, row(4, [3]))
+    assert plan.misses == [3] and plan.waves == [(3, 0, True)]
+    assert sim.snapshot() == [7, 1]
+    assert sim.stats["prefetch_wasted"] == 0 and sim.stats["evictions"] == 1
+    plan = sim.visit(2, row(4, [0, 1]))            # the re-targeted prefetch is used; (0,0) has to come back
+    assert plan.hits == [1] and plan.misses == [0]
+    assert sim.stats["prefetch_used"] == 2 and sim.stats["bytes_h2d"] == 4 * W
+
+
+def test_next_use_estimate_follows_the_supplied_predictions(Sim=CacheSim):
+    """est_next_use: inside the supplied predictions an expert's next use is the first visit of its layer that predicts
+    it.  2 layers x 2 experts, 2 slots.  v0: (0,0) -> slot 0; v1: (1,0) -> slot 1.  After v1 the predictor says v2 = {1},
+    v3 = {0}.  (0,1) is wanted for v2: (0,0) is NOT predicted at v2, so its next use is v4 (layer 0's following visit, no
+    prediction supplied: assume used); (1,0) is predicted at v3.  Both are later than the target v2; the farther one,
+    (0,0), goes.  Ignoring the predictions, (0,0) would be 'needed at v2' and (1,0) would be the victim."""
+    sim = Sim(2, 2, 2, W)
+    sim.visit(0, row(2, [0])); sim.visit(1, row(2, [0]))
+    assert sim.snapshot() == [0, 2]
+    assert sim.prefetch(1, [row(2, [1]), row(2, [0])]) == 1
+    assert sim.snapshot() == [1, 2]
+    plan = sim.visit(2, row(2, [1]))
+    assert plan.hits == [1] and plan.misses == []
+
+
+def test_misprefetched_victims_oldest_first(Sim=CacheSim):
+    """Class 1 order: among several mis-prefetched experts the one loaded first goes first.  One layer x 4 experts,
+    3 slots: {0, 1, 2} prefetched for v0 (slots 0, 1, 2); v0 selects {2, 3}: 2 hits, 3 takes expert 0's slot."""
+    sim = Sim(1, 4, 3, W)
+    sim.prefetch(-1, [row(4, [0, 1, 2])])
+    sim.visit(0, row(4, [2, 3]))
+    assert sim.snapshot() == [3, 1, 2]
+
+
+def test_phase_a_never_destroys_a_still_useful_prefetch(Sim=CacheSim):
+    """Phase A takes victims from classes 0-2 only.  2 layers x 3 experts, 2 slots: (0,0) prefetched for v0 (slot 0), (1,0)
+    for v1 (slot 1).  v0 selects {0, 1}: 0 hits; for 1 the only unlocked slot holds a prefetch whose visit is still to
+    come, so the load WAITS for phase B and then reuses the slot of this visit's completed hit (class 2 beats class 3);
+    the prefetch for v1 survives and nothing is wasted."""
+    sim = Sim(2, 3, 2, W)
+    assert sim.prefetch(-1, [row(3, [0]), row(3, [0])]) == 2
+    assert sim.snapshot() == [0, 3]
+    plan = sim.visit(0, row(3, [0, 1]))
+    assert plan.waves == [(0, 0, False), (1, 0, True)]
+    assert sim.snapshot() == [1, 3] and sim.stats["prefetch_wasted"] == 0
+    assert sim.visit(1, row(3, [0])).hits == [0]
+
+
+def test_hits_of_the_visit_are_never_phase_a_victims(Sim=CacheSim):
+    """One layer x 3 experts, 2 slots holding {0, 1}; v1 selects {0, 1, 2}: both residents are this visit's hits (locked),
+    so 2 waits for phase B and then takes the older hit's slot -- after that hit's wave was enqueued (R9)."""
+    sim = Sim(1, 3, 2, W)
+    sim.visit(0, row(3, [0, 1]))
+    plan = sim.visit(1, row(3, [0, 1, 2]))
+    assert plan.waves == [(0, 0, False), (1, 1, False), (2, 0, True)]
+    assert sim.snapshot() == [2, 1]
 
 
 # ------------------------------------------------------------------------------------------------
@@ -251,11 +418,11 @@ def one_hot_counts(E, e):
     return c
 
 
-def test_lru_matches_the_textbook_reference_string():
+def test_lru_matches_the_textbook_reference_string(Sim=CacheSim):
     """The classic page-replacement reference string (20 references, 3 frames): LRU takes 12 faults -- one access
     per visit, so the batch semantics (hits before misses) play no part."""
     ref = [7, 0, 1, 2, 0, 3, 0, 4, 2, 3, 0, 3, 2, 1, 2, 0, 1, 7, 0, 1]
-    sim = CacheSim(1, 8, 3, W, policy="lru")
+    sim = Sim(1, 8, 3, W, policy="lru")
     for v, e in enumerate(ref):
         sim.visit(v, one_hot_counts(8, e))
     assert sim.stats["misses"] == 12 and sim.stats["hits"] == 8
@@ -265,12 +432,12 @@ def test_lru_matches_the_textbook_reference_string():
 
 
 @pytest.mark.parametrize("policy,L", [("lru", 1), ("lru", 3), ("layer_lru", 3)])
-def test_lru_against_an_independent_ordered_dict(policy, L):
+def test_lru_against_an_independent_ordered_dict(policy, L, Sim=CacheSim):
     from collections import OrderedDict
     E, S, n = 12, 6, 400
     g = np.random.default_rng(3)
     seq = g.integers(0, E, size=n)
-    sim = CacheSim(L, E, S, W, policy=policy)
+    sim = Sim(L, E, S, W, policy=policy)
     sim.prefetch(-1, ones(4, E))                                   # ignored by the baselines
     caches = [OrderedDict() for _ in range(L if policy == "layer_lru" else 1)]
     cap = S // L if policy == "layer_lru" else S
@@ -295,8 +462,8 @@ def test_lru_against_an_independent_ordered_dict(policy, L):
             assert gid < 0 or gid // E == s // (S // L)
 
 
-def test_lru_batch_visit_never_evicts_its_own_experts_while_others_remain():
-    sim = CacheSim(1, 8, 4, W, policy="lru")
+def test_lru_batch_visit_never_evicts_its_own_experts_while_others_remain(Sim=CacheSim):
+    sim = Sim(1, 8, 4, W, policy="lru")
     sim.visit(0, row(8, [0, 1, 2, 3]))
     plan = sim.visit(1, row(8, [2, 3, 4, 5]))                      # hits 2, 3 are locked: 4, 5 replace 0, 1
     assert plan.hits == [2, 3] and plan.misses == [4, 5]
@@ -306,13 +473,109 @@ def test_lru_batch_visit_never_evicts_its_own_experts_while_others_remain():
     assert len(set(x for x in sim.snapshot())) == 4
 
 
-def test_plec_beats_both_lru_baselines_on_the_stack_trace():
+def test_plec_beats_both_lru_baselines_on_the_stack_trace(Sim=CacheSim):
     """The paper's claim in kind (Fig. 9): with a predicted path, PLEC's hit ratio is far above on-demand LRU's."""
     cfg = wl.scaled(wl.CONFIGS["stack_decode"], d_model=64, d_ff=128, T=16, n_layers=8, n_slots=16)
-    plec = run_trace(cfg, H=1, n_steps=10)
+    plec = run_trace(cfg, H=1, n_steps=10, Sim=Sim)
     tr = wl.routing_trace(cfg, 10)
     for policy in ("lru", "layer_lru"):
-        sim = CacheSim(cfg.n_layers, cfg.n_experts, cfg.n_slots, W, policy=policy)
+        sim = Sim(cfg.n_layers, cfg.n_experts, cfg.n_slots, W, policy=policy)
         for v in range(10 * cfg.n_layers):
             sim.visit(v, np.bincount(tr.sets[v].ravel(), minlength=cfg.n_experts))
         assert plec.hit_ratio() > sim.hit_ratio() + 0.2, policy
+
+
+# ------------------------------------------------------------------------------------------------
+# The pins above are only worth something if a plausible mistake in the simulator turns one of them red.  This test
+# re-runs every scenario test of this file against one-line MUTANTS of oracle/cache_sim.py (source text edited in
+# memory, never written back) and demands that each mutant fails at least one of them (DESIGN.md section 2 has the table
+# mutant -> failing pin).  One mutant is EQUIVALENT and says so: not stopping a refill at the first expert without a
+# victim cannot change anything, because victims for a later target are a subset of those for an earlier one.
+# ------------------------------------------------------------------------------------------------
+MUTANTS = [
+    ("R8: nearest next use evicted first among completed", "key = (2, -nu, self.slot_stamp[s], s)", "key = (2, nu, self.slot_stamp[s], s)"),
+    ("R8: most recently used evicted first among completed", "key = (2, -nu, self.slot_stamp[s], s)", "key = (2, -nu, -self.slot_stamp[s], s)"),
+    ("R11: nearest next use evicted first in the last resort", "key = (3, -nu, self.slot_stamp[s], s)", "key = (3, nu, self.slot_stamp[s], s)"),
+    ("class 2 admits a next use AT the target", "nu > target", "nu >= target"),
+    ("R12: misses served in descending order", "for e in plan.misses:", "for e in reversed(plan.misses):"),
+    ("R12: prefetches issued in descending order", "for e in sorted(self.pred[t]):", "for e in sorted(self.pred[t], reverse=True):"),
+    ("prefetch walks the visits backwards", "for t in range(v_now + 1, hi + 1):", "for t in range(hi, v_now, -1):"),
+    ("R25: no re-target", "self.slot_pred_for[s] = t   # R25", "pass   # R25"),
+    ("P:L130: mis-prefetched demoted below completed", "key = (1, 0, self.slot_stamp[s], s)", "key = (2.5, 0, self.slot_stamp[s], s)"),
+    ("class 1: newest mis-prefetch first", "key = (1, 0, self.slot_stamp[s], s)", "key = (1, 0, -self.slot_stamp[s], s)"),
+    ("a prefetch is mis-prefetched only after its visit", "self.slot_pred_for[s] <= v_now:\n                key = (1,", "self.slot_pred_for[s] < v_now:\n                key = (1,"),
+    ("hits are not locked during phase A", "self.slot_stamp[s] = self.tick\n            locked.add(gid(e))", "self.slot_stamp[s] = self.tick"),
+    ("phase A may take a still-useful prefetch", "self._victim(v, v, allow3=False, locked=locked)", "self._victim(v, v, allow3=True, locked=locked)"),
+    ("next-use estimate ignores the predictions", "while v2 in self.pred and e not in self.pred[v2]:", "while False:"),
+    ("a hit does not refresh the LRU stamp", "self.tick += 1\n            self.slot_stamp[s] = self.tick\n            locked.add", "locked.add"),
+    ("R10: the horizon is ignored", "(min(self.H, n_ahead) if self.H > 0 else n_ahead)", "n_ahead"),
+    ("empty slots are not preferred", "key = (0, 0, 0, s)", "key = (9, 0, 0, s)"),
+    ("highest empty slot first", "key = (0, 0, 0, s)", "key = (0, 0, 0, -s)"),
+    ("a prefetched expert counts as used from the start", "self.slot_used[s] = False\n        self.tick += 1", "self.slot_used[s] = pred_for != -1\n        self.tick += 1"),
+]
+EQUIVALENT_MUTANTS = [
+    ("prefetch does not stop at the first expert without a victim", "return issued               # pool is full", "continue                    # pool is full"),
+]
+
+
+def _mutant(old, new):
+    import oracle.cache_sim as cs
+    src = open(cs.__file__).read()
+    assert src.count(old) == 1, f"mutation site not unique / not found: {old!r}"
+    import sys
+    import types
+    mod = types.ModuleType("oracle_cache_sim_mutant")
+    sys.modules[mod.__name__] = mod              # dataclasses looks the defining module up by name
+    try:
+        exec(compile(src.replace(old, new), cs.__file__ + "<mutant>", "exec"), mod.__dict__)
+    finally:
+        del sys.modules[mod.__name__]
+    return mod.CacheSim
+
+
+def _scenario_tests():
+    import inspect
+    out = []
+    for name, fn in sorted(globals().items()):
+        if name.startswith("test_") and callable(fn) and "Sim" in inspect.signature(fn).parameters:
+            others = [p for p in inspect.signature(fn).parameters.values() if p.name != "Sim" and p.default is p.empty]
+            if not others:
+                out.append((name, fn))
+    return out
+
+
+def _failing_pins(Sim):
+    failed = []
+    for name, fn in _scenario_tests():
+        try:
+            fn(Sim=Sim)
+        except Exception:            # an assertion, or the mutant running into a dead end
+            failed.append(name)
+    return failed
+
+
+def test_the_unmutated_simulator_passes_every_scenario():
+    assert len(_scenario_tests()) >= 25
+    assert _failing_pins(CacheSim) == []
+
+
+@pytest.mark.parametrize("what,old,new", MUTANTS, ids=[m[0] for m in MUTANTS])
+def test_every_mutation_of_the_simulator_fails_a_pin(what, old, new):
+    failed = _failing_pins(_mutant(old, new))
+    assert failed, f"mutant survives every pin: {what}"
+
+
+@pytest.mark.parametrize("what,old,new", EQUIVALENT_MUTANTS, ids=[m[0] for m in EQUIVALENT_MUTANTS])
+def test_equivalent_mutants_really_are_equivalent(what, old, new):
+    """Stop rule of the refill: after the first expert that finds no class 0-2 victim nothing later in
+    the same call can find one -- est_next_use does not depend on the target, a later target only shrinks class 2, no
+    stale prefetch is left to re-target (it would have been a class-1 victim) -- so 'stop' and 'skip' are the same
+    policy.  Checked on seeded traces, state and log compared after every call."""
+    Mut = _mutant(old, new)
+    assert _failing_pins(Mut) == []
+    for name, H, kw in (("mixtral_decode", 1, {}), ("mixtral_decode", 0, {}), ("stack_decode", 0, dict(T=16, n_layers=6, n_slots=12)),
+                        ("stack_decode", 2, dict(T=8, n_layers=5, n_slots=7))):
+        cfg = wl.scaled(wl.CONFIGS[name], d_model=64, d_ff=128, **kw)
+        a = run_trace(cfg, H, n_steps=40, Sim=CacheSim)
+        b = run_trace(cfg, H, n_steps=40, Sim=Mut)
+        assert a.log == b.log and a.stats == b.stats and a.snapshot() == b.snapshot()
