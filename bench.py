@@ -34,14 +34,29 @@ DUAL_FAMILIES, DUAL_FAMILY_PROB = 2, 0.9     # dual_batch_stack: latent token gr
 METRIC = "moe_layer_tokens_per_s"
 UNIT = "tokens/s"
 
-# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel (GEMM1) per launch, from the
-# committed `ncu --set full` captures (never measured by this script, which never runs under a profiler):
-#   mixtral_prefill: profiles/r1f_ffn_prefill_ncu_full.md -- the 6 GEMM1 launches of one steady-state streaming step
-#                    (2.0711 GB in all); resident leg: the one launch over all 8 experts (2.0716 GB)
-#   mixtral_decode : profiles/r1f_ffn_decode_ncu_full.md  -- 4 GEMM1 launches of a streaming step (three single-expert
-#                    waves and one 5-expert wave, 1.8975 GB in all); resident leg: one launch over 7 experts (1.6523 GB)
-NCU_TRAFFIC_BYTES = {"mixtral_prefill": 2.0711e9 / 6, "mixtral_decode": 1.8975e9 / 4}
-NCU_TRAFFIC_BYTES_RESIDENT = {"mixtral_prefill": 2.0716e9, "mixtral_decode": 1.6523e9}
+# roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, from the committed
+# `ncu --set full` captures (this script never runs under a profiler).  profiles/ncu_traffic.json records the numbers
+# together with the git blob hash of csrc/ffn_tc.cu they were taken at; when the kernel source has changed since, the
+# line says traffic: null, traffic_stale: true instead of quoting a number that no longer describes the code.
+def git_blob_hash(path: str) -> str:
+    import hashlib
+    data = open(path, "rb").read()
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
+def ncu_traffic(workload: str, leg: str):
+    """(bytes per launch or None, stale flag, source text) for leg in {"in_step", "resident"}."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(path):
+        return None, False, "no profiles/ncu_traffic.json"
+    rec = json.load(open(path))
+    ent = rec.get("workloads", {}).get(workload, {}).get(leg)
+    if ent is None:
+        return None, False, "no ncu capture of this workload / leg in profiles/ncu_traffic.json"
+    cur = git_blob_hash(os.path.join(ROOT, "paper_2410_17954_b200", "csrc", "ffn_tc.cu"))
+    if cur != rec.get("ffn_tc_blob"):
+        return None, True, f"capture taken at ffn_tc.cu blob {rec.get('ffn_tc_blob', '?')[:12]}, source is now {cur[:12]}"
+    return ent["bytes_per_launch"], False, ent.get("source", "profiles/ncu_traffic.json")
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -167,9 +182,12 @@ def workload_config(cfg, world, extra=None):
     c = {"workload": cfg.name, "tokens_per_step_per_gpu": cfg.T, "visits_per_step": cfg.n_layers,
          "d_model": cfg.d_model, "d_ff": cfg.d_ff, "n_layers": cfg.n_layers, "n_experts": cfg.n_experts,
          "top_k": cfg.top_k, "cache_slots": cfg.n_slots, "n_shared": cfg.n_shared, "expert_bytes": cfg.expert_bytes,
-         "prefetch_horizon": cfg.horizon, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-         "l2_policy": "inputs larger than L2: every step reads >= 0.69 GB of expert weights from HBM slots that the "
-                      "copy stream rewrites, against a 126 MB L2; no explicit flush"}
+         "prefetch_horizon": cfg.horizon, "parallelism": f"replicas x{world}" if world > 1 else "single GPU"}
+    # expert weights a step reads from HBM slots (every active expert once; the copy stream rewrites the slots it evicts)
+    act = min(cfg.n_experts, cfg.T * cfg.top_k) * cfg.n_layers
+    c["l2_policy"] = (f"inputs larger than L2: a step reads up to {act} experts x {cfg.expert_bytes / 1e6:.1f} MB = "
+                      f"{act * cfg.expert_bytes / 1e9:.2f} GB of weights out of HBM slots against a 126 MB L2; no explicit "
+                      "flush in the streaming step (the resident leg flushes when its weights would fit)")
     if extra:
         c.update(extra)
     return c
@@ -178,7 +196,7 @@ def workload_config(cfg, world, extra=None):
 # ---------------------------------------------------------------------------------------------------
 # the reference arm / cpu_baseline: the oracle as it stands, on host cores, bounded sample
 # ---------------------------------------------------------------------------------------------------
-def oracle_sample(cfg, n_tokens: int, n_layers: int, cache=None):
+def oracle_sample(cfg, n_tokens: int, n_layers: int, cache=None, real: str = "double"):
     """Time the oracle on a bounded sample of one step: the first n_tokens tokens through the first n_layers
     layers (whole layer each: route, permute, FFN, combine[, rmsnorm + residual]).  Returns tokens/s scaled to a
     whole step (time * L / n_layers), seconds spent, threads used, and a description."""
@@ -212,18 +230,18 @@ def oracle_sample(cfg, n_tokens: int, n_layers: int, cache=None):
     h = x
     for l in range(n_layers):
         if L > 1:
-            u = oracle.round_bf16(oracle.rmsnorm(h, 1e-5))
+            u = oracle.round_bf16(oracle.rmsnorm(h, 1e-5, real=real), real=real)
             ref = oracle.layer_forward(u, wrs[l], biases[l], lambda e, l=l: get(l, e), cfg.top_k, cfg.renorm,
-                                       shared=shared[l], res=h)
-            h = oracle.round_bf16(ref.out)
+                                       shared=shared[l], res=h, real=real)
+            h = oracle.round_bf16(ref.out, real=real)
         else:
             oracle.layer_forward(h, wrs[l], biases[l], lambda e, l=l: get(l, e), cfg.top_k, cfg.renorm,
-                                 shared=shared[l])
+                                 shared=shared[l], real=real)
     dt = time.perf_counter() - t0
     step_s = dt * L / n_layers
     what = (f"first {n_tokens} of {cfg.T} tokens through the first {n_layers} of {L} layer visit(s) of one step of "
-            f"{cfg.name}, whole layer in fp64 ({dt:.1f} s; scaled x{L / n_layers:g} to a step), weights pre-generated, "
-            "no host<->device traffic, no cache")
+            f"{cfg.name}, whole layer in {'fp64' if real == 'double' else 'fp32'} ({dt:.1f} s; scaled x{L / n_layers:g} to a "
+            "step), weights pre-generated, no host<->device traffic, no cache")
     return n_tokens / step_s, dt, oracle.num_threads(), what
 
 
@@ -275,7 +293,8 @@ def run_reference(args):
     n_tok, n_lay = ref_sample_size(cfg, args)
     cache = {}
     vals = []
-    sample = oracle_sample_dual if cfg.name == "dual_batch_stack" else oracle_sample
+    real = "float" if args.ref_precision == "fp32" and cfg.name != "dual_batch_stack" else "double"
+    sample = oracle_sample_dual if cfg.name == "dual_batch_stack" else (lambda c, t, l, ca: oracle_sample(c, t, l, ca, real=real))
     for i in range(args.warmup + args.steps):
         v, dt, cores, what = sample(cfg, n_tok, n_lay, cache)
         if i >= args.warmup:
@@ -284,8 +303,10 @@ def run_reference(args):
     ms = float(np.mean([dt for _, dt in vals])) * 1e3
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, world),
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+            "dtype": "f64" if real == "double" else "f32", "data": "synthetic",
+            "config": workload_config(cfg, world, {"phys_host_experts": cfg.n_layers * cfg.n_experts, "cache_policy": args.policy}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what,
+                             "precision": "fp64" if real == "double" else "fp32"},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -423,6 +444,134 @@ def measure_pinned_h2d(dev, nbytes: int, reps: int = 10) -> float:
     return best
 
 
+def cpu_baseline_block(cfg, args):
+    """The oracle as it stands on the host cores, bounded sample: fp64 (the oracle's default, what the parity tests use)
+    and the same C file built with -DORC_REAL=float (the fp32 oracle BASELINE.json's north_star describes)."""
+    n_tok, n_lay = ref_sample_size(cfg, args)
+    cache = {}
+    v, dt, cores, what = oracle_sample(cfg, n_tok, n_lay, cache)
+    v32, dt32, _, what32 = oracle_sample(cfg, n_tok, n_lay, cache, real="float")
+    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what, "precision": "fp64",
+            "fp32": {"value": v32, "unit": UNIT, "cores": cores, "kind": "oracle", "precision": "fp32", "sample": what32}}
+
+
+def measure_fill_peak(dev):
+    """L2 -> SM fill ceiling of this device, from the DIAGNOSTIC library's probe kernel (ef_diag.h): the
+    product library carries no probe.  None when libef_diag.so has not been built."""
+    from paper_2410_17954_b200 import EfContext, EfError
+    try:
+        ctx = EfContext(1, 8, 1, 256, 512, 1, 0, 16, 0, dev.index, 0, diag=True)
+    except (EfError, OSError):
+        return None
+    try:
+        return ctx.ef_diag_tma_fill_gbs(64 << 20, 2000)
+    finally:
+        ctx.close()
+
+
+def measure_workload(cfg, args, dev, plan, world, peaks, log, steps, warmup, want_e2e=True, want_resident=True, fill_peak=None,
+                     sample_clocks=True, local=0, rank=0):
+    """One workload through the whole path: device-resident leg (+ per-launch FFN roofline), optional end-to-end leg,
+    optional resident-FFN leg.  Returns a dict of the pieces of the JSON line."""
+    import torch
+    phys = args.phys_experts
+    need = cfg.n_layers * cfg.n_experts * cfg.expert_bytes
+    if phys == 0:
+        try:
+            avail = int(next(l for l in open("/proc/meminfo") if l.startswith("MemAvailable")).split()[1]) * 1024
+        except Exception:
+            avail = need * 4
+        if need * world > 0.6 * avail:
+            phys = max(cfg.n_experts, int(0.5 * avail / world / cfg.expert_bytes))
+            log(f"pinned pool of {need / 1e9:.1f} GB does not fit comfortably in {avail / 1e9:.1f} GB of host memory: "
+                f"aliasing {cfg.n_layers * cfg.n_experts} logical experts onto {phys} physical buffers")
+    steps_total = 2 * (steps + warmup) + 2
+    drv = Driver(cfg, dev, plan["x_stream"], steps_total, phys, log, args.policy)
+    runner = drv.runner
+    runner.ctx.ef_sync()                 # the warm-up prefetch must not share the link with the peak measurement
+    h2d_peak = measure_pinned_h2d(dev, cfg.expert_bytes) if rank == 0 else None
+
+    def timed(e2e, n_steps, n_warm, with_kernel_times=False):
+        for _ in range(n_warm):
+            drv.step(e2e)
+        drv.adopt_gate_prediction()
+        runner.ctx.ef_sync()
+        runner.ctx.ef_cache_reset_stats()               # also clears the copy-busy accumulator
+        if with_kernel_times:
+            runner.ctx.ef_get_kernel_times(reset=True)
+            runner.ctx.ef_get_launch_log(reset=True)
+            runner.ctx.ef_set_kernel_timing(True)
+        l0 = runner.ctx.ef_launch_count()
+        dist_barrier(); torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n_steps):
+            drv.step(e2e)
+        e1.record()
+        runner.ctx.ef_sync()
+        torch.cuda.synchronize(); dist_barrier()
+        ms = e0.elapsed_time(e1)
+        kt = lg = None
+        if with_kernel_times:
+            kt = runner.ctx.ef_get_kernel_times(reset=True)
+            lg = runner.ctx.ef_get_launch_log(reset=True)
+            runner.ctx.ef_set_kernel_timing(False)
+        st = runner.ctx.ef_cache_get_stats()
+        copy_ms = runner.ctx.ef_copy_busy_ms()
+        return ms, runner.ctx.ef_launch_count() - l0, kt, lg, st, copy_ms
+
+    sampler = ClockSampler(local) if sample_clocks else None
+    if sampler:
+        sampler.start()
+    ms, launches, kt, lg, st, copy_ms = timed(False, steps, warmup, with_kernel_times=True)
+    clocks = sampler.stop() if sampler else None
+    ms_max = dist_max(ms, dev)
+    value = plan["global_tokens"] * steps / (ms_max * 1e-3)
+    res = {"value": value, "ms_per_step": ms_max / steps, "clocks": clocks, "gpu_launches": launches}
+
+    if want_e2e:
+        ms_e2e, _, _, _, st_e2e, _ = timed(True, steps, max(1, warmup // 2))
+        ms_e2e_max = dist_max(ms_e2e, dev)
+        io_h2d, io_d2h = drv.io_bytes()
+        res["e2e"] = {"value": plan["global_tokens"] * steps / (ms_e2e_max * 1e-3), "unit": UNIT,
+                      "h2d_bytes_per_step": io_h2d + int(st_e2e["bytes_h2d"] / steps), "d2h_bytes_per_step": io_d2h,
+                      "ms_per_step": ms_e2e_max / steps,
+                      "expert_loads_per_step": (st_e2e["ondemand_loads"] + st_e2e["prefetch_issued"]) / steps,
+                      "note": "step inputs (x, per-token router bias) from pinned host memory and out back to pinned "
+                              "host memory every step; expert weights stream from the pinned host pool in both legs. "
+                              "Trace workloads: this leg continues the routing trace after the device-resident leg, so "
+                              "its steps move a different number of experts over the link (expert_loads_per_step here "
+                              "against h2d.loads_per_step) and, the step being link-bound, take proportionally long"}
+
+    d, f = cfg.d_model, cfg.d_ff
+    decode = cfg.name in ("mixtral_decode", "stack_decode", "dual_batch_stack")
+    power_capped = bool(clocks and "sw_power_cap" in (clocks.get("reasons") or []))
+    roofline = ffn_roofline(lg, kt, d, f, peaks, decode, "streaming step (a wave of hits + waves of misses, one launch per wave)",
+                            gated=cfg.expert_kind == "swiglu", fill_peak=fill_peak, power_capped=power_capped)
+    tr, stale, src = ncu_traffic(cfg.name, "in_step")
+    roofline.update({"traffic": tr, "traffic_stale": stale, "traffic_source": src})
+    res["roofline"] = roofline
+
+    res["h2d"] = {"bytes_per_step": st["bytes_h2d"] / steps, "loads_per_step": (st["ondemand_loads"] + st["prefetch_issued"]) / steps,
+                  "copy_busy_ms_per_step": copy_ms / steps,
+                  "achieved_gbs": (st["bytes_h2d"] / (copy_ms * 1e-3) / 1e9) if copy_ms > 0 else None,
+                  "peak_gbs": h2d_peak, "peak_source": "measured in this run on an idle device: pinned->device cudaMemcpyAsync, best of 10 over one "
+                                 "expert-sized and one 1 GiB buffer",
+                  "frac": (st["bytes_h2d"] / (copy_ms * 1e-3) / 1e9 / h2d_peak) if copy_ms > 0 and h2d_peak else None,
+                  "gbs_over_step": st["bytes_h2d"] / (ms * 1e-3) / 1e9,
+                  "step_ms_lower_bound_from_link": (st["bytes_h2d"] / steps / (h2d_peak * 1e9) * 1e3) if h2d_peak else None,
+                  "copy_overlap": "copies run on the library's copy stream concurrently with the grouped-FFN waves"}
+    res["cache"] = dict(st, hit_ratio=st["hits"] / max(1, st["lookups"]))
+    res["phys"] = drv.phys or cfg.n_layers * cfg.n_experts
+
+    counts = runner.counts.cpu().numpy()
+    res["aux_roofline"] = aux_rooflines(runner, cfg, peaks, dev) if rank == 0 else None
+    drv.close()
+    if want_resident and rank == 0:
+        res["roofline_resident"] = resident_leg(cfg, counts, peaks, dev, args, decode, fill_peak)
+    return res
+
+
 def run_ours(args):
     import torch
 
@@ -435,121 +584,40 @@ def run_ours(args):
     plan = replica_plan(rank, world, cfg.T)
     peaks = measured_peaks()
     log = (lambda m: print(f"[bench] {m}", file=sys.stderr, flush=True)) if rank == 0 else (lambda m: None)
+    fill_peak = measure_fill_peak(dev) if rank == 0 else None
 
-    # host memory check for the pinned pool (cfg 5: 90 GB); alias onto fewer physical buffers if it cannot fit
-    phys = args.phys_experts
-    need = cfg.n_layers * cfg.n_experts * cfg.expert_bytes
-    if phys == 0:
-        try:
-            avail = int(next(l for l in open("/proc/meminfo") if l.startswith("MemAvailable")).split()[1]) * 1024
-        except Exception:
-            avail = need * 4
-        if need * world > 0.6 * avail:
-            phys = max(cfg.n_experts, int(0.5 * avail / world / cfg.expert_bytes))
-            log(f"pinned pool of {need / 1e9:.1f} GB does not fit comfortably in {avail / 1e9:.1f} GB of host memory: "
-                f"aliasing {cfg.n_layers * cfg.n_experts} logical experts onto {phys} physical buffers")
-    steps_total = 2 * (args.steps + args.warmup) + 2
-    drv = Driver(cfg, dev, plan["x_stream"], steps_total, phys, log, args.policy)
-    runner = drv.runner
-    runner.ctx.ef_sync()                 # the warm-up prefetch must not share the link with the peak measurement
-    h2d_peak = measure_pinned_h2d(dev, cfg.expert_bytes) if rank == 0 else None
+    main = measure_workload(cfg, args, dev, plan, world, peaks, log, args.steps, args.warmup, want_e2e=True,
+                            want_resident=not args.no_resident, fill_peak=fill_peak, local=local, rank=rank)
 
-    def timed(e2e, steps, warmup, with_kernel_times=False):
-        for _ in range(warmup):
-            drv.step(e2e)
-        drv.adopt_gate_prediction()
-        runner.ctx.ef_sync()
-        runner.ctx.ef_cache_reset_stats()               # also clears the copy-busy accumulator
-        if with_kernel_times:
-            runner.ctx.ef_get_kernel_times(reset=True)
-            runner.ctx.ef_set_kernel_timing(True)
-        l0 = runner.ctx.ef_launch_count()
-        dist_barrier(); torch.cuda.synchronize()
-        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(steps):
-            drv.step(e2e)
-        e1.record()
-        runner.ctx.ef_sync()
-        torch.cuda.synchronize(); dist_barrier()
-        ms = e0.elapsed_time(e1)
-        kt = None
-        if with_kernel_times:
-            kt = runner.ctx.ef_get_kernel_times(reset=True)
-            runner.ctx.ef_set_kernel_timing(False)
-        st = runner.ctx.ef_cache_get_stats()
-        copy_ms = runner.ctx.ef_copy_busy_ms()
-        return ms, runner.ctx.ef_launch_count() - l0, kt, st, copy_ms
-
-    sampler = ClockSampler(local)
-    sampler.start()
-    ms, launches, kt, st, copy_ms = timed(False, args.steps, args.warmup, with_kernel_times=True)
-    clocks = sampler.stop()
-    ms_max = dist_max(ms, dev)
-    value = plan["global_tokens"] * args.steps / (ms_max * 1e-3)
-
-    ms_e2e, _, _, st_e2e, _ = timed(True, args.steps, max(1, args.warmup // 2))
-    ms_e2e_max = dist_max(ms_e2e, dev)
-    e2e_value = plan["global_tokens"] * args.steps / (ms_e2e_max * 1e-3)
-    io_h2d, io_d2h = drv.io_bytes()
-
-    d, f = cfg.d_model, cfg.d_ff
-    decode = cfg.T * cfg.top_k / cfg.n_experts < 249 and cfg.name in ("mixtral_decode", "stack_decode")
-    fill_peak = None
-    if rank == 0 and not decode:
-        runner.ctx.ef_sync()
-        fill_peak = runner.ctx.ef_debug_tma_fill_gbs(64 << 20, 2000)
-    roofline = ffn_roofline(kt, d, f, peaks, decode, "streaming step (one wave of hits + batched waves of misses)",
-                            gated=cfg.expert_kind == "swiglu", fill_peak=fill_peak)
-    roofline["traffic"] = NCU_TRAFFIC_BYTES.get(cfg.name)
-    roofline["traffic_source"] = ("bytes per GEMM1 launch from the committed ncu capture under profiles/ (see NCU_TRAFFIC_BYTES)"
-                                  if cfg.name in NCU_TRAFFIC_BYTES else "no ncu capture for this workload")
-    roofline["algorithmic_bytes_per_launch"] = ((4.0 if cfg.expert_kind == "swiglu" else 2.0) * d * f * kt["groups"]
-                                                + 2.0 * d * kt["rows"] + 2.0 * f * kt["rows"]) / max(1, kt["gemm1_launches"])
-
-    h2d = {"bytes_per_step": st["bytes_h2d"] / args.steps, "loads_per_step": (st["ondemand_loads"] + st["prefetch_issued"]) / args.steps,
-           "copy_busy_ms_per_step": copy_ms / args.steps,
-           "achieved_gbs": (st["bytes_h2d"] / (copy_ms * 1e-3) / 1e9) if copy_ms > 0 else None,
-           "peak_gbs": h2d_peak, "peak_source": "measured in this run on an idle device: pinned->device cudaMemcpyAsync, best of 10 over one "
-                          "expert-sized and one 1 GiB buffer",
-           "frac": (st["bytes_h2d"] / (copy_ms * 1e-3) / 1e9 / h2d_peak) if copy_ms > 0 and h2d_peak else None,
-           "gbs_over_step": st["bytes_h2d"] / (ms * 1e-3) / 1e9,
-           "step_ms_lower_bound_from_link": (st["bytes_h2d"] / args.steps / (h2d_peak * 1e9) * 1e3) if h2d_peak else None,
-           "copy_overlap": "copies run on the library's copy stream concurrently with the grouped-FFN waves"}
-    cache = dict(st)
-    cache["hit_ratio"] = st["hits"] / max(1, st["lookups"])
-
-    resident = None
-    if rank == 0 and not args.no_resident:
-        counts = runner.counts.cpu().numpy()
-        drv.close()
-        resident = resident_leg(cfg, counts, peaks, dev, args, decode, fill_peak)
-    else:
-        drv.close()
+    # The default line also vouches for the other two north_star targets (BASELINE.json): decode expert-weight reads
+    # against HBM (configs[2]) and the many-expert prefill GEMM against the tensor peak (configs[3]) -- short runs of
+    # the same path on those workloads, each with its in-step and resident FFN roofline.
+    extra = {}
+    if args.workload == "mixtral_prefill" and world == 1 and not args.no_extra:
+        for key, name, n_steps in (("decode", "mixtral_decode", 12), ("many_expert", "many_expert_prefill", 4)):
+            c2 = wl.CONFIGS[name]
+            p2 = replica_plan(rank, world, c2.T)
+            r2 = measure_workload(c2, args, dev, p2, world, peaks, log, n_steps, 3, want_e2e=False, want_resident=True,
+                                  fill_peak=fill_peak, local=local, rank=rank)
+            extra[key] = {"config": workload_config(c2, world, {"phys_host_experts": r2["phys"], "cache_policy": args.policy}),
+                          "steps": n_steps, "warmup": 3, "value": r2["value"], "unit": UNIT, "ms_per_step": r2["ms_per_step"],
+                          "clocks": r2["clocks"], "gpu_launches": r2["gpu_launches"], "roofline": r2["roofline"],
+                          "roofline_resident": r2.get("roofline_resident"), "h2d": r2["h2d"], "cache": r2["cache"],
+                          "aux_roofline": r2["aux_roofline"]}
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        n_tok, n_lay = ref_sample_size(cfg, args)
-        v, dt, cores, what = oracle_sample(cfg, n_tok, n_lay)
-        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}
+        cpu_baseline = cpu_baseline_block(cfg, args)
 
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                "config": workload_config(cfg, world, {"phys_host_experts": drv.phys or cfg.n_layers * cfg.n_experts,
-                                                       "cache_policy": args.policy}),
-                "clocks": clocks,
-                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_h2d + int(st_e2e["bytes_h2d"] / args.steps),
-                        "d2h_bytes_per_step": io_d2h, "ms_per_step": ms_e2e_max / args.steps,
-                        "expert_loads_per_step": (st_e2e["ondemand_loads"] + st_e2e["prefetch_issued"]) / args.steps,
-                        "note": "step inputs (x, per-token router bias) from pinned host memory and out back to pinned "
-                                "host memory every step; expert weights stream from the pinned host pool in both legs. "
-                                "Trace workloads: this leg continues the routing trace after the device-resident leg, so "
-                                "its steps move a different number of experts over the link (expert_loads_per_step here "
-                                "against h2d.loads_per_step) and, the step being link-bound, take proportionally long"},
-                "gpu_launches": launches, "roofline": roofline, "roofline_resident": resident,
-                "h2d": h2d, "cache": cache, "cpu_baseline": cpu_baseline}
+                "config": workload_config(cfg, world, {"phys_host_experts": main["phys"], "cache_policy": args.policy}),
+                "clocks": main["clocks"], "e2e": main["e2e"], "gpu_launches": main["gpu_launches"],
+                "roofline": main["roofline"], "roofline_resident": main.get("roofline_resident"),
+                "aux_roofline": main["aux_roofline"], "h2d": main["h2d"], "cache": main["cache"], "cpu_baseline": cpu_baseline}
+        line.update(extra)
         print(json.dumps(line), flush=True)
 
 
@@ -641,7 +709,8 @@ def run_dual_batch(args):
             step(sched, e2e)
         runner.ctx.ef_sync(); runner.ctx.ef_cache_reset_stats()
         if with_kernel_times:
-            runner.ctx.ef_get_kernel_times(reset=True); runner.ctx.ef_set_kernel_timing(True)
+            runner.ctx.ef_get_kernel_times(reset=True); runner.ctx.ef_get_launch_log(reset=True)
+            runner.ctx.ef_set_kernel_timing(True)
         l0 = runner.ctx.ef_launch_count()
         dist_barrier(); torch.cuda.synchronize()
         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
@@ -651,12 +720,13 @@ def run_dual_batch(args):
         e1.record()
         runner.ctx.ef_sync(); torch.cuda.synchronize(); dist_barrier()
         ms = dist_max(e0.elapsed_time(e1), dev)
-        kt = None
+        kt = lg = None
         if with_kernel_times:
-            kt = runner.ctx.ef_get_kernel_times(reset=True); runner.ctx.ef_set_kernel_timing(False)
+            kt = runner.ctx.ef_get_kernel_times(reset=True); lg = runner.ctx.ef_get_launch_log(reset=True)
+            runner.ctx.ef_set_kernel_timing(False)
         st = runner.ctx.ef_cache_get_stats()
         copy_ms = runner.ctx.ef_copy_busy_ms()
-        return {"ms": ms, "launches": runner.ctx.ef_launch_count() - l0, "kt": kt, "st": st, "copy_ms": copy_ms}
+        return {"ms": ms, "launches": runner.ctx.ef_launch_count() - l0, "kt": kt, "lg": lg, "st": st, "copy_ms": copy_ms}
 
     def arm_summary(res, steps):
         st = res["st"]
@@ -683,7 +753,7 @@ def run_dual_batch(args):
     e1.record(); e1.synchronize()
     sched_us = e0.elapsed_time(e1) / 20 * 1e3
     objs = np.array(objs)
-    roofline = ffn_roofline(on["kt"], d, f, peaks, True, "streaming steps with the Token Scheduler on")
+    roofline = ffn_roofline(on["lg"], on["kt"], d, f, peaks, True, "streaming steps with the Token Scheduler on")
     st = on["st"]
     h2d = {"bytes_per_step": st["bytes_h2d"] / args.steps, "copy_busy_ms_per_step": on["copy_ms"] / args.steps,
            "achieved_gbs": st["bytes_h2d"] / (on["copy_ms"] * 1e-3) / 1e9 if on["copy_ms"] > 0 else None, "peak_gbs": h2d_peak,
@@ -693,7 +763,7 @@ def run_dual_batch(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n_tok, n_lay = ref_sample_size(cfg, args)
         v, dt, cores, what = oracle_sample_dual(cfg, n_tok, n_lay)
-        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what, "precision": "fp64"}
     if rank == 0:
         a_on, a_off = arm_summary(on, args.steps), arm_summary(off, args.steps)
         io_h2d = N * d * 2 + N * L * E * 4 + N * L * E
@@ -720,51 +790,75 @@ def run_dual_batch(args):
         print(json.dumps(line), flush=True)
 
 
-def ffn_roofline(kt, d, f, peaks, decode, where, gated=True, fill_peak=None):
-    """Roofline of the dominant kernel (GEMM1 of the grouped FFN) from the library's per-launch CUDA events.
-    gated: SwiGLU experts (GEMM1 contracts against gate AND up: 4 d f FLOP per row); else ReLU experts (2 d f)."""
-    t1, t2 = kt["gemm1_ms"] * 1e-3, kt["gemm2_ms"] * 1e-3
-    n1, n2 = max(1, kt["gemm1_launches"]), max(1, kt["gemm2_launches"])
+def ffn_roofline(lg, kt, d, f, peaks, decode, where, gated=True, fill_peak=None, power_capped=False, burst_only=False):
+    """Roofline of the dominant kernel -- the grouped-FFN wave kernel (both GEMMs of a wave in one launch; a wave whose
+    expert is still arriving in two chunks runs them as two launches) -- from the library's per-launch CUDA events.
+    lg: the launch log (ef_get_launch_log), kt: the totals (ef_get_kernel_times).
+    Algorithmic work of a launch over `rows` routed rows in `groups` experts (gated = SwiGLU experts):
+      GEMM1  (4 | 2) d f FLOP per row, (4 | 2) d f weight bytes per expert, 2 d read + 2 f written per row
+      GEMM2        2 d f FLOP per row,       2 d f weight bytes per expert, 2 f read + 2 d written per row
+    `frac` holds the whole path against ONE roofline (tensor peak for prefill, HBM for decode); `frac_of_launch_bound`
+    holds every launch against ITS OWN bound max(FLOP / tensor peak, bytes / HBM bandwidth), which is the honest figure
+    for waves of a few small experts that no tensor pipe could keep busy (their weights have to come out of HBM once)."""
     g1 = 4.0 if gated else 2.0
+    burst, sust, hbm = peaks["bf16_tflops"], peaks.get("bf16_tflops_sustained") or peaks["bf16_tflops"], peaks["hbm_gbs"]
+    tot = {"t": 0.0, "flop": 0.0, "wbytes": 0.0, "bytes": 0.0, "bound_burst": 0.0, "bound_sust": 0.0}
+    kinds = {1: dict(t=0.0, n=0, flop=0.0, wbytes=0.0), 2: dict(t=0.0, n=0, flop=0.0, wbytes=0.0), 3: dict(t=0.0, n=0, flop=0.0, wbytes=0.0)}
+    for r in lg:
+        w1, w2 = (1 if r["which"] & 1 else 0), (1 if r["which"] & 2 else 0)
+        flop = (w1 * g1 + w2 * 2.0) * d * f * r["rows"]
+        wb = (w1 * g1 + w2 * 2.0) * d * f * r["groups"]
+        ab = (w1 + w2) * (2.0 * d + 2.0 * f) * r["rows"]
+        t = r["ms"] * 1e-3
+        tot["t"] += t; tot["flop"] += flop; tot["wbytes"] += wb; tot["bytes"] += wb + ab
+        tot["bound_burst"] += max(flop / (burst * 1e12), (wb + ab) / (hbm * 1e9))
+        tot["bound_sust"] += max(flop / (sust * 1e12), (wb + ab) / (hbm * 1e9))
+        k = kinds[r["which"]]
+        k["t"] += t; k["n"] += 1; k["flop"] += flop; k["wbytes"] += wb
+    T = max(tot["t"], 1e-12)
+    n = max(1, len(lg))
+
+    def kind_view(k):
+        if not k["n"]:
+            return None
+        v = {"launches": k["n"], "avg_launch_ms": k["t"] * 1e3 / k["n"], "tflops": k["flop"] / k["t"] / 1e12,
+             "weight_gbs": k["wbytes"] / k["t"] / 1e9}
+        v["frac"] = v["weight_gbs"] / hbm if decode else v["tflops"] / burst
+        return v
+    out = {"kernel": f"ffn_wave_kernel (tcgen05 grouped GEMM1 + GEMM2 of a wave, one launch), {where}",
+           "launches": len(lg), "avg_launch_ms": tot["t"] * 1e3 / n, "rows_per_launch": sum(r["rows"] for r in lg) / n,
+           "groups_per_launch": sum(r["groups"] for r in lg) / n,
+           "algorithmic_bytes_per_launch": tot["bytes"] / n, "algorithmic_flop_per_launch": tot["flop"] / n,
+           "frac_of_launch_bound": tot["bound_burst"] / T,
+           "frac_of_launch_bound_note": "sum over launches of max(FLOP / burst bf16 peak, algorithmic bytes / HBM copy bandwidth) "
+                                        "divided by the sum of their measured durations",
+           "by_launch_kind": {"wave (GEMM1+GEMM2, one launch)": kind_view(kinds[3]), "gemm1 only": kind_view(kinds[1]),
+                              "gemm2 only": kind_view(kinds[2])}}
     if decode:
-        b1, b2 = g1 * d * f * kt["groups"], 2.0 * d * f * kt["groups"]      # weight bytes read once per active expert
-        peak = peaks["hbm_gbs"]
-        a1 = b1 / t1 / 1e9 if t1 > 0 else 0.0
-        a2 = b2 / t2 / 1e9 if t2 > 0 else 0.0
-        return {"bound": "hbm", "kernel": f"ffn_gemm_kernel<swiglu> (GEMM1), {where}", "achieved": a1, "peak": peak,
-                "unit": "GB/s", "frac": a1 / peak, "peak_source": f"{peaks['source']} HBM copy bandwidth", "traffic": None,
-                "launches": kt["gemm1_launches"], "avg_launch_ms": t1 * 1e3 / n1, "groups_per_launch": kt["groups"] / n1,
-                "gemm2": {"achieved": a2, "frac": a2 / peak, "avg_launch_ms": t2 * 1e3 / n2},
-                "ffn": {"achieved": (b1 + b2) / (t1 + t2) / 1e9 if t1 + t2 > 0 else 0.0,
-                        "frac": (b1 + b2) / (t1 + t2) / 1e9 / peak if t1 + t2 > 0 else 0.0}}
-    fl1, fl2 = g1 * d * f * kt["rows"], 2.0 * d * f * kt["rows"]
-    peak = peaks["bf16_tflops_sustained"] or peaks["bf16_tflops"]
-    a1 = fl1 / t1 / 1e12 if t1 > 0 else 0.0
-    a2 = fl2 / t2 / 1e12 if t2 > 0 else 0.0
-    # second ceiling: the operand bytes TMA stages into shared memory (from the tile plan) against the measured TMA fill
-    # rate of the device -- the L2 -> SM fabric, which is what the prefill GEMM actually runs into (DESIGN.md 6.1)
-    fab = None
-    if fill_peak and kt.get("gemm1_fill_bytes"):
-        f1 = kt["gemm1_fill_bytes"] / t1 / 1e9 if t1 > 0 else 0.0
-        f2 = kt["gemm2_fill_bytes"] / t2 / 1e9 if t2 > 0 else 0.0
-        fab = {"bound": "l2_to_sm", "achieved": f1, "peak": fill_peak, "unit": "GB/s", "frac": f1 / fill_peak,
-               "bytes_per_launch": kt["gemm1_fill_bytes"] / n1, "flop_per_fill_byte": fl1 / max(1, kt["gemm1_fill_bytes"]),
-               "tflops_at_fill_peak": fl1 / max(1, kt["gemm1_fill_bytes"]) * fill_peak / 1e3,
-               "gemm2": {"achieved": f2, "frac": f2 / fill_peak, "flop_per_fill_byte": fl2 / max(1, kt["gemm2_fill_bytes"])},
-               "peak_source": "measured in this run: ef_debug_tma_fill_gbs, every SM streaming 32 KB TMA boxes out of a "
-                              "64 MB L2-resident region"}
-    return {"bound": "tensor", "l2_to_sm": fab, "kernel": f"ffn_gemm_kernel<swiglu> (GEMM1), {where}", "achieved": a1, "peak": peak,
-            "unit": "TFLOP/s", "frac": a1 / peak,
-            "peak_source": f"{peaks['source']} bf16 sustained (kernel timed inside a long step)", "traffic": None,
-            "launches": kt["gemm1_launches"], "avg_launch_ms": t1 * 1e3 / n1, "rows_per_launch": kt["rows"] / n1,
-            "gemm2": {"achieved": a2, "frac": a2 / peak, "avg_launch_ms": t2 * 1e3 / n2},
-            "ffn": {"achieved": (fl1 + fl2) / (t1 + t2) / 1e12 if t1 + t2 > 0 else 0.0,
-                    "frac": (fl1 + fl2) / (t1 + t2) / 1e12 / peak if t1 + t2 > 0 else 0.0}}
+        a = tot["wbytes"] / T / 1e9
+        out.update({"bound": "hbm", "achieved": a, "peak": hbm, "unit": "GB/s", "frac": a / hbm,
+                    "peak_source": f"{peaks['source']} HBM copy bandwidth (read + write; a read-only stream measures higher)"})
+    else:
+        a = tot["flop"] / T / 1e12
+        # a link-bound step leaves the GPU idle most of the time: its kernels run at burst clocks unless the sampled
+        # clocks say the power cap was active; the resident leg is always a kernel timed alone (burst)
+        use_burst = burst_only or not power_capped
+        out.update({"bound": "tensor", "achieved": a, "peak": burst if use_burst else sust, "unit": "TFLOP/s",
+                    "frac": a / (burst if use_burst else sust), "frac_burst": a / burst, "frac_sustained": a / sust,
+                    "peak_source": f"{peaks['source']} bf16 " + ("burst (kernel timed alone, or inside a step whose sampled clocks "
+                                   "show no power cap)" if use_burst else "sustained (power cap active in the sampled clocks)")})
+        if fill_peak and kt and kt.get("gemm1_fill_bytes"):
+            fb = kt["gemm1_fill_bytes"] + kt["gemm2_fill_bytes"]
+            out["l2_to_sm"] = {"bound": "l2_to_sm", "achieved": fb / T / 1e9, "peak": fill_peak, "unit": "GB/s",
+                               "frac": fb / T / 1e9 / fill_peak, "bytes_per_launch": fb / n, "flop_per_fill_byte": tot["flop"] / fb,
+                               "peak_source": "measured in this run by the diagnostic library's probe (ef_diag_tma_fill_gbs): every "
+                                              "SM streaming 32 KB TMA boxes out of a 64 MB L2-resident region"}
+    return out
 
 
 def resident_leg(cfg, counts, peaks, dev, args, decode, fill_peak=None):
-    """The grouped FFN alone with every active expert of one visit resident (kernel-only roofline): one launch
-    pair over all groups, timed by the library's CUDA events on the compute stream, weights > L2."""
+    """The grouped FFN alone with every active expert of one visit resident (kernel-only roofline): ONE launch over all
+    groups running both GEMMs, timed by the library's CUDA events on the compute stream, weights > L2 or L2 flushed."""
     import torch
     from paper_2410_17954_b200 import EfContext
     E = cfg.n_experts
@@ -781,7 +875,7 @@ def resident_leg(cfg, counts, peaks, dev, args, decode, fill_peak=None):
     y = torch.empty((R, cfg.d_model), dtype=torch.bfloat16, device=dev)
     act = [e for e in range(E) if counts[e] > 0]
     rb, rw, sl = [int(offs[e]) for e in act], [int(counts[e]) for e in act], [slot_of[e] for e in act]
-    # when the active experts' weights fit in L2 (cfg 4: 64 x 17 MB > 126 MB still; tiny: no) flush between launches
+    # when the active experts' weights could stay in L2 between launches, flush it
     flush = None
     if len(act) * cfg.expert_bytes < 512e6:
         flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -790,23 +884,77 @@ def resident_leg(cfg, counts, peaks, dev, args, decode, fill_peak=None):
         ctx.ef_expert_ffn_grouped_resident(x_perm, rb, rw, sl, y)
     ctx.ef_sync()
     ctx.ef_set_kernel_timing(True)
-    ctx.ef_get_kernel_times(reset=True)
+    ctx.ef_get_kernel_times(reset=True); ctx.ef_get_launch_log(reset=True)
     n = max(5, args.steps)
     for _ in range(n):
         if flush is not None:
             flush.zero_()
         ctx.ef_expert_ffn_grouped_resident(x_perm, rb, rw, sl, y)
     kt = ctx.ef_get_kernel_times(reset=True)
-    res = ffn_roofline(kt, cfg.d_model, cfg.d_ff, dict(peaks, bf16_tflops_sustained=None), decode,
+    lg = ctx.ef_get_launch_log(reset=True)
+    res = ffn_roofline(lg, kt, cfg.d_model, cfg.d_ff, peaks, decode,
                        "all active experts of one visit resident, one launch over all groups",
-                       gated=cfg.expert_kind == "swiglu", fill_peak=fill_peak)
-    if not decode:
-        res["peak_source"] = f"{peaks['source']} bf16 burst (kernel timed alone)"
-    res["traffic"] = NCU_TRAFFIC_BYTES_RESIDENT.get(cfg.name)
+                       gated=cfg.expert_kind == "swiglu", fill_peak=fill_peak, burst_only=True)
+    tr, stale, src = ncu_traffic(cfg.name, "resident")
+    res.update({"traffic": tr, "traffic_stale": stale, "traffic_source": src})
     res["rows_per_expert"] = [int(c) for c in counts]
     res["l2"] = "256 MB flush write between launches" if flush is not None else "weights exceed L2 between launches"
     ctx.close()
     return res
+
+
+def aux_rooflines(runner, cfg, peaks, dev):
+    """HBM rooflines of the memory-bound kernels of the path (S 8(d): route, permute = index + gather, combine, rmsnorm):
+    algorithmic bytes per call / CUDA-event time per call / measured HBM copy bandwidth.  Each kernel is timed over back to
+    back calls that rotate through enough input / output buffer sets to exceed L2 (so no call re-reads what the previous
+    one left there), after a warm-up; the buffers are scratch copies, the runner's own state is not touched."""
+    import torch
+    T, d, k, E = cfg.T, cfg.d_model, cfg.top_k, cfg.n_experts
+    R = T * k
+    c = runner.ctx
+    hbm = peaks["hbm_gbs"]
+    per_set = max(1, R * d * 2 + T * d * 2)
+    n_sets = int(min(64, max(2, (300 << 20) // per_set + 1)))
+    bf = torch.bfloat16
+    xs = [torch.randn((T, d), device=dev, dtype=torch.float32).to(bf) for _ in range(n_sets)]
+    xps = [torch.empty((R, d), dtype=bf, device=dev) for _ in range(n_sets)]
+    outs = [torch.empty((T, d), dtype=bf, device=dev) for _ in range(n_sets)]
+    layer = 0
+    wr, bias = runner.w_router[layer], runner.bias[layer]
+    idx = torch.empty((T, k), dtype=torch.int32, device=dev); w = torch.empty((T, k), dtype=torch.float32, device=dev)
+    counts = torch.empty((E,), dtype=torch.int32, device=dev); offsets = torch.empty((E + 1,), dtype=torch.int32, device=dev)
+    src = torch.empty((R,), dtype=torch.int32, device=dev); inv = torch.empty((R,), dtype=torch.int32, device=dev)
+    c.ef_route_topk(xs[0], wr, bias, T, cfg.renorm, idx, w, None)
+    c.ef_permute(idx, xs[0], T, xps[0], counts, offsets, src, inv)
+    torch.cuda.synchronize()
+    reps = 3 * n_sets
+
+    def timed(fn):
+        for i in range(n_sets):
+            fn(i)
+        torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(reps):
+            fn(i % n_sets)
+        e1.record(); e1.synchronize()
+        return e0.elapsed_time(e1) * 1e-3 / reps
+    rows = {}
+
+    def add(name, secs, nbytes, what):
+        rows[name] = {"bound": "hbm", "us_per_call": secs * 1e6, "algorithmic_bytes": nbytes, "achieved": nbytes / secs / 1e9,
+                      "peak": hbm, "unit": "GB/s", "frac": nbytes / secs / 1e9 / hbm, "bytes": what}
+    add("route_topk", timed(lambda i: c.ef_route_topk(xs[i], wr, bias, T, cfg.renorm, idx, w, None)),
+        T * d * 2 + E * d * 2 + T * k * 8, "x [T,d] bf16 + router [E,d] bf16 read, idx + w [T,k] written")
+    add("permute (index + gather)", timed(lambda i: c.ef_permute(idx, xs[i], T, xps[i], counts, offsets, src, inv)),
+        T * d * 2 + R * d * 2 + R * 12, "x [T,d] read once (k-fold re-read from L2), x_perm [R,d] written, idx read + src + inv written")
+    add("combine", timed(lambda i: c.ef_combine(xps[i], inv, w, T, None, None, outs[i])),
+        R * d * 2 + T * d * 2 + R * 8, "y_perm [R,d] read, out [T,d] written, inv + w read")
+    if cfg.n_layers > 1:
+        add("rmsnorm", timed(lambda i: c.ef_rmsnorm(xs[i], T, 1e-5, outs[i])), 2 * T * d * 2, "x [T,d] read, out [T,d] written")
+    return {"kernels": rows, "peak_source": f"{peaks['source']} HBM copy bandwidth",
+            "how": f"CUDA events over {reps} back-to-back calls rotating through {n_sets} buffer sets "
+                   f"({n_sets * per_set / 1e6:.0f} MB > L2), after {n_sets} warm-up calls"}
 
 
 def main():
@@ -818,6 +966,9 @@ def main():
     ap.add_argument("--workload", default="mixtral_prefill", choices=sorted(wl.CONFIGS))
     ap.add_argument("--ref-tokens", type=int, default=0, help="tokens in the bounded oracle sample (0 = per-workload default)")
     ap.add_argument("--ref-layers", type=int, default=0, help="layer visits in the bounded oracle sample (0 = default)")
+    ap.add_argument("--ref-precision", default="fp64", choices=["fp64", "fp32"],
+                    help="--impl reference: the oracle as the parity tests use it (fp64) or the same C file built with "
+                         "-DORC_REAL=float")
     ap.add_argument("--phys-experts", type=int, default=0,
                     help="alias the logical experts onto this many physical pinned host buffers (0 = one per expert "
                          "if host memory allows)")
@@ -828,6 +979,8 @@ def main():
                          "share, or PLEC prefetching every expert of the next layer (the baselines of P:L230 as policy sketches)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-resident", action="store_true")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="default workload only: skip the decode / many_expert blocks (the other two north_star targets)")
     args = ap.parse_args()
     if args.horizon is not None:
         wl.CONFIGS[args.workload] = wl.scaled(wl.CONFIGS[args.workload], horizon=args.horizon)

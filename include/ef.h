@@ -18,7 +18,13 @@
  *     arena, copy stream, events, workspaces, the slot table and -- after ef_host_expert_register --
  *     a packed copy of each expert in its own pinned host pool (every expert is backed up
  *     on the host, so eviction needs no write-back).
- *   - One ctx per GPU; calls on one ctx must not run concurrently.
+ *   - One ctx per GPU; calls on one ctx must not run concurrently (no two host threads inside the library at once).
+ *   - Streams: the library's workspaces are per ctx, not per stream.  The LAYER calls (ef_rmsnorm, ef_route_topk,
+ *     ef_permute, ef_expert_ffn_grouped[_resident], ef_shared_ffn, ef_combine) form one lane and the TOKEN-SCHEDULER
+ *     calls (ef_token_schedule, ef_path_hamming, ef_reindex_rows) another; the two lanes share nothing and may run
+ *     on different streams concurrently.  Inside a lane, a call on a stream other than the lane's previous one is
+ *     ordered behind everything the lane has enqueued so far (the library inserts the event wait), so changing
+ *     streams is safe but never concurrent.
  *   - Shape limits: d_model % 64 == 0, d_ff % 128 == 0, 1 <= top_k <= 8, top_k <= n_experts <= 256.
  *
  * Logical clock: visit = step * n_layers + layer.  The cache policy depends only on the sequence
@@ -107,9 +113,11 @@ int32_t ef_route_topk(ef_ctx* ctx, void* stream, const void* x, const void* w_ro
 
 /* Stable counting sort of the flat pairs p = t*k + j by topk_idx[p]:
  *   counts[E], offsets[E+1] (exclusive scan), inv[p] = row, src[row] = p, x_perm[row,:] = x[p / k,:].
- * All device.  counts_host_pinned: nullable PINNED host int32[E] that also receives counts; when
- * NULL the library mirrors counts into its own pinned buffer.  Either way an internal event marks
- * the mirror complete and ef_expert_ffn_grouped(counts_host = NULL) waits on it. */
+ * All device.  counts_host_pinned: nullable PINNED host int32[E] that also receives counts (it must stay valid until
+ * the next ef_permute); when NULL the library mirrors counts into its own pinned buffer.  Either way an internal
+ * event marks the mirror complete, and ef_expert_ffn_grouped(counts_host = NULL) waits on it and reads that mirror.
+ * A topk_idx entry outside [0, E) is not routed anywhere: the pair is skipped (inv = -1) and the next
+ * ef_expert_ffn_grouped(counts_host = NULL) fails with EF_ERR_INVALID_ARG. */
 int32_t ef_permute(ef_ctx* ctx, void* stream, const int32_t* topk_idx, const void* x, int32_t T, void* x_perm,
                    int32_t* counts, int32_t* offsets, int32_t* src, int32_t* inv, int32_t* counts_host_pinned);
 
@@ -214,9 +222,6 @@ int32_t ef_token_schedule(ef_ctx* ctx, void* stream, const uint8_t* paths, int32
  * 16, 16-byte aligned), out of place; perm DEVICE int32[n_rows] (need not be a permutation).  Asynchronous. */
 int32_t ef_reindex_rows(ef_ctx* ctx, void* stream, const void* src, const int32_t* perm, int32_t n_rows,
                         int64_t row_bytes, void* dst);
-/* Problems with N <= 256 (decode batches) run in one single-CTA kernel with the distance matrix in shared memory;
- * larger ones in the multi-kernel path.  Test hook: 1 = always take the multi-kernel path.  Results are identical. */
-int32_t ef_set_token_sched_path(ef_ctx* ctx, int32_t force_multi_kernel);
 /* The Hamming distance matrix of Eq. 6 alone: dist_out DEVICE uint16[N, N] (16-byte aligned), d_ij = number of
  * (layer, expert) entries in which r_i and r_j differ; S_ij = 1 - d_ij / LE.  N need not be even here. */
 int32_t ef_path_hamming(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, uint16_t* dist_out);
@@ -228,48 +233,59 @@ int32_t ef_sync(ef_ctx* ctx);
 const char* ef_last_error(ef_ctx* ctx);
 /* Number of kernels this ctx has launched since creation (for bench.py's gpu_launches). */
 int64_t ef_launch_count(ef_ctx* ctx);
-/* Per-kernel device timing of the grouped FFN, for roofline reporting (bench.py).  When on, every
- * grouped-GEMM launch is bracketed by CUDA events on the compute stream.  ef_get_kernel_times waits for
- * the recorded events (synchronous), returns the totals since the last reset and optionally resets.
- * rows = sum over launches of the routed rows they processed (algorithmic FLOPs: gemm1 4*d*f per row,
- * gemm2 2*d*f per row; algorithmic weight bytes: groups * 3*d*f*2). */
+/* Per-launch device timing of the grouped FFN, for roofline reporting (bench.py).  When on, every grouped-FFN launch is
+ * bracketed by CUDA events on the compute stream.  A wave is ONE launch that runs both GEMMs (`which` = 3); a wave whose
+ * expert is still arriving in two chunks runs GEMM1 (`which` = 1) and GEMM2 (`which` = 2) as two launches gated on
+ * different events.  ef_get_kernel_times waits for the recorded events (synchronous), returns the totals since the last
+ * reset and optionally resets; ef_get_launch_log returns the same launches one by one (oldest first), so that a caller can
+ * hold every launch against ITS OWN roofline bound max(FLOP / peak, bytes / bandwidth).
+ * Algorithmic work of a launch over `rows` routed rows in `groups` experts (SwiGLU): GEMM1 4*d*f FLOP per row and 4*d*f
+ * weight bytes per group, GEMM2 2*d*f and 2*d*f (ReLU experts: 2*d*f for both GEMMs). */
 typedef struct {
-    double gemm1_ms, gemm2_ms;
-    int64_t gemm1_launches, gemm2_launches;
-    int64_t rows;     /* routed rows processed (each counted once per FFN, not per GEMM) */
-    int64_t groups;   /* expert groups processed */
-    int64_t gemm1_fill_bytes, gemm2_fill_bytes;   /* bytes the launches' TMA loads staged into shared memory (weight
-                         boxes + token boxes over every tile and k-block, from the tile plan): the L2 -> SM traffic */
+    double gemm1_ms, gemm2_ms, wave_ms;               /* device time of the which = 1 / 2 / 3 launches */
+    int64_t gemm1_launches, gemm2_launches, wave_launches;
+    int64_t gemm1_rows, gemm2_rows, wave_rows;        /* routed rows those launches processed */
+    int64_t gemm1_groups, gemm2_groups, wave_groups;  /* expert groups those launches processed */
+    int64_t gemm1_fill_bytes, gemm2_fill_bytes;       /* bytes the launches' TMA loads staged into shared memory for GEMM1 /
+                         GEMM2 units (weight boxes + token boxes over every tile and k-block, from the tile plan): the
+                         L2 -> SM traffic */
 } ef_kernel_times;
+typedef struct {
+    int32_t which;     /* 1 GEMM1 only, 2 GEMM2 only, 3 both GEMMs in one launch */
+    int32_t groups;    /* experts in the launch */
+    int64_t rows;      /* routed rows in the launch */
+    float ms;          /* device time between the events around the launch */
+} ef_launch_record;
 int32_t ef_set_kernel_timing(ef_ctx* ctx, int32_t on);
 int32_t ef_get_kernel_times(ef_ctx* ctx, ef_kernel_times* out, int32_t reset);
-/* Tail split-K of the grouped GEMM: 0 = automatic (default: split the tiles of the last, partly
- * filled round along K so that every SM stays busy), 1 = never split, 2..16 = split EVERY tile into that many
- * K parts (test hook: exercises the partial-sum workspace on small shapes).  Results differ between modes only
- * by fp32 summation order. */
-int32_t ef_set_splitk(ef_ctx* ctx, int32_t mode);
-/* Physical scheduling of on-demand loads (never part of the policy or its counters):
- * ef_set_wave_bytes: consecutive on-demand experts of a visit are computed by one grouped launch per `bytes` of
- *   expert weights on the link (default 128 MiB; an expert larger than that, and always the last miss of a visit, is
- *   its own launch; 0 = one launch pair per miss).
- * ef_set_chunk_min_bytes: experts of at least `bytes` (default 32 MiB) are copied as two chunks -- first-GEMM weights,
- *   then the down projection -- each with its own "ready" event, so GEMM1 overlaps the second chunk's transfer
- *   (0 = always one copy per expert).  Results are identical in every setting. */
-int32_t ef_set_wave_bytes(ef_ctx* ctx, int64_t bytes);
-int32_t ef_set_chunk_min_bytes(ef_ctx* ctx, int64_t bytes);
-/* Diagnostic: the rate at which TMA can fill shared memory on this device, i.e. the L2 -> SM fabric ceiling that bounds
- * the grouped GEMM's operand traffic.  One persistent CTA per SM streams 32 KB boxes (64 x 256 bf16, the
- * GEMM's weight box) through a 4-stage ring, `iters` boxes per CTA, out of a scratch region of region_bytes (<= 126 MB
- * stays in L2; larger streams from HBM).  gbs_out: HOST double, delivered GB/s.  Synchronous; allocates and frees the
- * region. */
-int32_t ef_debug_tma_fill_gbs(ef_ctx* ctx, int64_t region_bytes, int32_t iters, double* gbs_out);
-/* Diagnostic, only in libraries built with -DEF_KPROF (EF_ERR_UNSUPPORTED otherwise): the first call arms the
- * counters, later calls return, per CTA of the last GEMM1 (which = 1) or GEMM2 (which = 2) launch, the cycles the
- * MMA-issuing lane spent {in total, waiting for a tile ticket, waiting for the epilogue to free TMEM, waiting for
- * TMA to fill a stage} and the units it processed.  out: HOST int64[5 * SM count].  Synchronous. */
-int32_t ef_debug_kprof(ef_ctx* ctx, int32_t which, int64_t* out);
-/* 0 = tcgen05 kernels (default); 1 = plain-FMA debug kernels for the grouped FFN (bring-up aid, slow). */
-int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on);
+/* out: HOST ef_launch_record[max_records]; *n_out = records written (the log keeps at most 65536).  Synchronous. */
+int32_t ef_get_launch_log(ef_ctx* ctx, ef_launch_record* out, int32_t max_records, int32_t* n_out, int32_t reset);
+
+/* Physical-scheduling knobs and test hooks.  None of them changes what is computed or any cache counter (results differ
+ * between EF_OPT_SPLITK settings only by fp32 summation order):
+ * EF_OPT_SPLITK          tail split-K of the grouped GEMM: 0 = automatic (default: the tiles of the last,
+ *                        partly filled round are split along K so that every SM stays busy), 1 = never, 2..16 = split
+ *                        EVERY tile into that many K parts (test hook: exercises the partial-sum workspace on small shapes).
+ * EF_OPT_WAVE_BYTES      consecutive on-demand experts of a visit are computed by one grouped launch per `value` bytes of
+ *                        expert weights on the link (default 128 MiB; an expert larger than that, and always the last
+ *                        miss of a visit, is its own launch; 0 = one launch per miss) -- SURVEY.md 8(f).3.
+ * EF_OPT_CHUNK_MIN_BYTES experts of at least `value` bytes (default 32 MiB) are copied as two chunks -- first-GEMM weights,
+ *                        then the down projection -- each with its own "ready" event, so GEMM1 of the visit's last wave
+ *                        overlaps the second chunk's transfer (0 = always one copy per expert).
+ * EF_OPT_FUSED_WAVES     1 (default) = a wave is one launch running both GEMMs; 0 = always two launches (test hook).
+ * EF_OPT_TOKEN_SCHED_PATH problems with N <= 256 (decode batches) run in one single-CTA kernel with the distance matrix in
+ *                        shared memory, larger ones in the multi-kernel path; 1 = always the multi-kernel path (test hook).
+ * EF_OPT_COPY_ORDER      order in which the on-demand copies of one visit are put on the link: 0 = policy order (ascending
+ *                        expert id, R12), 1 (default) = experts with more routed rows first, so the largest GEMMs start
+ *                        earliest (the paper's "high-priority queue").  Which slot an expert takes
+ *                        and every counter are decided in policy order either way. */
+#define EF_OPT_SPLITK 1
+#define EF_OPT_WAVE_BYTES 2
+#define EF_OPT_CHUNK_MIN_BYTES 3
+#define EF_OPT_FUSED_WAVES 4
+#define EF_OPT_TOKEN_SCHED_PATH 5
+#define EF_OPT_COPY_ORDER 6
+int32_t ef_set_option(ef_ctx* ctx, int32_t key, int64_t value);
 
 #ifdef __cplusplus
 }

@@ -11,16 +11,21 @@ from dataclasses import dataclass
 import numpy as np
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
-_LIB = None
+_LIBS: dict = {}
 
+# include/ef.h
 DECLARED_SYMBOLS = [
     "ef_create", "ef_destroy", "ef_host_expert_register", "ef_host_expert_alias", "ef_route_topk", "ef_permute",
     "ef_expert_ffn_grouped", "ef_expert_ffn_grouped_resident", "ef_shared_ffn", "ef_combine", "ef_rmsnorm",
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
-    "ef_cache_clear", "ef_copy_busy_ms", "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_debug_simt_ffn", "ef_set_kernel_timing",
-    "ef_get_kernel_times", "ef_set_splitk", "ef_debug_kprof", "ef_token_schedule", "ef_path_hamming", "ef_set_token_sched_path", "ef_reindex_rows",
-    "ef_set_wave_bytes", "ef_set_chunk_min_bytes", "ef_debug_tma_fill_gbs", "ef_set_cache_policy",
+    "ef_cache_clear", "ef_set_cache_policy", "ef_copy_busy_ms", "ef_token_schedule", "ef_reindex_rows", "ef_path_hamming",
+    "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_kernel_timing", "ef_get_kernel_times", "ef_get_launch_log",
+    "ef_set_option",
 ]
+# include/ef_diag.h: only libef_diag.so (the diagnostic build) has these
+DIAG_SYMBOLS = ["ef_diag_set_simt_ffn", "ef_diag_tma_fill_gbs", "ef_diag_kprof"]
+
+EF_OPT_SPLITK, EF_OPT_WAVE_BYTES, EF_OPT_CHUNK_MIN_BYTES, EF_OPT_FUSED_WAVES, EF_OPT_TOKEN_SCHED_PATH, EF_OPT_COPY_ORDER = 1, 2, 3, 4, 5, 6
 
 
 class EfError(RuntimeError):
@@ -43,26 +48,31 @@ class CacheStats(ctypes.Structure):
 
 
 class KernelTimes(ctypes.Structure):
-    _fields_ = [("gemm1_ms", ctypes.c_double), ("gemm2_ms", ctypes.c_double), ("gemm1_launches", ctypes.c_int64),
-                ("gemm2_launches", ctypes.c_int64), ("rows", ctypes.c_int64), ("groups", ctypes.c_int64),
-                ("gemm1_fill_bytes", ctypes.c_int64), ("gemm2_fill_bytes", ctypes.c_int64)]
+    _fields_ = ([(n, ctypes.c_double) for n in ("gemm1_ms", "gemm2_ms", "wave_ms")] +
+                [(n, ctypes.c_int64) for n in ("gemm1_launches", "gemm2_launches", "wave_launches", "gemm1_rows", "gemm2_rows",
+                                               "wave_rows", "gemm1_groups", "gemm2_groups", "wave_groups",
+                                               "gemm1_fill_bytes", "gemm2_fill_bytes")])
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
 
 
-def library_path() -> str:
-    return os.path.join(_PKG, "libef.so")
+class LaunchRecord(ctypes.Structure):
+    _fields_ = [("which", ctypes.c_int32), ("groups", ctypes.c_int32), ("rows", ctypes.c_int64), ("ms", ctypes.c_float)]
 
 
-def load_library() -> ctypes.CDLL:
-    """Load libef.so (built by ``python -m paper_2410_17954_b200.build``).  Fails loudly if absent."""
-    global _LIB
-    if _LIB is None:
-        path = library_path()
+def library_path(diag: bool = False) -> str:
+    return os.path.join(_PKG, "libef_diag.so" if diag else "libef.so")
+
+
+def load_library(diag: bool = False) -> ctypes.CDLL:
+    """Load libef.so (built by ``python -m paper_2410_17954_b200.build``), or with diag=True the diagnostic build
+    libef_diag.so (``... .build --diag``; include/ef_diag.h).  Fails loudly if absent."""
+    if diag not in _LIBS:
+        path = library_path(diag)
         if not os.path.exists(path):
-            raise EfError(-100, f"{path} not found: build it with `python -m paper_2410_17954_b200.build` "
-                                "(there is no CPU fallback)")
+            raise EfError(-100, f"{path} not found: build it with `python -m paper_2410_17954_b200.build"
+                                f"{' --diag' if diag else ''}` (there is no CPU fallback)")
         lib = ctypes.CDLL(path)
         vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
         sig = {
@@ -85,20 +95,18 @@ def load_library() -> ctypes.CDLL:
             "ef_cache_clear": [vp],
             "ef_copy_busy_ms": [vp, ctypes.POINTER(ctypes.c_float)],
             "ef_sync": [vp],
-            "ef_set_debug_simt_ffn": [vp, i32],
             "ef_set_kernel_timing": [vp, i32],
-            "ef_set_splitk": [vp, i32],
-            "ef_debug_kprof": [vp, i32, vp],
             "ef_get_kernel_times": [vp, ctypes.POINTER(KernelTimes), i32],
+            "ef_get_launch_log": [vp, ctypes.POINTER(LaunchRecord), i32, ctypes.POINTER(i32), i32],
             "ef_token_schedule": [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp],
             "ef_reindex_rows": [vp, vp, vp, vp, i32, i64, vp],
             "ef_path_hamming": [vp, vp, vp, i32, i32, vp],
-            "ef_set_token_sched_path": [vp, i32],
-            "ef_debug_tma_fill_gbs": [vp, i64, i32, ctypes.POINTER(ctypes.c_double)],
             "ef_set_cache_policy": [vp, i32],
-            "ef_set_wave_bytes": [vp, i64],
-            "ef_set_chunk_min_bytes": [vp, i64],
+            "ef_set_option": [vp, i32, i64],
         }
+        if diag:
+            sig.update({"ef_diag_set_simt_ffn": [vp, i32], "ef_diag_kprof": [vp, i32, vp],
+                        "ef_diag_tma_fill_gbs": [vp, i64, i32, ctypes.POINTER(ctypes.c_double)]})
         for name, args in sig.items():
             fn = getattr(lib, name)
             fn.argtypes = args
@@ -107,13 +115,13 @@ def load_library() -> ctypes.CDLL:
         lib.ef_last_error.restype = ctypes.c_char_p
         lib.ef_launch_count.argtypes = [vp]
         lib.ef_launch_count.restype = i64
-        _LIB = lib
-    return _LIB
+        _LIBS[diag] = lib
+    return _LIBS[diag]
 
 
-def exported_symbols() -> list[str]:
-    lib = load_library()
-    return [s for s in DECLARED_SYMBOLS if hasattr(lib, s)]
+def exported_symbols(diag: bool = False) -> list[str]:
+    lib = load_library(diag)
+    return [s for s in DECLARED_SYMBOLS + DIAG_SYMBOLS if hasattr(lib, s)]
 
 
 def _dp(t):
@@ -140,8 +148,9 @@ class EfContext:
     """One ef_ctx.  Method names and argument order follow include/ef.h."""
 
     def __init__(self, n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared=0, max_tokens=1,
-                 prefetch_horizon=0, device=0, expert_kind=0):
-        self.lib = load_library()
+                 prefetch_horizon=0, device=0, expert_kind=0, diag=False):
+        self.lib = load_library(diag)
+        self.diag = diag
         self.cfg = EfConfig(n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared, max_tokens,
                             prefetch_horizon, device, expert_kind)
         h = ctypes.c_void_p()
@@ -244,9 +253,6 @@ class EfContext:
         row_bytes = src.element_size() * (src.numel() // max(1, src.shape[0]))
         self._chk(self.lib.ef_reindex_rows(self.h, _stream(), _dp(src), _dp(perm), n, row_bytes, _dp(dst)))
 
-    def ef_set_token_sched_path(self, force_multi_kernel: bool):
-        self._chk(self.lib.ef_set_token_sched_path(self.h, 1 if force_multi_kernel else 0))
-
     def ef_path_hamming(self, paths, dist_out):
         N = paths.shape[0]
         LE = paths.numel() // max(1, N)
@@ -279,31 +285,26 @@ class EfContext:
     def ef_launch_count(self) -> int:
         return int(self.lib.ef_launch_count(self.h))
 
-    def ef_set_debug_simt_ffn(self, on: bool):
-        self._chk(self.lib.ef_set_debug_simt_ffn(self.h, 1 if on else 0))
-
-    def ef_set_splitk(self, mode: int):
-        self._chk(self.lib.ef_set_splitk(self.h, int(mode)))
+    def ef_set_option(self, key: int, value: int):
+        self._chk(self.lib.ef_set_option(self.h, int(key), int(value)))
 
     POLICIES = {"plec": 0, "lru": 1, "layer_lru": 2}
 
     def ef_set_cache_policy(self, policy):
         self._chk(self.lib.ef_set_cache_policy(self.h, self.POLICIES.get(policy, policy)))
 
-    def ef_set_wave_bytes(self, nbytes: int):
-        self._chk(self.lib.ef_set_wave_bytes(self.h, int(nbytes)))
+    # -- include/ef_diag.h (diag=True contexts only)
+    def ef_diag_set_simt_ffn(self, on: bool):
+        self._chk(self.lib.ef_diag_set_simt_ffn(self.h, 1 if on else 0))
 
-    def ef_set_chunk_min_bytes(self, nbytes: int):
-        self._chk(self.lib.ef_set_chunk_min_bytes(self.h, int(nbytes)))
-
-    def ef_debug_tma_fill_gbs(self, region_bytes: int, iters: int = 2000) -> float:
+    def ef_diag_tma_fill_gbs(self, region_bytes: int, iters: int = 2000) -> float:
         out = ctypes.c_double()
-        self._chk(self.lib.ef_debug_tma_fill_gbs(self.h, int(region_bytes), int(iters), ctypes.byref(out)))
+        self._chk(self.lib.ef_diag_tma_fill_gbs(self.h, int(region_bytes), int(iters), ctypes.byref(out)))
         return float(out.value)
 
-    def ef_debug_kprof(self, which: int, n_sms: int = 148):
+    def ef_diag_kprof(self, which: int, n_sms: int = 148):
         out = np.zeros((n_sms, 5), np.int64)
-        self._chk(self.lib.ef_debug_kprof(self.h, int(which), out.ctypes.data_as(ctypes.c_void_p)))
+        self._chk(self.lib.ef_diag_kprof(self.h, int(which), out.ctypes.data_as(ctypes.c_void_p)))
         return out
 
     def ef_set_kernel_timing(self, on: bool):
@@ -313,3 +314,9 @@ class EfContext:
         kt = KernelTimes()
         self._chk(self.lib.ef_get_kernel_times(self.h, ctypes.byref(kt), 1 if reset else 0))
         return kt.as_dict()
+
+    def ef_get_launch_log(self, reset: bool = True, max_records: int = 65536) -> list[dict]:
+        buf = (LaunchRecord * max_records)()
+        n = ctypes.c_int32()
+        self._chk(self.lib.ef_get_launch_log(self.h, buf, max_records, ctypes.byref(n), 1 if reset else 0))
+        return [{"which": int(r.which), "groups": int(r.groups), "rows": int(r.rows), "ms": float(r.ms)} for r in buf[:n.value]]

@@ -38,7 +38,7 @@ combine_kernel(const uint4* __restrict__ y_perm, const int32_t* __restrict__ inv
     for (int j = 0; j < k; ++j) {
         const int row = inv[t * k + j];
         const float s = w[t * k + j];
-        fma8(acc, y_perm[(int64_t)row * d8 + c], s);
+        if (row >= 0) fma8(acc, y_perm[(int64_t)row * d8 + c], s);      // -1: a pair ef_permute could not route
     }
     for (int s = 0; s < n_shared; ++s) fma8(acc, y_shared[((int64_t)s * T + t) * d8 + c], 1.f);
     uint4 o;

@@ -1,6 +1,6 @@
-// Diagnostics that are not on the hot path.
+// Diagnostics that are not on the hot path.  libef_diag only (include/ef_diag.h).
 //
-// ef_debug_tma_fill_gbs: how fast TMA can fill shared memory on this device.  The grouped GEMM (ffn_tc.cu) stages
+// ef_diag_tma_fill_gbs: how fast TMA can fill shared memory on this device.  The grouped GEMM (ffn_tc.cu) stages
 // 48 KB of operands per CTA per k-block (1024 tensor cycles at full rate), i.e. it asks the L2 -> SM path for 48 bytes
 // per clock and SM; how close that is to what the device can deliver decides whether the tensor pipe can be kept fed
 // (contiguous 32 KB boxes fill at 18-21 TB/s, the same box gathered from 256 strided rows at
@@ -10,6 +10,7 @@
 #include <algorithm>
 
 #include "ef_internal.h"
+#include "ef_diag.h"
 
 namespace {
 
@@ -79,10 +80,10 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 
 }  // namespace
 
-extern "C" int32_t ef_debug_tma_fill_gbs(ef_ctx* ctx, int64_t region_bytes, int32_t iters, double* gbs_out) {
+extern "C" int32_t ef_diag_tma_fill_gbs(ef_ctx* ctx, int64_t region_bytes, int32_t iters, double* gbs_out) {
     EF_CHECK_CTX(ctx);
     if (!gbs_out || iters < 1 || region_bytes < BOX_BYTES)
-        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_debug_tma_fill_gbs: need gbs_out, iters >= 1, region_bytes >= %d", BOX_BYTES);
+        return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_diag_tma_fill_gbs: need gbs_out, iters >= 1, region_bytes >= %d", BOX_BYTES);
     void* fp = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qres) != cudaSuccess ||
@@ -91,7 +92,7 @@ extern "C" int32_t ef_debug_tma_fill_gbs(ef_ctx* ctx, int64_t region_bytes, int3
     const int n_boxes = (int)std::min<int64_t>(region_bytes / BOX_BYTES, 1 << 20);
     void* buf = nullptr;
     cudaError_t e = cudaMalloc(&buf, (size_t)n_boxes * BOX_BYTES);
-    if (e != cudaSuccess) return ef_fail(ctx, EF_ERR_OOM, "ef_debug_tma_fill_gbs: scratch region: %s", cudaGetErrorString(e));
+    if (e != cudaSuccess) return ef_fail(ctx, EF_ERR_OOM, "ef_diag_tma_fill_gbs: scratch region: %s", cudaGetErrorString(e));
     int32_t rc = EF_OK;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     do {
@@ -123,6 +124,6 @@ extern "C" int32_t ef_debug_tma_fill_gbs(ef_ctx* ctx, int64_t region_bytes, int3
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
     cudaFree(buf);
-    if (e != cudaSuccess) { ctx->sticky = EF_ERR_CUDA; return ef_fail(ctx, EF_ERR_CUDA, "ef_debug_tma_fill_gbs: %s", cudaGetErrorString(e)); }
+    if (e != cudaSuccess) { ctx->sticky = EF_ERR_CUDA; return ef_fail(ctx, EF_ERR_CUDA, "ef_diag_tma_fill_gbs: %s", cudaGetErrorString(e)); }
     return rc;
 }

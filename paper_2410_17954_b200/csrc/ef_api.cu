@@ -54,6 +54,45 @@ static cudaError_t ring_wait(ef_ctx* ctx, cudaStream_t waiter, const EvHandle& h
     return cudaStreamWaitEvent(waiter, ctx->ev_ring[f.idx], 0);
 }
 
+// The library's workspaces are per ctx, not per stream (ef.h, "Streams").  Every stream-taking call of a lane passes
+// through here first: a call on a stream other than the lane's previous one is ordered behind everything the lane has
+// enqueued so far, so that two streams can never interleave inside the split-K workspace, the h workspace, the
+// scheduler blocks or a slot that a copy is about to overwrite.
+static int32_t enter_lane(ef_ctx* ctx, cudaStream_t st, cudaStream_t* last, bool* has_last) {
+    if (*has_last && *last != st) {
+        cudaError_t e;
+        EvHandle h = ring_record(ctx, *last, &e);
+        EF_CUDA(ctx, e);
+        EF_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_ring[h.idx], 0));
+    }
+    *last = st;
+    *has_last = true;
+    return EF_OK;
+}
+#define EF_ENTER_LAYER(ctx, st)                                                                   \
+    do {                                                                                          \
+        int32_t rc__ = enter_lane((ctx), (st), &(ctx)->last_compute, &(ctx)->has_last_compute);  \
+        if (rc__ != EF_OK) return rc__;                                                           \
+    } while (0)
+#define EF_ENTER_SCHED(ctx, st)                                                               \
+    do {                                                                                      \
+        int32_t rc__ = enter_lane((ctx), (st), &(ctx)->last_sched, &(ctx)->has_last_sched);  \
+        if (rc__ != EF_OK) return rc__;                                                       \
+    } while (0)
+
+// timing-enabled events are pooled: creating one costs microseconds, which is visible next to a 50 us decode wave
+int32_t efk_timing_events(ef_ctx* ctx, cudaEvent_t* e0, cudaEvent_t* e1) {
+    for (cudaEvent_t* e : {e0, e1}) {
+        if (!ctx->timing_pool.empty()) {
+            *e = ctx->timing_pool.back();
+            ctx->timing_pool.pop_back();
+        } else {
+            EF_CUDA(ctx, cudaEventCreate(e));
+        }
+    }
+    return EF_OK;
+}
+
 // ---------------------------------------------------------------------------------------------------
 // lifetime
 // ---------------------------------------------------------------------------------------------------
@@ -89,13 +128,14 @@ extern "C" int32_t ef_create(const ef_config* cfg, ef_ctx** out) {
     ctx->h_rows = (int64_t)c.max_tokens * (c.top_k + c.n_shared);
     if ((e = cudaMalloc(&ctx->h_ws, (size_t)ctx->h_rows * c.d_ff * 2)) != cudaSuccess)
         return bail(EF_ERR_OOM, "h workspace", e);
-    if ((e = cudaHostAlloc((void**)&ctx->counts_pinned, sizeof(int32_t) * c.n_experts, cudaHostAllocDefault)) !=
+    if ((e = cudaHostAlloc((void**)&ctx->counts_pinned, sizeof(int32_t) * (c.n_experts + 1), cudaHostAllocDefault)) !=
         cudaSuccess)
         return bail(EF_ERR_OOM, "pinned counts", e);
     if ((e = cudaEventCreateWithFlags(&ctx->counts_event, cudaEventDisableTiming)) != cudaSuccess)
         return bail(EF_ERR_CUDA, "event", e);
     if ((e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
         return bail(EF_ERR_CUDA, "copy stream", e);
+    memset(ctx->counts_pinned, 0, sizeof(int32_t) * (c.n_experts + 1));
     ctx->ev_ring.resize(kRing, nullptr);
     ctx->ev_gen.assign(kRing, 0);
     for (int i = 0; i < kRing; ++i)
@@ -103,6 +143,8 @@ extern "C" int32_t ef_create(const ef_config* cfg, ef_ctx** out) {
             return bail(EF_ERR_CUDA, "event ring", e);
     ctx->host_expert.assign((size_t)c.n_layers * c.n_experts, nullptr);
     ctx->host_owned.assign((size_t)c.n_layers * c.n_experts, 0);
+    ctx->host_aliases.assign((size_t)c.n_layers * c.n_experts, 0);
+    ctx->alias_src.assign((size_t)c.n_layers * c.n_experts, -1);
     ctx->shared_registered.assign((size_t)c.n_layers * std::max(1, c.n_shared), 0);
     ctx->slots.assign(c.n_slots, EfSlot());
     ctx->slot_of.assign((size_t)c.n_layers * c.n_experts, -1);
@@ -123,6 +165,7 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
     cudaDeviceSynchronize();
     for (auto& sp : ctx->copy_spans) { cudaEventDestroy(sp.first); cudaEventDestroy(sp.second); }
     for (auto& k : ctx->kspans) { cudaEventDestroy(k.e0); cudaEventDestroy(k.e1); }
+    for (auto ev : ctx->timing_pool) cudaEventDestroy(ev);
     for (auto ev : ctx->ev_ring) if (ev) cudaEventDestroy(ev);
     if (ctx->counts_event) cudaEventDestroy(ctx->counts_event);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
@@ -189,6 +232,19 @@ extern "C" int32_t ef_host_expert_register(ef_ctx* ctx, int32_t layer, int32_t e
         expert < -c.n_shared)
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_register: bad layer/expert/pointer");
     EF_CUDA(ctx, cudaSetDevice(c.device));
+    if (expert >= 0) {
+        // re-registration replaces the packed host copy: not while another expert aliases it (the alias would dangle) and
+        // not while a slot holds or is receiving the old weights (the hit would serve stale data, a copy in flight would
+        // read freed pinned memory)
+        const size_t g = (size_t)layer * c.n_experts + expert;
+        if (ctx->host_expert[g] && ctx->host_aliases[g] > 0)
+            return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_register: (layer %d, expert %d) is aliased by %d other expert(s)",
+                           layer, expert, ctx->host_aliases[g]);
+        if (ctx->host_expert[g] && ctx->slot_of[g] >= 0)
+            return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_register: (layer %d, expert %d) is resident; ef_cache_evict it first",
+                           layer, expert);
+        if (ctx->host_expert[g]) EF_CUDA(ctx, cudaStreamSynchronize(ctx->copy_stream));   // an evicted expert's copy may still be in flight
+    }
     void* buf = nullptr;
     cudaError_t e = cudaHostAlloc(&buf, (size_t)ctx->W, cudaHostAllocDefault);
     if (e != cudaSuccess) return ef_fail(ctx, EF_ERR_OOM, "pinned host pool: %s", cudaGetErrorString(e));
@@ -196,6 +252,7 @@ extern "C" int32_t ef_host_expert_register(ef_ctx* ctx, int32_t layer, int32_t e
     if (expert >= 0) {
         size_t g = (size_t)layer * c.n_experts + expert;
         if (ctx->host_expert[g] && ctx->host_owned[g]) cudaFreeHost(ctx->host_expert[g]);
+        else if (ctx->host_expert[g]) ctx->host_aliases[ctx->alias_src[g]]--;      // it was an alias until now
         ctx->host_expert[g] = buf;
         ctx->host_owned[g] = 1;
         return EF_OK;
@@ -218,9 +275,19 @@ extern "C" int32_t ef_host_expert_alias(ef_ctx* ctx, int32_t layer, int32_t expe
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_alias: bad ids");
     size_t g = (size_t)layer * c.n_experts + expert, sg = (size_t)src_layer * c.n_experts + src_expert;
     if (!ctx->host_expert[sg]) return ef_fail(ctx, EF_ERR_NOT_REGISTERED, "ef_host_expert_alias: source not registered");
-    if (ctx->host_expert[g] && ctx->host_owned[g]) cudaFreeHost(ctx->host_expert[g]);
+    if (g == sg) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_alias: an expert cannot alias itself");
+    if (!ctx->host_owned[sg]) sg = (size_t)ctx->alias_src[sg];                    // alias of an alias: count on the owner
+    if (ctx->host_expert[g]) {
+        if (ctx->host_aliases[g] > 0 || ctx->slot_of[g] >= 0)
+            return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_host_expert_alias: the target is aliased by others or resident");
+        EF_CUDA(ctx, cudaStreamSynchronize(ctx->copy_stream));
+        if (ctx->host_owned[g]) cudaFreeHost(ctx->host_expert[g]);
+        else ctx->host_aliases[ctx->alias_src[g]]--;
+    }
     ctx->host_expert[g] = ctx->host_expert[sg];
     ctx->host_owned[g] = 0;
+    ctx->alias_src[g] = (int32_t)sg;
+    ctx->host_aliases[sg]++;
     return EF_OK;
 }
 
@@ -236,6 +303,7 @@ extern "C" int32_t ef_route_topk(ef_ctx* ctx, void* stream, const void* x, const
     if (T > ctx->cfg.max_tokens) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_route_topk: T > max_tokens");
     if (bias && bias_token_stride != 0 && bias_token_stride < ctx->cfg.n_experts)
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_route_topk: bias_token_stride must be 0 or >= E");
+    EF_ENTER_LAYER(ctx, (cudaStream_t)stream);
     return efk_route_topk(ctx, (cudaStream_t)stream, x, w_router, bias, bias_token_stride, T, renorm ? 1 : 0,
                           topk_idx, topk_w, logits_out);
 }
@@ -247,10 +315,14 @@ extern "C" int32_t ef_permute(ef_ctx* ctx, void* stream, const int32_t* topk_idx
     if (T < 0 || !counts || !offsets || (T > 0 && (!topk_idx || !x || !x_perm || !src || !inv)))
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_permute: null pointer or negative T");
     if (T > ctx->cfg.max_tokens) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_permute: T > max_tokens");
+    EF_ENTER_LAYER(ctx, (cudaStream_t)stream);
     int32_t* mirror = counts_host_pinned ? counts_host_pinned : ctx->counts_pinned;
-    int32_t rc = efk_permute(ctx, (cudaStream_t)stream, topk_idx, x, T, x_perm, counts, offsets, src, inv, mirror);
+    int32_t* err = ctx->counts_pinned + ctx->cfg.n_experts;
+    *err = 0;
+    int32_t rc = efk_permute(ctx, (cudaStream_t)stream, topk_idx, x, T, x_perm, counts, offsets, src, inv, mirror, err);
     if (rc != EF_OK) return rc;
-    if (!counts_host_pinned) EF_CUDA(ctx, cudaEventRecord(ctx->counts_event, (cudaStream_t)stream));
+    ctx->counts_mirror = mirror;       // what ef_expert_ffn_grouped(counts_host = NULL) reads once the event has fired
+    EF_CUDA(ctx, cudaEventRecord(ctx->counts_event, (cudaStream_t)stream));
     return EF_OK;
 }
 
@@ -260,12 +332,14 @@ extern "C" int32_t ef_combine(ef_ctx* ctx, void* stream, const void* y_perm, con
     if (T < 0 || (T > 0 && (!y_perm || !inv || !topk_w || !out)))
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_combine: null pointer or negative T");
     if (y_shared && ctx->cfg.n_shared == 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_combine: y_shared given but n_shared == 0");
+    EF_ENTER_LAYER(ctx, (cudaStream_t)stream);
     return efk_combine(ctx, (cudaStream_t)stream, y_perm, inv, topk_w, T, residual, y_shared, out);
 }
 
 extern "C" int32_t ef_rmsnorm(ef_ctx* ctx, void* stream, const void* x, int32_t T, float eps, void* out) {
     EF_CHECK_CTX(ctx);
     if (T < 0 || (T > 0 && (!x || !out))) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_rmsnorm: null pointer or negative T");
+    EF_ENTER_LAYER(ctx, (cudaStream_t)stream);
     return efk_rmsnorm(ctx, (cudaStream_t)stream, x, T, eps, out);
 }
 
@@ -365,9 +439,11 @@ int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
     EfPhys& ph = ctx->phys[slot];
     EF_CUDA(ctx, ring_wait(ctx, ctx->copy_stream, ph.free_, ctx->last_compute, ctx->has_last_compute));
     cudaEvent_t t0, t1;
-    if (ctx->copy_spans.size() > 8192) drain_copy_spans(ctx, false, nullptr);
-    EF_CUDA(ctx, cudaEventCreate(&t0));
-    EF_CUDA(ctx, cudaEventCreate(&t1));
+    if (ctx->copy_spans.size() > 1024) drain_copy_spans(ctx, false, nullptr);
+    {
+        int32_t rc = efk_timing_events(ctx, &t0, &t1);
+        if (rc != EF_OK) return rc;
+    }
     EF_CUDA(ctx, cudaEventRecord(t0, ctx->copy_stream));
     // Finer-grained streaming: a large expert travels as two copies -- the first-GEMM weights
     // (packed W13, or W1), then Wd -- with a "ready" event after each, so GEMM1 of the wave that waits for this
@@ -407,8 +483,8 @@ void drain_copy_spans(ef_ctx* ctx, bool wait, float* acc_ms) {
         if (done) {
             float ms = 0.f;
             if (cudaEventElapsedTime(&ms, v[i].first, v[i].second) == cudaSuccess) ctx->copy_ms += ms;
-            cudaEventDestroy(v[i].first);
-            cudaEventDestroy(v[i].second);
+            ctx->timing_pool.push_back(v[i].first);
+            ctx->timing_pool.push_back(v[i].second);
         } else {
             v[keep++] = v[i];
         }
@@ -436,31 +512,49 @@ int32_t wait_slot_ready(ef_ctx* ctx, cudaStream_t st, EfPhys& ph, int which) {
     return EF_OK;
 }
 
-int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm, const std::vector<WaveItem>& items) {
+// One wave.  Normally ONE launch that runs both GEMMs (ffn_tc.cu) once every member's weights have landed.  Only the
+// LAST wave of a visit may run as two launches when its expert is still arriving in two chunks: GEMM1 is gated on the
+// first chunk (W13 / W1) and overlaps the transfer of Wd, so the tail of the visit after its final copy is one GEMM2.  For
+// every earlier wave that overlap buys nothing -- the next wave's copies are on the link anyway -- and one launch is faster.
+int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm, const std::vector<WaveItem>& items,
+                 bool last_of_visit = false) {
     if (items.empty()) return EF_OK;
     auto& phys = ctx->phys;
     int32_t rc;
-    for (int which = 1; which <= 2; ++which) {
-        for (const WaveItem& it : items)
-            if ((rc = wait_slot_ready(ctx, st, phys[it.slot], which)) != EF_OK) return rc;
+    bool two_launches = !ctx->fused_waves;
+    if (last_of_visit)
+        for (const WaveItem& it : items) {
+            const EfPhys& ph = phys[it.slot];
+            if (ph.ready1.idx >= 0 && !(ph.waited == st && (ph.waited_mask & 2))) two_launches = true;
+        }
+    auto launch = [&](int phase) -> int32_t {
         for (size_t base = 0; base < items.size(); base += EF_MAX_GROUPS) {
-            EfGroupTable tab;
-            int32_t h_row0[EF_MAX_GROUPS];
+            EfWaveTable tab;
             tab.n = (int32_t)std::min<size_t>(EF_MAX_GROUPS, items.size() - base);
             for (int i = 0; i < tab.n; ++i) {
                 const WaveItem& it = items[base + i];
-                tab.g[i] = EfGroup{it.row0, it.row0, it.rows, it.slot};
-                h_row0[i] = it.row0;
+                tab.g[i] = EfWaveGroup{it.row0, it.row0, it.row0, it.rows, it.slot};
             }
-            if ((rc = efk_ffn_grouped(ctx, st, x_perm, y_perm, tab, h_row0, which)) != EF_OK) return rc;
+            int32_t r = efk_ffn_grouped(ctx, st, x_perm, y_perm, tab, phase);
+            if (r != EF_OK) return r;
         }
+        return EF_OK;
+    };
+    if (two_launches) {
+        for (int which = 1; which <= 2; ++which) {
+            for (const WaveItem& it : items)
+                if ((rc = wait_slot_ready(ctx, st, phys[it.slot], which)) != EF_OK) return rc;
+            if ((rc = launch(which)) != EF_OK) return rc;
+        }
+    } else {
+        for (const WaveItem& it : items)
+            if ((rc = wait_slot_ready(ctx, st, phys[it.slot], 2)) != EF_OK) return rc;
+        if ((rc = launch(3)) != EF_OK) return rc;
     }
     cudaError_t e;
     EvHandle ev = ring_record(ctx, st, &e);
     EF_CUDA(ctx, e);
     for (const WaveItem& it : items) phys[it.slot].free_ = ev;
-    ctx->last_compute = st;
-    ctx->has_last_compute = true;
     return EF_OK;
 }
 
@@ -480,9 +574,9 @@ struct MissBatcher {
         for (const WaveItem& it : open) if (it.slot == slot) return true;
         return false;
     }
-    int32_t flush() {
+    int32_t flush(bool last_of_visit = false) {
         if (open.empty()) return EF_OK;
-        int32_t rc = run_wave(ctx, st, x_perm, y_perm, open);
+        int32_t rc = run_wave(ctx, st, x_perm, y_perm, open, last_of_visit);
         open.clear();
         return rc;
     }
@@ -490,17 +584,18 @@ struct MissBatcher {
         int32_t rc = EF_OK;
         if (last_of_visit && !open.empty() && (rc = flush()) != EF_OK) return rc;
         open.push_back(it);
-        if ((int)open.size() >= per_wave || last_of_visit) rc = flush();
+        if ((int)open.size() >= per_wave || last_of_visit) rc = flush(last_of_visit);
         return rc;
     }
 };
 
 }  // namespace
 
-int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                        const int32_t* h_row0, int phase) {
-    if (ctx->debug_simt) return efk_ffn_simt(ctx, st, x, y, tab, h_row0, phase);
-    return efk_ffn_tc(ctx, st, x, y, tab, h_row0, phase);
+int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase) {
+#ifdef EF_DIAG
+    if (ctx->debug_simt) return efk_ffn_simt(ctx, st, x, y, tab, phase);     // bring-up aid, diag library only (ef_diag.h)
+#endif
+    return efk_ffn_tc(ctx, st, x, y, tab, phase);
 }
 
 extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visit, int32_t layer, const void* x_perm,
@@ -513,8 +608,11 @@ extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visi
     if (visit < 0 || (int32_t)(visit % c.n_layers) != layer)
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_expert_ffn_grouped: visit %% n_layers must equal layer");
     if (!counts_host) {
+        if (!ctx->counts_mirror) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_expert_ffn_grouped: counts_host is NULL and no ef_permute has run");
         EF_CUDA(ctx, cudaEventSynchronize(ctx->counts_event));   // the one device->host sync per visit
-        counts_host = ctx->counts_pinned;
+        counts_host = ctx->counts_mirror;
+        if (ctx->counts_pinned[c.n_experts])
+            return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_expert_ffn_grouped: the last ef_permute saw top-k indices outside [0, n_experts)");
     }
     const int E = c.n_experts;
     std::vector<int32_t> off(E + 1, 0);
@@ -524,8 +622,7 @@ extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visi
     }
     if ((int64_t)off[E] > (int64_t)c.max_tokens * c.top_k)
         return ef_fail(ctx, EF_ERR_CAPACITY, "ef_expert_ffn_grouped: sum(counts) > max_tokens * top_k");
-    ctx->last_compute = st;
-    ctx->has_last_compute = true;
+    EF_ENTER_LAYER(ctx, st);
 
     // lookup (R6)
     std::vector<int> hits, misses;
@@ -619,8 +716,7 @@ extern "C" int32_t ef_expert_ffn_grouped_resident(ef_ctx* ctx, void* stream, con
             return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_expert_ffn_grouped_resident: bad group %d", i);
         items.push_back(WaveItem{row_begin[i], rows[i], slots[i]});
     }
-    ctx->last_compute = st;
-    ctx->has_last_compute = true;
+    EF_ENTER_LAYER(ctx, st);
     return run_wave(ctx, st, x_perm, y_perm, items);
 }
 
@@ -632,17 +728,17 @@ extern "C" int32_t ef_shared_ffn(ef_ctx* ctx, void* stream, int32_t layer, const
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_shared_ffn: bad argument");
     if (T > c.max_tokens) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_shared_ffn: T > max_tokens");
     if (T == 0) return EF_OK;
-    EfGroupTable tab;
-    int32_t h_row0[EF_MAX_GROUPS];
+    EfWaveTable tab;
     if (c.n_shared > EF_MAX_GROUPS) return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_shared_ffn: too many shared experts");
     tab.n = c.n_shared;
     for (int s = 0; s < c.n_shared; ++s) {
         if (!ctx->shared_registered[(size_t)layer * c.n_shared + s])
             return ef_fail(ctx, EF_ERR_NOT_REGISTERED, "shared expert %d of layer %d not registered", s, layer);
-        tab.g[s] = EfGroup{0, s * T, T, c.n_slots + layer * c.n_shared + s};
-        h_row0[s] = c.max_tokens * c.top_k + s * c.max_tokens;   // shared region of the h workspace
+        // every token goes through every shared expert; their h rows live behind the routed region of the workspace
+        tab.g[s] = EfWaveGroup{0, c.max_tokens * c.top_k + s * c.max_tokens, s * T, T, c.n_slots + layer * c.n_shared + s};
     }
-    return efk_ffn_grouped(ctx, (cudaStream_t)stream, x, y_shared, tab, h_row0, 3);
+    EF_ENTER_LAYER(ctx, (cudaStream_t)stream);
+    return efk_ffn_grouped(ctx, (cudaStream_t)stream, x, y_shared, tab, 3);
 }
 
 extern "C" int32_t ef_cache_prefetch(ef_ctx* ctx, int64_t visit_now, const uint8_t* predicted, int32_t n_ahead) {
@@ -707,6 +803,7 @@ extern "C" int32_t ef_token_schedule(ef_ctx* ctx, void* stream, const uint8_t* p
         return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_token_schedule: need even N >= 2, distinct centroids in [0, N), max_iter >= 1");
     if (N > EF_TS_MAX_TOKENS || LE > 32767 || max_iter > 64)
         return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_token_schedule: N <= %d, LE <= 32767, max_iter <= 64", EF_TS_MAX_TOKENS);
+    EF_ENTER_SCHED(ctx, (cudaStream_t)stream);
     return efk_token_schedule(ctx, (cudaStream_t)stream, paths, N, LE, c0, c1, max_iter, batch_of, perm, info, batch_paths);
 }
 
@@ -718,13 +815,8 @@ extern "C" int32_t ef_reindex_rows(ef_ctx* ctx, void* stream, const void* src, c
     if ((row_bytes & 15) || ((uintptr_t)src & 15) || ((uintptr_t)dst & 15) || row_bytes / 16 > INT32_MAX)
         return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_reindex_rows: rows must be multiples of 16 bytes, 16-byte aligned");
     if (n_rows == 0 || row_bytes == 0) return EF_OK;
+    EF_ENTER_SCHED(ctx, (cudaStream_t)stream);
     return efk_reindex_rows(ctx, (cudaStream_t)stream, src, perm, n_rows, row_bytes, dst);
-}
-
-extern "C" int32_t ef_set_token_sched_path(ef_ctx* ctx, int32_t force_multi_kernel) {
-    EF_CHECK_CTX(ctx);
-    ctx->ts_force_multi = force_multi_kernel ? 1 : 0;
-    return EF_OK;
 }
 
 extern "C" int32_t ef_path_hamming(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE,
@@ -734,6 +826,7 @@ extern "C" int32_t ef_path_hamming(ef_ctx* ctx, void* stream, const uint8_t* pat
     if (N > EF_TS_MAX_TOKENS || LE > 32767 || ((uintptr_t)dist_out & 15))
         return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_path_hamming: N <= %d, LE <= 32767, dist_out 16-byte aligned", EF_TS_MAX_TOKENS);
     if (N == 0) return EF_OK;
+    EF_ENTER_SCHED(ctx, (cudaStream_t)stream);
     return efk_path_hamming(ctx, (cudaStream_t)stream, paths, N, LE, dist_out);
 }
 
@@ -788,12 +881,6 @@ extern "C" const char* ef_last_error(ef_ctx* ctx) { return ctx ? ctx->err.c_str(
 
 extern "C" int64_t ef_launch_count(ef_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
-extern "C" int32_t ef_set_debug_simt_ffn(ef_ctx* ctx, int32_t on) {
-    EF_CHECK_CTX(ctx);
-    ctx->debug_simt = on ? 1 : 0;
-    return EF_OK;
-}
-
 extern "C" int32_t ef_set_cache_policy(ef_ctx* ctx, int32_t policy) {
     EF_CHECK_CTX(ctx);
     if (policy != EF_POLICY_PLEC && policy != EF_POLICY_LRU && policy != EF_POLICY_LAYER_LRU)
@@ -806,51 +893,50 @@ extern "C" int32_t ef_set_cache_policy(ef_ctx* ctx, int32_t policy) {
     return EF_OK;
 }
 
-extern "C" int32_t ef_set_wave_bytes(ef_ctx* ctx, int64_t bytes) {
+extern "C" int32_t ef_set_option(ef_ctx* ctx, int32_t key, int64_t value) {
     EF_CHECK_CTX(ctx);
-    if (bytes < 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_wave_bytes: negative");
-    ctx->wave_bytes = bytes;
-    return EF_OK;
+    switch (key) {
+        case EF_OPT_SPLITK:
+            if (value < 0 || value > 16) return ef_fail(ctx, EF_ERR_INVALID_ARG, "EF_OPT_SPLITK: 0 (auto), 1 (off) or 2..16");
+            ctx->splitk_mode = (int32_t)value;
+            return EF_OK;
+        case EF_OPT_WAVE_BYTES:
+            if (value < 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "EF_OPT_WAVE_BYTES: negative");
+            ctx->wave_bytes = value;
+            return EF_OK;
+        case EF_OPT_CHUNK_MIN_BYTES:
+            if (value < 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "EF_OPT_CHUNK_MIN_BYTES: negative");
+            ctx->chunk_min_bytes = value;
+            return EF_OK;
+        case EF_OPT_FUSED_WAVES:
+            ctx->fused_waves = value ? 1 : 0;
+            return EF_OK;
+        case EF_OPT_TOKEN_SCHED_PATH:
+            ctx->ts_force_multi = value ? 1 : 0;
+            return EF_OK;
+        case EF_OPT_COPY_ORDER:
+            if (value != 0 && value != 1) return ef_fail(ctx, EF_ERR_INVALID_ARG, "EF_OPT_COPY_ORDER: 0 (policy order) or 1 (most rows first)");
+            ctx->copy_order = (int32_t)value;
+            return EF_OK;
+        default:
+            return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_option: unknown key %d", key);
+    }
 }
 
-extern "C" int32_t ef_set_chunk_min_bytes(ef_ctx* ctx, int64_t bytes) {
-    EF_CHECK_CTX(ctx);
-    if (bytes < 0) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_chunk_min_bytes: negative");
-    ctx->chunk_min_bytes = bytes;
-    return EF_OK;
-}
-
-extern "C" int32_t ef_set_splitk(ef_ctx* ctx, int32_t mode) {
-    EF_CHECK_CTX(ctx);
-    if (mode < 0 || mode > 16) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_set_splitk: mode must be 0 (auto), 1 (off) or 2..16");
-    ctx->splitk_mode = mode;
-    return EF_OK;
-}
-
-// Debug builds (-DEF_KPROF) only: per-CTA {total, wait ticket, wait TMEM, wait TMA, units} cycles of the MMA-issuing lane for
-// the last GEMM1 (which = 1) or GEMM2 (which = 2) launch.  out: HOST int64[n_sms * 5].  Synchronous.
-extern "C" int32_t ef_debug_kprof(ef_ctx* ctx, int32_t which, int64_t* out) {
-    EF_CHECK_CTX(ctx);
-#ifdef EF_KPROF
-    if (!out || (which != 1 && which != 2)) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_debug_kprof: bad argument");
-    const size_t bytes = sizeof(long long) * 5 * (size_t)ctx->n_sms;
-    for (long long** p : {&ctx->kprof1, &ctx->kprof2})
-        if (!*p) { EF_CUDA(ctx, cudaMalloc(p, bytes)); EF_CUDA(ctx, cudaMemset(*p, 0, bytes)); }
-    EF_CUDA(ctx, cudaDeviceSynchronize());
-    EF_CUDA(ctx, cudaMemcpy(out, which == 1 ? ctx->kprof1 : ctx->kprof2, bytes, cudaMemcpyDeviceToHost));
-    return EF_OK;
-#else
-    (void)which; (void)out;
-    return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_debug_kprof: library built without -DEF_KPROF");
-#endif
-}
-
+// wait for the recorded launch spans, fold them into the totals and the per-launch log, recycle their events
 static void drain_kernel_spans(ef_ctx* ctx) {
     for (auto& k : ctx->kspans) {
         cudaEventSynchronize(k.e1);
         float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, k.e0, k.e1) == cudaSuccess) (k.which == 1 ? ctx->ktimes.gemm1_ms : ctx->ktimes.gemm2_ms) += ms;
-        cudaEventDestroy(k.e0); cudaEventDestroy(k.e1);
+        if (cudaEventElapsedTime(&ms, k.e0, k.e1) == cudaSuccess) {
+            ef_kernel_times& t = ctx->ktimes;
+            if (k.which == 1) { t.gemm1_ms += ms; t.gemm1_launches++; t.gemm1_rows += k.rows; t.gemm1_groups += k.groups; }
+            else if (k.which == 2) { t.gemm2_ms += ms; t.gemm2_launches++; t.gemm2_rows += k.rows; t.gemm2_groups += k.groups; }
+            else { t.wave_ms += ms; t.wave_launches++; t.wave_rows += k.rows; t.wave_groups += k.groups; }
+            if (ctx->launch_log.size() < 65536) ctx->launch_log.push_back(ef_launch_record{k.which, k.groups, k.rows, ms});
+        }
+        ctx->timing_pool.push_back(k.e0);
+        ctx->timing_pool.push_back(k.e1);
     }
     ctx->kspans.clear();
 }
@@ -867,5 +953,16 @@ extern "C" int32_t ef_get_kernel_times(ef_ctx* ctx, ef_kernel_times* out, int32_
     drain_kernel_spans(ctx);
     *out = ctx->ktimes;
     if (reset) ctx->ktimes = ef_kernel_times();
+    return EF_OK;
+}
+
+extern "C" int32_t ef_get_launch_log(ef_ctx* ctx, ef_launch_record* out, int32_t max_records, int32_t* n_out, int32_t reset) {
+    EF_CHECK_CTX(ctx);
+    if (!n_out || max_records < 0 || (max_records > 0 && !out)) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_get_launch_log: bad argument");
+    drain_kernel_spans(ctx);
+    const int32_t n = (int32_t)std::min<size_t>((size_t)max_records, ctx->launch_log.size());
+    for (int32_t i = 0; i < n; ++i) out[i] = ctx->launch_log[i];
+    *n_out = n;
+    if (reset) ctx->launch_log.clear();
     return EF_OK;
 }

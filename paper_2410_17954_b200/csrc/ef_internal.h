@@ -12,7 +12,8 @@
 #include "ef.h"
 
 #define EF_MAX_GROUPS 64   // groups per grouped-GEMM launch (table travels in kernel params)
-#define EF_SCHED_RING 1024 // per-launch tile-scheduler word pairs (self-resetting; ring keeps in-flight launches apart)
+#define EF_SCHED_WORDS (1 << 20)  // int32 words of per-launch scheduler blocks {tickets, finished CTAs, one "h rows ready"
+                                 // counter per token tile}; self-resetting, carved out of a ring (ffn_tc.cu)
 #define EF_W13_BLOCK 128   // gate/up interleave granularity in the packed expert layout
 
 // ---- packed expert layout (library-defined; the caller never sees it) ----------------------------
@@ -35,16 +36,17 @@ __host__ __device__ inline int64_t ef_tiled_index(int64_t r, int64_t c, int64_t 
     return t * EF_TILE_ROWS * K + kb * h * EF_ROWLET + rr * EF_ROWLET + cc;
 }
 
-struct EfGroup {
-    int32_t a_row0;   // first row of A (x_perm or h)
-    int32_t c_row0;   // first row of the output
-    int32_t rows;     // M of this group (>0)
+// One wave of the grouped FFN: group i applies the expert in arena slot `slot` to `rows` token rows that start at
+// x_row0 in the input, h_row0 in the h workspace and y_row0 in the output.
+struct EfWaveGroup {
+    int32_t x_row0, h_row0, y_row0;
+    int32_t rows;     // M of this group (> 0)
     int32_t slot;     // arena slot holding the expert
 };
 
-struct EfGroupTable {
+struct EfWaveTable {
     int32_t n;
-    EfGroup g[EF_MAX_GROUPS];
+    EfWaveGroup g[EF_MAX_GROUPS];
 };
 
 // One slot's policy state (mirror of DESIGN.md §4; written independently of oracle/cache_sim.py).
@@ -78,7 +80,8 @@ struct ef_ctx {
     int32_t n_arena_slots = 0;
     void* h_ws = nullptr;          // bf16 [h_rows, f]
     int64_t h_rows = 0;
-    int32_t* counts_pinned = nullptr;   // pinned mirror of counts[E]
+    int32_t* counts_pinned = nullptr;   // pinned mirror of counts[E] + one word of permute error flags
+    const int32_t* counts_mirror = nullptr;   // where the last ef_permute mirrored counts (ours or the caller's)
     cudaEvent_t counts_event = nullptr;
     int32_t* permute_ws = nullptr;      // device scratch for ef_permute
     cudaStream_t copy_stream = nullptr;
@@ -86,11 +89,15 @@ struct ef_ctx {
     std::vector<uint32_t> ev_gen;
     int32_t ev_next = 0;
     std::vector<EfPhys> phys;           // [S]
-    cudaStream_t last_compute = nullptr;
+    cudaStream_t last_compute = nullptr;   // stream of the layer path's last call (route .. combine); see ef_enter_stream
     bool has_last_compute = false;
+    cudaStream_t last_sched = nullptr;     // stream of the token-scheduler path's last call
+    bool has_last_sched = false;
     // host pool
     std::vector<void*> host_expert;     // [L*E] packed pinned buffers (owned unless aliased)
     std::vector<char> host_owned;
+    std::vector<int32_t> host_aliases;  // [L*E] how many other experts alias this one's buffer
+    std::vector<int32_t> alias_src;     // [L*E] the owner an aliasing expert points at, else -1
     std::vector<char> shared_registered;  // [L*n_shared]
     // policy
     std::vector<EfSlot> slots;
@@ -101,8 +108,12 @@ struct ef_ctx {
     ef_cache_stats stats{};
     // tensor map over the whole arena as rowlets (2-D: 64 elements x total rowlets); both GEMMs use it
     CUtensorMap tm_w{};
+    CUtensorMap tm_h{};                 // the h workspace [h_rows, f] (fixed for the ctx's life)
+    CUtensorMap tm_x{};                 // the caller's x_perm [rows, d], re-encoded only when pointer or row count change
+    const void* tm_x_ptr = nullptr;
+    int64_t tm_x_rows = 0;
     bool tm_ok = false;
-    int32_t* sched_words = nullptr;     // device, [EF_SCHED_RING][2]
+    int32_t* sched_words = nullptr;     // device, [EF_SCHED_WORDS]
     int32_t sched_next = 0;
     // tail split-K of the grouped GEMM (ffn_tc.cu): fp32 partial slots + per-tile arrival counters
     float* splitk_ws = nullptr;
@@ -114,11 +125,14 @@ struct ef_ctx {
     // copy timing
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> copy_spans;
     float copy_ms = 0.f;
-    // optional per-kernel timing (ef_set_kernel_timing)
+    // optional per-launch timing (ef_set_kernel_timing): one pooled event pair per grouped-FFN launch
     int32_t time_kernels = 0;
-    struct KSpan { cudaEvent_t e0, e1; int which; };   // one grouped-GEMM launch (which = 1: GEMM1, 2: GEMM2)
+    struct KSpan { cudaEvent_t e0, e1; int which; int64_t rows; int32_t groups; };   // which: 1 GEMM1, 2 GEMM2, 3 both (one launch)
     std::vector<KSpan> kspans;
+    std::vector<cudaEvent_t> timing_pool;    // timing-enabled events, recycled by drain_kernel_spans / drain_copy_spans
+    std::vector<ef_launch_record> launch_log;
     ef_kernel_times ktimes{};
+    int32_t fused_waves = 1;            // EF_OPT_FUSED_WAVES: 0 = always two launches per wave (test hook)
     // token scheduler workspace (token_sched.cu): state words, packed paths + membership bits, distance matrix
     void* ts_state = nullptr;
     void* ts_small = nullptr;
@@ -130,9 +144,10 @@ struct ef_ctx {
     // physical scheduling knobs (never part of the policy): see ef_set_wave_bytes / ef_set_chunk_min_bytes
     int64_t wave_bytes = (int64_t)128 << 20;
     int64_t chunk_min_bytes = (int64_t)32 << 20;
+    int32_t copy_order = 1;             // EF_OPT_COPY_ORDER
     // misc
     int64_t launches = 0;
-    int32_t debug_simt = 0;
+    int32_t debug_simt = 0;             // diag builds only (ef_diag.h)
     bool route_smem_set = false;        // route kernel opted in to > 48 KB dynamic smem (E > 176)
     std::string err;
     int32_t sticky = EF_OK;
@@ -160,18 +175,18 @@ int32_t ef_fail(ef_ctx* ctx, int32_t code, const char* fmt, ...);
 int32_t efk_route_topk(ef_ctx* ctx, cudaStream_t st, const void* x, const void* wr, const float* bias,
                        int64_t bias_stride, int T, int renorm, int32_t* idx, float* w, float* logits);
 int32_t efk_permute(ef_ctx* ctx, cudaStream_t st, const int32_t* idx, const void* x, int T, void* x_perm,
-                    int32_t* counts, int32_t* offsets, int32_t* src, int32_t* inv, int32_t* counts_host);
+                    int32_t* counts, int32_t* offsets, int32_t* src, int32_t* inv, int32_t* counts_host, int32_t* err_host);
 int32_t efk_combine(ef_ctx* ctx, cudaStream_t st, const void* y_perm, const int32_t* inv, const float* w, int T,
                     const void* residual, const void* y_shared, void* out);
 int32_t efk_rmsnorm(ef_ctx* ctx, cudaStream_t st, const void* x, int T, float eps, void* out);
 
-// Grouped SwiGLU FFN over arena slots: x rows -> h workspace -> y rows.  tab.g[i] = {x_row0, y_row0, rows, slot};
-// h rows are placed at h_row0 + (x_row0 - tab.g[0].x_row0 is NOT assumed): h row of group i = h_row_of[i].
-// phase: bit 0 = launch GEMM1 (x -> h), bit 1 = launch GEMM2 (h -> y); 3 = both, back to back.
-int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& x_to_y,
-                        const int32_t* h_row0 /*[n]*/, int phase);
-int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                     const int32_t* h_row0, int phase);
+// Grouped FFN over arena slots: x rows -> h workspace -> y rows, one wave.
+// phase: bit 0 = GEMM1 (x -> h), bit 1 = GEMM2 (h -> y); 3 = both in ONE launch (ffn_tc.cu).
+int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase);
+#ifdef EF_DIAG
+int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase);
+#endif
+int32_t efk_timing_events(ef_ctx* ctx, cudaEvent_t* e0, cudaEvent_t* e1);   // a pooled pair of timing-enabled events
 int32_t efk_token_schedule(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, int c0, int c1,
                            int max_iter, int32_t* batch_of, int32_t* perm, int32_t* info, uint8_t* batch_paths);
 int32_t efk_reindex_rows(ef_ctx* ctx, cudaStream_t st, const void* src, const int32_t* perm, int n_rows, int64_t row_bytes,
@@ -179,5 +194,4 @@ int32_t efk_reindex_rows(ef_ctx* ctx, cudaStream_t st, const void* src, const in
 int32_t efk_path_hamming(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, uint16_t* dist_out);
 void efk_token_sched_free(ef_ctx* ctx);
 int32_t efk_ffn_tc_init(ef_ctx* ctx);   // build arena tensor maps, set smem attributes
-int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                   const int32_t* h_row0, int phase);
+int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase);

@@ -1,4 +1,4 @@
-// Plain-FMA grouped SwiGLU FFN.  BRING-UP AID ONLY (ef_set_debug_simt_ffn): a second, simple CUDA
+// Plain-FMA grouped SwiGLU FFN.  BRING-UP AID ONLY, libef_diag only (ef_diag_set_simt_ffn): a second, simple CUDA
 // implementation of a4 used to triangulate the tcgen05 kernels on the device.  Not the product path,
 // never selected automatically.  Reads the same packed expert layout (ef_internal.h).
 #include <cuda_bf16.h>
@@ -11,7 +11,10 @@ constexpr int TM = 64, TN = 64, TK = 16;
 
 __device__ __forceinline__ float bf2f(uint16_t b) { return __uint_as_float(((uint32_t)b) << 16); }
 
-__device__ __forceinline__ bool find_tile(const EfGroupTable& tab, int tile, int& g, int& mt) {
+struct SimtGroup { int32_t a_row0, c_row0, rows, slot; };
+struct SimtTable { int32_t n; SimtGroup g[EF_MAX_GROUPS]; };
+
+__device__ __forceinline__ bool find_tile(const SimtTable& tab, int tile, int& g, int& mt) {
     for (int i = 0; i < tab.n; ++i) {
         int nt = (tab.g[i].rows + TM - 1) / TM;
         if (tile < nt) { g = i; mt = tile; return true; }
@@ -24,19 +27,19 @@ __device__ __forceinline__ bool find_tile(const EfGroupTable& tab, int tile, int
 template <int kEpi>     // 0 plain, 1 SwiGLU (packed gate/up rows), 2 ReLU
 __global__ void __launch_bounds__(256)
 simt_gemm_kernel(const uint16_t* __restrict__ a, uint16_t* __restrict__ c, const char* __restrict__ arena, int64_t W,
-                 int64_t b_off_bytes, int K, int N, int b_rows, EfGroupTable tab, EfGroupTable ctab) {
+                 int64_t b_off_bytes, int K, int N, int b_rows, SimtTable tab) {
     constexpr bool kSwiglu = kEpi == 1;
     __shared__ float As[TK][TM + 1];
     __shared__ float B0[TK][TN + 1];
     __shared__ float B1[kSwiglu ? TK : 1][TN + 1];
     int g, mt;
     if (!find_tile(tab, blockIdx.y, g, mt)) return;
-    const EfGroup grp = tab.g[g];
+    const SimtGroup grp = tab.g[g];
     const int rows = grp.rows;
     const int m0 = mt * TM, n0 = blockIdx.x * TN;
     const uint16_t* A = a + (int64_t)grp.a_row0 * K;
     const uint16_t* Bbase = (const uint16_t*)(arena + (int64_t)grp.slot * W + b_off_bytes);
-    uint16_t* C = c + (int64_t)ctab.g[g].c_row0 * N;
+    uint16_t* C = c + (int64_t)grp.c_row0 * N;
     const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
     float acc0[4][4] = {}, acc1[4][4] = {};
     for (int k0 = 0; k0 < K; k0 += TK) {
@@ -94,31 +97,30 @@ simt_gemm_kernel(const uint16_t* __restrict__ a, uint16_t* __restrict__ c, const
 
 }  // namespace
 
-int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                     const int32_t* h_row0, int phase) {
+int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase) {
     const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
     int tiles = 0;
-    EfGroupTable t1 = tab, c1 = tab, t2 = tab, c2 = tab;
+    SimtTable t1, t2;
+    t1.n = t2.n = tab.n;
     for (int i = 0; i < tab.n; ++i) {
         tiles += (tab.g[i].rows + TM - 1) / TM;
-        c1.g[i].c_row0 = h_row0[i];          // GEMM1 writes h rows
-        t2.g[i].a_row0 = h_row0[i];          // GEMM2 reads them
-        c2.g[i].c_row0 = tab.g[i].c_row0;    // ... and writes y rows
+        t1.g[i] = SimtGroup{tab.g[i].x_row0, tab.g[i].h_row0, tab.g[i].rows, tab.g[i].slot};   // GEMM1: x rows -> h rows
+        t2.g[i] = SimtGroup{tab.g[i].h_row0, tab.g[i].y_row0, tab.g[i].rows, tab.g[i].slot};   // GEMM2: h rows -> y rows
     }
     if (tiles == 0) return EF_OK;
     const bool relu = ctx->cfg.expert_kind == 1;
     if (phase & 1) {
         if (relu)
             simt_gemm_kernel<2><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
-                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, f, t1, c1);
+                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, f, t1);
         else
             simt_gemm_kernel<1><<<dim3((f + TN - 1) / TN, tiles), 256, 0, st>>>(
-                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, 2 * f, t1, c1);
+                (const uint16_t*)x, (uint16_t*)ctx->h_ws, ctx->arena, ctx->W, 0, d, f, 2 * f, t1);
         ctx->launches++;
     }
     if (phase & 2) {
         simt_gemm_kernel<0><<<dim3((d + TN - 1) / TN, tiles), 256, 0, st>>>(
-            (const uint16_t*)ctx->h_ws, (uint16_t*)y, ctx->arena, ctx->W, (int64_t)(relu ? 1 : 2) * f * d * 2, f, d, d, t2, c2);
+            (const uint16_t*)ctx->h_ws, (uint16_t*)y, ctx->arena, ctx->W, (int64_t)(relu ? 1 : 2) * f * d * 2, f, d, d, t2);
         ctx->launches++;
     }
     EF_CUDA(ctx, cudaGetLastError());

@@ -1,9 +1,15 @@
-// a4: grouped SwiGLU expert FFN over cache slots -- tcgen05 / TMEM / TMA kernels for sm_100a.
+// a4: grouped SwiGLU expert FFN over cache slots -- tcgen05 / TMEM / TMA kernel for sm_100a.
 //
-// Two launches per wave, both instances of one persistent, warp-specialised grouped GEMM, computed TRANSPOSED
-// ("swap-AB"): the weight rows are the MMA M side (always full 128-lane accumulators), the ragged token rows are
-// the MMA N side, whose granularity is 16 -- so an expert with M_e routed rows costs ceil16(M_e) MMA columns, not
-// a multiple of 128 rows (BASELINE.json cfg 2: 4096 routed rows occupy 4144 MMA columns instead of 4608 rows).
+// ONE launch per wave: a persistent, warp-specialised grouped GEMM that runs BOTH GEMMs of the wave's experts.  Its work
+// list holds the GEMM1 units (x -> h) followed by the GEMM2 units (h -> y); a GEMM2 unit waits -- in its TMA producer
+// only, after the weight box of its first stage is already on its way -- until the GEMM1 units of its own token tile have
+// stored their h columns (one release counter per token tile, bumped once per weight tile).  There is no launch boundary,
+// no ramp and no tail between the two GEMMs: GEMM2 of the experts that finished early overlaps GEMM1 of the rest, h
+// is read back out of L2, and a decode wave streams W13 and Wd as one uninterrupted pass over the expert.
+// Both GEMMs are computed TRANSPOSED ("swap-AB"): the weight rows are the MMA M side (always full 128-lane
+// accumulators), the ragged token rows are the MMA N side, whose granularity is 16 -- so an expert with M_e routed rows
+// costs ceil16(M_e) MMA columns, not a multiple of 128 rows (BASELINE.json cfg 2: 4096 routed rows occupy 4144 MMA columns
+// instead of 4608 rows).
 //   D[w, t] = sum_k W_slot(g)[w, k] . A[t, k]          (bf16 x bf16 -> fp32 in TMEM; lanes = weight rows, columns = tokens)
 //   GEMM1: A = x_perm, W = packed W13 (gate/up interleaved by 128 rows): accumulator 0 = 128 gate rows, accumulator 1 =
 //          the matching 128 up rows, same lanes -> epilogue h = silu(g) * u -> bf16
@@ -30,18 +36,21 @@
 //   warp 2     TMEM allocator    : 512 columns per CTA.  A tile with > 128 tokens takes all of them (accumulators at
 //                                columns 0 and 256); tiles with <= 128 tokens alternate between the two 256-column
 //                                halves (accumulators at +0 and +128), so their epilogue overlaps the next tile's MMAs
+//   warp 3     prologue          : token tiling of the wave's groups into shared memory
 //   warps 4-11 epilogue          : tcgen05.ld 16x256b (the MMA C-fragment layout) -> SwiGLU / cast -> stmatrix.trans
 //                                into a [32 tokens][128 features] staging tile -> 16-byte global stores, 256
 //                                contiguous bytes per token row; warps w and w+4 share a TMEM lane quarter and
 //                                take alternate 32-token chunks; "accumulator free" arrives on the leader's barrier
-// Per-expert tile scheduling over ragged token counts: units are numbered longest-first -- every > 128-token tile
-// of every group (n-major inside a group, so the token tiles that share a weight tile are claimed back to back and
-// hit L2), then the <= 128-token tail tiles -- and claimed dynamically (greedy list scheduling).
-// Tail split-K: with T units on G pairs the last T mod G units (all of them when T < G -- decode, single-expert miss
-// waves) would leave most SMs idle for a whole tile time, so the host splits each of those units s ways along K.
-// A split unit writes its raw fp32 accumulators to a workspace slot, then bumps the tile's arrival counter; the
-// unit that arrives last sums the s partials in split order (deterministic) and runs the normal epilogue.  No
-// CTA ever waits for another cluster.
+// Per-expert tile scheduling over ragged token counts: inside a phase units are numbered longest-first -- every
+// > 128-token tile of every group (n-major inside a group, so the token tiles that share a weight tile are claimed back
+// to back and hit L2) with the <= 128-token tail tiles spread among them -- and claimed dynamically (greedy list
+// scheduling).
+// Tail split-K: with T units on G pairs the last T mod G units of a phase (all of them when T < G -- decode,
+// single-expert miss waves) would leave most SMs idle for a whole tile time, so the host splits each of those units s
+// ways along K.  A split unit writes its raw fp32 accumulators to a workspace slot, then bumps the tile's arrival
+// counter; the unit that arrives last sums the s partials in split order (deterministic) and runs the normal epilogue.
+// No CTA ever waits for another cluster on this path; the only cross-CTA wait is a GEMM2 producer's wait for h rows,
+// whose GEMM1 units were all claimed -- by CTAs that never wait themselves -- before any GEMM2 ticket was handed out.
 #include <cuda_bf16.h>
 
 #include "ef_internal.h"
@@ -85,11 +94,12 @@ struct __align__(8) SmemCtl {
     int32_t sched_tile[kSched];
     uint32_t tmem_base;
     int32_t split_last;                   // epilogue broadcast: this unit arrived last at its split tile
-    int32_t total_long;                   // number of > 128-token tiles (they come first)
-    int32_t gstart_long[EF_MAX_GROUPS + 1];
-    int32_t gstart_short[EF_MAX_GROUPS + 1];
-    int16_t g_tile_rows[EF_MAX_GROUPS];   // token tiling of each group (prologue): rows per tile ...
-    int16_t g_long[EF_MAX_GROUPS];        // ... and number of > 128-token tiles
+    // token tiling of the wave (prologue; the same for both GEMMs): exclusive prefix sums, over the groups, of the number
+    // of > 128-token ("long") tiles and of <= 128-token ("short") tail tiles; a phase multiplies them by its n_pairs_n
+    int32_t tl[EF_MAX_GROUPS + 1];
+    int32_t tsh[EF_MAX_GROUPS + 1];
+    int16_t g_tile_rows[EF_MAX_GROUPS];   // rows per token tile of each group ...
+    int16_t g_long[EF_MAX_GROUPS];        // ... and its number of long tiles
 };
 
 constexpr size_t kSmemBytes = 1024 /*align slack*/ + (size_t)kStages * STAGE_BYTES + 2 * STG_BYTES + sizeof(SmemCtl);
@@ -278,7 +288,26 @@ __device__ __forceinline__ void ws_sum32(const float* tile_slots, int s, int acc
 // barrier among the 8 epilogue warps only
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 
+// ---- one launch = one WAVE: both GEMMs of a set of experts --------------------------------------------------------------
+// Phase 0 ("GEMM1"): A = x rows, W = packed W13 / W1, epilogue SwiGLU / ReLU, C = h workspace.
+// Phase 1 ("GEMM2"): A = h rows, W = Wd,              epilogue plain,          C = y rows.
+// Tickets [0, p0.total) are phase-0 units, [p0.total, p0.total + p1.total) phase-1 units; either total may be 0 (a
+// single-GEMM launch: chunked expert copies gate the two GEMMs of a wave on different events, and the stage tests).
+struct PhaseArgs {
+    uint16_t* C;                   // output rows
+    int32_t ldc, n_cols;           // leading dimension and valid columns of C
+    int32_t KB;                    // k-blocks of 64
+    int32_t n_tiles_n, n_pairs_n;  // 256-row weight tiles of the matrix, CTA pairs per token tile (ceil(n_tiles_n / 2))
+    int32_t w_rows, base_rowlet;   // rows of the weight matrix, its first rowlet inside an arena slot
+    int32_t total;                 // tickets of this phase
+    int32_t n_plain, s;            // tickets [0, n_plain) are whole tiles; the rest are (tile, K part) pairs, part fastest;
+                                   // s = K parts per split tile (>= 2 when any tile is split)
+    float* ws;                     // [n_split_tiles * s * 2] slots of kSlotFloats fp32
+    int32_t* counters;             // [n_split_tiles * 2] arrival counters, zero between launches
+};
+
 struct Tile {
+    int phase;           // 0: GEMM1 unit, 1: GEMM2 unit
     int a_row, c_row;    // first token row in the A tensor / in the output
     int rows_valid;      // tokens of this tile (1..256)
     int n_mma;           // rows_valid rounded up to the MMA N granularity (16)
@@ -286,23 +315,18 @@ struct Tile {
     int n_pair, slot;    // n_pair: the pair's two adjacent weight tiles are 2 * n_pair + cluster rank
     int kb0, kb1;        // k-block range of this unit
     int tail, split_j;   // index among the split tiles (-1: whole tile) and which K part this unit is
+    int tid;             // token-tile id inside the launch: index of the "h rows ready" counter
 };
 
-struct SplitArgs {
-    int32_t n_plain;     // tickets [0, n_plain) are whole tiles; the rest are (tile, K part) pairs, part fastest
-    int32_t s;           // K parts per split tile (>= 2 when any tile is split)
-    float* ws;           // [n_split_tiles * s] slots of kSlotFloats fp32
-    int32_t* counters;   // [n_split_tiles] arrival counters, zero between launches
-};
-
-// number of "long" (129..256-token) tiles of a group; the remainder, if any, is one short tile per n
 // Token tiling of a group.  A tile narrower than ~170 tokens costs as much per k-block as a 170-token one (its 32 KB
-// weight stage has to be filled either way), so with a long K loop a group of 257..4096 rows is cut into
+// weight stage has to be filled either way), so with long K loops a group of 257..4096 rows is cut into
 // ceil(rows / 256) BALANCED tiles of b = ceil16(rows / tiles) rows instead of full 256-row tiles plus a small remainder
 // (593 rows: 208 + 208 + 177, not 256 + 256 + 81): measured +5 % / +3 % on GEMM1 / GEMM2 of the Mixtral shape.  With a
 // short K loop (K < 3072: the many-expert shapes) the fixed cost of one more 129..256-token tile -- its epilogue is not
 // overlapped, it owns all of TMEM -- outweighs that (measured -2 % / -6 %), so those keep 256-row tiles + remainder.
-// Tiles 0 .. n-2 hold b rows, the last one what is left; it is "short" (<= 128 tokens, half of TMEM) or "long".
+// Both GEMMs of a wave use the SAME tiling (balanced iff d and f are both >= 3072), so that a GEMM2 unit depends on
+// exactly one token tile of GEMM1.  Tiles 0 .. n-2 hold b rows, the last one what is left; it is "short" (<= 128
+// tokens, half of TMEM) or "long".
 constexpr int kBalancedMinK = 3072;
 __device__ __host__ __forceinline__ int group_tile_rows(int rows, bool balanced) {
     const int n = (rows + BT - 1) / BT;
@@ -322,27 +346,31 @@ __device__ __host__ __forceinline__ int group_has_short(int rows, bool balanced)
     return (r > 0 && r <= 128) ? 1 : 0;
 }
 
-__device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemCtl* ctl, int unit, const SplitArgs& sp,
-                                            int KB) {
+__device__ __forceinline__ Tile decode_tile(const EfWaveTable& tab, const SmemCtl* ctl, int unit, const PhaseArgs& p0,
+                                            const PhaseArgs& p1) {
     Tile t;
-    int g = 0, row_off;
-    int tile = unit;
-    t.kb0 = 0; t.kb1 = KB; t.tail = -1; t.split_j = 0;
-    if (unit >= sp.n_plain) {
-        const int v = unit - sp.n_plain;
-        t.tail = v / sp.s;
-        t.split_j = v - t.tail * sp.s;
-        tile = sp.n_plain + t.tail;
-        t.kb0 = (t.split_j * KB) / sp.s;
-        t.kb1 = ((t.split_j + 1) * KB) / sp.s;
+    t.phase = unit >= p0.total ? 1 : 0;
+    const PhaseArgs& p = t.phase ? p1 : p0;
+    const int u = unit - (t.phase ? p0.total : 0);
+    int g = 0, j;
+    int tile = u;
+    t.kb0 = 0; t.kb1 = p.KB; t.tail = -1; t.split_j = 0;
+    if (u >= p.n_plain) {
+        const int v = u - p.n_plain;
+        t.tail = v / p.s;
+        t.split_j = v - t.tail * p.s;
+        tile = p.n_plain + t.tail;
+        t.kb0 = (t.split_j * p.KB) / p.s;
+        t.kb1 = ((t.split_j + 1) * p.KB) / p.s;
     }
-    // Ticket order: long (129..256-token) tiles are tensor-bound, short ones are bound by streaming their weight tile,
-    // so a launch with many short tiles (many-expert prefill) spreads them evenly among the long ones -- both kinds
-    // are then in flight on different SMs at the same time -- and keeps only the last `tail_short` short tiles for the
-    // end of the list, where small units even out the finish (and where the split-K tail lives).
-    const int total_short = ctl->gstart_short[tab.n];
-    const int tail_short = min(total_short, (int)gridDim.x);
-    const int spread = total_short - tail_short, first = ctl->total_long + spread;
+    // Ticket order inside a phase: long (129..256-token) tiles are tensor-bound, short ones are bound by streaming their
+    // weight tile, so a launch with many short tiles (many-expert prefill) spreads them evenly among the long ones --
+    // both kinds are then in flight on different SMs at the same time -- and keeps only the last `tail_short` short
+    // tiles for the end of the list, where small units even out the finish (and where the split-K tail lives).
+    const int npn = p.n_pairs_n;
+    const int total_long = ctl->tl[tab.n] * npn, total_short = ctl->tsh[tab.n] * npn;
+    const int tail_short = min(total_short, (int)gridDim.x / 4);
+    const int spread = total_short - tail_short, first = total_long + spread;
     bool is_short;
     if (tile >= first) {
         is_short = true;
@@ -353,39 +381,171 @@ __device__ __forceinline__ Tile decode_tile(const EfGroupTable& tab, const SmemC
         tile = is_short ? sb : tile - sb;
     }
     if (!is_short) {
-        while (tile >= ctl->gstart_long[g + 1]) ++g;
-        const int local = tile - ctl->gstart_long[g];
+        while (tile >= ctl->tl[g + 1] * npn) ++g;
+        const int local = tile - ctl->tl[g] * npn;
         const int nl = ctl->g_long[g];
-        t.n_pair = local / nl;
-        row_off = (local - t.n_pair * nl) * ctl->g_tile_rows[g];
+        t.n_pair = local / nl;                  // n-major inside a group: the token tiles that share a weight tile are
+        j = local - t.n_pair * nl;              // claimed back to back and hit L2
         t.is_long = 1;
     } else {
-        const int ts = tile;
-        while (ts >= ctl->gstart_short[g + 1]) ++g;
-        t.n_pair = ts - ctl->gstart_short[g];
-        row_off = ctl->g_long[g] * ctl->g_tile_rows[g];
+        while (tile >= ctl->tsh[g + 1] * npn) ++g;
+        t.n_pair = tile - ctl->tsh[g] * npn;
+        j = ctl->g_long[g];
         t.is_long = 0;
     }
+    const int row_off = j * ctl->g_tile_rows[g];
+    t.tid = ctl->tl[g] + ctl->tsh[g] + j;
     t.rows_valid = min(tab.g[g].rows - row_off, (int)ctl->g_tile_rows[g]);
     t.n_mma = (t.rows_valid + 15) & ~15;
-    t.a_row = tab.g[g].a_row0 + row_off;
-    t.c_row = tab.g[g].c_row0 + row_off;
+    t.a_row = (t.phase ? tab.g[g].h_row0 : tab.g[g].x_row0) + row_off;
+    t.c_row = (t.phase ? tab.g[g].y_row0 : tab.g[g].h_row0) + row_off;
     t.slot = tab.g[g].slot;
     return t;
 }
 
-// kSwiglu: accumulator 0 = 128 gate rows, accumulator 1 = the matching up rows -> 128 output columns per weight tile;
-// else accumulators 0 / 1 = output columns [256 n, +128) / [256 n + 128, +128).  n_tiles_n = weight tiles, n_pairs_n =
-// ceil(n_tiles_n / 2) (an odd last tile leaves the peer CTA multiplying zero-filled rows).
-template <int kEpi>     // 0: plain (GEMM2), 1: SwiGLU (gated GEMM1), 2: ReLU (non-gated GEMM1 of Switch-style experts, R30)
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
-ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmW,
-                uint16_t* __restrict__ C, int ldc, int n_cols, int K, int n_tiles_n, int n_pairs_n, int total_tiles,
-                int w_rows, int slot_rowlets, int base_rowlet,
-                int32_t* __restrict__ sched, const SplitArgs sp, long long* __restrict__ kprof,
-                const __grid_constant__ EfGroupTable tab) {
+// "h rows of token tile tid are complete": GEMM1 units add 1 per weight tile stored, GEMM2 producers wait for all of them.
+__device__ __forceinline__ void signal_ready(int32_t* cnt) {
+    asm volatile("fence.proxy.async;" ::: "memory");
+    asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(cnt) : "memory");
+}
+__device__ __forceinline__ void wait_ready(const int32_t* cnt, int need) {
+    int v = 0;
+    for (long long spins = 0; spins < (1ll << 25); ++spins) {       // bounded (~ seconds): a lost signal traps, never hangs
+        asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(cnt) : "memory");
+        if (v >= need) break;
+        __nanosleep(100);
+    }
+    if (v < need) __trap();
+    asm volatile("fence.proxy.async;" ::: "memory");                // the rows were written through the generic proxy; TMA reads them
+}
+
+// Epilogue of one unit for the 8 epilogue warps of one CTA.  kEpi: 0 plain (GEMM2), 1 SwiGLU (gated GEMM1: accumulator 0
+// = 128 gate rows, accumulator 1 = the matching up rows -> 128 output columns per weight tile), 2 ReLU (non-gated GEMM1
+// of Switch-style experts, R30); for 0 and 2 accumulators 0 / 1 = output columns [256 n, +128) / [256 n + 128, +128).
+template <int kEpi>
+__device__ __forceinline__ void epilogue_unit(const Tile& t, const PhaseArgs& p, SmemCtl* ctl, uint8_t* stg_base, uint32_t tmem_base,
+                                              uint32_t rank, int warp, int lane, int b0, int nb, int32_t* ready, bool do_signal) {
     constexpr bool kSwiglu = kEpi == 1;
     constexpr bool kRelu = kEpi == 2;
+    const int q = warp & 3;
+    const int part = (warp - 4) >> 2;
+    const int lane128 = q * 32 + lane;            // accumulator lane = weight row inside the 128-row block
+    const int n_tile = 2 * t.n_pair + (int)rank;
+    const bool tile_ok = n_tile < p.n_tiles_n;    // false: the odd last weight tile's idle partner
+    const bool split = t.tail >= 0;
+    float* ws_mine = split ? p.ws + (((size_t)t.tail * p.s + t.split_j) * 2 + rank) * kSlotFloats : nullptr;
+    uint16_t* __restrict__ C = p.C;
+    const int ldc = p.ldc, n_cols = p.n_cols;
+    const uint32_t tb0 = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b0 * 256);
+    const uint32_t tb1 = tb0 + (t.is_long ? 256u : 128u);
+    const int n_chunks = tile_ok ? (t.rows_valid + 31) >> 5 : 0;
+    const int col0 = kSwiglu ? n_tile * ACC_M : n_tile * BW;      // first output column of accumulator 0
+    uint8_t* stg = stg_base + part * STG_BYTES;
+    // stmatrix row address of this thread: block i = lane / 8 (tokens 8i..8i+7), row lane % 8, + feature offset
+    const uint32_t st_row = smem_u32(stg) + (uint32_t)(lane * STG_LD + q * 64);
+#pragma unroll 1
+    for (int c = part; c < n_chunks; c += 2) {
+        const int n_rows = min(32, t.rows_valid - c * 32);
+        if (split) {
+            uint32_t a0[32];
+            tc_ld32(tb0 + c * 32, a0);
+            tc_wait_ld();
+            ws_store32(ws_mine, 0, c, lane128, a0);
+            tc_ld32(tb1 + c * 32, a0);
+            tc_wait_ld();
+            ws_store32(ws_mine, 1, c, lane128, a0);
+            continue;
+        }
+#pragma unroll 1
+        for (int acc = 0; acc < (kSwiglu ? 1 : 2); ++acc) {
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+                const uint32_t lane_off = (uint32_t)(hh * 16) << 16;
+                uint32_t r[8];
+                if (kSwiglu) {
+                    uint32_t g[16], u[16];
+                    tc_ld16x256b_x4(tb0 + lane_off + c * 32, g);
+                    tc_ld16x256b_x4(tb1 + lane_off + c * 32, u);
+                    tc_wait_ld();
+#pragma unroll
+                    for (int i = 0; i < 8; ++i)
+                        r[i] = pack_bf16(silu_mul(__uint_as_float(g[2 * i]), __uint_as_float(u[2 * i])),
+                                         silu_mul(__uint_as_float(g[2 * i + 1]), __uint_as_float(u[2 * i + 1])));
+                } else {
+                    uint32_t v[16];
+                    tc_ld16x256b_x4((acc ? tb1 : tb0) + lane_off + c * 32, v);
+                    tc_wait_ld();
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        float lo = __uint_as_float(v[2 * i]), hi = __uint_as_float(v[2 * i + 1]);
+                        if (kRelu) { lo = fmaxf(lo, 0.f); hi = fmaxf(hi, 0.f); }
+                        r[i] = pack_bf16(lo, hi);
+                    }
+                }
+                // r[2j] = lanes 0-7 of this half, r[2j+1] = lanes 8-15; token block j
+                stmatrix_x4_trans(st_row + hh * 32, r[0], r[2], r[4], r[6]);
+                stmatrix_x4_trans(st_row + hh * 32 + 16, r[1], r[3], r[5], r[7]);
+            }
+            stage_to_global(stg, C, ldc, (int64_t)t.c_row + c * 32, n_rows, col0 + acc * ACC_M, n_cols, lane128, 2 + part);
+        }
+    }
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0)
+        for (int h = 0; h < nb; ++h) mbar_arrive_remote(mapa(&ctl->tmem_empty[b0 + h], 0));
+    bool stored = !split && tile_ok;              // this CTA has written its part of the output tile
+    if (split && tile_ok) {
+        // publish the partial, count arrivals; the last unit of the tile reduces all s partials in split order
+        __threadfence();
+        epi_bar();
+        if (threadIdx.x == 4 * 32) {
+            int32_t* cnt = p.counters + t.tail * 2 + rank;
+            const int old = atomicAdd(cnt, 1);
+            const int last = (old == p.s - 1) ? 1 : 0;
+            if (last) *cnt = 0;                          // re-arm for the next launch
+            ctl->split_last = last;
+        }
+        epi_bar();
+        const bool last = ctl->split_last != 0;          // rewritten only after the next split unit's first barrier
+        if (last) {
+            __threadfence();
+            const float* ws_tile = p.ws + ((size_t)t.tail * p.s * 2 + rank) * kSlotFloats;
+#pragma unroll 1
+            for (int c = part; c < n_chunks; c += 2) {
+                const int n_rows = min(32, t.rows_valid - c * 32);
+                uint32_t a0[32], a1[32];
+                ws_sum32(ws_tile, p.s, 0, c, lane128, a0);
+                ws_sum32(ws_tile, p.s, 1, c, lane128, a1);
+                uint16_t* srow = reinterpret_cast<uint16_t*>(stg) + lane128;       // [token][feature], 2-byte stores
+#pragma unroll 1
+                for (int acc = 0; acc < (kSwiglu ? 1 : 2); ++acc) {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        float v = kSwiglu ? silu_mul(__uint_as_float(a0[i]), __uint_as_float(a1[i]))
+                                          : __uint_as_float(acc ? a1[i] : a0[i]);
+                        if (kRelu) v = fmaxf(v, 0.f);
+                        srow[i * (STG_LD / 2)] = bf16_bits(v);
+                    }
+                    stage_to_global(stg, C, ldc, (int64_t)t.c_row + c * 32, n_rows, col0 + acc * ACC_M, n_cols, lane128, 2 + part);
+                }
+            }
+            stored = true;
+        }
+    }
+    // GEMM1 of a fused wave: tell the GEMM2 units of this token tile that one more weight tile's h columns are in place
+    if (do_signal && stored) {
+        __threadfence();
+        epi_bar();
+        if (threadIdx.x == 4 * 32) signal_ready(ready + t.tid);
+    }
+}
+
+template <bool kReluExperts>     // false: SwiGLU experts (gated GEMM1); true: Switch-style ReLU experts
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmH,
+                const __grid_constant__ CUtensorMap tmW, const PhaseArgs p0, const PhaseArgs p1, int slot_rowlets,
+                int balanced, int n_token_tiles, int32_t* __restrict__ sched /* {tickets, finished CTAs, ready[n_token_tiles]} */,
+                long long* __restrict__ kprof, const __grid_constant__ EfWaveTable tab) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t* stg_base = smem + (size_t)kStages * STAGE_BYTES;
@@ -393,9 +553,14 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
     const bool leader = rank == 0;
+    const int total_tiles = p0.total + p1.total;
+    int32_t* ready = sched + 2;
+    // a GEMM2 unit waits for the h columns of all real weight tiles of GEMM1 (only when GEMM1 runs in this launch)
+    const int ready_need = (p0.total > 0 && p1.total > 0) ? p0.n_tiles_n : 0;
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmX) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmH) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmW) : "memory");
     }
     if (warp == 1 && lane == 0) {
@@ -412,30 +577,27 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
         // per-group token tiling (lanes in parallel), then the exclusive scans of the tile counts (one lane)
         for (int g = lane; g < tab.n; g += 32) {
             const int rows = tab.g[g].rows;
-            const bool bal = K >= kBalancedMinK;
-            const int nlg = group_long_tiles(rows, bal);
-            ctl->g_tile_rows[g] = (int16_t)group_tile_rows(rows, bal);
+            const int nlg = group_long_tiles(rows, balanced != 0);
+            ctl->g_tile_rows[g] = (int16_t)group_tile_rows(rows, balanced != 0);
             ctl->g_long[g] = (int16_t)nlg;
-            ctl->gstart_long[g + 1] = nlg * n_pairs_n;
-            ctl->gstart_short[g + 1] = group_has_short(rows, bal) * n_pairs_n;
+            ctl->tl[g + 1] = nlg;
+            ctl->tsh[g + 1] = group_has_short(rows, balanced != 0);
         }
         __syncwarp();
         if (lane == 0) {
             int nl = 0, ns = 0;
-            ctl->gstart_long[0] = 0;
-            ctl->gstart_short[0] = 0;
+            ctl->tl[0] = 0;
+            ctl->tsh[0] = 0;
             for (int g = 1; g <= tab.n; ++g) {
-                nl += ctl->gstart_long[g];  ctl->gstart_long[g] = nl;
-                ns += ctl->gstart_short[g]; ctl->gstart_short[g] = ns;
+                nl += ctl->tl[g];  ctl->tl[g] = nl;
+                ns += ctl->tsh[g]; ctl->tsh[g] = ns;
             }
-            ctl->total_long = nl;
         }
     }
     tc_fence_before();
     cluster_sync();               // barriers of both CTAs are initialised before any remote arrive / multicast commit
     tc_fence_after();
     const uint32_t tmem_base = ctl->tmem_base;
-    const int KB = K / BK;
 
     if (warp == 0) {
         // ===== tile scheduler (leader) + TMA producer (both) =====
@@ -457,25 +619,34 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                     mbar_arrive_remote(mapa(&ctl->sched_empty[ss], 0));
                 }
                 if (tile >= total_tiles) break;
-                const Tile t = decode_tile(tab, ctl, tile, sp, KB);
+                const Tile t = decode_tile(tab, ctl, tile, p0, p1);
+                const PhaseArgs& p = t.phase ? p1 : p0;
+                const CUtensorMap* tmA = t.phase ? &tmH : &tmX;
                 const int half = t.n_mma >> 1;                               // token rows this CTA stages
                 const int n_box = (half + XBOX - 1) / XBOX;
                 const uint32_t bytes = (uint32_t)(W_BYTES + n_box * XBOX_BYTES);
                 // weight tile -> rowlet coordinates in the arena (tiled layout, ef_internal.h): a k-block of the tile is
                 // h_t contiguous rowlets.  The odd last pair's idle partner re-reads tile 0 (its lanes are never stored);
                 // a short last tile's box runs on into the next k-block's rowlets (lanes >= h_t, never stored either)
-                const int w_tile = (2 * t.n_pair + (int)rank) < n_tiles_n ? 2 * t.n_pair + (int)rank : 0;
-                const int h_t = min(BW, w_rows - w_tile * BW);
-                const int w_rowlet0 = t.slot * slot_rowlets + base_rowlet + w_tile * BW * KB;
+                const int w_tile = (2 * t.n_pair + (int)rank) < p.n_tiles_n ? 2 * t.n_pair + (int)rank : 0;
+                const int h_t = min(BW, p.w_rows - w_tile * BW);
+                const int w_rowlet0 = t.slot * slot_rowlets + p.base_rowlet + w_tile * BW * p.KB;
                 const int x_row = t.a_row + (int)rank * half;
+                bool must_wait = t.phase == 1 && ready_need > 0;
                 for (int kb = t.kb0; kb < t.kb1; ++kb) {
                     mbar_wait(&ctl->empty[stage], phase ^ 1);
                     uint8_t* sw = smem + (size_t)stage * STAGE_BYTES;
                     if (leader) mbar_expect_tx(&ctl->full[stage], 2 * bytes);  // both CTAs' boxes land on this barrier
                     const uint32_t bar = mapa(&ctl->full[stage], 0);
                     tma_load_2d(sw, &tmW, bar, 0, w_rowlet0 + kb * h_t);
+                    if (must_wait) {
+                        // the weights do not depend on GEMM1: their box is already on its way while this lane waits for
+                        // the h rows of its token tile (written by the GEMM1 units of this same launch)
+                        wait_ready(ready + t.tid, ready_need);
+                        must_wait = false;
+                    }
                     for (int j = 0; j < n_box; ++j)
-                        tma_load_2d(sw + W_BYTES + j * XBOX_BYTES, &tmX, bar, kb * BK, x_row + j * XBOX);
+                        tma_load_2d(sw + W_BYTES + j * XBOX_BYTES, tmA, bar, kb * BK, x_row + j * XBOX);
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
@@ -495,7 +666,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                 mbar_arrive(&ctl->sched_empty[ss]);
                 if (tile >= total_tiles) break;
                 KPROF(++kp_units;)
-                const Tile t = decode_tile(tab, ctl, tile, sp, KB);
+                const Tile t = decode_tile(tab, ctl, tile, p0, p1);
                 const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
                 KPROF(long long kp_b = clock64();)
                 for (int h = 0; h < nb; ++h) mbar_wait_cluster(&ctl->tmem_empty[b0 + h], ((bphase >> (b0 + h)) & 1u) ^ 1u);
@@ -534,9 +705,6 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
         }
     } else if (warp >= 4) {
         // ===== epilogue: warps w and w+4 share TMEM lane quarter (w % 4) and take alternate 32-token chunks =====
-        const int q = warp & 3;
-        const int part = (warp - 4) >> 2;
-        const int lane128 = q * 32 + lane;            // accumulator lane = weight row inside the 128-row block
         int buf = 0; uint32_t bphase = 0;
         for (int it = 0;; ++it) {
             const int ss = it % kSched;
@@ -545,112 +713,18 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
             __syncwarp();
             if (lane == 0) mbar_arrive_remote(mapa(&ctl->sched_empty[ss], 0));
             if (tile >= total_tiles) break;
-            const Tile t = decode_tile(tab, ctl, tile, sp, KB);
-            const int n_tile = 2 * t.n_pair + (int)rank;
-            const bool tile_ok = n_tile < n_tiles_n;   // false: the odd last weight tile's idle partner
+            const Tile t = decode_tile(tab, ctl, tile, p0, p1);
             const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
-            const bool split = t.tail >= 0;
-            float* ws_mine = split ? sp.ws + (((size_t)t.tail * sp.s + t.split_j) * 2 + rank) * kSlotFloats : nullptr;
             for (int h = 0; h < nb; ++h) {
                 mbar_wait(&ctl->tmem_full[b0 + h], (bphase >> (b0 + h)) & 1u);
                 bphase ^= 1u << (b0 + h);
             }
             tc_fence_after();
-            const uint32_t tb0 = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b0 * 256);
-            const uint32_t tb1 = tb0 + (t.is_long ? 256u : 128u);
-            const int n_chunks = tile_ok ? (t.rows_valid + 31) >> 5 : 0;
-            const int col0 = kSwiglu ? n_tile * ACC_M : n_tile * BW;      // first output column of accumulator 0
-            uint8_t* stg = stg_base + part * STG_BYTES;
-            // stmatrix row address of this thread: block i = lane / 8 (tokens 8i..8i+7), row lane % 8, + feature offset
-            const uint32_t st_row = smem_u32(stg) + (uint32_t)(lane * STG_LD + q * 64);
-#pragma unroll 1
-            for (int c = part; c < n_chunks; c += 2) {
-                const int n_rows = min(32, t.rows_valid - c * 32);
-                if (split) {
-                    uint32_t a0[32];
-                    tc_ld32(tb0 + c * 32, a0);
-                    tc_wait_ld();
-                    ws_store32(ws_mine, 0, c, lane128, a0);
-                    tc_ld32(tb1 + c * 32, a0);
-                    tc_wait_ld();
-                    ws_store32(ws_mine, 1, c, lane128, a0);
-                    continue;
-                }
-#pragma unroll 1
-                for (int acc = 0; acc < (kSwiglu ? 1 : 2); ++acc) {
-#pragma unroll
-                    for (int hh = 0; hh < 2; ++hh) {
-                        const uint32_t lane_off = (uint32_t)(hh * 16) << 16;
-                        uint32_t r[8];
-                        if (kSwiglu) {
-                            uint32_t g[16], u[16];
-                            tc_ld16x256b_x4(tb0 + lane_off + c * 32, g);
-                            tc_ld16x256b_x4(tb1 + lane_off + c * 32, u);
-                            tc_wait_ld();
-#pragma unroll
-                            for (int i = 0; i < 8; ++i)
-                                r[i] = pack_bf16(silu_mul(__uint_as_float(g[2 * i]), __uint_as_float(u[2 * i])),
-                                                 silu_mul(__uint_as_float(g[2 * i + 1]), __uint_as_float(u[2 * i + 1])));
-                        } else {
-                            uint32_t v[16];
-                            tc_ld16x256b_x4((acc ? tb1 : tb0) + lane_off + c * 32, v);
-                            tc_wait_ld();
-#pragma unroll
-                            for (int i = 0; i < 8; ++i) {
-                                float lo = __uint_as_float(v[2 * i]), hi = __uint_as_float(v[2 * i + 1]);
-                                if (kRelu) { lo = fmaxf(lo, 0.f); hi = fmaxf(hi, 0.f); }
-                                r[i] = pack_bf16(lo, hi);
-                            }
-                        }
-                        // r[2j] = lanes 0-7 of this half, r[2j+1] = lanes 8-15; token block j
-                        stmatrix_x4_trans(st_row + hh * 32, r[0], r[2], r[4], r[6]);
-                        stmatrix_x4_trans(st_row + hh * 32 + 16, r[1], r[3], r[5], r[7]);
-                    }
-                    stage_to_global(stg, C, ldc, (int64_t)t.c_row + c * 32, n_rows, col0 + acc * ACC_M, n_cols, lane128, 2 + part);
-                }
-            }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0)
-                for (int h = 0; h < nb; ++h) mbar_arrive_remote(mapa(&ctl->tmem_empty[b0 + h], 0));
+            if (t.phase == 0)
+                epilogue_unit<kReluExperts ? 2 : 1>(t, p0, ctl, stg_base, tmem_base, rank, warp, lane, b0, nb, ready, ready_need > 0);
+            else
+                epilogue_unit<0>(t, p1, ctl, stg_base, tmem_base, rank, warp, lane, b0, nb, ready, false);
             buf = t.is_long ? 0 : (b0 ^ 1);
-            if (split && tile_ok) {
-                // publish the partial, count arrivals; the last unit of the tile reduces all s partials in split order
-                __threadfence();
-                epi_bar();
-                if (threadIdx.x == 4 * 32) {
-                    int32_t* cnt = sp.counters + t.tail * 2 + rank;
-                    const int old = atomicAdd(cnt, 1);
-                    const int last = (old == sp.s - 1) ? 1 : 0;
-                    if (last) *cnt = 0;                          // re-arm for the next launch
-                    ctl->split_last = last;
-                }
-                epi_bar();
-                const bool last = ctl->split_last != 0;          // rewritten only after the next split unit's first barrier
-                if (last) {
-                    __threadfence();
-                    const float* ws_tile = sp.ws + ((size_t)t.tail * sp.s * 2 + rank) * kSlotFloats;
-#pragma unroll 1
-                    for (int c = part; c < n_chunks; c += 2) {
-                        const int n_rows = min(32, t.rows_valid - c * 32);
-                        uint32_t a0[32], a1[32];
-                        ws_sum32(ws_tile, sp.s, 0, c, lane128, a0);
-                        ws_sum32(ws_tile, sp.s, 1, c, lane128, a1);
-                        uint16_t* srow = reinterpret_cast<uint16_t*>(stg) + lane128;       // [token][feature], 2-byte stores
-#pragma unroll 1
-                        for (int acc = 0; acc < (kSwiglu ? 1 : 2); ++acc) {
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) {
-                                float v = kSwiglu ? silu_mul(__uint_as_float(a0[i]), __uint_as_float(a1[i]))
-                                                  : __uint_as_float(acc ? a1[i] : a0[i]);
-                                if (kRelu) v = fmaxf(v, 0.f);
-                                srow[i * (STG_LD / 2)] = bf16_bits(v);
-                            }
-                            stage_to_global(stg, C, ldc, (int64_t)t.c_row + c * 32, n_rows, col0 + acc * ACC_M, n_cols, lane128, 2 + part);
-                        }
-                    }
-                }
-            }
         }
     }
 
@@ -660,11 +734,14 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
     }
-    // the last CTA to finish re-arms the scheduler words for the launch that reuses them (every leader has drawn its
-    // terminal ticket by now, so nobody reads the counter again)
+    // the last CTA to finish re-arms the scheduler words and the ready counters for the launch that reuses them (every
+    // leader has drawn its terminal ticket and every GEMM2 producer has seen its counter by now)
     if (threadIdx.x == 0) {
         __threadfence();
-        if (atomicAdd(sched + 1, 1) == (int)gridDim.x - 1) { sched[0] = 0; sched[1] = 0; }
+        if (atomicAdd(sched + 1, 1) == (int)gridDim.x - 1) {
+            for (int i = 0; i < n_token_tiles; ++i) ready[i] = 0;
+            sched[0] = 0; sched[1] = 0;
+        }
     }
 }
 
@@ -717,15 +794,16 @@ int32_t make_map_arena(ef_ctx* ctx, CUtensorMap* tm, const void* base) {
     return EF_OK;
 }
 
-// per-launch scheduler words {ticket counter, finished CTAs}; the kernel zeroes them again when it ends, and a
-// ring of EF_SCHED_RING pairs keeps launches that may still be in flight apart
-int32_t* next_sched(ef_ctx* ctx) {
-    int32_t* p = ctx->sched_words + 2 * (size_t)ctx->sched_next;
-    ctx->sched_next = (ctx->sched_next + 1) % EF_SCHED_RING;
+// per-launch scheduler block {ticket counter, finished CTAs, ready[n_token_tiles]}; the kernel zeroes it again when it
+// ends, and the blocks are carved out of a ring that is far longer than anything that can be in flight on one stream
+int32_t* next_sched(ef_ctx* ctx, int n_words) {
+    if (ctx->sched_next + n_words > EF_SCHED_WORDS) ctx->sched_next = 0;
+    int32_t* p = ctx->sched_words + ctx->sched_next;
+    ctx->sched_next += n_words;
     return p;
 }
 
-// Tail split-K plan for one launch: `tiles` tickets in scheduler order with `n_short` short ones at the end, G CTAs,
+// Tail split-K plan for one phase: `tiles` tickets in scheduler order with `n_short` short ones at the end, G CTA pairs,
 // KB k-blocks per tile.  Costs are in k-block times of a 256-row tile (1024 tensor cycles): a whole tail tile holds
 // an SM for KB (KB/2 if short) of them; a split unit adds a partial write and the finaliser reads s partials
 // (~0.03 per valid row each, from the measured ~50 GB/s per-SM global bandwidth).
@@ -757,12 +835,12 @@ SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, d
     return p;
 }
 
-// bytes one launch's TMA loads stage into shared memory (what crosses the L2 -> SM fabric): per token tile and weight-tile
+// bytes one phase's TMA loads stage into shared memory (what crosses the L2 -> SM fabric): per token tile and weight-tile
 // pair, per k-block, each CTA of the pair pulls its 32 KB weight box plus the 8 KB token boxes covering its half tile
-int64_t launch_fill_bytes(const EfGroupTable& tab, int npn, int KB) {
+int64_t phase_fill_bytes(const EfWaveTable& tab, bool balanced, int npn, int KB) {
     int64_t per_kb = 0;
     for (int i = 0; i < tab.n; ++i)
-        for (int off = 0, b = group_tile_rows(tab.g[i].rows, KB * BK >= kBalancedMinK); off < tab.g[i].rows; off += b) {
+        for (int off = 0, b = group_tile_rows(tab.g[i].rows, balanced); off < tab.g[i].rows; off += b) {
             const int n_mma = (std::min(tab.g[i].rows - off, b) + 15) & ~15;
             const int n_box = (n_mma / 2 + XBOX - 1) / XBOX;
             per_kb += 2 * (int64_t)(W_BYTES + n_box * XBOX_BYTES);
@@ -776,105 +854,91 @@ int32_t efk_ffn_tc_init(ef_ctx* ctx) {
     static_assert(BK == EF_ROWLET && BW == EF_TILE_ROWS, "the packed layout is tiled for this kernel's stage shape");
     int32_t rc = make_map_arena(ctx, &ctx->tm_w, ctx->arena);
     if (rc != EF_OK) return rc;
-    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
-    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
-    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
-    EF_CUDA(ctx, cudaMalloc(&ctx->sched_words, sizeof(int32_t) * 2 * EF_SCHED_RING));
-    EF_CUDA(ctx, cudaMemset(ctx->sched_words, 0, sizeof(int32_t) * 2 * EF_SCHED_RING));
-    ctx->splitk_max_units = ctx->n_sms;      // pair units; each has one workspace slot and one counter per CTA of the pair
-    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_ws, sizeof(float) * kSlotFloats * 2 * (size_t)ctx->splitk_max_units));
-    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_counters, sizeof(int32_t) * 2 * ctx->splitk_max_units));
-    EF_CUDA(ctx, cudaMemset(ctx->splitk_counters, 0, sizeof(int32_t) * 2 * ctx->splitk_max_units));
+    if ((rc = make_map_2d(ctx, &ctx->tm_h, ctx->h_ws, ctx->h_rows, ctx->cfg.d_ff)) != EF_OK) return rc;   // fixed for the ctx's life
+    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_wave_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+    EF_CUDA(ctx, cudaFuncSetAttribute(ffn_wave_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+    EF_CUDA(ctx, cudaMalloc(&ctx->sched_words, sizeof(int32_t) * EF_SCHED_WORDS));
+    EF_CUDA(ctx, cudaMemset(ctx->sched_words, 0, sizeof(int32_t) * EF_SCHED_WORDS));
+    // split-K: pair units; each has one workspace slot and one counter per CTA of the pair; one region per GEMM of a wave
+    ctx->splitk_max_units = ctx->n_sms;
+    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_ws, sizeof(float) * kSlotFloats * 2 * 2 * (size_t)ctx->splitk_max_units));
+    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_counters, sizeof(int32_t) * 2 * 2 * ctx->splitk_max_units));
+    EF_CUDA(ctx, cudaMemset(ctx->splitk_counters, 0, sizeof(int32_t) * 2 * 2 * ctx->splitk_max_units));
     ctx->tm_ok = true;
     return EF_OK;
 }
 
-int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfGroupTable& tab,
-                   const int32_t* h_row0, int phase) {
+// One wave: phase bit 0 = GEMM1 (x -> h), bit 1 = GEMM2 (h -> y).  phase == 3 is ONE launch: the GEMM2 units are ticketed
+// behind the GEMM1 units and wait, per token tile, for that tile's h columns (see the kernel).
+int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase) {
     const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
-    if (tab.n == 0) return EF_OK;
-    int64_t rows_total = 0;
-    // tiles per n column (every group's long tiles plus its short tail tile) under the tiling GEMM1 / GEMM2 will use
-    int mtiles1 = 0, mshort1 = 0, mtiles2 = 0, mshort2 = 0;
-    const bool bal1 = d >= kBalancedMinK, bal2 = f >= kBalancedMinK;
-    EfGroupTable t1 = tab, t2 = tab;
+    if (tab.n == 0 || !(phase & 3)) return EF_OK;
+    const bool relu = ctx->cfg.expert_kind == 1;
+    const bool bal = d >= kBalancedMinK && f >= kBalancedMinK;
+    int64_t rows_total = 0, x_rows = 0;
+    int mtiles = 0, mshort = 0;       // token tiles of the wave (every group's long tiles plus its short tail tile)
     for (int i = 0; i < tab.n; ++i) {
         rows_total += tab.g[i].rows;
-        mtiles1 += group_long_tiles(tab.g[i].rows, bal1) + group_has_short(tab.g[i].rows, bal1);
-        mshort1 += group_has_short(tab.g[i].rows, bal1);
-        mtiles2 += group_long_tiles(tab.g[i].rows, bal2) + group_has_short(tab.g[i].rows, bal2);
-        mshort2 += group_has_short(tab.g[i].rows, bal2);
-        t1.g[i].c_row0 = h_row0[i];   // GEMM1: x rows -> h rows
-        t2.g[i].a_row0 = h_row0[i];   // GEMM2: h rows -> y rows
+        x_rows = std::max<int64_t>(x_rows, (int64_t)tab.g[i].x_row0 + tab.g[i].rows);
+        mtiles += group_long_tiles(tab.g[i].rows, bal) + group_has_short(tab.g[i].rows, bal);
+        mshort += group_has_short(tab.g[i].rows, bal);
     }
     const int n_pairs = ctx->n_sms / 2;     // CTA pairs (clusters of 2), one CTA per SM
-    const bool relu = ctx->cfg.expert_kind == 1;
-    const int w1_rows = relu ? f : 2 * f;                             // W1 of a non-gated expert, or packed W13
+    const int w1_rows = relu ? f : 2 * f;   // W1 of a non-gated expert, or packed W13
     const int slot_rowlets = (int)(ctx->W / (EF_ROWLET * 2));
-    // optional per-launch timing (ef_set_kernel_timing): one event pair per GEMM launch
-    auto span_begin = [&](ef_ctx::KSpan& sp, int which) -> cudaError_t {
-        sp.which = which;
-        cudaError_t e = cudaEventCreate(&sp.e0);
-        if (e == cudaSuccess) e = cudaEventCreate(&sp.e1);
-        if (e == cudaSuccess) e = cudaEventRecord(sp.e0, st);
-        return e;
-    };
-    if (phase & 1) {
-        int64_t x_rows = 0;
-        for (int i = 0; i < tab.n; ++i) x_rows = std::max<int64_t>(x_rows, (int64_t)tab.g[i].a_row0 + tab.g[i].rows);
-        CUtensorMap tmX;
-        int32_t rc = make_map_2d(ctx, &tmX, x, x_rows, d);
-        if (rc != EF_OK) return rc;
-        ef_ctx::KSpan span{};
-        if (ctx->time_kernels) EF_CUDA(ctx, span_begin(span, 1));
-        const int ntn = relu ? (f + BW - 1) / BW : f / 128;      // 256 packed W13 rows -> 128 h columns; 256 W1 rows -> 256
-        const int npn = (ntn + 1) / 2;
-        const int tiles = mtiles1 * npn;
-        const SplitPlan pl = plan_split(ctx, tiles, mshort1 * npn, n_pairs, d / BK, (double)rows_total / mtiles1);
-        const int total = pl.n_plain + pl.n_tail * pl.s;
-        const int grid = 2 * std::min(total, n_pairs);
-        const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
-        if (relu)
-            ffn_gemm_kernel<2><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
-                                                                   total, w1_rows, slot_rowlets, 0, next_sched(ctx), sp, ctx->kprof1, t1);
-        else
-            ffn_gemm_kernel<1><<<grid, kThreads, kSmemBytes, st>>>(tmX, ctx->tm_w, (uint16_t*)ctx->h_ws, f, f, d, ntn, npn,
-                                                                   total, w1_rows, slot_rowlets, 0, next_sched(ctx), sp, ctx->kprof1, t1);
-        ctx->launches++;
-        EF_CUDA(ctx, cudaGetLastError());
-        if (ctx->time_kernels) {
-            EF_CUDA(ctx, cudaEventRecord(span.e1, st));
-            ctx->kspans.push_back(span);
-            ctx->ktimes.gemm1_launches++;
-            ctx->ktimes.gemm1_fill_bytes += launch_fill_bytes(tab, npn, d / BK);
-            ctx->ktimes.rows += rows_total;
-            ctx->ktimes.groups += tab.n;
-        }
+    const double avg_rows = (double)rows_total / mtiles;
+    PhaseArgs pa[2] = {};
+    // GEMM1: 256 packed W13 rows -> 128 h columns; 256 W1 rows -> 256
+    const int ntn1 = relu ? (f + BW - 1) / BW : f / 128, ntn2 = (d + BW - 1) / BW;
+    pa[0] = PhaseArgs{(uint16_t*)ctx->h_ws, f, f, d / BK, ntn1, (ntn1 + 1) / 2, w1_rows, 0, 0, 0, 1, ctx->splitk_ws, ctx->splitk_counters};
+    pa[1] = PhaseArgs{(uint16_t*)y, d, d, f / BK, ntn2, (ntn2 + 1) / 2, d, (int)((int64_t)w1_rows * d / EF_ROWLET), 0, 0, 1,
+                      ctx->splitk_ws + (size_t)kSlotFloats * 2 * ctx->splitk_max_units, ctx->splitk_counters + 2 * ctx->splitk_max_units};
+    for (int ph = 0; ph < 2; ++ph) {
+        if (!(phase & (1 << ph))) continue;
+        PhaseArgs& p = pa[ph];
+        const int tiles = mtiles * p.n_pairs_n;
+        // GEMM1 of a fused wave is followed by GEMM2 units that depend on it: its tail cannot be filled by them when the wave
+        // is one token tile deep, so it is split like a launch of its own
+        const SplitPlan pl = plan_split(ctx, tiles, mshort * p.n_pairs_n, n_pairs, p.KB, avg_rows);
+        p.n_plain = pl.n_plain;
+        p.s = pl.s;
+        p.total = pl.n_plain + pl.n_tail * pl.s;
     }
-    if (phase & 2) {
-        CUtensorMap tmH;
-        int32_t rc = make_map_2d(ctx, &tmH, ctx->h_ws, ctx->h_rows, f);
-        if (rc != EF_OK) return rc;
-        ef_ctx::KSpan span{};
-        if (ctx->time_kernels) EF_CUDA(ctx, span_begin(span, 2));
-        const int ntn = (d + BW - 1) / BW;
-        const int npn = (ntn + 1) / 2;
-        const int tiles = mtiles2 * npn;
-        const SplitPlan pl = plan_split(ctx, tiles, mshort2 * npn, n_pairs, f / BK, (double)rows_total / mtiles2);
-        const int total = pl.n_plain + pl.n_tail * pl.s;
-        const int grid = 2 * std::min(total, n_pairs);
-        const SplitArgs sp{pl.n_plain, pl.s, ctx->splitk_ws, ctx->splitk_counters};
-        ffn_gemm_kernel<0><<<grid, kThreads, kSmemBytes, st>>>(tmH, ctx->tm_w, (uint16_t*)y, d, d, f, ntn, npn,
-                                                                   total, d, slot_rowlets, (int)((int64_t)w1_rows * d / EF_ROWLET),
-                                                                   next_sched(ctx), sp, ctx->kprof2, t2);
-        ctx->launches++;
-        EF_CUDA(ctx, cudaGetLastError());
-        if (ctx->time_kernels) {
-            EF_CUDA(ctx, cudaEventRecord(span.e1, st));
-            ctx->kspans.push_back(span);
-            ctx->ktimes.gemm2_launches++;
-            ctx->ktimes.gemm2_fill_bytes += launch_fill_bytes(tab, npn, f / BK);
+    const int total = pa[0].total + pa[1].total;
+    const int grid = 2 * std::min(total, n_pairs);
+    if (2 + mtiles > EF_SCHED_WORDS) return ef_fail(ctx, EF_ERR_CAPACITY, "grouped FFN: too many token tiles in one wave");
+    if (phase & 1) {
+        if (ctx->tm_x_ptr != x || ctx->tm_x_rows != x_rows) {      // the caller's x_perm buffer rarely changes: encode once
+            int32_t rc = make_map_2d(ctx, &ctx->tm_x, x, x_rows, d);
+            if (rc != EF_OK) return rc;
+            ctx->tm_x_ptr = x;
+            ctx->tm_x_rows = x_rows;
         }
+    } else if (!ctx->tm_x_ptr) {
+        ctx->tm_x = ctx->tm_h;                                      // never dereferenced by a GEMM2-only launch
+    }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->time_kernels) {
+        int32_t rc = efk_timing_events(ctx, &e0, &e1);
+        if (rc != EF_OK) return rc;
+        EF_CUDA(ctx, cudaEventRecord(e0, st));
+    }
+    int32_t* sched = next_sched(ctx, 2 + mtiles);
+    long long* kprof = (phase & 1) ? ctx->kprof1 : ctx->kprof2;
+    if (relu)
+        ffn_wave_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(ctx->tm_x, ctx->tm_h, ctx->tm_w, pa[0], pa[1], slot_rowlets,
+                                                                  bal ? 1 : 0, mtiles, sched, kprof, tab);
+    else
+        ffn_wave_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(ctx->tm_x, ctx->tm_h, ctx->tm_w, pa[0], pa[1], slot_rowlets,
+                                                                   bal ? 1 : 0, mtiles, sched, kprof, tab);
+    ctx->launches++;
+    EF_CUDA(ctx, cudaGetLastError());
+    if (ctx->time_kernels) {
+        EF_CUDA(ctx, cudaEventRecord(e1, st));
+        ef_ctx::KSpan span{e0, e1, phase & 3, rows_total, tab.n};
+        ctx->kspans.push_back(span);
+        if (phase & 1) ctx->ktimes.gemm1_fill_bytes += phase_fill_bytes(tab, bal, pa[0].n_pairs_n, pa[0].KB);
+        if (phase & 2) ctx->ktimes.gemm2_fill_bytes += phase_fill_bytes(tab, bal, pa[1].n_pairs_n, pa[1].KB);
     }
     return EF_OK;
 }

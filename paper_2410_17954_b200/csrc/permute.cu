@@ -47,7 +47,7 @@ __device__ __forceinline__ int32_t ld_dsmem(const int32_t* p, uint32_t rank) {
 __global__ void __launch_bounds__(kIdxWarps * 32)
 permute_index_kernel(const int32_t* __restrict__ idx, int R, int E, int32_t* __restrict__ counts,
                      int32_t* __restrict__ offsets, int32_t* __restrict__ src, int32_t* __restrict__ inv,
-                     int32_t* counts_host) {
+                     int32_t* counts_host, int32_t* err_host) {
     extern __shared__ int32_t sm[];
     int32_t* hist = sm;                       // [kIdxWarps][E]
     int32_t* s_off = sm + kIdxWarps * E;      // [E + 1]
@@ -75,8 +75,11 @@ permute_index_kernel(const int32_t* __restrict__ idx, int R, int E, int32_t* __r
 #pragma unroll
         for (int u = 0; u < kBatch; ++u) {
             if (base0 + u * 32 >= hi) break;
-            const bool valid = base0 + u * 32 + lane < hi;
-            const int key = keys[u];
+            // a key outside [0, E) (caller-supplied top-k indices are not trusted) is routed nowhere: it gets a lane-unique
+            // key like the lanes past the end, is left out of every count, and raises the error word the host checks
+            const bool in_range = (unsigned)keys[u] < (unsigned)E;
+            const bool valid = base0 + u * 32 + lane < hi && in_range;
+            const int key = in_range ? keys[u] : (E + lane);
             const unsigned mask = __match_any_sync(0xffffffffu, key);
             if (valid && lane == (__ffs(mask) - 1)) myh[key] += __popc(mask);
             __syncwarp();
@@ -118,7 +121,6 @@ permute_index_kernel(const int32_t* __restrict__ idx, int R, int E, int32_t* __r
     __syncthreads();
     if (crank == 0) {
         for (int e = threadIdx.x; e <= E; e += blockDim.x) offsets[e] = s_off[e];
-        if (counts_host) __threadfence_system();
     }
 
     for (int base0 = lo; base0 < hi; base0 += 32 * kBatch) {
@@ -132,28 +134,34 @@ permute_index_kernel(const int32_t* __restrict__ idx, int R, int E, int32_t* __r
         for (int u = 0; u < kBatch; ++u) {
             if (base0 + u * 32 >= hi) break;
             const int p = base0 + u * 32 + lane;
-            const bool valid = p < hi;
-            const int key = keys[u];
+            const bool in_range = (unsigned)keys[u] < (unsigned)E;
+            const bool valid = p < hi && in_range;
+            const int key = in_range ? keys[u] : (E + lane);
             const unsigned mask = __match_any_sync(0xffffffffu, key);
             const int rank = __popc(mask & ((1u << lane) - 1u));
             if (valid) {
                 const int row = s_off[key] + s_base[key] + myh[key] + rank;
                 inv[p] = row;
                 src[row] = p;
+            } else if (p < hi) {
+                inv[p] = -1;                      // ef_combine skips it
+                if (err_host) *err_host = 1;
             }
             __syncwarp();
             if (valid && lane == (__ffs(mask) - 1)) myh[key] += __popc(mask);
             __syncwarp();
         }
     }
+    if (counts_host || err_host) __threadfence_system();
     cluster_sync();                           // no CTA exits while a peer may still read its totals
 }
 
 __global__ void __launch_bounds__(256)
 gather_rows_kernel(const uint4* __restrict__ x, const int32_t* __restrict__ src, int R, int k, int d8,
-                   uint4* __restrict__ x_perm) {
+                   uint4* __restrict__ x_perm, const int32_t* __restrict__ n_rows_dev) {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= R) return;
+    if (n_rows_dev && warp >= *n_rows_dev) return;     // dispatch: rows past offsets[E] exist only if pairs were skipped
     const int t = src[warp] / k;
     const uint4* in = x + (int64_t)t * d8;
     uint4* out = x_perm + (int64_t)warp * d8;
@@ -168,14 +176,14 @@ gather_rows_kernel(const uint4* __restrict__ x, const int32_t* __restrict__ src,
 }  // namespace
 
 int32_t efk_permute(ef_ctx* ctx, cudaStream_t st, const int32_t* idx, const void* x, int T, void* x_perm,
-                    int32_t* counts, int32_t* offsets, int32_t* src, int32_t* inv, int32_t* counts_host) {
+                    int32_t* counts, int32_t* offsets, int32_t* src, int32_t* inv, int32_t* counts_host, int32_t* err_host) {
     const int E = ctx->cfg.n_experts, k = ctx->cfg.top_k, d = ctx->cfg.d_model;
     const int R = T * k;
     size_t smem = ((size_t)kIdxWarps * E + 3 * (size_t)E + 1) * sizeof(int32_t);
     // one cluster: a CTA per ~1024 pairs (one 32-pair step per warp), at most 8 (the portable cluster size)
     const int n_cta = std::max(1, std::min(8, (R + 1023) / 1024));
     if (n_cta == 1) {     // a launch without cluster dimensions is a cluster of one CTA
-        permute_index_kernel<<<1, kIdxWarps * 32, smem, st>>>(idx, R, E, counts, offsets, src, inv, counts_host);
+        permute_index_kernel<<<1, kIdxWarps * 32, smem, st>>>(idx, R, E, counts, offsets, src, inv, counts_host, err_host);
         EF_CUDA(ctx, cudaGetLastError());
     } else {
     cudaLaunchConfig_t cfg = {};
@@ -188,12 +196,12 @@ int32_t efk_permute(ef_ctx* ctx, cudaStream_t st, const int32_t* idx, const void
     attr[0].val.clusterDim.x = n_cta; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    EF_CUDA(ctx, cudaLaunchKernelEx(&cfg, permute_index_kernel, idx, R, E, counts, offsets, src, inv, counts_host));
+    EF_CUDA(ctx, cudaLaunchKernelEx(&cfg, permute_index_kernel, idx, R, E, counts, offsets, src, inv, counts_host, err_host));
     }
     ctx->launches++;
     if (R > 0) {
         int blocks = (R * 32 + 255) / 256;
-        gather_rows_kernel<<<blocks, 256, 0, st>>>((const uint4*)x, src, R, k, d / 8, (uint4*)x_perm);
+        gather_rows_kernel<<<blocks, 256, 0, st>>>((const uint4*)x, src, R, k, d / 8, (uint4*)x_perm, offsets + E);
         ctx->launches++;
         EF_CUDA(ctx, cudaGetLastError());
     }
@@ -206,7 +214,7 @@ int32_t efk_reindex_rows(ef_ctx* ctx, cudaStream_t st, const void* src, const in
                          void* dst) {
     if (n_rows == 0) return EF_OK;
     const int blocks = (n_rows * 32 + 255) / 256;
-    gather_rows_kernel<<<blocks, 256, 0, st>>>((const uint4*)src, perm, n_rows, 1, (int)(row_bytes / 16), (uint4*)dst);
+    gather_rows_kernel<<<blocks, 256, 0, st>>>((const uint4*)src, perm, n_rows, 1, (int)(row_bytes / 16), (uint4*)dst, nullptr);
     ctx->launches++;
     EF_CUDA(ctx, cudaGetLastError());
     return EF_OK;

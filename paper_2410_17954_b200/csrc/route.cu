@@ -126,12 +126,16 @@ route_topk_kernel(const uint4* __restrict__ x, const uint4* __restrict__ wr, con
         const float* lg = s_logits + r * E;
         if (logits_out)
             for (int e = lane; e < E; e += 32) logits_out[(int64_t)t * E + e] = lg[e];
-        // candidates: lane owns experts lane, lane+32, ...
+        // candidates: lane owns experts lane, lane+32, ...  A NaN logit (NaN in x, the router or the bias: undefined input,
+        // R2) ranks as -inf, and among equal candidates the lowest untaken index wins, so every pick is a valid expert id
+        // whatever the input (an all-NaN row selects experts 0 .. k-1, as the oracle's strict '>' scan does).
         float v[8];
+        unsigned taken = 0;                       // bit i: expert lane + 32 i has been picked
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             int e = lane + 32 * i;
             v[i] = (e < E) ? lg[e] : -INFINITY;
+            if (v[i] != v[i]) v[i] = -INFINITY;
         }
         float zall = 0.f, m = 0.f, zsel = 0.f, my_val = 0.f;
         int my_idx = 0;
@@ -141,7 +145,7 @@ route_topk_kernel(const uint4* __restrict__ x, const uint4* __restrict__ wr, con
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
                 int e = lane + 32 * i;
-                if (e < E && (v[i] > bv || (v[i] == bv && e < bi))) { bv = v[i]; bi = e; }
+                if (e < E && !((taken >> i) & 1u) && (v[i] > bv || (v[i] == bv && e < bi))) { bv = v[i]; bi = e; }
             }
             warp_argmax(bv, bi);
             if (j == 0) {
@@ -154,11 +158,7 @@ route_topk_kernel(const uint4* __restrict__ x, const uint4* __restrict__ wr, con
             }
             zsel += expf(bv - m);
             if (lane == j) { my_val = bv; my_idx = bi; }
-            if ((bi & 31) == lane) {
-#pragma unroll
-                for (int i = 0; i < 8; ++i)
-                    if (i == (bi >> 5)) v[i] = -INFINITY;   // taken; E real logits are finite
-            }
+            if ((bi & 31) == lane) taken |= 1u << (bi >> 5);
         }
         if (lane < k) {
             const float Z = renorm ? zsel : zall;

@@ -26,7 +26,7 @@ def bits_from_bf16_tensor(t: torch.Tensor) -> np.ndarray:
 
 class MoELayerRunner:
     def __init__(self, n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared=0, max_tokens=1,
-                 prefetch_horizon=0, renorm=1, device=0, expert_kind=0):
+                 prefetch_horizon=0, renorm=1, device=0, expert_kind=0, diag=False):
         if not torch.cuda.is_available():
             raise RuntimeError("MoELayerRunner needs a CUDA device; there is no CPU fallback")
         self.dev = torch.device("cuda", device)
@@ -34,7 +34,7 @@ class MoELayerRunner:
         self.L, self.E, self.k, self.d, self.f = n_layers, n_experts, top_k, d_model, d_ff
         self.n_shared, self.renorm, self.max_tokens = n_shared, renorm, max_tokens
         self.ctx = EfContext(n_layers, n_experts, top_k, d_model, d_ff, n_slots, n_shared, max_tokens,
-                             prefetch_horizon, device, expert_kind)
+                             prefetch_horizon, device, expert_kind, diag=diag)
         T, k, E, d = max_tokens, top_k, n_experts, d_model
         dev = self.dev
         self.w_router = [None] * n_layers

@@ -13,12 +13,14 @@ torch = pytest.importorskip("torch")
 
 from test_gpu_stages import bf, check_float, dev_bf16, to_bits  # noqa: E402
 
+EF_OPT_WAVE_BYTES, EF_OPT_CHUNK_MIN_BYTES, EF_OPT_FUSED_WAVES = 2, 3, 4      # include/ef.h
 
-def build_runner(cfg, horizon=None, experts=None, max_tokens=None):
+
+def build_runner(cfg, horizon=None, experts=None, max_tokens=None, diag=False):
     from paper_2410_17954_b200 import MoELayerRunner
     r = MoELayerRunner(cfg.n_layers, cfg.n_experts, cfg.top_k, cfg.d_model, cfg.d_ff, cfg.n_slots, cfg.n_shared,
                        max_tokens or cfg.T, cfg.horizon if horizon is None else horizon, cfg.renorm,
-                       expert_kind=1 if cfg.expert_kind == "relu" else 0)
+                       expert_kind=1 if cfg.expert_kind == "relu" else 0, diag=diag)
     experts = experts or {}
     for l in range(cfg.n_layers):
         r.set_router(l, wl.router_weight(cfg, l), wl.static_router_bias(cfg, l))
@@ -44,8 +46,9 @@ def assert_cache_equal(runner, sim):
 @pytest.mark.parametrize("simt", [True, False], ids=["simt_debug", "tcgen05"])
 def test_cfg1_tiny_end_to_end(simt):
     cfg = wl.CONFIGS["tiny"]
-    r, ex = build_runner(cfg)
-    r.ctx.ef_set_debug_simt_ffn(simt)
+    r, ex = build_runner(cfg, diag=simt)
+    if simt:
+        r.ctx.ef_diag_set_simt_ffn(True)
     x = wl.activations(cfg)
     ref = oracle.layer_forward(x, wl.router_weight(cfg), None, [ex[(0, e)] for e in range(cfg.n_experts)], cfg.top_k)
     predicted = (ref.counts > 0).astype(np.uint8)[None, :]          # "a routing path that is 100% correct"
@@ -116,14 +119,17 @@ def test_cfg4_reduced_shared_experts_and_zipf():
 # neither the result nor the accounting -- down to pools so small that a miss takes the slot of a miss of the same visit
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n_slots", [1, 2, 5, 24])
-@pytest.mark.parametrize("wave_bytes,chunk_min", [(0, 0), (1 << 40, 0), (0, 1), (1 << 40, 1), (None, None)],
-                         ids=["single_waves", "batched", "chunked", "batched_chunked", "defaults"])
-def test_miss_wave_batching_and_chunked_copies(n_slots, wave_bytes, chunk_min):
+@pytest.mark.parametrize("wave_bytes,chunk_min,fused", [(0, 0, 1), (1 << 40, 0, 1), (0, 1, 1), (1 << 40, 1, 1), (None, None, 1),
+                                                        (0, 1, 0), (1 << 40, 0, 0)],
+                         ids=["single_waves", "batched", "chunked", "batched_chunked", "defaults", "chunked_two_launches",
+                              "batched_two_launches"])
+def test_miss_wave_batching_and_chunked_copies(n_slots, wave_bytes, chunk_min, fused):
     cfg = wl.scaled(wl.CONFIGS["many_expert_prefill"], T=256, d_model=256, d_ff=384, n_slots=n_slots)
     r, ex = build_runner(cfg)
+    r.ctx.ef_set_option(EF_OPT_FUSED_WAVES, fused)
     if wave_bytes is not None:
-        r.ctx.ef_set_wave_bytes(wave_bytes)
-        r.ctx.ef_set_chunk_min_bytes(chunk_min)
+        r.ctx.ef_set_option(EF_OPT_WAVE_BYTES, wave_bytes)
+        r.ctx.ef_set_option(EF_OPT_CHUNK_MIN_BYTES, chunk_min)
     x = wl.activations(cfg)
     ref = oracle.layer_forward(x, wl.router_weight(cfg), wl.static_router_bias(cfg),
                                [ex[(0, e)] for e in range(cfg.n_experts)], cfg.top_k,
@@ -256,8 +262,8 @@ def test_long_trace_wraps_the_event_ring():
     L, E = cfg.n_layers, cfg.n_experts
     n_steps = 170
     r, ex = build_runner(cfg, horizon=0)
-    r.ctx.ef_set_chunk_min_bytes(1)                      # two copies + two ready events per load
-    r.ctx.ef_set_wave_bytes(0)                           # one wave (and one free event) per miss
+    r.ctx.ef_set_option(EF_OPT_CHUNK_MIN_BYTES, 1)                      # two copies + two ready events per load
+    r.ctx.ef_set_option(EF_OPT_WAVE_BYTES, 0)                           # one wave (and one free event) per miss
     tr = wl.routing_trace(cfg, n_steps)
     sim = CacheSim(L, E, cfg.n_slots, cfg.expert_bytes, 0)
     nv = n_steps * L
@@ -326,4 +332,125 @@ def test_evict_and_clear_match_simulator():
     assert_cache_equal(r, sim)
     r.ctx.ef_cache_clear()
     assert r.ctx.ef_cache_snapshot() == [-1] * cfg.n_slots
+    r.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# boundary behaviour stated in include/ef.h
+# ------------------------------------------------------------------------------------------------
+def test_permute_with_caller_mirror_then_ffn_with_null_counts():
+    """ef.h (ef_permute): with a caller-supplied pinned mirror the internal event is still recorded, and
+    ef_expert_ffn_grouped(counts_host = NULL) waits on it and reads THAT mirror."""
+    cfg = wl.scaled(wl.CONFIGS["tiny"], n_slots=8)
+    r, ex = build_runner(cfg)
+    x = wl.activations(cfg)
+    ref = oracle.layer_forward(x, wl.router_weight(cfg), None, [ex[(0, e)] for e in range(cfg.n_experts)], cfg.top_k)
+    c, T = r.ctx, cfg.T
+    xd = dev_bf16(x)
+    mine = torch.full((cfg.n_experts,), -7, dtype=torch.int32).pin_memory()
+    out = torch.empty((T, cfg.d_model), dtype=torch.bfloat16, device="cuda")
+    for rep in range(2):                                  # the second pass must not see the first pass's event / mirror
+        mine.fill_(-7)
+        c.ef_route_topk(xd, r.w_router[0], None, T, 1, r.topk_idx, r.topk_w, None)
+        c.ef_permute(r.topk_idx, xd, T, r.x_perm, r.counts, r.offsets, r.src, r.inv, mine)
+        c.ef_expert_ffn_grouped(rep, 0, r.x_perm, None, r.y_perm)
+        assert np.array_equal(mine.numpy(), ref.counts)   # the call waited for the mirror
+        c.ef_combine(r.y_perm, r.inv, r.topk_w, T, None, None, out)
+        c.ef_sync()
+        check_float(bf(to_bits(out)), ref.out)
+    assert c.ef_cache_get_stats()["lookups"] == 2 * int((ref.counts > 0).sum())
+    r.close()
+
+
+def test_out_of_range_topk_index_is_skipped_and_flagged():
+    """ef.h (ef_permute): a top-k index outside [0, E) is routed nowhere (inv = -1, left out of every count) and the
+    next ef_expert_ffn_grouped(counts_host = NULL) refuses to run; ef_combine skips the pair."""
+    from paper_2410_17954_b200 import EfError
+    cfg = wl.scaled(wl.CONFIGS["tiny"], n_slots=8)
+    r, ex = build_runner(cfg)
+    T, k, E = cfg.T, cfg.top_k, cfg.n_experts
+    g = np.random.default_rng(0)
+    idx = np.stack([g.choice(E, k, replace=False) for _ in range(T)]).astype(np.int32)
+    bad = [(3, 0, E), (40, 1, -1), (63, 1, 1 << 20)]
+    for t, j, v in bad:
+        idx[t, j] = v
+    xd = dev_bf16(wl.activations(cfg))
+    r.topk_idx.copy_(torch.from_numpy(idx))
+    r.ctx.ef_permute(r.topk_idx, xd, T, r.x_perm, r.counts, r.offsets, r.src, r.inv)
+    torch.cuda.synchronize()
+    good = np.ones((T, k), bool)
+    for t, j, _ in bad:
+        good[t, j] = False
+    counts_ref = np.bincount(idx[good], minlength=E)
+    assert np.array_equal(r.counts.cpu().numpy(), counts_ref)
+    inv = r.inv.cpu().numpy().reshape(T, k)
+    assert (inv[~good] == -1).all() and sorted(inv[good]) == list(range(int(counts_ref.sum())))
+    with pytest.raises(EfError) as e:
+        r.ctx.ef_expert_ffn_grouped(0, 0, r.x_perm, None, r.y_perm)
+    assert e.value.code == -1
+    r.y_perm.zero_(); r.topk_w.fill_(1.0)
+    out = torch.empty((T, cfg.d_model), dtype=torch.bfloat16, device="cuda")
+    r.ctx.ef_combine(r.y_perm, r.inv, r.topk_w, T, None, None, out)       # must not read row -1
+    r.ctx.ef_sync()
+    assert float(out.float().abs().max()) == 0.0
+    r.close()
+
+
+def test_nan_activations_still_route_to_valid_experts():
+    """R2: NaN logits are undefined input, but the router must never emit an index outside [0, E): a NaN logit ranks as
+    -inf and the lowest untaken index wins, exactly what the oracle's strict '>' scan does on an all-NaN row."""
+    cfg = wl.scaled(wl.CONFIGS["tiny"], n_slots=8)
+    r, _ = build_runner(cfg)
+    T, k, E = cfg.T, cfg.top_k, cfg.n_experts
+    x = bf(wl.activations(cfg)).astype(np.float32)
+    x[5, :] = np.nan
+    xd = torch.from_numpy(x).cuda().to(torch.bfloat16)
+    r.ctx.ef_route_topk(xd, r.w_router[0], None, T, 1, r.topk_idx, r.topk_w, r.logits)
+    torch.cuda.synchronize()
+    idx = r.topk_idx.cpu().numpy()
+    assert idx.min() >= 0 and idx.max() < E
+    assert list(idx[5]) == list(range(k))
+    idx_ref, _ = oracle.topk_gate(r.logits.cpu().numpy().astype(np.float64), k, 1)
+    assert np.array_equal(idx, idx_ref)
+    r.ctx.ef_permute(r.topk_idx, xd, T, r.x_perm, r.counts, r.offsets, r.src, r.inv)
+    r.ctx.ef_sync()
+    assert int(r.counts.sum()) == T * k
+    r.close()
+
+
+def test_calls_on_a_second_stream_are_ordered_behind_the_first():
+    """ef.h (Streams): the layer calls share per-ctx workspaces; a call on another stream is serialised behind what the
+    lane has enqueued so far.  Two visits on two streams, no host synchronisation in between."""
+    cfg = wl.scaled(wl.CONFIGS["tiny"], T=64, d_model=512, d_ff=1024, n_slots=8)
+    r, ex = build_runner(cfg)
+    x = wl.activations(cfg)
+    ref = oracle.layer_forward(x, wl.router_weight(cfg), None, [ex[(0, e)] for e in range(cfg.n_experts)], cfg.top_k)
+    xd = dev_bf16(x)
+    outs = [torch.empty((cfg.T, cfg.d_model), dtype=torch.bfloat16, device="cuda") for _ in range(6)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    for v in range(6):
+        with torch.cuda.stream(streams[v & 1]):
+            r.visit(v, xd, outs[v])
+    r.ctx.ef_sync()
+    for o in outs:
+        check_float(bf(to_bits(o)), ref.out)
+    r.close()
+
+
+def test_reregistering_a_resident_or_aliased_expert_is_refused():
+    from paper_2410_17954_b200 import EfError
+    cfg = wl.scaled(wl.CONFIGS["tiny"], n_slots=4)
+    r, ex = build_runner(cfg)
+    c = r.ctx
+    c.ef_host_expert_alias(0, 7, 0, 2)                       # expert 7 now shares expert 2's packed host buffer
+    with pytest.raises(EfError):
+        c.ef_host_expert_register(0, 2, *ex[(0, 2)])         # would pull the buffer from under the alias
+    c.ef_cache_prefetch(-1, np.array([[1, 0, 0, 0, 0, 0, 0, 0]], np.uint8))
+    with pytest.raises(EfError):
+        c.ef_host_expert_register(0, 0, *ex[(0, 0)])         # resident: the slot would keep serving the old weights
+    c.ef_cache_evict(0, [0])
+    c.ef_host_expert_register(0, 0, *ex[(0, 1)])             # evicted: allowed (waits for the copy stream first)
+    c.ef_host_expert_register(0, 7, *ex[(0, 7)])             # an alias may become an owner again ...
+    c.ef_host_expert_register(0, 2, *ex[(0, 2)])             # ... which frees its former source for re-registration
     r.close()

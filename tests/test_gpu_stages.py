@@ -146,13 +146,15 @@ def test_permute_bit_exact(T, k, E, d):
 # ------------------------------------------------------------------------------------------------
 # a4 grouped FFN (resident experts)
 # ------------------------------------------------------------------------------------------------
-def run_resident_ffn(ctx, E, d, f, counts, seed, simt, splitk=0, expert_kind="swiglu"):
+def run_resident_ffn(ctx, E, d, f, counts, seed, simt, splitk=0, expert_kind="swiglu", fused=True):
     """Load experts 0..E-1 into slots via the cache, run the grouped FFN on oracle-permuted rows."""
     cfg = wl.scaled(wl.CONFIGS["tiny"], d_model=d, d_ff=f, n_experts=E, seed=seed, expert_kind=expert_kind)
     experts = [wl.expert_weights(cfg, 0, e) for e in range(E)]
-    for e in range(E):
-        ctx.ef_host_expert_register(0, e, *experts[e])
-    ctx.ef_cache_prefetch(-1, np.ones((1, E), np.uint8))
+    if not getattr(ctx, "_experts_loaded", False):       # repeated calls on one ctx reuse the resident experts
+        for e in range(E):
+            ctx.ef_host_expert_register(0, e, *experts[e])
+        ctx.ef_cache_prefetch(-1, np.ones((1, E), np.uint8))
+        ctx._experts_loaded = True
     snap = ctx.ef_cache_snapshot()
     slot_of = {g: s for s, g in enumerate(snap) if g >= 0}
     assert len(slot_of) == E
@@ -160,8 +162,11 @@ def run_resident_ffn(ctx, E, d, f, counts, seed, simt, splitk=0, expert_kind="sw
     x_perm = wl.normal_bf16(seed, "xperm", (R, d), 1.0)
     offs = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
     y = torch.full((R, d), float("nan"), dtype=torch.bfloat16, device="cuda")
-    ctx.ef_set_debug_simt_ffn(simt)
-    ctx.ef_set_splitk(splitk)
+    from paper_2410_17954_b200 import EF_OPT_FUSED_WAVES, EF_OPT_SPLITK
+    if simt:
+        ctx.ef_diag_set_simt_ffn(True)       # the plain-FMA bring-up backend exists in the diag library only
+    ctx.ef_set_option(EF_OPT_SPLITK, splitk)
+    ctx.ef_set_option(EF_OPT_FUSED_WAVES, 1 if fused else 0)
     act = [e for e in range(E) if counts[e] > 0]
     ctx.ef_expert_ffn_grouped_resident(dev_bf16(x_perm), [offs[e] for e in act], [counts[e] for e in act],
                                        [slot_of[e] for e in act], y)
@@ -179,22 +184,28 @@ FFN_CASES = [
     (5, 512, 1408 - 1408 % 128, [300, 7, 0, 513, 64]),
     (2, 64, 128, [1, 1]),
     (2, 1024, 384, [257, 255]),
-    # K >= 3072 switches the token tiling to balanced tiles (593 -> 208 + 208 + 177): GEMM1 (K = d), then GEMM2 (K = f)
+    # long K loops on one side only keep 256-row tiles + remainder (both GEMMs of a wave share ONE token tiling)
     (2, 3072, 256, [300, 593]),
     (3, 256, 3072, [513, 257, 130]),
+    # d and f both >= 3072 switch the wave to balanced tiles (593 -> 208 + 208 + 177)
+    (2, 3072, 3072, [593, 300]),
 ]
 
+# variant ids: simt = the diag library's plain-FMA backend; splitk 0 = automatic tail split-K (these launches have fewer
+# tiles than SMs, so it engages), 1 = off, 2 / 3 / 5 = every tile split into that many K parts (uneven k-block ranges,
+# partial-sum workspace, last-arriver reduction); fused = one launch runs both GEMMs (GEMM2 units wait for their token
+# tile's h columns), else two launches
+FFN_VARIANTS = [(True, 0, True), (False, 1, True), (False, 0, True), (False, 2, True), (False, 3, True), (False, 5, True),
+                (False, 0, False), (False, 3, False)]
+FFN_VARIANT_IDS = ["simt_debug", "tcgen05_nosplit", "tcgen05_auto", "tcgen05_split2", "tcgen05_split3", "tcgen05_split5",
+                   "two_launches_auto", "two_launches_split3"]
 
-# splitk: 0 = automatic tail split-K (these launches have fewer tiles than SMs, so it engages), 1 = off,
-# 2 / 3 / 5 = every tile split into that many K parts (uneven k-block ranges, partial-sum workspace, last-arriver
-# reduction)
-@pytest.mark.parametrize("simt,splitk", [(True, 0), (False, 1), (False, 0), (False, 2), (False, 3), (False, 5)],
-                         ids=["simt_debug", "tcgen05_nosplit", "tcgen05_auto", "tcgen05_split2", "tcgen05_split3",
-                              "tcgen05_split5"])
+
+@pytest.mark.parametrize("simt,splitk,fused", FFN_VARIANTS, ids=FFN_VARIANT_IDS)
 @pytest.mark.parametrize("E,d,f,counts", FFN_CASES)
-def test_ffn_grouped_resident(E, d, f, counts, simt, splitk):
-    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)))
-    got, ref = run_resident_ffn(ctx, E, d, f, counts, seed=13, simt=simt, splitk=splitk)
+def test_ffn_grouped_resident(E, d, f, counts, simt, splitk, fused):
+    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)), diag=simt)
+    got, ref = run_resident_ffn(ctx, E, d, f, counts, seed=13, simt=simt, splitk=splitk, fused=fused)
     assert not np.isnan(got).any()          # every routed row was written
     check_float(got, ref)
     ctx.close()
@@ -202,15 +213,31 @@ def test_ffn_grouped_resident(E, d, f, counts, simt, splitk):
 
 # Switch-style non-gated ReLU experts (expert_kind = 1, R30): W1 tiles of 256 rows (f = 384: a ragged last
 # weight tile, an odd tile count for the CTA pair), all kernel variants
-@pytest.mark.parametrize("simt,splitk", [(True, 0), (False, 1), (False, 0), (False, 3)],
-                         ids=["simt_debug", "tcgen05_nosplit", "tcgen05_auto", "tcgen05_split3"])
+@pytest.mark.parametrize("simt,splitk,fused", [(True, 0, True), (False, 1, True), (False, 0, True), (False, 3, True), (False, 0, False)],
+                         ids=["simt_debug", "tcgen05_nosplit", "tcgen05_auto", "tcgen05_split3", "two_launches_auto"])
 @pytest.mark.parametrize("E,d,f,counts", [(4, 256, 512, [40, 0, 1, 87]), (3, 768, 3072, [300, 129, 16]),
                                           (2, 1024, 384, [257, 255]), (2, 64, 128, [1, 1])])
-def test_ffn_grouped_resident_relu_experts(E, d, f, counts, simt, splitk):
-    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)), expert_kind=1)
-    got, ref = run_resident_ffn(ctx, E, d, f, counts, seed=29, simt=simt, splitk=splitk, expert_kind="relu")
+def test_ffn_grouped_resident_relu_experts(E, d, f, counts, simt, splitk, fused):
+    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)), expert_kind=1, diag=simt)
+    got, ref = run_resident_ffn(ctx, E, d, f, counts, seed=29, simt=simt, splitk=splitk, expert_kind="relu", fused=fused)
     assert not np.isnan(got).any()
     check_float(got, ref)
+    ctx.close()
+
+
+def test_ffn_many_groups_many_waves_in_one_launch():
+    """64 groups of ragged sizes in ONE launch (the many-expert shape, reduced): more GEMM1 units than CTA pairs, so GEMM2
+    units of the early groups run while GEMM1 units of the late groups are still in flight, and every token tile's
+    ready counter is exercised; repeated launches re-arm the counters."""
+    E, d, f = 64, 256, 384
+    g = wl.stream(5, "ffn.many")
+    counts = [int(c) for c in g.integers(0, 300, size=E)]
+    counts[3], counts[17], counts[40] = 0, 700, 1
+    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)))
+    for rep in range(3):
+        got, ref = run_resident_ffn(ctx, E, d, f, counts, seed=31, simt=False)
+        assert not np.isnan(got).any()
+        check_float(got, ref)
     ctx.close()
 
 
@@ -320,11 +347,11 @@ def test_errors_are_codes_not_crashes():
 # ------------------------------------------------------------------------------------------------
 def test_tma_fill_rate_and_fill_byte_accounting():
     E, d, f, counts = 2, 512, 1024, [300, 17]
-    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)))
-    gbs = ctx.ef_debug_tma_fill_gbs(32 << 20, 500)
+    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=int(np.sum(counts)), diag=True)
+    gbs = ctx.ef_diag_tma_fill_gbs(32 << 20, 500)
     assert 2000.0 < gbs < 40000.0                     # an L2-resident region: several TB/s on a B200
     with pytest.raises(Exception):
-        ctx.ef_debug_tma_fill_gbs(16, 500)            # smaller than one box
+        ctx.ef_diag_tma_fill_gbs(16, 500)             # smaller than one box
     ctx.ef_set_kernel_timing(True)
     ctx.ef_get_kernel_times(reset=True)
     run_resident_ffn(ctx, E, d, f, counts, seed=3, simt=False, splitk=1)
@@ -339,5 +366,8 @@ def test_tma_fill_rate_and_fill_byte_accounting():
     npn1, npn2 = (f // 128 + 1) // 2, ((d + 255) // 256 + 1) // 2
     assert kt["gemm1_fill_bytes"] == tiles * npn1 * (d // 64)
     assert kt["gemm2_fill_bytes"] == tiles * npn2 * (f // 64)
-    assert kt["rows"] == sum(counts) and kt["groups"] == 2
+    assert kt["wave_rows"] == sum(counts) and kt["wave_groups"] == 2 and kt["wave_launches"] == 1
+    assert kt["gemm1_launches"] == 0 and kt["gemm2_launches"] == 0          # one launch ran both GEMMs
+    log = ctx.ef_get_launch_log()
+    assert [(r["which"], r["groups"], r["rows"]) for r in log] == [(3, 2, sum(counts))] and log[0]["ms"] > 0
     ctx.close()

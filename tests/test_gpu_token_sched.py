@@ -41,7 +41,7 @@ def check_against_oracle(ctx, r, c0, c1, max_iter=16):
     """Both device paths (single-CTA for N <= 256, multi-kernel) against the oracle."""
     ref = ots.schedule(r, c0, c1, max_iter)
     for force_multi in (False, True):
-        ctx.ef_set_token_sched_path(force_multi)
+        ctx.ef_set_option(5, 1 if force_multi else 0)          # EF_OPT_TOKEN_SCHED_PATH
         b, p, info, bp = run_schedule(ctx, r, c0, c1, max_iter)
         assert np.array_equal(b, ref.batch_of), force_multi
         for c in (0, 1):
@@ -49,7 +49,7 @@ def check_against_oracle(ctx, r, c0, c1, max_iter=16):
         assert np.array_equal(p, ref.perm), force_multi
         assert info[:6].tolist() == [ref.iters, int(ref.converged), ref.centroids[0], ref.centroids[1], ref.objective,
                                      ref.objective_before], force_multi
-    ctx.ef_set_token_sched_path(False)
+    ctx.ef_set_option(5, 0)
     return ref
 
 

@@ -8,15 +8,22 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def header_symbols():
-    txt = open(os.path.join(ROOT, "include", "ef.h")).read()
+def header_symbols(name="ef.h"):
+    txt = open(os.path.join(ROOT, "include", name)).read()
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
     return sorted(set(re.findall(r"\b(ef_[a-z0-9_]+)\s*\(", txt)))
 
 
+def dynamic_symbols(lib_path):
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", lib_path], capture_output=True, text=True, check=True).stdout
+    return sorted(l.split()[-1] for l in out.splitlines() if l.split()[-1].startswith("ef_"))
+
+
 def test_header_and_binding_agree():
-    from paper_2410_17954_b200 import DECLARED_SYMBOLS
-    assert sorted(DECLARED_SYMBOLS) == header_symbols()
+    from paper_2410_17954_b200 import DECLARED_SYMBOLS, DIAG_SYMBOLS
+    assert sorted(DECLARED_SYMBOLS) == header_symbols("ef.h")
+    assert sorted(DIAG_SYMBOLS) == header_symbols("ef_diag.h")
 
 
 def test_library_exports_every_declared_symbol():
@@ -24,6 +31,20 @@ def test_library_exports_every_declared_symbol():
     b.build()
     from paper_2410_17954_b200 import exported_symbols, DECLARED_SYMBOLS
     assert sorted(exported_symbols()) == sorted(DECLARED_SYMBOLS)
+
+
+def test_product_library_exports_nothing_but_the_header():
+    """No bring-up backend, probe kernel or debug hook ships in libef.so: its ef_* exports are exactly include/ef.h; the
+    diagnostic build adds exactly include/ef_diag.h."""
+    from paper_2410_17954_b200 import build as b
+    from paper_2410_17954_b200 import library_path
+    b.build()
+    assert dynamic_symbols(library_path()) == header_symbols("ef.h")
+    b.build_diag()
+    assert dynamic_symbols(library_path(diag=True)) == sorted(header_symbols("ef.h") + header_symbols("ef_diag.h"))
+    import subprocess
+    kernels = subprocess.run(["cuobjdump", "-elf", library_path()], capture_output=True, text=True).stdout
+    assert "simt_gemm_kernel" not in kernels and "tma_fill_kernel" not in kernels
 
 
 def test_product_path_does_not_touch_oracle():
