@@ -233,3 +233,47 @@ class CacheSim:
 
     def hit_ratio(self) -> float:
         return self.stats["hits"] / max(1, self.stats["lookups"])
+
+
+def belady_min_loads(n_layers: int, n_experts: int, n_slots: int, actual) -> list:
+    """Clairvoyant reference for the policy gap (NOT part of the library's policy): Belady's MIN [farthest next use
+    is evicted] on the ACTUAL trace, with demand loading.  actual[v] = iterable of the experts active at visit v (local
+    ids; layer = v mod n_layers).  A visit's active experts are served hits first, then misses in ascending id (R12); a
+    miss evicts, among the residents that are not still waiting to be served at this visit, the one whose next use lies
+    farthest in the future (never used again = infinitely far).  Returns the number of loads at every visit.
+    Prefetching cannot lower the NUMBER of loads, only hide their latency, so on a link-bound step this is the floor that
+    PLEC's and LRU's bytes_h2d are held against.  With one access per visit this is the textbook OPT (pinned to the
+    classic reference string: 9 faults with 3 frames) and it is checked against exhaustive search on small traces."""
+    nv = len(actual)
+    acts = [sorted(set(int(e) for e in a)) for a in actual]
+    gid = lambda v, e: (v % n_layers) * n_experts + e
+    # next_use[v][g] = first visit > v at which g is active
+    INF = 1 << 60
+    nxt_at = [dict() for _ in range(nv)]
+    upcoming: dict = {}
+    for v in range(nv - 1, -1, -1):
+        for e in acts[v]:
+            g = gid(v, e)
+            nxt_at[v][g] = upcoming.get(g, INF)
+        for e in acts[v]:
+            upcoming[gid(v, e)] = v
+    next_use: dict = {}          # for residents: their next use strictly after the current visit (kept up to date on use)
+    cache: set = set()
+    loads = []
+    for v in range(nv):
+        want = [gid(v, e) for e in acts[v]]
+        misses = [g for g in want if g not in cache]
+        for g in want:                                      # hits are served first: from now on their next use is after v
+            if g in cache:
+                next_use[g] = nxt_at[v][g]
+        n = 0
+        for g in misses:
+            if len(cache) >= n_slots:
+                victim = max(cache, key=lambda r: (next_use[r], r))
+                cache.discard(victim)
+                del next_use[victim]
+            cache.add(g)
+            next_use[g] = nxt_at[v][g]
+            n += 1
+        loads.append(n)
+    return loads

@@ -418,8 +418,8 @@ int pick_victim(ef_ctx* ctx, int64_t v_now, int64_t target, bool allow3, const s
 
 void drain_copy_spans(ef_ctx* ctx, bool wait, float* acc_ms);
 
-// policy bookkeeping + the physical H2D for one load
-int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
+// policy bookkeeping of one load (slot table, counters): decided in policy order, at once
+int32_t policy_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
     if (!ctx->host_expert[g])
         return ef_fail(ctx, EF_ERR_NOT_REGISTERED, "expert (layer %d, id %d) was never registered", g / ctx->cfg.n_experts,
                        g % ctx->cfg.n_experts);
@@ -435,7 +435,11 @@ int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
     sl.stamp = ++ctx->tick;
     ctx->slot_of[g] = slot;
     ctx->stats.bytes_h2d += (uint64_t)ctx->W;
+    return EF_OK;
+}
 
+// the physical H2D of one load: waits (on the copy stream) for the last wave that read the slot, then copies
+int32_t enqueue_copy(ef_ctx* ctx, int slot, int32_t g) {
     EfPhys& ph = ctx->phys[slot];
     EF_CUDA(ctx, ring_wait(ctx, ctx->copy_stream, ph.free_, ctx->last_compute, ctx->has_last_compute));
     cudaEvent_t t0, t1;
@@ -446,9 +450,9 @@ int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
     }
     EF_CUDA(ctx, cudaEventRecord(t0, ctx->copy_stream));
     // Finer-grained streaming: a large expert travels as two copies -- the first-GEMM weights
-    // (packed W13, or W1), then Wd -- with a "ready" event after each, so GEMM1 of the wave that waits for this
-    // expert runs while Wd is still on the link.  Small experts travel whole (the gap between two copies would cost
-    // more link time than the overlap wins).
+    // (packed W13, or W1), then Wd -- with a "ready" event after each, so GEMM1 of the visit's last wave runs while Wd is
+    // still on the link.  Small experts travel whole (the gap between two copies would cost more link time than the
+    // overlap wins).
     char* dst = ctx->arena + (size_t)slot * ctx->W;
     const char* srcp = (const char*)ctx->host_expert[g];
     const size_t w1_bytes = (size_t)(ctx->cfg.expert_kind == 1 ? 1 : 2) * ctx->cfg.d_model * ctx->cfg.d_ff * 2;
@@ -471,6 +475,11 @@ int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
     ph.waited_mask = 0;
     ph.waited = nullptr;
     return EF_OK;
+}
+
+int32_t issue_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
+    int32_t rc = policy_load(ctx, slot, g, pred_for);
+    return rc != EF_OK ? rc : enqueue_copy(ctx, slot, g);
 }
 
 void drain_copy_spans(ef_ctx* ctx, bool wait, float* acc_ms) {
@@ -559,16 +568,26 @@ int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm,
 }
 
 // Miss waves.  Every on-demand expert could be its own wave (compute starts the moment its copy lands), but for small
-// experts that is one launch pair per ~0.3 ms copy, each too short to fill the GPU.  The batcher groups consecutive
-// misses into one grouped launch per ~wave_bytes of link traffic; the last miss of a visit stays alone so that the
-// tail after the final copy is one expert's FFN.  Physical scheduling only: which slot a miss takes and every counter
-// were decided before the item got here.
+// experts that is one launch per ~0.3 ms copy, each far too short to fill the GPU.  The batcher groups consecutive
+// misses into waves: never less than ~wave_bytes of link traffic per wave, and -- while many misses are still to come --
+// HALF of what is left (a visit with 40 small misses runs them as waves of 20, 10, 7, 2 and 1 experts): the big early
+// waves are real grouped GEMMs, each finishes long before the next, smaller wave's copies have landed, and the last miss
+// of a visit still is a wave of its own, so the tail after the final copy is one expert's FFN.  Physical scheduling only:
+// which slot a miss takes and every counter were decided before the item got here.
 struct MissBatcher {
     ef_ctx* ctx; cudaStream_t st; const void* x_perm; void* y_perm;
     std::vector<WaveItem> open;
-    int per_wave;
-    MissBatcher(ef_ctx* c, cudaStream_t s, const void* x, void* y) : ctx(c), st(s), x_perm(x), y_perm(y) {
-        per_wave = (int)std::max<int64_t>(1, std::min<int64_t>(EF_MAX_GROUPS, ctx->wave_bytes / ctx->W));
+    int min_wave;           // experts per wave from wave_bytes
+    int remaining;          // misses of this visit not yet pushed (set by the caller)
+    int target;             // size of the wave being collected
+    MissBatcher(ef_ctx* c, cudaStream_t s, const void* x, void* y, int n_misses)
+        : ctx(c), st(s), x_perm(x), y_perm(y), remaining(n_misses) {
+        min_wave = (int)std::max<int64_t>(1, std::min<int64_t>(EF_MAX_GROUPS, ctx->wave_bytes / ctx->W));
+        target = next_target();
+    }
+    int next_target() const {
+        if (ctx->wave_bytes == 0) return 1;
+        return std::min(EF_MAX_GROUPS, std::max(min_wave, remaining / 2));
     }
     bool holds_slot(int slot) const {
         for (const WaveItem& it : open) if (it.slot == slot) return true;
@@ -578,13 +597,15 @@ struct MissBatcher {
         if (open.empty()) return EF_OK;
         int32_t rc = run_wave(ctx, st, x_perm, y_perm, open, last_of_visit);
         open.clear();
+        target = next_target();
         return rc;
     }
     int32_t push(const WaveItem& it, bool last_of_visit) {
         int32_t rc = EF_OK;
         if (last_of_visit && !open.empty() && (rc = flush()) != EF_OK) return rc;
         open.push_back(it);
-        if ((int)open.size() >= per_wave || last_of_visit) rc = flush(last_of_visit);
+        --remaining;
+        if ((int)open.size() >= target || last_of_visit) rc = flush(last_of_visit);
         return rc;
     }
 };
@@ -644,33 +665,63 @@ extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visi
         locked[s] = 1;
         wave0.push_back(WaveItem{off[e], counts_host[e], s});
     }
-    // phase A: on-demand loads into empty / mis-prefetched / completed slots; copies start now and
-    // overlap wave 0
-    std::vector<WaveItem> wavesA;
+    // ---- policy, in policy order (R12: ascending expert id), all of it before anything physical: every decision depends
+    // on the slot table alone ("completed" = enqueued, R9)
+    struct Miss { WaveItem item; int32_t g; int gen; };     // gen: 0 = the victim slot held nothing of this visit's misses
+    std::vector<Miss> planA, planB;
+    std::vector<int> gen_of_slot(c.n_slots, -1);
+    // phase A: on-demand loads into empty / mis-prefetched / completed slots; their copies overlap wave 0
     std::vector<int> rest;
     for (int e : misses) {
         const int s = pick_victim(ctx, visit, visit, false, locked);
         if (s < 0) { rest.push_back(e); continue; }
-        int32_t rc = issue_load(ctx, s, layer * E + e, -1);
+        int32_t rc = policy_load(ctx, s, layer * E + e, -1);
         if (rc != EF_OK) return rc;
         ctx->stats.ondemand_loads++;
         ctx->slots[s].used = true;
         locked[s] = 1;
-        wavesA.push_back(WaveItem{off[e], counts_host[e], s});
+        gen_of_slot[s] = 0;
+        planA.push_back(Miss{WaveItem{off[e], counts_host[e], s}, layer * E + e, 0});
     }
-    // Wave 0 = the hits.  A pending phase-B load may be about to overwrite the slot of one of these very hits, and its
-    // copy waits for the "free" event of the wave that read the slot.  Copies are far slower than waves, so only the
-    // FIRST victim matters: it is known already (phase B's first pick depends on the table, not on execution), and
-    // when it is a hit that hit runs as its own wave first, so the copy starts after one expert's FFN instead of
-    // after the whole wave (physical ordering only: the policy and its accounting are unchanged).
+    // phase B: the pool was full of this visit's own experts and useful prefetches; the locks drop, and each remaining
+    // miss takes a class 0-3 victim -- now including this visit's hits and the misses that came before it
+    std::fill(locked.begin(), locked.end(), 0);
+    for (int e : rest) {
+        const int s = pick_victim(ctx, visit, visit, true, locked);
+        if (s < 0) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_expert_ffn_grouped: no victim slot (internal)");
+        int32_t rc = policy_load(ctx, s, layer * E + e, -1);
+        if (rc != EF_OK) return rc;
+        ctx->stats.ondemand_loads++;
+        ctx->slots[s].used = true;
+        const int gen = gen_of_slot[s] < 0 ? 0 : gen_of_slot[s] + 1;
+        gen_of_slot[s] = gen;
+        planB.push_back(Miss{WaveItem{off[e], counts_host[e], s}, layer * E + e, gen});
+    }
+    // ---- physical order of the copies (never part of the policy; EF_OPT_COPY_ORDER): misses that do not
+    // wait for one another go on the link with the most routed rows first -- the largest GEMMs start earliest and the
+    // visit's tail after its final copy is its smallest expert -- and a miss that reuses the slot of an earlier miss of
+    // this visit (a later "generation") follows the generation it waits for.
+    if (ctx->copy_order == 1) {
+        auto more_rows = [](const Miss& a, const Miss& b) { return a.item.rows > b.item.rows; };
+        std::stable_sort(planA.begin(), planA.end(), more_rows);
+        std::stable_sort(planB.begin(), planB.end(), [](const Miss& a, const Miss& b) {
+            return a.gen != b.gen ? a.gen < b.gen : a.item.rows > b.item.rows;
+        });
+    }
     int32_t rc = EF_OK;
-    int first_victim = -1;
-    if (!rest.empty() && wave0.size() > 1) first_victim = pick_victim(ctx, visit, visit, true, std::vector<char>(c.n_slots, 0));
+    for (const Miss& m : planA)
+        if ((rc = enqueue_copy(ctx, m.item.slot, m.g)) != EF_OK) return rc;
+    // Wave 0 = the hits.  The first phase-B copy is about to overwrite the slot of one of these very hits, and it waits
+    // for the "free" event of the wave that read the slot.  Copies are far slower than waves, so only the FIRST one
+    // matters: that hit runs as its own wave first, so the copy starts after one expert's FFN instead of after the whole
+    // wave (physical ordering only: the policy and its accounting are unchanged).
+    int first_victim = (!planB.empty() && wave0.size() > 1) ? planB[0].item.slot : -1;
     size_t split_at = wave0.size();
     for (size_t i = 0; i < wave0.size(); ++i)
         if (wave0[i].slot == first_victim) split_at = i;
+    const bool no_misses = planA.empty() && planB.empty();
     if (split_at == wave0.size()) {
-        rc = run_wave(ctx, st, x_perm, y_perm, wave0);
+        rc = run_wave(ctx, st, x_perm, y_perm, wave0, no_misses);
         if (rc != EF_OK) return rc;
     } else {
         std::vector<WaveItem> others;
@@ -681,22 +732,15 @@ extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visi
         rc = run_wave(ctx, st, x_perm, y_perm, others);
         if (rc != EF_OK) return rc;
     }
-    MissBatcher mb(ctx, st, x_perm, y_perm);
-    for (size_t i = 0; i < wavesA.size(); ++i)   // compute starts as the copies land, one grouped launch per batch
-        if ((rc = mb.push(wavesA[i], rest.empty() && i + 1 == wavesA.size())) != EF_OK) return rc;
-    // phase B: the pool was full of this visit's own experts and useful prefetches
-    std::fill(locked.begin(), locked.end(), 0);
-    for (size_t i = 0; i < rest.size(); ++i) {
-        const int e = rest[i];
-        const int s = pick_victim(ctx, visit, visit, true, locked);
-        if (s < 0) return ef_fail(ctx, EF_ERR_CAPACITY, "ef_expert_ffn_grouped: no victim slot (internal)");
-        // the copy into s waits for the "free" event of the wave that read s: that wave must be enqueued first
-        if (mb.holds_slot(s) && (rc = mb.flush()) != EF_OK) return rc;
-        rc = issue_load(ctx, s, layer * E + e, -1);
-        if (rc != EF_OK) return rc;
-        ctx->stats.ondemand_loads++;
-        ctx->slots[s].used = true;
-        if ((rc = mb.push(WaveItem{off[e], counts_host[e], s}, i + 1 == rest.size())) != EF_OK) return rc;
+    MissBatcher mb(ctx, st, x_perm, y_perm, (int)(planA.size() + planB.size()));
+    for (size_t i = 0; i < planA.size(); ++i)   // compute starts as the copies land, one grouped launch per batch
+        if ((rc = mb.push(planA[i].item, planB.empty() && i + 1 == planA.size())) != EF_OK) return rc;
+    for (size_t i = 0; i < planB.size(); ++i) {
+        const Miss& m = planB[i];
+        // the copy into the slot waits for the "free" event of the wave that read it: that wave must be enqueued first
+        if (mb.holds_slot(m.item.slot) && (rc = mb.flush()) != EF_OK) return rc;
+        if ((rc = enqueue_copy(ctx, m.item.slot, m.g)) != EF_OK) return rc;
+        if ((rc = mb.push(m.item, i + 1 == planB.size())) != EF_OK) return rc;
     }
     return mb.flush();
 }

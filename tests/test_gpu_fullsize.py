@@ -116,9 +116,9 @@ def decode_case(cfg, n_steps, sample_tokens, phys=0, forced_tokens=()):
       * `forced_tokens` (stacks only): before each visit the GPU's rows for these tokens are overwritten with the
         ORACLE's bf16 layer input, so every layer is compared on identical inputs under the per-layer north_star
         tolerance (teacher forcing from the oracle side, as in test_gpu_stages.py);
-      * `sample_tokens` run free on the GPU through all L layers; after l+1 layers the per-layer rounding errors
-        (independent, propagation gain ~1 in a pre-norm residual stack) add in quadrature, so the bound is the
-        per-layer one times sqrt(l+1) (error budget)."""
+      * `sample_tokens` run free on the GPU through all L layers; their error against the oracle's own chain is
+        measured after every layer and returned (free_err: mean relative, free_max: max abs / max|ref|) -- the caller
+        asserts on the measurement."""
     L, E, k = cfg.n_layers, cfg.n_experts, cfg.top_k
     n_phys = phys if phys else L * E
     gen = wl.scaled(cfg, phys_experts=phys)
@@ -147,6 +147,7 @@ def decode_case(cfg, n_steps, sample_tokens, phys=0, forced_tokens=()):
     n_free = len(free)
     forced_dev = torch.as_tensor(forced, dtype=torch.long, device="cuda")
     worst = {"free": 0.0, "forced": 0.0}
+    free_err, free_max = np.zeros(L), np.zeros(L)
     for s in range(n_steps):
         h0 = wl.activations(cfg, s)
         hd = dev_bf16(h0)
@@ -179,21 +180,28 @@ def decode_case(cfg, n_steps, sample_tokens, phys=0, forced_tokens=()):
             if forced:
                 _, m = check_float(got[n_free:], ref.out[n_free:])
                 worst["forced"] = max(worst["forced"], m)
-            if free and (l == L - 1 or l in (0, 7)):
-                g = np.sqrt(l + 1.0)
-                _, m = check_float(got[:n_free], ref.out[:n_free], max_tol=2e-2 * g, mean_tol=5e-3 * g)
-                worst["free"] = max(worst["free"], m / g)
+            if free and L > 1:
+                # free-running tokens: measured, not assumed -- the error after every layer goes into free_err
+                fr, rf = got[:n_free], ref.out[:n_free]
+                free_err[l] = max(free_err[l], np.abs(fr - rf).sum() / np.abs(rf).sum())
+                free_max[l] = max(free_max[l], np.abs(fr - rf).max() / np.abs(rf).max())
+            elif free:
+                _, m = check_float(got[:n_free], ref.out[:n_free])
+                worst["free"] = max(worst["free"], m)
             hd = dst
     r.ctx.ef_sync()
     st = r.ctx.ef_cache_get_stats()
     r.close()
-    print(f"{cfg.name}: worst mean-rel error forced {worst['forced']:.2e}, free/sqrt(layers) {worst['free']:.2e}")
-    return st, sim
+    print(f"{cfg.name}: worst mean-rel error forced {worst['forced']:.2e}, free (single layer) {worst['free']:.2e}")
+    if free and L > 1:
+        print("free-running mean-rel error by layer:", " ".join(f"{e:.2e}" for e in free_err))
+        print("free-running max-abs/max|ref| by layer:", " ".join(f"{e:.2e}" for e in free_max))
+    return st, sim, free_err, free_max
 
 
 def test_cfg3_mixtral_decode_full_size():
     cfg = wl.CONFIGS["mixtral_decode"]
-    st, sim = decode_case(cfg, n_steps=12, sample_tokens=range(cfg.T))
+    st, sim, _, _ = decode_case(cfg, n_steps=12, sample_tokens=range(cfg.T))
     assert st["hits"] + st["misses"] == st["lookups"] > 0
     assert st["bytes_h2d"] == cfg.expert_bytes * (st["ondemand_loads"] + st["prefetch_issued"])
 
@@ -202,6 +210,87 @@ def test_cfg5_stack_decode_full_shape():
     """32 layers x 8 experts at Mixtral shapes, 64 slots, 64 tokens; the 256 logical experts alias 16 physical host
     buffers so the test needs 5.6 GB of host memory, not 90 GB.  Two steps = 64 visits."""
     cfg = wl.CONFIGS["stack_decode"]
-    st, sim = decode_case(cfg, n_steps=2, sample_tokens=[0, 21], phys=16, forced_tokens=[42, 63])
+    st, sim, free_err, free_max = decode_case(cfg, n_steps=2, sample_tokens=[0, 9, 21, 30, 51, 58], phys=16,
+                                              forced_tokens=[42, 63])
     assert st["prefetch_issued"] > 0 and st["prefetch_used"] > 0
     assert st["hits"] + st["misses"] == st["lookups"] == sim.stats["lookups"]
+    # The FORCED tokens (oracle's bf16 input fed to every layer) hold the plain north_star tolerance at every layer: that
+    # is the parity claim, asserted inside decode_case.  The FREE-running tokens compare two chains that each round the
+    # hidden state to bf16 after every layer (the GPU's and the oracle's), so they drift apart; the drift is MEASURED at
+    # every layer and asserted to behave like accumulated rounding noise, not like a defect (DESIGN.md section 6):
+    #  (1) it stays inside the per-layer tolerance times sqrt(depth) at EVERY depth (measured on B200, 6 tokens x 2 steps:
+    #      2.5e-3 after layer 1, 1.2e-2 after 8, 2.6e-2 after 32 = 0.93 of the envelope);
+    #  (2) it grows sub-linearly with depth -- the fitted exponent of err ~ depth^p is 0.65 (a systematic error,
+    #      e.g. a biased rounding or a dropped term, accumulates with p >= 1);
+    #  (3) a single layer applied to the drifted state adds no more than a fresh layer does: err[l+1] - err[l] never
+    #      exceeds the first layer's own error by more than 50 %.
+    L = cfg.n_layers
+    depth = np.arange(1, L + 1)
+    assert (free_err <= 5e-3 * np.sqrt(depth)).all(), free_err / np.sqrt(depth)
+    assert (free_max <= 2e-2 * np.sqrt(depth)).all(), free_max / np.sqrt(depth)
+    p_fit = np.polyfit(np.log(depth), np.log(free_err), 1)[0]
+    print(f"free-running drift: err ~ depth^{p_fit:.2f}; err/envelope at the last layer {free_err[-1] / (5e-3 * np.sqrt(L)):.2f}")
+    assert 0.3 <= p_fit <= 0.85, p_fit
+    assert (np.diff(free_err) <= 1.5 * free_err[0]).all(), np.diff(free_err)
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json states configs[2] "for 256 steps" and configs[4] "for 128 steps": the WHOLE traces, at reduced d_model /
+# d_ff (the routing trace, the pool, the horizon and therefore every policy decision do not depend on them), with the slot
+# table and all nine counters compared with the simulator after EVERY visit.
+# ------------------------------------------------------------------------------------------------
+def full_trace_accounting(name, horizon, d_model=128, d_ff=256, phys=8):
+    base = wl.CONFIGS[name]
+    cfg = wl.scaled(base, d_model=d_model, d_ff=d_ff, horizon=horizon)
+    L, E, k, T, n_steps = cfg.n_layers, cfg.n_experts, cfg.top_k, cfg.T, cfg.n_steps
+    assert (n_steps, T, cfg.n_slots) == (base.n_steps, base.T, base.n_slots)
+    gen = wl.scaled(cfg, phys_experts=phys)
+    store = {p: wl.expert_weights(gen, p // E, p % E) for p in range(phys)}
+    ex = {(l, e): store[(l * E + e) % phys] for l in range(L) for e in range(E)}
+    r = make_runner(cfg, ex)
+    tr = wl.routing_trace(cfg, n_steps)
+    sim = CacheSim(L, E, cfg.n_slots, cfg.expert_bytes, cfg.horizon)
+    nv = n_steps * L
+    look = L if cfg.horizon <= 0 else cfg.horizon
+    window = lambda v: tr.predicted[v + 1:min(nv, v + 1 + look)]
+    w0 = window(-1)
+    sim.prefetch(-1, w0); r.ctx.ef_cache_prefetch(-1, w0)
+    bufs = [torch.empty((T, cfg.d_model), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    lookups = 0
+    for s in range(n_steps):
+        hd = dev_bf16(wl.activations(cfg, s))
+        for l in range(L):
+            v = s * L + l
+            win = window(v)
+            dst = bufs[l & 1]
+            r.visit(v, hd, dst, token_bias=torch.from_numpy(wl.trace_bias(cfg, tr, v)).cuda(),
+                    predicted_next=win if len(win) else None, residual=hd if L > 1 else None,
+                    pre_norm_eps=1e-5 if L > 1 else None)
+            counts = np.bincount(tr.sets[v].ravel(), minlength=E)
+            lookups += int((counts > 0).sum())
+            sim.visit(v, counts)
+            if len(win):
+                sim.prefetch(v, win)
+            assert_cache_equal(r, sim)                                        # slot table + 9 counters, every visit
+            hd = dst
+    r.ctx.ef_sync()
+    assert np.array_equal(r.counts.cpu().numpy(), counts)                     # the trace bias drove the router to the end
+    st = r.ctx.ef_cache_get_stats()
+    assert st["lookups"] == lookups == st["hits"] + st["misses"] and st["ondemand_loads"] == st["misses"]
+    assert st["bytes_h2d"] == cfg.expert_bytes * (st["ondemand_loads"] + st["prefetch_issued"])
+    r.close()
+    return cfg, st
+
+
+def test_cfg3_whole_trace_256_steps_accounting():
+    cfg, st = full_trace_accounting("mixtral_decode", horizon=None or wl.CONFIGS["mixtral_decode"].horizon)
+    assert cfg.n_steps == 256 and st["lookups"] > 256 * 4
+    assert 0.5 < st["hits"] / st["lookups"] < 0.95                  # 6 of 8 slots, ~7.8 active experts per step (S 8(d))
+
+
+@pytest.mark.parametrize("horizon", [0, 1], ids=["fill", "one_visit_ahead"])
+def test_cfg5_whole_trace_128_steps_accounting(horizon):
+    """32 layers x 128 steps = 4096 visits, 64 tokens, 64 slots, both prefetch horizons (R10)."""
+    cfg, st = full_trace_accounting("stack_decode", horizon=horizon)
+    assert cfg.n_steps == 128 and cfg.n_layers == 32
+    assert st["lookups"] >= 4096 * 7 and st["prefetch_issued"] > 0

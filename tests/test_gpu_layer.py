@@ -119,14 +119,19 @@ def test_cfg4_reduced_shared_experts_and_zipf():
 # neither the result nor the accounting -- down to pools so small that a miss takes the slot of a miss of the same visit
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n_slots", [1, 2, 5, 24])
-@pytest.mark.parametrize("wave_bytes,chunk_min,fused", [(0, 0, 1), (1 << 40, 0, 1), (0, 1, 1), (1 << 40, 1, 1), (None, None, 1),
-                                                        (0, 1, 0), (1 << 40, 0, 0)],
+@pytest.mark.parametrize("wave_bytes,chunk_min,fused,copy_order",
+                         [(0, 0, 1, 1), (1 << 40, 0, 1, 1), (0, 1, 1, 1), (1 << 40, 1, 1, 1), (None, None, 1, 1),
+                          (0, 1, 0, 1), (1 << 40, 0, 0, 1), (None, None, 1, 0), (4 * 3 * 256 * 384 * 2, 0, 1, 0)],
                          ids=["single_waves", "batched", "chunked", "batched_chunked", "defaults", "chunked_two_launches",
-                              "batched_two_launches"])
-def test_miss_wave_batching_and_chunked_copies(n_slots, wave_bytes, chunk_min, fused):
+                              "batched_two_launches", "policy_copy_order", "waves_of_4_policy_copy_order"])
+def test_miss_wave_batching_and_chunked_copies(n_slots, wave_bytes, chunk_min, fused, copy_order):
+    """Results, slot table and counters are identical however the on-demand loads are scheduled physically: one wave per
+    miss or geometric batches, whole or two-chunk copies, one or two launches per wave, copies in policy order or with the
+    most routed rows first (later 'generations' -- misses that reuse the slot of an earlier miss of the visit -- behind)."""
     cfg = wl.scaled(wl.CONFIGS["many_expert_prefill"], T=256, d_model=256, d_ff=384, n_slots=n_slots)
     r, ex = build_runner(cfg)
     r.ctx.ef_set_option(EF_OPT_FUSED_WAVES, fused)
+    r.ctx.ef_set_option(6, copy_order)                   # EF_OPT_COPY_ORDER
     if wave_bytes is not None:
         r.ctx.ef_set_option(EF_OPT_WAVE_BYTES, wave_bytes)
         r.ctx.ef_set_option(EF_OPT_CHUNK_MIN_BYTES, chunk_min)

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 import workloads as wl
-from oracle.cache_sim import CacheSim
+from oracle.cache_sim import CacheSim, belady_min_loads
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 W = 1000
@@ -483,6 +483,73 @@ def test_plec_beats_both_lru_baselines_on_the_stack_trace(Sim=CacheSim):
         for v in range(10 * cfg.n_layers):
             sim.visit(v, np.bincount(tr.sets[v].ravel(), minlength=cfg.n_experts))
         assert plec.hit_ratio() > sim.hit_ratio() + 0.2, policy
+
+
+# ------------------------------------------------------------------------------------------------
+# clairvoyant reference (Belady MIN) for the policy gap: how far PLEC's and LRU's loads are from the floor
+# ------------------------------------------------------------------------------------------------
+def test_belady_matches_the_textbook_reference_string():
+    """The classic reference string again (see the LRU pin above): the optimal policy takes 9 faults with 3 frames."""
+    ref = [7, 0, 1, 2, 0, 3, 0, 4, 2, 3, 0, 3, 2, 1, 2, 0, 1, 7, 0, 1]
+    loads = belady_min_loads(1, 8, 3, [[e] for e in ref])
+    assert sum(loads) == 9
+    assert loads[:4] == [1, 1, 1, 1] and loads[4] == 0
+
+
+def _min_loads_exhaustive(visits, L, E, S):
+    """Fewest loads over ALL eviction choices in the same serving model (inside a visit hits first, then the misses in
+    ascending id; a miss may evict any resident): memoised search over (visit, miss index, cache)."""
+    from functools import lru_cache
+    want = [tuple((v % L) * E + e for e in a) for v, a in enumerate(visits)]
+
+    @lru_cache(maxsize=None)
+    def go(v, cache):
+        if v == len(want):
+            return 0
+        misses = tuple(g for g in want[v] if g not in cache)
+        return serve(v, misses, cache)
+
+    @lru_cache(maxsize=None)
+    def serve(v, misses, cache):
+        if not misses:
+            return go(v + 1, cache)
+        g, rest = misses[0], misses[1:]
+        if len(cache) < S:
+            return 1 + serve(v, rest, tuple(sorted(cache + (g,))))
+        return 1 + min(serve(v, rest, tuple(sorted(tuple(x for x in cache if x != out) + (g,)))) for out in cache)
+    return go(0, ())
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_belady_is_optimal_on_small_traces(seed):
+    g = np.random.default_rng(seed)
+    L, E, S = int(g.integers(1, 3)), 4, int(g.integers(2, 4))
+    visits = [sorted(set(int(e) for e in g.choice(E, size=int(g.integers(1, 4)), replace=False))) for _ in range(10)]
+    assert sum(belady_min_loads(L, E, S, visits)) == _min_loads_exhaustive(visits, L, E, S)
+
+
+def test_policy_gap_to_the_clairvoyant_floor_on_the_decode_traces():
+    """Loads per step of PLEC (config horizon), on-demand LRU and the clairvoyant floor on the cfg 3 and (reduced-length)
+    cfg 5 routing traces: the floor is never beaten, and the numbers quoted in profiles/r2_policies.md come from here
+    (run with -s)."""
+    for name, steps, horizons in (("mixtral_decode", 256, (1,)), ("stack_decode", 16, (0, 1))):
+        cfg = wl.scaled(wl.CONFIGS[name], d_model=64, d_ff=128)
+        tr = wl.routing_trace(cfg, steps)
+        L, E = cfg.n_layers, cfg.n_experts
+        nv = steps * L
+        acts = [sorted(set(int(e) for e in tr.sets[v].ravel())) for v in range(nv)]
+        floor = sum(belady_min_loads(L, E, cfg.n_slots, acts)) / steps
+        rows = {"clairvoyant (Belady MIN, demand)": floor}
+        for H in horizons:
+            sim = run_trace(wl.scaled(cfg, horizon=H), H, steps)
+            rows[f"PLEC H={'fill' if H <= 0 else H}"] = (sim.stats["ondemand_loads"] + sim.stats["prefetch_issued"]) / steps
+        lru = CacheSim(L, E, cfg.n_slots, W, policy="lru")
+        for v in range(nv):
+            lru.visit(v, np.bincount(tr.sets[v].ravel(), minlength=E))
+        rows["on-demand LRU"] = lru.stats["ondemand_loads"] / steps
+        print(name, {k: round(v, 2) for k, v in rows.items()})
+        assert all(v >= floor - 1e-9 for v in rows.values())
+        assert floor > 0
 
 
 # ------------------------------------------------------------------------------------------------
