@@ -70,7 +70,8 @@ constexpr int kThreads = 384;
 constexpr int kEpiWarps = 8;
 constexpr int kSched = 4;               // depth of the tile-broadcast ring
 constexpr int kTmemCols = 512;
-constexpr int kSlotFloats = 2 * 128 * 256;   // split-K workspace slot: two 128-lane x 256-column fp32 accumulators
+constexpr int kSlotFloats = 2 * 128 * 256;   // LARGEST split-K workspace slot: two 128-lane x 256-column fp32 accumulators; a wave whose
+                                             // token tiles are narrower uses proportionally smaller slots (PhaseArgs::ws_acc_f4)
 // Epilogue staging (transpose): per column-parity group of 4 warps one [32 tokens][128 features] bf16 tile, rows
 // padded by 16 B so that stmatrix rows (stride 272 B) and 16-byte read-backs are bank-conflict free
 constexpr int STG_LD = ACC_M * 2 + 16;
@@ -78,6 +79,13 @@ constexpr int STG_BYTES = 32 * STG_LD;
 
 // -DEF_KPROF: the MMA-issuing lane of every CTA accumulates the cycles it spends waiting for a tile ticket, for the
 // epilogue to free TMEM and for TMA to fill a stage, and dumps them per CTA (ef_debug_kprof).  Off in normal builds.
+// -DEF_KTIME (with -DEF_KPROF): instead of the wait cycles, the same five words hold a TIMELINE of the pair in globaltimer
+// nanoseconds: {prologue done, first stage full, last GEMM1 unit issued, first GEMM2 stage full, last unit issued}.
+#ifdef EF_KTIME
+#define KTIME(...) __VA_ARGS__
+#else
+#define KTIME(...)
+#endif
 #ifdef EF_KPROF
 #define KPROF(...) __VA_ARGS__
 #else
@@ -257,27 +265,28 @@ __device__ __forceinline__ void stage_to_global(const uint8_t* stg, uint16_t* __
     named_bar(bar_id, 128);
 }
 
-// split-K workspace slot layout: [accumulator][column / 4][lane][4 floats] -- a warp's float4 accesses are contiguous
-__device__ __forceinline__ void ws_store32(float* slot, int acc, int c, int lane128, const uint32_t (&v)[32]) {
-    float4* p = reinterpret_cast<float4*>(slot) + (size_t)acc * (ACC_M * BT / 4) + (size_t)(c * 8) * ACC_M + lane128;
+// split-K workspace slot layout: [accumulator][column / 4][lane][4 floats] -- a warp's float4 accesses are contiguous;
+// acc_f4 = float4 words per accumulator = 8 * 128 * (32-token chunks of the wave's widest tile)
+__device__ __forceinline__ void ws_store32(float* slot, int acc_f4, int acc, int c, int lane128, const uint32_t (&v)[32]) {
+    float4* p = reinterpret_cast<float4*>(slot) + (size_t)acc * acc_f4 + (size_t)(c * 8) * ACC_M + lane128;
 #pragma unroll
     for (int i = 0; i < 8; ++i)
         p[(size_t)i * ACC_M] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
                                            __uint_as_float(v[4 * i + 3]));
 }
 // sum over the s partial slots of a tile, in slot order; L2-only loads (the partials were written by other SMs)
-__device__ __forceinline__ void ws_sum32(const float* tile_slots, int s, int acc, int c, int lane128, uint32_t (&out)[32]) {
+__device__ __forceinline__ void ws_sum32(const float* tile_slots, int acc_f4, int s, int acc, int c, int lane128, uint32_t (&out)[32]) {
     float4 sum[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) sum[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    const float4* p = reinterpret_cast<const float4*>(tile_slots) + (size_t)acc * (ACC_M * BT / 4) + (size_t)(c * 8) * ACC_M + lane128;
+    const float4* p = reinterpret_cast<const float4*>(tile_slots) + (size_t)acc * acc_f4 + (size_t)(c * 8) * ACC_M + lane128;
     for (int j = 0; j < s; ++j) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const float4 v = __ldcg(p + (size_t)i * ACC_M);
             sum[i].x += v.x; sum[i].y += v.y; sum[i].z += v.z; sum[i].w += v.w;
         }
-        p += 2 * (kSlotFloats / 4);      // slots alternate between the two CTAs of the pair
+        p += 2 * (2 * acc_f4);           // slots alternate between the two CTAs of the pair
     }
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
@@ -302,7 +311,8 @@ struct PhaseArgs {
     int32_t total;                 // tickets of this phase
     int32_t n_plain, s;            // tickets [0, n_plain) are whole tiles; the rest are (tile, K part) pairs, part fastest;
                                    // s = K parts per split tile (>= 2 when any tile is split)
-    float* ws;                     // [n_split_tiles * s * 2] slots of kSlotFloats fp32
+    int32_t ws_acc_f4;             // float4 words per accumulator in a workspace slot (a slot = 2 accumulators)
+    float* ws;                     // [n_split_tiles * s * 2] slots of 8 * ws_acc_f4 fp32
     int32_t* counters;             // [n_split_tiles * 2] arrival counters, zero between launches
 };
 
@@ -433,7 +443,8 @@ __device__ __forceinline__ void epilogue_unit(const Tile& t, const PhaseArgs& p,
     const int n_tile = 2 * t.n_pair + (int)rank;
     const bool tile_ok = n_tile < p.n_tiles_n;    // false: the odd last weight tile's idle partner
     const bool split = t.tail >= 0;
-    float* ws_mine = split ? p.ws + (((size_t)t.tail * p.s + t.split_j) * 2 + rank) * kSlotFloats : nullptr;
+    const size_t slot_floats = (size_t)8 * p.ws_acc_f4;
+    float* ws_mine = split ? p.ws + (((size_t)t.tail * p.s + t.split_j) * 2 + rank) * slot_floats : nullptr;
     uint16_t* __restrict__ C = p.C;
     const int ldc = p.ldc, n_cols = p.n_cols;
     const uint32_t tb0 = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b0 * 256);
@@ -450,10 +461,10 @@ __device__ __forceinline__ void epilogue_unit(const Tile& t, const PhaseArgs& p,
             uint32_t a0[32];
             tc_ld32(tb0 + c * 32, a0);
             tc_wait_ld();
-            ws_store32(ws_mine, 0, c, lane128, a0);
+            ws_store32(ws_mine, p.ws_acc_f4, 0, c, lane128, a0);
             tc_ld32(tb1 + c * 32, a0);
             tc_wait_ld();
-            ws_store32(ws_mine, 1, c, lane128, a0);
+            ws_store32(ws_mine, p.ws_acc_f4, 1, c, lane128, a0);
             continue;
         }
 #pragma unroll 1
@@ -509,20 +520,32 @@ __device__ __forceinline__ void epilogue_unit(const Tile& t, const PhaseArgs& p,
         const bool last = ctl->split_last != 0;          // rewritten only after the next split unit's first barrier
         if (last) {
             __threadfence();
-            const float* ws_tile = p.ws + ((size_t)t.tail * p.s * 2 + rank) * kSlotFloats;
+            const float* ws_tile = p.ws + ((size_t)t.tail * p.s * 2 + rank) * slot_floats;
+            uint16_t* srow = reinterpret_cast<uint16_t*>(stg) + lane128;           // [token][feature], 2-byte stores
+            if (kSwiglu) {
 #pragma unroll 1
-            for (int c = part; c < n_chunks; c += 2) {
-                const int n_rows = min(32, t.rows_valid - c * 32);
-                uint32_t a0[32], a1[32];
-                ws_sum32(ws_tile, p.s, 0, c, lane128, a0);
-                ws_sum32(ws_tile, p.s, 1, c, lane128, a1);
-                uint16_t* srow = reinterpret_cast<uint16_t*>(stg) + lane128;       // [token][feature], 2-byte stores
+                for (int c = part; c < n_chunks; c += 2) {
+                    const int n_rows = min(32, t.rows_valid - c * 32);
+                    uint32_t a0[32], a1[32];
+                    ws_sum32(ws_tile, p.ws_acc_f4, p.s, 0, c, lane128, a0);
+                    ws_sum32(ws_tile, p.ws_acc_f4, p.s, 1, c, lane128, a1);
+#pragma unroll
+                    for (int i = 0; i < 32; ++i)
+                        srow[i * (STG_LD / 2)] = bf16_bits(silu_mul(__uint_as_float(a0[i]), __uint_as_float(a1[i])));
+                    stage_to_global(stg, C, ldc, (int64_t)t.c_row + c * 32, n_rows, col0, n_cols, lane128, 2 + part);
+                }
+            } else {
+                // the two accumulators are independent output columns: the (chunk, accumulator) items alternate between the
+                // two warp groups, so a one-chunk decode tile is reduced by both groups at once
 #pragma unroll 1
-                for (int acc = 0; acc < (kSwiglu ? 1 : 2); ++acc) {
+                for (int w = part; w < 2 * n_chunks; w += 2) {
+                    const int c = w >> 1, acc = w & 1;
+                    const int n_rows = min(32, t.rows_valid - c * 32);
+                    uint32_t a0[32];
+                    ws_sum32(ws_tile, p.ws_acc_f4, p.s, acc, c, lane128, a0);
 #pragma unroll
                     for (int i = 0; i < 32; ++i) {
-                        float v = kSwiglu ? silu_mul(__uint_as_float(a0[i]), __uint_as_float(a1[i]))
-                                          : __uint_as_float(acc ? a1[i] : a0[i]);
+                        float v = __uint_as_float(a0[i]);
                         if (kRelu) v = fmaxf(v, 0.f);
                         srow[i * (STG_LD / 2)] = bf16_bits(v);
                     }
@@ -547,6 +570,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                 int balanced, int n_token_tiles, int32_t* __restrict__ sched /* {tickets, finished CTAs, ready[n_token_tiles]} */,
                 long long* __restrict__ kprof, const __grid_constant__ EfWaveTable tab) {
     extern __shared__ uint8_t smem_raw[];
+    KTIME(long long kt_entry; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(kt_entry));)
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t* stg_base = smem + (size_t)kStages * STAGE_BYTES;
     SmemCtl* ctl = (SmemCtl*)(stg_base + 2 * STG_BYTES);
@@ -657,6 +681,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
             int stage = 0; uint32_t phase = 0;
             int buf = 0; uint32_t bphase = 0;          // bit b = phase of TMEM half b
             KPROF(long long kp_t0 = clock64(); long long kp_sched = 0, kp_tmem = 0, kp_full = 0; int kp_units = 0;)
+            KTIME(long long kt[5] = {kt_entry, 0, 0, 0, 0}; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(kt[1]));)
             for (int it = 0;; ++it) {
                 const int ss = it % kSched;
                 KPROF(long long kp_a = clock64();)
@@ -679,6 +704,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                     KPROF(long long kp_c = clock64();)
                     mbar_wait(&ctl->full[stage], phase);
                     KPROF(kp_full += clock64() - kp_c;)
+                    KTIME(if (t.phase == 1 && !kt[3]) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(kt[3]));)
                     tc_fence_after();
                     const uint32_t sw = smem_u32(smem + (size_t)stage * STAGE_BYTES);
                     const uint32_t sx = sw + W_BYTES;
@@ -697,7 +723,9 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                     bphase ^= 1u << (b0 + h);
                 }
                 buf = t.is_long ? 0 : (b0 ^ 1);
+                KTIME(asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(kt[t.phase == 0 ? 2 : 4]));)
             }
+            KTIME(if (kprof) { long long* o = kprof + (size_t)(blockIdx.x >> 1) * 5; for (int i = 0; i < 5; ++i) o[i] = kt[i]; kprof = nullptr; })
             KPROF(if (kprof) {
                 long long* o = kprof + (size_t)(blockIdx.x >> 1) * 5;
                 o[0] = clock64() - kp_t0; o[1] = kp_sched; o[2] = kp_tmem; o[3] = kp_full; o[4] = kp_units;
@@ -734,6 +762,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
     }
+    KTIME(if (threadIdx.x == 0 && kprof) { long long te; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(te)); kprof[(size_t)(148 / 2) * 5 + blockIdx.x] = te; })
     // the last CTA to finish re-arms the scheduler words and the ready counters for the launch that reuses them (every
     // leader has drawn its terminal ticket and every GEMM2 producer has seen its counter by now)
     if (threadIdx.x == 0) {
@@ -806,10 +835,11 @@ int32_t* next_sched(ef_ctx* ctx, int n_words) {
 // Tail split-K plan for one phase: `tiles` tickets in scheduler order with `n_short` short ones at the end, G CTA pairs,
 // KB k-blocks per tile.  Costs are in k-block times of a 256-row tile (1024 tensor cycles): a whole tail tile holds
 // an SM for KB (KB/2 if short) of them; a split unit adds a partial write and the finaliser reads s partials
-// (~0.03 per valid row each, from the measured ~50 GB/s per-SM global bandwidth).
+// (~0.03 per valid row each, from the measured ~50 GB/s per-SM global bandwidth, and never less than a dependent
+// round trip each).
 struct SplitPlan { int n_plain, n_tail, s; };
 
-SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, double avg_rows) {
+SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, double avg_rows, int max_units) {
     SplitPlan p{tiles, 0, 1};
     if (ctx->splitk_mode == 1 || tiles == 0) return p;
     int r = tiles % G;
@@ -817,7 +847,7 @@ SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, d
     if (ctx->splitk_mode >= 2) {                       // forced (tests): split every tile
         p.s = std::min(ctx->splitk_mode, std::max(1, KB));
         if (p.s < 2) return SplitPlan{tiles, 0, 1};
-        p.n_tail = std::min(tiles, ctx->splitk_max_units / p.s);
+        p.n_tail = std::min(tiles, max_units / p.s);
         p.n_plain = tiles - p.n_tail;
         return p.n_tail ? p : SplitPlan{tiles, 0, 1};
     }
@@ -827,8 +857,12 @@ SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, d
     const int smax = std::min(16, KB / 4);
     double best = KB * w;                              // s = 1: one more round of whole tiles
     for (int s = 2; s <= smax; ++s) {
-        if (r * s > ctx->splitk_max_units) break;
-        const double cost = (double)((r * s + G - 1) / G) * (KB * w / s) + 1.0 + ovh * (1 + s);
+        if (r * s > max_units) break;
+        // the finaliser walks the s partials one after the other: bandwidth for wide tiles (ovh per partial), a dependent
+        // L2 round trip per partial and accumulator for narrow ones (measured on a 5-token decode tile: ~4 us for s = 5,
+        // which turned a 48 us GEMM1 into 68 us -- a decode GEMM1 is not split, its HBM stream is what bounds it)
+        const double fin = std::max(ovh * (1 + s), 1.5 * s);
+        const double cost = (double)((r * s + G - 1) / G) * (KB * w / s) + 1.0 + fin;
         if (cost < best * 0.9) { best = cost; p.s = s; }
     }
     if (p.s > 1) { p.n_tail = r; p.n_plain = tiles - r; }
@@ -860,10 +894,12 @@ int32_t efk_ffn_tc_init(ef_ctx* ctx) {
     EF_CUDA(ctx, cudaMalloc(&ctx->sched_words, sizeof(int32_t) * EF_SCHED_WORDS));
     EF_CUDA(ctx, cudaMemset(ctx->sched_words, 0, sizeof(int32_t) * EF_SCHED_WORDS));
     // split-K: pair units; each has one workspace slot and one counter per CTA of the pair; one region per GEMM of a wave
+    // (splitk_max_units full-size slots per CTA of the pair; a wave of narrower token tiles cuts the same memory into up to
+    // 8x as many smaller slots -- a decode wave's tile is one 32-token chunk wide -- hence 8x the arrival counters)
     ctx->splitk_max_units = ctx->n_sms;
     EF_CUDA(ctx, cudaMalloc(&ctx->splitk_ws, sizeof(float) * kSlotFloats * 2 * 2 * (size_t)ctx->splitk_max_units));
-    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_counters, sizeof(int32_t) * 2 * 2 * ctx->splitk_max_units));
-    EF_CUDA(ctx, cudaMemset(ctx->splitk_counters, 0, sizeof(int32_t) * 2 * 2 * ctx->splitk_max_units));
+    EF_CUDA(ctx, cudaMalloc(&ctx->splitk_counters, sizeof(int32_t) * 2 * 2 * 8 * ctx->splitk_max_units));
+    EF_CUDA(ctx, cudaMemset(ctx->splitk_counters, 0, sizeof(int32_t) * 2 * 2 * 8 * ctx->splitk_max_units));
     ctx->tm_ok = true;
     return EF_OK;
 }
@@ -877,8 +913,10 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     const bool bal = d >= kBalancedMinK && f >= kBalancedMinK;
     int64_t rows_total = 0, x_rows = 0;
     int mtiles = 0, mshort = 0;       // token tiles of the wave (every group's long tiles plus its short tail tile)
+    int widest = 1;                   // rows of the wave's widest token tile
     for (int i = 0; i < tab.n; ++i) {
         rows_total += tab.g[i].rows;
+        widest = std::max(widest, std::min(tab.g[i].rows, group_tile_rows(tab.g[i].rows, bal)));
         x_rows = std::max<int64_t>(x_rows, (int64_t)tab.g[i].x_row0 + tab.g[i].rows);
         mtiles += group_long_tiles(tab.g[i].rows, bal) + group_has_short(tab.g[i].rows, bal);
         mshort += group_has_short(tab.g[i].rows, bal);
@@ -890,16 +928,22 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     PhaseArgs pa[2] = {};
     // GEMM1: 256 packed W13 rows -> 128 h columns; 256 W1 rows -> 256
     const int ntn1 = relu ? (f + BW - 1) / BW : f / 128, ntn2 = (d + BW - 1) / BW;
-    pa[0] = PhaseArgs{(uint16_t*)ctx->h_ws, f, f, d / BK, ntn1, (ntn1 + 1) / 2, w1_rows, 0, 0, 0, 1, ctx->splitk_ws, ctx->splitk_counters};
-    pa[1] = PhaseArgs{(uint16_t*)y, d, d, f / BK, ntn2, (ntn2 + 1) / 2, d, (int)((int64_t)w1_rows * d / EF_ROWLET), 0, 0, 1,
-                      ctx->splitk_ws + (size_t)kSlotFloats * 2 * ctx->splitk_max_units, ctx->splitk_counters + 2 * ctx->splitk_max_units};
+    // split-K workspace slots are as wide as the wave's widest tile (in 32-token chunks): a decode wave gets 8x the units
+    const int chunks = (widest + 31) / 32;
+    const int acc_f4 = chunks * 8 * ACC_M;
+    const int max_units = ctx->splitk_max_units * (BT / 32) / chunks;
+    pa[0] = PhaseArgs{(uint16_t*)ctx->h_ws, f, f, d / BK, ntn1, (ntn1 + 1) / 2, w1_rows, 0, 0, 0, 1, acc_f4, ctx->splitk_ws,
+                      ctx->splitk_counters};
+    pa[1] = PhaseArgs{(uint16_t*)y, d, d, f / BK, ntn2, (ntn2 + 1) / 2, d, (int)((int64_t)w1_rows * d / EF_ROWLET), 0, 0, 1, acc_f4,
+                      ctx->splitk_ws + (size_t)kSlotFloats * 2 * ctx->splitk_max_units,
+                      ctx->splitk_counters + 2 * 8 * ctx->splitk_max_units};
     for (int ph = 0; ph < 2; ++ph) {
         if (!(phase & (1 << ph))) continue;
         PhaseArgs& p = pa[ph];
         const int tiles = mtiles * p.n_pairs_n;
         // GEMM1 of a fused wave is followed by GEMM2 units that depend on it: its tail cannot be filled by them when the wave
         // is one token tile deep, so it is split like a launch of its own
-        const SplitPlan pl = plan_split(ctx, tiles, mshort * p.n_pairs_n, n_pairs, p.KB, avg_rows);
+        const SplitPlan pl = plan_split(ctx, tiles, mshort * p.n_pairs_n, n_pairs, p.KB, avg_rows, max_units);
         p.n_plain = pl.n_plain;
         p.s = pl.s;
         p.total = pl.n_plain + pl.n_tail * pl.s;
