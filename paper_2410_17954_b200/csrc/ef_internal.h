@@ -140,8 +140,8 @@ struct ef_ctx {
     void* ts_dist = nullptr;
     size_t ts_dist_bytes = 0;
     bool ts_small_attr = false;         // ts_small_kernel opted in to > 48 KB dynamic smem
-    int32_t ts_force_multi = 0;         // test hook (ef_set_token_sched_path): 1 = never take the single-CTA path
-    // physical scheduling knobs (never part of the policy): see ef_set_wave_bytes / ef_set_chunk_min_bytes
+    int32_t ts_force_multi = 0;         // test hook (EF_OPT_TOKEN_SCHED_PATH): 1 = never take the single-CTA path
+    // physical scheduling knobs (never part of the policy): ef_set_option(EF_OPT_WAVE_BYTES / EF_OPT_CHUNK_MIN_BYTES)
     int64_t wave_bytes = (int64_t)128 << 20;
     int64_t chunk_min_bytes = (int64_t)32 << 20;
     int32_t copy_order = 1;             // EF_OPT_COPY_ORDER

@@ -78,7 +78,7 @@ constexpr int STG_LD = ACC_M * 2 + 16;
 constexpr int STG_BYTES = 32 * STG_LD;
 
 // -DEF_KPROF: the MMA-issuing lane of every CTA accumulates the cycles it spends waiting for a tile ticket, for the
-// epilogue to free TMEM and for TMA to fill a stage, and dumps them per CTA (ef_debug_kprof).  Off in normal builds.
+// epilogue to free TMEM and for TMA to fill a stage, and dumps them per CTA (ef_diag_kprof, diag library).  Off in normal builds.
 // -DEF_KTIME (with -DEF_KPROF): instead of the wait cycles, the same five words hold a TIMELINE of the pair in globaltimer
 // nanoseconds: {prologue done, first stage full, last GEMM1 unit issued, first GEMM2 stage full, last unit issued}.
 #ifdef EF_KTIME
@@ -419,13 +419,23 @@ __device__ __forceinline__ void signal_ready(int32_t* cnt) {
     asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(cnt) : "memory");
 }
 __device__ __forceinline__ void wait_ready(const int32_t* cnt, int need) {
+    // The GEMM1 units this waits for were all claimed before the first GEMM2 ticket was handed out, by CTAs that never wait
+    // themselves, so the wait is bounded by one unit's duration.  A signal that never comes would be a bug in this file:
+    // after 10 s of wall time (globaltimer; robust against slow clocks, preemption and profilers' replays) the kernel
+    // traps -- a sticky CUDA error at the C ABI -- instead of hanging the device.
     int v = 0;
-    for (long long spins = 0; spins < (1ll << 25); ++spins) {       // bounded (~ seconds): a lost signal traps, never hangs
+    unsigned long long t0 = 0;
+    for (unsigned spins = 0;; ++spins) {
         asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(cnt) : "memory");
         if (v >= need) break;
         __nanosleep(100);
+        if ((spins & 1023u) == 1023u) {
+            unsigned long long t;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+            if (t0 == 0) t0 = t;
+            else if (t - t0 > 10000000000ull) __trap();
+        }
     }
-    if (v < need) __trap();
     asm volatile("fence.proxy.async;" ::: "memory");                // the rows were written through the generic proxy; TMA reads them
 }
 

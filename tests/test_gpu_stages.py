@@ -241,6 +241,44 @@ def test_ffn_many_groups_many_waves_in_one_launch():
     ctx.close()
 
 
+def test_fused_wave_is_bit_identical_to_two_launches_and_to_itself():
+    """Race detector for the in-launch GEMM1 -> GEMM2 hand-over (per-token-tile ready counters, generic-proxy stores read
+    back through TMA): both modes use the same tiling and the same split-K plan, so ONE launch must give bit for bit what
+    two launches give, on every repetition, for ragged random waves that mix empty, tiny, 129..256-row and multi-tile
+    groups (more units than CTA pairs, so GEMM2 units of early groups run while late GEMM1 units are in flight)."""
+    from paper_2410_17954_b200 import EF_OPT_FUSED_WAVES
+    E, d, f = 24, 512, 768
+    g = wl.stream(9, "ffn.fused")
+    ctx = make_ctx(n_experts=E, top_k=1, d_model=d, d_ff=f, n_slots=E, max_tokens=6000)
+    cfg = wl.scaled(wl.CONFIGS["tiny"], d_model=d, d_ff=f, n_experts=E, seed=41)
+    for e in range(E):
+        ctx.ef_host_expert_register(0, e, *wl.expert_weights(cfg, 0, e))
+    ctx.ef_cache_prefetch(-1, np.ones((1, E), np.uint8))
+    slot_of = {gid: s for s, gid in enumerate(ctx.ef_cache_snapshot())}
+    for trial in range(10):
+        kind = g.integers(0, 4, size=E)
+        counts = np.where(kind == 0, 0, np.where(kind == 1, g.integers(1, 40, size=E),
+                          np.where(kind == 2, g.integers(129, 257, size=E), g.integers(257, 700, size=E)))).astype(int)
+        if counts.sum() == 0:
+            counts[0] = 5
+        offs = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+        R = int(offs[-1])
+        x = dev_bf16(wl.normal_bf16(100 + trial, "xperm", (R, d), 1.0))
+        act = [e for e in range(E) if counts[e] > 0]
+        args = ([int(offs[e]) for e in act], [int(counts[e]) for e in act], [slot_of[e] for e in act])
+        outs = []
+        for fused in (1, 0, 1, 1):
+            y = torch.full((R, d), float("nan"), dtype=torch.bfloat16, device="cuda")
+            ctx.ef_set_option(EF_OPT_FUSED_WAVES, fused)
+            ctx.ef_expert_ffn_grouped_resident(x, *args, y)
+            ctx.ef_sync()
+            outs.append(to_bits(y))
+        assert not np.isnan(bf(outs[0])).any()
+        for o in outs[1:]:
+            assert np.array_equal(o, outs[0]), (trial, counts.tolist())
+    ctx.close()
+
+
 def test_ffn_splitk_repeated_launches_rearm_counters():
     """The arrival counters and scheduler words re-arm themselves: many launches in a row, alternating split
     factors, all give the same answer as the unsplit kernel up to fp32 summation order."""
