@@ -25,6 +25,11 @@
  *     on different streams concurrently.  Inside a lane, a call on a stream other than the lane's previous one is
  *     ordered behind everything the lane has enqueued so far (the library inserts the event wait), so changing
  *     streams is safe but never concurrent.
+ *   - CUDA graphs: the memory-bound calls (ef_rmsnorm, ef_route_topk, ef_permute, ef_combine, ef_reindex_rows) may be
+ *     issued on a stream that is being captured; the library then inserts no cross-stream ordering (ordering the replayed
+ *     graph against other work on the same ctx is the caller's job) and a captured ef_permute leaves no counts mirror
+ *     behind for ef_expert_ffn_grouped(counts_host = NULL).  The grouped-FFN calls wait on copy-stream events, and
+ *     ef_expert_ffn_grouped on the gate's counts on the host: they are not capturable.
  *   - Shape limits: d_model % 64 == 0, d_ff % 128 == 0, 1 <= top_k <= 8, top_k <= n_experts <= 256.
  *
  * Logical clock: visit = step * n_layers + layer.  The cache policy depends only on the sequence

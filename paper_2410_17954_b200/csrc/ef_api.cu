@@ -59,6 +59,11 @@ static cudaError_t ring_wait(ef_ctx* ctx, cudaStream_t waiter, const EvHandle& h
 // enqueued so far, so that two streams can never interleave inside the split-K workspace, the h workspace, the
 // scheduler blocks or a slot that a copy is about to overwrite.
 static int32_t enter_lane(ef_ctx* ctx, cudaStream_t st, cudaStream_t* last, bool* has_last) {
+    // A stream that is being captured into a CUDA graph executes nothing now: ordering the replayed graph against the
+    // lane's other work is the capturer's business (ef.h), and an event recorded outside the capture could not be waited
+    // on from inside it anyway.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap == cudaStreamCaptureStatusActive) return EF_OK;
     if (*has_last && *last != st) {
         cudaError_t e;
         EvHandle h = ring_record(ctx, *last, &e);
@@ -321,6 +326,11 @@ extern "C" int32_t ef_permute(ef_ctx* ctx, void* stream, const int32_t* topk_idx
     *err = 0;
     int32_t rc = efk_permute(ctx, (cudaStream_t)stream, topk_idx, x, T, x_perm, counts, offsets, src, inv, mirror, err);
     if (rc != EF_OK) return rc;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing((cudaStream_t)stream, &cap) == cudaSuccess && cap == cudaStreamCaptureStatusActive) {
+        ctx->counts_mirror = nullptr;  // captured into a graph: nothing has run, there is no mirror to wait for
+        return EF_OK;
+    }
     ctx->counts_mirror = mirror;       // what ef_expert_ffn_grouped(counts_host = NULL) reads once the event has fired
     EF_CUDA(ctx, cudaEventRecord(ctx->counts_event, (cudaStream_t)stream));
     return EF_OK;

@@ -459,3 +459,44 @@ def test_reregistering_a_resident_or_aliased_expert_is_refused():
     c.ef_host_expert_register(0, 7, *ex[(0, 7)])             # an alias may become an owner again ...
     c.ef_host_expert_register(0, 2, *ex[(0, 2)])             # ... which frees its former source for re-registration
     r.close()
+
+
+def test_memory_bound_calls_can_be_captured_into_a_cuda_graph():
+    """ef.h (CUDA graphs): rmsnorm -> route -> permute and combine, captured once and replayed, give what the eager calls
+    give; a captured ef_permute leaves no counts mirror behind."""
+    from paper_2410_17954_b200 import EfError
+    cfg = wl.scaled(wl.CONFIGS["tiny"], n_slots=8)
+    r, ex = build_runner(cfg)
+    c, T = r.ctx, cfg.T
+    x = dev_bf16(wl.activations(cfg))
+    normed = torch.empty_like(x)
+    out_e = torch.empty_like(x); out_g = torch.empty_like(x)
+
+    def front():
+        c.ef_rmsnorm(x, T, 1e-5, normed)
+        c.ef_route_topk(normed, r.w_router[0], None, T, 1, r.topk_idx, r.topk_w, None)
+        c.ef_permute(r.topk_idx, normed, T, r.x_perm, r.counts, r.offsets, r.src, r.inv)
+    front()
+    c.ef_expert_ffn_grouped(0, 0, r.x_perm, None, r.y_perm)
+    c.ef_combine(r.y_perm, r.inv, r.topk_w, T, x, None, out_e)
+    c.ef_sync()
+    eager = [t.clone() for t in (r.topk_idx, r.topk_w, r.counts, r.offsets, r.src, r.inv, r.x_perm)]
+    for t in (r.topk_idx, r.counts, r.offsets, r.src, r.inv):
+        t.fill_(-1)
+    r.x_perm.zero_()
+    g1, g2 = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    with torch.cuda.graph(g1, stream=s):
+        front()
+    with pytest.raises(EfError):                       # nothing ran: there is no mirror to wait for
+        c.ef_expert_ffn_grouped(1, 0, r.x_perm, None, r.y_perm)
+    with torch.cuda.graph(g2, stream=s):
+        c.ef_combine(r.y_perm, r.inv, r.topk_w, T, x, None, out_g)
+    g1.replay()
+    torch.cuda.synchronize()
+    for a, b in zip(eager, (r.topk_idx, r.topk_w, r.counts, r.offsets, r.src, r.inv, r.x_perm)):
+        assert torch.equal(a, b)
+    g2.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out_e, out_g)
+    r.close()

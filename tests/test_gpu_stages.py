@@ -380,6 +380,24 @@ def test_errors_are_codes_not_crashes():
     ctx.close()
 
 
+def test_set_option_validates_keys_and_values():
+    from paper_2410_17954_b200 import (EF_OPT_CHUNK_MIN_BYTES, EF_OPT_COPY_ORDER, EF_OPT_FUSED_WAVES, EF_OPT_SPLITK,
+                                       EF_OPT_TOKEN_SCHED_PATH, EF_OPT_WAVE_BYTES, EfError)
+    ctx = make_ctx()
+    for key, good, bad in ((EF_OPT_SPLITK, (0, 1, 16), (-1, 17)), (EF_OPT_WAVE_BYTES, (0, 1 << 40), (-1,)),
+                           (EF_OPT_CHUNK_MIN_BYTES, (0, 1), (-5,)), (EF_OPT_COPY_ORDER, (0, 1), (2, -1)),
+                           (EF_OPT_FUSED_WAVES, (0, 1), ()), (EF_OPT_TOKEN_SCHED_PATH, (0, 1), ())):
+        for v in good:
+            ctx.ef_set_option(key, v)
+        for v in bad:
+            with pytest.raises(EfError) as e:
+                ctx.ef_set_option(key, v)
+            assert e.value.code == -1
+    with pytest.raises(EfError):
+        ctx.ef_set_option(99, 0)
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------------
 # diagnostics used by bench.py's second roofline
 # ------------------------------------------------------------------------------------------------
