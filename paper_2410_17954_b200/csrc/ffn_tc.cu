@@ -161,8 +161,18 @@ __device__ __forceinline__ uint32_t mapa(const void* p, uint32_t rank) {
 __device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
-__device__ __forceinline__ void st_remote_u32(uint32_t cluster_addr, uint32_t v) {
-    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
+// Remote arrive that publishes nothing through memory (a consumer handing a ring slot or a TMEM half back: what it read is
+// ordered before the arrive by its own data dependence / tcgen05.fence::before_thread_sync).  No cluster-scope release:
+// that is a MEMBAR.GPU, ~1 us during which the arriving warp also waits for every global store it has in flight -- on the
+// TMEM hand-over that delay is the MMA lane's.
+__device__ __forceinline__ void mbar_arrive_remote_relaxed(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// 4 bytes into the peer's shared memory that complete 4 bytes of the transaction count of a barrier there: data and
+// signal in one asynchronous operation, no fence in the sender (the receiver arms the barrier with expect_tx itself)
+__device__ __forceinline__ void st_async_u32(uint32_t cluster_addr, uint32_t v, uint32_t cluster_bar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.u32 [%0], %1, [%2];" ::"r"(cluster_addr), "r"(v), "r"(cluster_bar)
+                 : "memory");
 }
 __device__ __forceinline__ void cluster_sync() {
     asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
@@ -513,7 +523,7 @@ __device__ __forceinline__ void epilogue_unit(const Tile& t, const PhaseArgs& p,
     tc_fence_before();
     __syncwarp();
     if (lane == 0)
-        for (int h = 0; h < nb; ++h) mbar_arrive_remote(mapa(&ctl->tmem_empty[b0 + h], 0));
+        for (int h = 0; h < nb; ++h) mbar_arrive_remote_relaxed(mapa(&ctl->tmem_empty[b0 + h], 0));
     bool stored = !split && tile_ok;              // this CTA has written its part of the output tile
     if (split && tile_ok) {
         // publish the partial, count arrivals; the last unit of the tile reduces all s partials in split order
@@ -644,13 +654,14 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                     mbar_wait_cluster(&ctl->sched_empty[ss], ((it / kSched) & 1) ^ 1);
                     tile = atomicAdd(sched, 1);
                     ctl->sched_tile[ss] = tile;
-                    st_remote_u32(mapa(&ctl->sched_tile[ss], 1), (uint32_t)tile);
                     mbar_arrive(&ctl->sched_full[ss]);                       // release.cta: local waiters
-                    mbar_arrive_remote(mapa(&ctl->sched_full[ss], 1));       // release.cluster: the peer's waiters
+                    // the peer's copy and its barrier's 4 transaction bytes in one st.async (its producer lane arms them)
+                    st_async_u32(mapa(&ctl->sched_tile[ss], 1), (uint32_t)tile, mapa(&ctl->sched_full[ss], 1));
                 } else {
+                    mbar_expect_tx(&ctl->sched_full[ss], 4);                 // this lap's arrival + the leader's 4 bytes
                     mbar_wait_cluster(&ctl->sched_full[ss], (it / kSched) & 1);
                     tile = ctl->sched_tile[ss];
-                    mbar_arrive_remote(mapa(&ctl->sched_empty[ss], 0));
+                    mbar_arrive_remote_relaxed(mapa(&ctl->sched_empty[ss], 0));
                 }
                 if (tile >= total_tiles) break;
                 const Tile t = decode_tile(tab, ctl, tile, p0, p1);
@@ -749,7 +760,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
             mbar_wait_cluster(&ctl->sched_full[ss], (it / kSched) & 1);
             const int tile = ctl->sched_tile[ss];
             __syncwarp();
-            if (lane == 0) mbar_arrive_remote(mapa(&ctl->sched_empty[ss], 0));
+            if (lane == 0) mbar_arrive_remote_relaxed(mapa(&ctl->sched_empty[ss], 0));
             if (tile >= total_tiles) break;
             const Tile t = decode_tile(tab, ctl, tile, p0, p1);
             const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
