@@ -158,9 +158,6 @@ __device__ __forceinline__ uint32_t mapa(const void* p, uint32_t rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(p)), "r"(rank));
     return r;
 }
-__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
-}
 // Remote arrive that publishes nothing through memory (a consumer handing a ring slot or a TMEM half back: what it read is
 // ordered before the arrive by its own data dependence / tcgen05.fence::before_thread_sync).  No cluster-scope release:
 // that is a MEMBAR.GPU, ~1 us during which the arriving warp also waits for every global store it has in flight -- on the
@@ -342,12 +339,13 @@ struct Tile {
 // weight stage has to be filled either way), so with long K loops a group of 257..4096 rows is cut into
 // ceil(rows / 256) BALANCED tiles of b = ceil16(rows / tiles) rows instead of full 256-row tiles plus a small remainder
 // (593 rows: 208 + 208 + 177, not 256 + 256 + 81): measured +5 % / +3 % on GEMM1 / GEMM2 of the Mixtral shape.  With a
-// short K loop (K < 3072: the many-expert shapes) the fixed cost of one more 129..256-token tile -- its epilogue is not
-// overlapped, it owns all of TMEM -- outweighs that (measured -2 % / -6 %), so those keep 256-row tiles + remainder.
-// Both GEMMs of a wave use the SAME tiling (balanced iff d and f are both >= 3072), so that a GEMM2 unit depends on
-// exactly one token tile of GEMM1.  Tiles 0 .. n-2 hold b rows, the last one what is left; it is "short" (<= 128
-// tokens, half of TMEM) or "long".
-constexpr int kBalancedMinK = 3072;
+// short K loop (the many-expert shapes) one more 129..256-token tile has a fixed cost -- its epilogue is not overlapped,
+// it owns all of TMEM: while the TMEM hand-over still paid a cluster-scope release that outweighed the balance (-2 % /
+// -6 %) and those shapes kept 256-row tiles + remainder (kBalancedMinK = 3072); with the relaxed hand-over balanced
+// tiles win there too (cfg 4, all experts resident: 389 -> 385 us), so every shape is balanced now.
+// Both GEMMs of a wave use the SAME tiling, so that a GEMM2 unit depends on exactly one token tile of GEMM1.  Tiles
+// 0 .. n-2 hold b rows, the last one what is left; it is "short" (<= 128 tokens, half of TMEM) or "long".
+constexpr int kBalancedMinK = 0;
 __device__ __host__ __forceinline__ int group_tile_rows(int rows, bool balanced) {
     const int n = (rows + BT - 1) / BT;
     if (!balanced || n < 2 || n > 16) return BT;
@@ -671,9 +669,12 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                 const int n_box = (half + XBOX - 1) / XBOX;
                 const uint32_t bytes = (uint32_t)(W_BYTES + n_box * XBOX_BYTES);
                 // weight tile -> rowlet coordinates in the arena (tiled layout, ef_internal.h): a k-block of the tile is
-                // h_t contiguous rowlets.  The odd last pair's idle partner re-reads tile 0 (its lanes are never stored);
-                // a short last tile's box runs on into the next k-block's rowlets (lanes >= h_t, never stored either)
-                const int w_tile = (2 * t.n_pair + (int)rank) < p.n_tiles_n ? 2 * t.n_pair + (int)rank : 0;
+                // h_t contiguous rowlets.  The odd last pair's partner has no weight tile: it stages only its half of the
+                // tokens (the MMA multiplies whatever its weight stage holds; its lanes are never stored).  A short last
+                // tile's box runs on into the next k-block's rowlets (lanes >= h_t, never stored either)
+                const bool peer_idle = 2 * t.n_pair + 1 >= p.n_tiles_n;
+                const bool w_idle = peer_idle && rank == 1;
+                const int w_tile = w_idle ? 0 : 2 * t.n_pair + (int)rank;
                 const int h_t = min(BW, p.w_rows - w_tile * BW);
                 const int w_rowlet0 = t.slot * slot_rowlets + p.base_rowlet + w_tile * BW * p.KB;
                 const int x_row = t.a_row + (int)rank * half;
@@ -681,9 +682,9 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                 for (int kb = t.kb0; kb < t.kb1; ++kb) {
                     mbar_wait(&ctl->empty[stage], phase ^ 1);
                     uint8_t* sw = smem + (size_t)stage * STAGE_BYTES;
-                    if (leader) mbar_expect_tx(&ctl->full[stage], 2 * bytes);  // both CTAs' boxes land on this barrier
+                    if (leader) mbar_expect_tx(&ctl->full[stage], 2 * bytes - (peer_idle ? (uint32_t)W_BYTES : 0u));  // both CTAs' boxes land here
                     const uint32_t bar = mapa(&ctl->full[stage], 0);
-                    tma_load_2d(sw, &tmW, bar, 0, w_rowlet0 + kb * h_t);
+                    if (!w_idle) tma_load_2d(sw, &tmW, bar, 0, w_rowlet0 + kb * h_t);
                     if (must_wait) {
                         // the weights do not depend on GEMM1: their box is already on its way while this lane waits for
                         // the h rows of its token tile (written by the GEMM1 units of this same launch)
@@ -891,16 +892,18 @@ SplitPlan plan_split(const ef_ctx* ctx, int tiles, int n_short, int G, int KB, d
 }
 
 // bytes one phase's TMA loads stage into shared memory (what crosses the L2 -> SM fabric): per token tile and weight-tile
-// pair, per k-block, each CTA of the pair pulls its 32 KB weight box plus the 8 KB token boxes covering its half tile
-int64_t phase_fill_bytes(const EfWaveTable& tab, bool balanced, int npn, int KB) {
+// pair, per k-block, each CTA of the pair pulls its 32 KB weight box (if it has a weight tile) plus the 8 KB token boxes
+// covering its half tile
+int64_t phase_fill_bytes(const EfWaveTable& tab, bool balanced, int npn, int n_tiles_n, int KB) {
     int64_t per_kb = 0;
     for (int i = 0; i < tab.n; ++i)
         for (int off = 0, b = group_tile_rows(tab.g[i].rows, balanced); off < tab.g[i].rows; off += b) {
             const int n_mma = (std::min(tab.g[i].rows - off, b) + 15) & ~15;
             const int n_box = (n_mma / 2 + XBOX - 1) / XBOX;
-            per_kb += 2 * (int64_t)(W_BYTES + n_box * XBOX_BYTES);
+            // every CTA of every pair stages its token boxes; one weight box per real weight tile
+            per_kb += (int64_t)npn * 2 * n_box * XBOX_BYTES + (int64_t)n_tiles_n * W_BYTES;
         }
-    return per_kb * npn * KB;
+    return per_kb * KB;
 }
 
 }  // namespace
@@ -1002,8 +1005,8 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         EF_CUDA(ctx, cudaEventRecord(e1, st));
         ef_ctx::KSpan span{e0, e1, phase & 3, rows_total, tab.n};
         ctx->kspans.push_back(span);
-        if (phase & 1) ctx->ktimes.gemm1_fill_bytes += phase_fill_bytes(tab, bal, pa[0].n_pairs_n, pa[0].KB);
-        if (phase & 2) ctx->ktimes.gemm2_fill_bytes += phase_fill_bytes(tab, bal, pa[1].n_pairs_n, pa[1].KB);
+        if (phase & 1) ctx->ktimes.gemm1_fill_bytes += phase_fill_bytes(tab, bal, pa[0].n_pairs_n, pa[0].n_tiles_n, pa[0].KB);
+        if (phase & 2) ctx->ktimes.gemm2_fill_bytes += phase_fill_bytes(tab, bal, pa[1].n_pairs_n, pa[1].n_tiles_n, pa[1].KB);
     }
     return EF_OK;
 }

@@ -184,11 +184,13 @@ FFN_CASES = [
     (5, 512, 1408 - 1408 % 128, [300, 7, 0, 513, 64]),
     (2, 64, 128, [1, 1]),
     (2, 1024, 384, [257, 255]),
-    # long K loops on one side only keep 256-row tiles + remainder (both GEMMs of a wave share ONE token tiling)
+    # long K loop on one GEMM, short on the other, long on both (balanced tiles: 593 -> 208 + 208 + 177, 300 -> 160 + 140,
+    # 513 -> 176 + 176 + 161, 257 -> 144 + 113; both GEMMs of a wave share ONE token tiling)
     (2, 3072, 256, [300, 593]),
     (3, 256, 3072, [513, 257, 130]),
-    # d and f both >= 3072 switch the wave to balanced tiles (593 -> 208 + 208 + 177)
     (2, 3072, 3072, [593, 300]),
+    # odd numbers of weight tiles on both GEMMs (f / 128 = 3, d / 256 = 3): the last pair's partner has no weight tile
+    (3, 768, 384, [260, 90, 3]),
 ]
 
 # variant ids: simt = the diag library's plain-FMA backend; splitk 0 = automatic tail split-K (these launches have fewer
@@ -413,12 +415,13 @@ def test_tma_fill_rate_and_fill_byte_accounting():
     run_resident_ffn(ctx, E, d, f, counts, seed=3, simt=False, splitk=1)
     kt = ctx.ef_get_kernel_times(reset=True)
     ctx.ef_set_kernel_timing(False)
-    # tile plan (K < 3072: 256-row tiles + remainder): expert 0 = tiles of 256 and 44 rows, expert 1 = one tile of 17 rows.  Per k-block a CTA pair stages
-    # 2 x 32 KB of weights and, per CTA, the 8 KB token boxes covering half of the tile rounded up to 16 rows
+    # tile plan (balanced tiles: ceil(rows / 256) tiles of ceil16(rows / tiles) rows): expert 0 = tiles of 160 and 140 rows,
+    # expert 1 = one tile of 17 rows.  Per k-block a CTA pair stages 2 x 32 KB of weights (both weight-tile counts are even
+    # here: no pair has an idle partner) and, per CTA, the 8 KB token boxes covering half of the tile rounded up to 16 rows
     def per_kb(rows):
         n_mma = (rows + 15) // 16 * 16
         return 2 * (32768 + -(-(n_mma // 2) // 64) * 8192)
-    tiles = per_kb(256) + per_kb(44) + per_kb(17)
+    tiles = per_kb(160) + per_kb(140) + per_kb(17)
     npn1, npn2 = (f // 128 + 1) // 2, ((d + 255) // 256 + 1) // 2
     assert kt["gemm1_fill_bytes"] == tiles * npn1 * (d // 64)
     assert kt["gemm2_fill_bytes"] == tiles * npn2 * (f // 64)
