@@ -580,10 +580,12 @@ int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm,
 // Miss waves.  Every on-demand expert could be its own wave (compute starts the moment its copy lands), but for small
 // experts that is one launch per ~0.3 ms copy, each far too short to fill the GPU.  The batcher groups consecutive
 // misses into waves: never less than ~wave_bytes of link traffic per wave, and -- while many misses are still to come --
-// HALF of what is left (a visit with 40 small misses runs them as waves of 20, 10, 7, 2 and 1 experts): the big early
-// waves are real grouped GEMMs, each finishes long before the next, smaller wave's copies have landed, and the last miss
-// of a visit still is a wave of its own, so the tail after the final copy is one expert's FFN.  Physical scheduling only:
-// which slot a miss takes and every counter were decided before the item got here.
+// HALF of what is left (a visit with 40 small misses runs them as waves of 20, 10, 7 and 3 experts): the big early
+// waves are real grouped GEMMs, each finishes long before the next, smaller wave's copies have landed.  When an expert is
+// large enough to be copied in two chunks (>= chunk_min_bytes: its FFN is a good fraction of a millisecond) the last miss
+// of a visit is a wave of its own, so the tail after the final copy is one expert's GEMM2; for small experts the last
+// misses stay together -- a launch per 17 MB expert costs more in ramp and tail than the others add to the wave.
+// Physical scheduling only: which slot a miss takes and every counter were decided before the item got here.
 struct MissBatcher {
     ef_ctx* ctx; cudaStream_t st; const void* x_perm; void* y_perm;
     std::vector<WaveItem> open;
@@ -612,7 +614,8 @@ struct MissBatcher {
     }
     int32_t push(const WaveItem& it, bool last_of_visit) {
         int32_t rc = EF_OK;
-        if (last_of_visit && !open.empty() && (rc = flush()) != EF_OK) return rc;
+        const bool alone = ctx->chunk_min_bytes > 0 && ctx->W >= ctx->chunk_min_bytes;
+        if (last_of_visit && alone && !open.empty() && (rc = flush()) != EF_OK) return rc;
         open.push_back(it);
         --remaining;
         if ((int)open.size() >= target || last_of_visit) rc = flush(last_of_visit);
