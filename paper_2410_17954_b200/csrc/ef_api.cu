@@ -580,7 +580,7 @@ int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm,
 // Miss waves.  Every on-demand expert could be its own wave (compute starts the moment its copy lands), but for small
 // experts that is one launch per ~0.3 ms copy, each far too short to fill the GPU.  The batcher groups consecutive
 // misses into waves: never less than ~wave_bytes of link traffic per wave, and -- while many misses are still to come --
-// HALF of what is left (a visit with 40 small misses runs them as waves of 20, 10, 7 and 3 experts): the big early
+// HALF of what is left (a visit with 40 small misses runs them as waves of 20, 10 and 10 experts): the big early
 // waves are real grouped GEMMs, each finishes long before the next, smaller wave's copies have landed.  When an expert is
 // large enough to be copied in two chunks (>= chunk_min_bytes: its FFN is a good fraction of a millisecond) the last miss
 // of a visit is a wave of its own, so the tail after the final copy is one expert's GEMM2; for small experts the last
@@ -599,8 +599,12 @@ struct MissBatcher {
     }
     int next_target() const {
         if (ctx->wave_bytes == 0) return 1;
-        return std::min(EF_MAX_GROUPS, std::max(min_wave, remaining / 2));
+        int t = std::min(EF_MAX_GROUPS, std::max(min_wave, remaining / 2));
+        // small experts: no trailing wave of one or two -- what is left joins this wave (see push)
+        if (!last_alone() && remaining - t < std::max(2, min_wave / 2) && remaining <= EF_MAX_GROUPS) t = std::max(t, remaining);
+        return t;
     }
+    bool last_alone() const { return ctx->chunk_min_bytes > 0 && ctx->W >= ctx->chunk_min_bytes; }
     bool holds_slot(int slot) const {
         for (const WaveItem& it : open) if (it.slot == slot) return true;
         return false;
@@ -614,8 +618,7 @@ struct MissBatcher {
     }
     int32_t push(const WaveItem& it, bool last_of_visit) {
         int32_t rc = EF_OK;
-        const bool alone = ctx->chunk_min_bytes > 0 && ctx->W >= ctx->chunk_min_bytes;
-        if (last_of_visit && alone && !open.empty() && (rc = flush()) != EF_OK) return rc;
+        if (last_of_visit && last_alone() && !open.empty() && (rc = flush()) != EF_OK) return rc;
         open.push_back(it);
         --remaining;
         if ((int)open.size() >= target || last_of_visit) rc = flush(last_of_visit);
