@@ -21,6 +21,13 @@ int32_t ef_diag_set_simt_ffn(ef_ctx* ctx, int32_t on);
  * weight box) through a 4-stage ring, `iters` boxes per CTA, out of a scratch region of region_bytes (<= 126 MB stays in
  * L2; larger streams from HBM).  gbs_out: HOST double, delivered GB/s.  Synchronous; allocates and frees the region. */
 int32_t ef_diag_tma_fill_gbs(ef_ctx* ctx, int64_t region_bytes, int32_t iters, double* gbs_out);
+/* What a cross-CTA hand-back costs on this device ("hand-overs"): n_ctas CTAs (1..SM count; even for the
+ * pair modes) stream the same boxes; mode -1: every CTA on its own (the stream above on fewer SMs); mode 0 / 1: CTA PAIRS
+ * (clusters of 2) run the grouped GEMM's protocol -- both CTAs' boxes complete on the leader's barrier, the leader's
+ * consumer lane hands each stage back to the peer's producer with a remote mbarrier arrive that is a cluster-scope
+ * RELEASE (0) or RELAXED (1).  The release is a MEMBAR.GPU per stage and throttles the stream to about a third.
+ * gbs_out: HOST double, delivered GB/s over all n_ctas.  Synchronous; allocates and frees the region. */
+int32_t ef_diag_pair_handoff_gbs(ef_ctx* ctx, int64_t region_bytes, int32_t iters, int32_t n_ctas, int32_t mode, double* gbs_out);
 /* Only in a diag library built with -DEF_KPROF as well (EF_ERR_UNSUPPORTED otherwise): the first call arms the counters,
  * later calls return, per CTA pair of the last launch that ran GEMM1 units (which = 1) or only GEMM2 units (which = 2),
  * the cycles the MMA-issuing lane spent {in total, waiting for a tile ticket, waiting for the epilogue to free TMEM,

@@ -23,7 +23,7 @@ DECLARED_SYMBOLS = [
     "ef_set_option",
 ]
 # include/ef_diag.h: only libef_diag.so (the diagnostic build) has these
-DIAG_SYMBOLS = ["ef_diag_set_simt_ffn", "ef_diag_tma_fill_gbs", "ef_diag_kprof"]
+DIAG_SYMBOLS = ["ef_diag_set_simt_ffn", "ef_diag_tma_fill_gbs", "ef_diag_pair_handoff_gbs", "ef_diag_kprof"]
 
 EF_OPT_SPLITK, EF_OPT_WAVE_BYTES, EF_OPT_CHUNK_MIN_BYTES, EF_OPT_FUSED_WAVES, EF_OPT_TOKEN_SCHED_PATH, EF_OPT_COPY_ORDER = 1, 2, 3, 4, 5, 6
 
@@ -106,7 +106,8 @@ def load_library(diag: bool = False) -> ctypes.CDLL:
         }
         if diag:
             sig.update({"ef_diag_set_simt_ffn": [vp, i32], "ef_diag_kprof": [vp, i32, vp],
-                        "ef_diag_tma_fill_gbs": [vp, i64, i32, ctypes.POINTER(ctypes.c_double)]})
+                        "ef_diag_tma_fill_gbs": [vp, i64, i32, ctypes.POINTER(ctypes.c_double)],
+                        "ef_diag_pair_handoff_gbs": [vp, i64, i32, i32, i32, ctypes.POINTER(ctypes.c_double)]})
         for name, args in sig.items():
             fn = getattr(lib, name)
             fn.argtypes = args
@@ -300,6 +301,11 @@ class EfContext:
     def ef_diag_tma_fill_gbs(self, region_bytes: int, iters: int = 2000) -> float:
         out = ctypes.c_double()
         self._chk(self.lib.ef_diag_tma_fill_gbs(self.h, int(region_bytes), int(iters), ctypes.byref(out)))
+        return float(out.value)
+
+    def ef_diag_pair_handoff_gbs(self, region_bytes: int, iters: int, n_ctas: int, mode: int) -> float:
+        out = ctypes.c_double()
+        self._chk(self.lib.ef_diag_pair_handoff_gbs(self.h, int(region_bytes), int(iters), int(n_ctas), int(mode), ctypes.byref(out)))
         return float(out.value)
 
     def ef_diag_kprof(self, which: int, n_sms: int = 148):

@@ -28,8 +28,8 @@
 //
 // Warp roles (384 threads, 1 CTA/SM, persistent; both CTAs unless stated):
 //   warp 0     TMA producer + tile scheduler : the LEADER claims the next unit with one atomicAdd on a per-launch
-//                                counter and hands it to both CTAs' roles through 4-deep smem rings (remote store +
-//                                remote mbarrier arrive for the peer); each CTA's producer then issues its own boxes,
+//                                counter and hands it to both CTAs' roles through 4-deep smem rings (the peer's copy
+//                                by one st.async that also completes its barrier); each CTA's producer then issues its own boxes,
 //                                all completing on the leader's "full" barrier
 //   warp 1     MMA issuer (leader only) : one lane issues the two MMAs per k-step; tcgen05.commit multicasts the
 //                                "stage free" / "accumulator ready" arrivals to both CTAs
@@ -41,6 +41,8 @@
 //                                into a [32 tokens][128 features] staging tile -> 16-byte global stores, 256
 //                                contiguous bytes per token row; warps w and w+4 share a TMEM lane quarter and
 //                                take alternate 32-token chunks; "accumulator free" arrives on the leader's barrier
+// Hand-backs across the pair (ring slots, drained TMEM halves) are RELAXED remote arrives: a cluster-scope release is a
+// MEMBAR.GPU on this device and made the MMA lane wait ~1 us for TMEM on every unit ("hand-overs").
 // Per-expert tile scheduling over ragged token counts: inside a phase units are numbered longest-first -- every
 // > 128-token tile of every group (n-major inside a group, so the token tiles that share a weight tile are claimed back
 // to back and hit L2) with the <= 128-token tail tiles spread among them -- and claimed dynamically (greedy list

@@ -410,6 +410,14 @@ def test_tma_fill_rate_and_fill_byte_accounting():
     assert 2000.0 < gbs < 40000.0                     # an L2-resident region: several TB/s on a B200
     with pytest.raises(Exception):
         ctx.ef_diag_tma_fill_gbs(16, 500)             # smaller than one box
+    # hand-back between the CTAs of a pair: a cluster-scope RELEASE arrive per stage throttles the stream,
+    # a RELAXED one does not -- the reason the grouped GEMM hands ring slots and TMEM halves back with relaxed arrives
+    own = ctx.ef_diag_pair_handoff_gbs(32 << 20, 500, 16, -1)
+    rel = ctx.ef_diag_pair_handoff_gbs(32 << 20, 500, 16, 0)
+    rlx = ctx.ef_diag_pair_handoff_gbs(32 << 20, 500, 16, 1)
+    assert rlx > 1.5 * rel and own > rel, (own, rel, rlx)
+    with pytest.raises(Exception):
+        ctx.ef_diag_pair_handoff_gbs(32 << 20, 500, 15, 1)   # pairs need an even number of CTAs
     ctx.ef_set_kernel_timing(True)
     ctx.ef_get_kernel_times(reset=True)
     run_resident_ffn(ctx, E, d, f, counts, seed=3, simt=False, splitk=1)
