@@ -167,6 +167,11 @@ __device__ __forceinline__ uint32_t mapa(const void* p, uint32_t rank) {
 __device__ __forceinline__ void mbar_arrive_remote_relaxed(uint32_t cluster_addr) {
     asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
+// ... handing back a ring slot: `read` is the value read out of the slot, an operand of the instruction only so that the
+// arrive cannot issue before that shared-memory load has delivered it (the data dependence the comment above relies on)
+__device__ __forceinline__ void mbar_arrive_remote_relaxed_after(uint32_t cluster_addr, int read) {
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];  // after %1" ::"r"(cluster_addr), "r"(read) : "memory");
+}
 // 4 bytes into the peer's shared memory that complete 4 bytes of the transaction count of a barrier there: data and
 // signal in one asynchronous operation, no fence in the sender (the receiver arms the barrier with expect_tx itself)
 __device__ __forceinline__ void st_async_u32(uint32_t cluster_addr, uint32_t v, uint32_t cluster_bar) {
@@ -661,7 +666,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                     mbar_expect_tx(&ctl->sched_full[ss], 4);                 // this lap's arrival + the leader's 4 bytes
                     mbar_wait_cluster(&ctl->sched_full[ss], (it / kSched) & 1);
                     tile = ctl->sched_tile[ss];
-                    mbar_arrive_remote_relaxed(mapa(&ctl->sched_empty[ss], 0));
+                    mbar_arrive_remote_relaxed_after(mapa(&ctl->sched_empty[ss], 0), tile);
                 }
                 if (tile >= total_tiles) break;
                 const Tile t = decode_tile(tab, ctl, tile, p0, p1);
@@ -763,7 +768,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
             mbar_wait_cluster(&ctl->sched_full[ss], (it / kSched) & 1);
             const int tile = ctl->sched_tile[ss];
             __syncwarp();
-            if (lane == 0) mbar_arrive_remote_relaxed(mapa(&ctl->sched_empty[ss], 0));
+            if (lane == 0) mbar_arrive_remote_relaxed_after(mapa(&ctl->sched_empty[ss], 0), tile);
             if (tile >= total_tiles) break;
             const Tile t = decode_tile(tab, ctl, tile, p0, p1);
             const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
