@@ -487,6 +487,9 @@ def measure_workload(cfg, args, dev, plan, world, peaks, log, steps, warmup, wan
                 f"aliasing {cfg.n_layers * cfg.n_experts} logical experts onto {phys} physical buffers")
     steps_total = 2 * (steps + warmup) + 2
     drv = Driver(cfg, dev, plan["x_stream"], steps_total, phys, log, args.policy)
+    if args.no_early_release:
+        from paper_2410_17954_b200 import EF_OPT_EARLY_RELEASE
+        drv.runner.ctx.ef_set_option(EF_OPT_EARLY_RELEASE, 0)
     runner = drv.runner
     runner.ctx.ef_sync()                 # the warm-up prefetch must not share the link with the peak measurement
     h2d_peak = measure_pinned_h2d(dev, cfg.expert_bytes) if rank == 0 else None
@@ -983,6 +986,8 @@ def main():
                          "if host memory allows)")
     ap.add_argument("--horizon", type=int, default=None,
                     help="override the workload's prefetch horizon H in visits (<= 0: as far as the supplied path reaches; R10)")
+    ap.add_argument("--no-early-release", action="store_true",
+                    help="EF_OPT_EARLY_RELEASE = 0: the first-victim hit always runs as a wave of its own (A/B arm)")
     ap.add_argument("--policy", default="plec", choices=["plec", "lru", "layer_lru", "next_layer_all"],
                     help="cache policy arm: the paper's PLEC (default), on-demand LRU over the pool, LRU inside a per-layer "
                          "share, or PLEC prefetching every expert of the next layer (the baselines of P:L230 as policy sketches)")

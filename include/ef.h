@@ -283,13 +283,19 @@ int32_t ef_get_launch_log(ef_ctx* ctx, ef_launch_record* out, int32_t max_record
  * EF_OPT_COPY_ORDER      order in which the on-demand copies of one visit are put on the link: 0 = policy order (ascending
  *                        expert id, R12), 1 (default) = experts with more routed rows first, so the largest GEMMs start
  *                        earliest (the paper's "high-priority queue").  Which slot an expert takes
- *                        and every counter are decided in policy order either way. */
+ *                        and every counter are decided in policy order either way.
+ * EF_OPT_EARLY_RELEASE   1 (default) = the hit whose slot the visit's first pending copy will overwrite is handed back from
+ *                        INSIDE the hits' wave (its units are ticketed first and count themselves done on a device word
+ *                        the copy stream waits for) when that wave consists of short (<= 128-token) tiles only, i.e. of
+ *                        decode-sized experts; 0 = that hit always runs as a wave of its own first.
+ *                        Physical scheduling only. */
 #define EF_OPT_SPLITK 1
 #define EF_OPT_WAVE_BYTES 2
 #define EF_OPT_CHUNK_MIN_BYTES 3
 #define EF_OPT_FUSED_WAVES 4
 #define EF_OPT_TOKEN_SCHED_PATH 5
 #define EF_OPT_COPY_ORDER 6
+#define EF_OPT_EARLY_RELEASE 7
 int32_t ef_set_option(ef_ctx* ctx, int32_t key, int64_t value);
 
 #ifdef __cplusplus

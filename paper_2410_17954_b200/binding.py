@@ -26,6 +26,7 @@ DECLARED_SYMBOLS = [
 DIAG_SYMBOLS = ["ef_diag_set_simt_ffn", "ef_diag_tma_fill_gbs", "ef_diag_pair_handoff_gbs", "ef_diag_kprof"]
 
 EF_OPT_SPLITK, EF_OPT_WAVE_BYTES, EF_OPT_CHUNK_MIN_BYTES, EF_OPT_FUSED_WAVES, EF_OPT_TOKEN_SCHED_PATH, EF_OPT_COPY_ORDER = 1, 2, 3, 4, 5, 6
+EF_OPT_EARLY_RELEASE = 7
 
 
 class EfError(RuntimeError):

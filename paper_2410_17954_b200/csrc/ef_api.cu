@@ -154,6 +154,18 @@ extern "C" int32_t ef_create(const ef_config* cfg, ef_ctx** out) {
     ctx->slots.assign(c.n_slots, EfSlot());
     ctx->slot_of.assign((size_t)c.n_layers * c.n_experts, -1);
     ctx->phys.assign(c.n_slots, EfPhys());
+    // early hand-back of a slot from inside a wave (run_wave): a device word and the driver's stream wait on it; without
+    // the entry point the first-victim hit simply keeps running as a wave of its own
+    {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess && fn) {
+            if ((e = cudaMalloc((void**)&ctx->early_flag, 256)) != cudaSuccess) return bail(EF_ERR_OOM, "early-release word", e);
+            if ((e = cudaMemset(ctx->early_flag, 0, 256)) != cudaSuccess) return bail(EF_ERR_CUDA, "early-release word", e);
+            ctx->wait_value_fn = fn;
+        }
+    }
     int32_t rc = efk_ffn_tc_init(ctx);
     if (rc != EF_OK) {
         g_create_err = "ef_create: " + ctx->err;
@@ -184,6 +196,7 @@ extern "C" int32_t ef_destroy(ef_ctx* ctx) {
     if (ctx->splitk_counters) cudaFree(ctx->splitk_counters);
     efk_token_sched_free(ctx);
     if (ctx->h_ws) cudaFree(ctx->h_ws);
+    if (ctx->early_flag) cudaFree(ctx->early_flag);
     if (ctx->arena) cudaFree(ctx->arena);
     delete ctx;
     return EF_OK;
@@ -451,7 +464,16 @@ int32_t policy_load(ef_ctx* ctx, int slot, int32_t g, int64_t pred_for) {
 // the physical H2D of one load: waits (on the copy stream) for the last wave that read the slot, then copies
 int32_t enqueue_copy(ef_ctx* ctx, int slot, int32_t g) {
     EfPhys& ph = ctx->phys[slot];
-    EF_CUDA(ctx, ring_wait(ctx, ctx->copy_stream, ph.free_, ctx->last_compute, ctx->has_last_compute));
+    if (ph.has_flag) {
+        // the slot's last reader hands it back from inside its launch: wait for the device word, not for the launch's end
+        typedef CUresult (*WaitValueFn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+        CUresult r = ((WaitValueFn)ctx->wait_value_fn)((CUstream)ctx->copy_stream, (CUdeviceptr)(uintptr_t)ctx->early_flag, ph.flag_target,
+                                                       CU_STREAM_WAIT_VALUE_GEQ);
+        if (r != CUDA_SUCCESS) return ef_fail(ctx, EF_ERR_CUDA, "cuStreamWaitValue32 failed: %d", (int)r);
+        ph.has_flag = false;
+    } else {
+        EF_CUDA(ctx, ring_wait(ctx, ctx->copy_stream, ph.free_, ctx->last_compute, ctx->has_last_compute));
+    }
     cudaEvent_t t0, t1;
     if (ctx->copy_spans.size() > 1024) drain_copy_spans(ctx, false, nullptr);
     {
@@ -535,9 +557,14 @@ int32_t wait_slot_ready(ef_ctx* ctx, cudaStream_t st, EfPhys& ph, int which) {
 // LAST wave of a visit may run as two launches when its expert is still arriving in two chunks: GEMM1 is gated on the
 // first chunk (W13 / W1) and overlaps the transfer of Wd, so the tail of the visit after its final copy is one GEMM2.  For
 // every earlier wave that overlap buys nothing -- the next wave's copies are on the link anyway -- and one launch is faster.
-int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm, const std::vector<WaveItem>& items,
-                 bool last_of_visit = false) {
-    if (items.empty()) return EF_OK;
+// early_slot >= 0: that member's slot is about to be overwritten by a copy that is enqueued right after this wave; it goes
+// first in the wave's table and, if the wave's tiling allows (efk_ffn_tc), is handed back from inside the launch.
+int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm, const std::vector<WaveItem>& items_in,
+                 bool last_of_visit = false, int early_slot = -1) {
+    if (items_in.empty()) return EF_OK;
+    std::vector<WaveItem> items = items_in;
+    if (early_slot >= 0)
+        std::stable_partition(items.begin(), items.end(), [&](const WaveItem& it) { return it.slot == early_slot; });
     auto& phys = ctx->phys;
     int32_t rc;
     bool two_launches = !ctx->fused_waves;
@@ -554,8 +581,15 @@ int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm,
                 const WaveItem& it = items[base + i];
                 tab.g[i] = EfWaveGroup{it.row0, it.row0, it.row0, it.rows, it.slot};
             }
-            int32_t r = efk_ffn_grouped(ctx, st, x_perm, y_perm, tab, phase);
+            EfEarly early;
+            early.want = early_slot >= 0 && base == 0 && phase == 3 && tab.g[0].slot == early_slot;
+            int32_t r = efk_ffn_grouped(ctx, st, x_perm, y_perm, tab, phase, &early);
             if (r != EF_OK) return r;
+            if (early.used) {
+                ctx->early_target += early.add;
+                phys[early_slot].has_flag = true;
+                phys[early_slot].flag_target = ctx->early_target;
+            }
         }
         return EF_OK;
     };
@@ -573,8 +607,28 @@ int32_t run_wave(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm,
     cudaError_t e;
     EvHandle ev = ring_record(ctx, st, &e);
     EF_CUDA(ctx, e);
-    for (const WaveItem& it : items) phys[it.slot].free_ = ev;
+    for (const WaveItem& it : items) {
+        phys[it.slot].free_ = ev;
+        if (it.slot != early_slot) phys[it.slot].has_flag = false;
+    }
     return EF_OK;
+}
+
+// would run_wave(items, false, early_slot) hand that slot back from inside its launch?
+bool wave_can_release_early(ef_ctx* ctx, cudaStream_t st, const void* x_perm, void* y_perm, const std::vector<WaveItem>& items_in, int early_slot) {
+    if (!ctx->early_release || !ctx->fused_waves || !ctx->early_flag || !ctx->wait_value_fn || items_in.size() > (size_t)EF_MAX_GROUPS) return false;
+#ifdef EF_DIAG
+    if (ctx->debug_simt) return false;
+#endif
+    std::vector<WaveItem> items = items_in;
+    std::stable_partition(items.begin(), items.end(), [&](const WaveItem& it) { return it.slot == early_slot; });
+    EfWaveTable tab;
+    tab.n = (int32_t)items.size();
+    for (int i = 0; i < tab.n; ++i) tab.g[i] = EfWaveGroup{items[i].row0, items[i].row0, items[i].row0, items[i].rows, items[i].slot};
+    EfEarly q;
+    q.want = true;
+    q.dry = true;
+    return efk_ffn_tc(ctx, st, x_perm, y_perm, tab, 3, &q) == EF_OK && q.used;
 }
 
 // Miss waves.  Every on-demand expert could be its own wave (compute starts the moment its copy lands), but for small
@@ -628,11 +682,11 @@ struct MissBatcher {
 
 }  // namespace
 
-int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase) {
+int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase, EfEarly* early) {
 #ifdef EF_DIAG
     if (ctx->debug_simt) return efk_ffn_simt(ctx, st, x, y, tab, phase);     // bring-up aid, diag library only (ef_diag.h)
 #endif
-    return efk_ffn_tc(ctx, st, x, y, tab, phase);
+    return efk_ffn_tc(ctx, st, x, y, tab, phase, early);
 }
 
 extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visit, int32_t layer, const void* x_perm,
@@ -740,13 +794,20 @@ extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visi
         rc = run_wave(ctx, st, x_perm, y_perm, wave0, no_misses);
         if (rc != EF_OK) return rc;
     } else {
-        std::vector<WaveItem> others;
-        for (size_t i = 0; i < wave0.size(); ++i)
-            if (i != split_at) others.push_back(wave0[i]);
-        rc = run_wave(ctx, st, x_perm, y_perm, std::vector<WaveItem>{wave0[split_at]});
-        if (rc != EF_OK) return rc;
-        rc = run_wave(ctx, st, x_perm, y_perm, others);
-        if (rc != EF_OK) return rc;
+        if (wave_can_release_early(ctx, st, x_perm, y_perm, wave0, first_victim)) {
+            // ONE wave: the first victim's units are ticketed first and hand its slot back from inside the launch
+            // (EF_OPT_EARLY_RELEASE; the copy waits on a device word instead of on an event behind a launch of its own)
+            rc = run_wave(ctx, st, x_perm, y_perm, wave0, false, first_victim);
+            if (rc != EF_OK) return rc;
+        } else {
+            std::vector<WaveItem> others;
+            for (size_t i = 0; i < wave0.size(); ++i)
+                if (i != split_at) others.push_back(wave0[i]);
+            rc = run_wave(ctx, st, x_perm, y_perm, std::vector<WaveItem>{wave0[split_at]});
+            if (rc != EF_OK) return rc;
+            rc = run_wave(ctx, st, x_perm, y_perm, others);
+            if (rc != EF_OK) return rc;
+        }
     }
     MissBatcher mb(ctx, st, x_perm, y_perm, (int)(planA.size() + planB.size()));
     for (size_t i = 0; i < planA.size(); ++i)   // compute starts as the copies land, one grouped launch per batch
@@ -973,6 +1034,9 @@ extern "C" int32_t ef_set_option(ef_ctx* ctx, int32_t key, int64_t value) {
             return EF_OK;
         case EF_OPT_TOKEN_SCHED_PATH:
             ctx->ts_force_multi = value ? 1 : 0;
+            return EF_OK;
+        case EF_OPT_EARLY_RELEASE:
+            ctx->early_release = value ? 1 : 0;
             return EF_OK;
         case EF_OPT_COPY_ORDER:
             if (value != 0 && value != 1) return ef_fail(ctx, EF_ERR_INVALID_ARG, "EF_OPT_COPY_ORDER: 0 (policy order) or 1 (most rows first)");

@@ -68,6 +68,8 @@ struct EfPhys {
                                      // (W13 / W1) have landed, before the copy of Wd starts
     EvHandle ready;                  // recorded on the copy stream after the whole H2D into the slot
     EvHandle free_;                  // recorded on the compute stream after the last wave reading the slot
+    bool has_flag = false;           // the slot is handed back from inside its last wave: a copy into it waits for
+    uint32_t flag_target = 0;        // *ctx->early_flag to reach this value instead of for `free_`
     uint8_t waited_mask = 0;         // bit 0 / bit 1: stream `waited` has waited on ready1 / ready since the load
     cudaStream_t waited = nullptr;   // (the legacy default stream is a valid value: 0)
 };
@@ -145,6 +147,10 @@ struct ef_ctx {
     int64_t wave_bytes = (int64_t)128 << 20;
     int64_t chunk_min_bytes = (int64_t)32 << 20;
     int32_t copy_order = 1;             // EF_OPT_COPY_ORDER
+    int32_t early_release = 1;          // EF_OPT_EARLY_RELEASE
+    uint32_t* early_flag = nullptr;     // device word the wave kernel adds finished k-blocks of an early-released slot to
+    uint32_t early_target = 0;          // the sum expected so far (host side; compared cyclically)
+    void* wait_value_fn = nullptr;      // cuStreamWaitValue32, if the driver has it
     // misc
     int64_t launches = 0;
     int32_t debug_simt = 0;             // diag builds only (ef_diag.h)
@@ -182,7 +188,8 @@ int32_t efk_rmsnorm(ef_ctx* ctx, cudaStream_t st, const void* x, int T, float ep
 
 // Grouped FFN over arena slots: x rows -> h workspace -> y rows, one wave.
 // phase: bit 0 = GEMM1 (x -> h), bit 1 = GEMM2 (h -> y); 3 = both in ONE launch (ffn_tc.cu).
-int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase);
+struct EfEarly;
+int32_t efk_ffn_grouped(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase, EfEarly* early = nullptr);
 #ifdef EF_DIAG
 int32_t efk_ffn_simt(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase);
 #endif
@@ -194,4 +201,12 @@ int32_t efk_reindex_rows(ef_ctx* ctx, cudaStream_t st, const void* src, const in
 int32_t efk_path_hamming(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, uint16_t* dist_out);
 void efk_token_sched_free(ef_ctx* ctx);
 int32_t efk_ffn_tc_init(ef_ctx* ctx);   // build arena tensor maps, set smem attributes
-int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase);
+// Early hand-back of the slot of group 0 from INSIDE a fused wave (ffn_tc.cu, EarlyArgs): the launch adds `add` to
+// ctx->early_flag in total, the last of it as soon as nothing of the launch reads that slot any more.
+struct EfEarly {
+    bool want = false;     // in: hand group 0's slot back early if this wave can
+    bool dry = false;      // in: only say whether it could (no launch)
+    bool used = false;     // out
+    uint32_t add = 0;      // out
+};
+int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase, EfEarly* early = nullptr);

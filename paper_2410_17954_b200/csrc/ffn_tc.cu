@@ -330,6 +330,18 @@ struct PhaseArgs {
     int32_t* counters;             // [n_split_tiles * 2] arrival counters, zero between launches
 };
 
+// Early hand-back of ONE expert's slot (ef_internal.h, EfEarly): group 0 of the table is the hit whose slot the visit's first
+// pending copy will overwrite.  Its GEMM2 units -- canonical units [p0.total, p0.total + n2) -- are ticketed at position `a`
+// (one round of other GEMM1 units behind its own GEMM1 units, which are the first tickets) instead of behind every GEMM1
+// unit of the wave, and each of them adds its k-blocks to *flag once its MMAs have completed, i.e. once nothing of the unit
+// reads the slot any more; the copy stream waits for the sum (cuStreamWaitValue32), not for the end of the launch.
+// (a = the number of group 0's GEMM1 units: measured, one more round of other units in between changes nothing.)
+struct EarlyArgs {
+    int32_t a, n2;          // n2 == 0: off
+    uint32_t* flag;
+    int32_t split0, t2, tail0;   // split0: group 0's t2 GEMM2 tiles are split p1.s ways; tail0 = split tiles of the phase's tail
+};
+
 struct Tile {
     int phase;           // 0: GEMM1 unit, 1: GEMM2 unit
     int a_row, c_row;    // first token row in the A tensor / in the output
@@ -340,6 +352,7 @@ struct Tile {
     int kb0, kb1;        // k-block range of this unit
     int tail, split_j;   // index among the split tiles (-1: whole tile) and which K part this unit is
     int tid;             // token-tile id inside the launch: index of the "h rows ready" counter
+    int g;               // group (index into the wave table)
 };
 
 // Token tiling of a group.  A tile narrower than ~170 tokens costs as much per k-block as a 170-token one (its 32 KB
@@ -372,15 +385,35 @@ __device__ __host__ __forceinline__ int group_has_short(int rows, bool balanced)
 }
 
 __device__ __forceinline__ Tile decode_tile(const EfWaveTable& tab, const SmemCtl* ctl, int unit, const PhaseArgs& p0,
-                                            const PhaseArgs& p1) {
+                                            const PhaseArgs& p1, const EarlyArgs& early) {
     Tile t;
+    // ticket -> canonical unit (all GEMM1 units, then all GEMM2 units): group 0's GEMM2 units are pulled forward to ticket a
+    if (early.n2 > 0 && unit >= early.a && unit < p0.total + early.n2)
+        unit = unit < early.a + early.n2 ? p0.total + (unit - early.a) : unit - early.n2;
     t.phase = unit >= p0.total ? 1 : 0;
     const PhaseArgs& p = t.phase ? p1 : p0;
-    const int u = unit - (t.phase ? p0.total : 0);
+    int u = unit - (t.phase ? p0.total : 0);
     int g = 0, j;
-    int tile = u;
     t.kb0 = 0; t.kb1 = p.KB; t.tail = -1; t.split_j = 0;
-    if (u >= p.n_plain) {
+    int tile = -1;
+    if (t.phase == 1 && early.split0) {
+        // group 0's GEMM2 tiles -- the first t2 whole tiles of the phase -- are split s ways as well (each unit is then short
+        // enough for the slot to come back about as early as from a launch of its own); their workspace slots and arrival
+        // counters follow the tail's
+        if (u < early.t2 * p.s) {
+            tile = u / p.s;
+            t.split_j = u - tile * p.s;
+            t.tail = early.tail0 + tile;
+            t.kb0 = (t.split_j * p.KB) / p.s;
+            t.kb1 = ((t.split_j + 1) * p.KB) / p.s;
+        } else {
+            u -= early.t2 * (p.s - 1);
+        }
+    }
+    if (tile >= 0) {
+    } else if (u < p.n_plain) {
+        tile = u;
+    } else {
         const int v = u - p.n_plain;
         t.tail = v / p.s;
         t.split_j = v - t.tail * p.s;
@@ -425,6 +458,7 @@ __device__ __forceinline__ Tile decode_tile(const EfWaveTable& tab, const SmemCt
     t.a_row = (t.phase ? tab.g[g].h_row0 : tab.g[g].x_row0) + row_off;
     t.c_row = (t.phase ? tab.g[g].y_row0 : tab.g[g].h_row0) + row_off;
     t.slot = tab.g[g].slot;
+    t.g = g;
     return t;
 }
 
@@ -593,7 +627,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmH,
                 const __grid_constant__ CUtensorMap tmW, const PhaseArgs p0, const PhaseArgs p1, int slot_rowlets,
                 int balanced, int n_token_tiles, int32_t* __restrict__ sched /* {tickets, finished CTAs, ready[n_token_tiles]} */,
-                long long* __restrict__ kprof, const __grid_constant__ EfWaveTable tab) {
+                long long* __restrict__ kprof, const EarlyArgs early, const __grid_constant__ EfWaveTable tab) {
     extern __shared__ uint8_t smem_raw[];
     KTIME(long long kt_entry; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(kt_entry));)
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -669,7 +703,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                     mbar_arrive_remote_relaxed_after(mapa(&ctl->sched_empty[ss], 0), tile);
                 }
                 if (tile >= total_tiles) break;
-                const Tile t = decode_tile(tab, ctl, tile, p0, p1);
+                const Tile t = decode_tile(tab, ctl, tile, p0, p1, early);
                 const PhaseArgs& p = t.phase ? p1 : p0;
                 const CUtensorMap* tmA = t.phase ? &tmH : &tmX;
                 const int half = t.n_mma >> 1;                               // token rows this CTA stages
@@ -720,7 +754,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                 mbar_arrive(&ctl->sched_empty[ss]);
                 if (tile >= total_tiles) break;
                 KPROF(++kp_units;)
-                const Tile t = decode_tile(tab, ctl, tile, p0, p1);
+                const Tile t = decode_tile(tab, ctl, tile, p0, p1, early);
                 const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
                 KPROF(long long kp_b = clock64();)
                 for (int h = 0; h < nb; ++h) mbar_wait_cluster(&ctl->tmem_empty[b0 + h], ((bphase >> (b0 + h)) & 1u) ^ 1u);
@@ -770,13 +804,16 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
             __syncwarp();
             if (lane == 0) mbar_arrive_remote_relaxed_after(mapa(&ctl->sched_empty[ss], 0), tile);
             if (tile >= total_tiles) break;
-            const Tile t = decode_tile(tab, ctl, tile, p0, p1);
+            const Tile t = decode_tile(tab, ctl, tile, p0, p1, early);
             const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
             for (int h = 0; h < nb; ++h) {
                 mbar_wait(&ctl->tmem_full[b0 + h], (bphase >> (b0 + h)) & 1u);
                 bphase ^= 1u << (b0 + h);
             }
             tc_fence_after();
+            // the unit's MMAs have completed: neither CTA's stages of it are read any more (early hand-back, see EarlyArgs)
+            if (early.n2 > 0 && t.phase == 1 && t.g == 0 && leader && threadIdx.x == 4 * 32)
+                asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(early.flag), "r"((uint32_t)(t.kb1 - t.kb0)) : "memory");
             if (t.phase == 0)
                 epilogue_unit<kReluExperts ? 2 : 1>(t, p0, ctl, stg_base, tmem_base, rank, warp, lane, b0, nb, ready, ready_need > 0);
             else
@@ -937,7 +974,7 @@ int32_t efk_ffn_tc_init(ef_ctx* ctx) {
 
 // One wave: phase bit 0 = GEMM1 (x -> h), bit 1 = GEMM2 (h -> y).  phase == 3 is ONE launch: the GEMM2 units are ticketed
 // behind the GEMM1 units and wait, per token tile, for that tile's h columns (see the kernel).
-int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase) {
+int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const EfWaveTable& tab, int phase, EfEarly* early) {
     const int d = ctx->cfg.d_model, f = ctx->cfg.d_ff;
     if (tab.n == 0 || !(phase & 3)) return EF_OK;
     const bool relu = ctx->cfg.expert_kind == 1;
@@ -979,6 +1016,47 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
         p.s = pl.s;
         p.total = pl.n_plain + pl.n_tail * pl.s;
     }
+    // Early hand-back of group 0's slot (EarlyArgs): only in a wave whose tiles are all SHORT (decode-sized experts: the
+    // canonical order of a phase is then group order, so group 0's units are its first ones, and a launch of its own for one
+    // such expert is mostly launch, hand-over and tail -- measured on cfg 3: FFN time per step -6 %, step time +0.2 %; for
+    // waves of long tiles a launch of its own is an efficient launch and hands the slot back 50-70 us earlier, cfg 2: step
+    // time +0.3 % for -2 % FFN time, so those keep it) and only when its GEMM1 units are whole and its GEMM2 units
+    // uniformly whole or uniformly split
+    EarlyArgs ea{0, 0, nullptr, 0, 0, 0};
+    if (early) {
+        early->used = false;
+        early->add = 0;
+        if (early->want && phase == 3 && tab.n >= 2 && ctx->splitk_mode <= 1 && ctx->early_flag) {
+            int wave_long = 0;
+            for (int i = 0; i < tab.n; ++i) wave_long += group_long_tiles(tab.g[i].rows, bal);
+            const int nt0 = group_long_tiles(tab.g[0].rows, bal) + group_has_short(tab.g[0].rows, bal);
+            const int n1 = nt0 * pa[0].n_pairs_n, t2 = nt0 * pa[1].n_pairs_n;
+            int n2 = 0;
+            if (wave_long == 0 && n1 <= pa[0].n_plain) {
+                if (t2 <= pa[1].n_plain) n2 = t2;
+                else if (pa[1].n_plain == 0) n2 = t2 * pa[1].s;
+            }
+            if (n2 > 0) {
+                ea = EarlyArgs{n1, n2, ctx->early_flag, 0, t2, 0};
+                // whole GEMM2 units of group 0: split them, with the tail's factor if the phase has a split tail, else
+                // with one that makes about half a round of units
+                if (n2 == t2 && pa[1].KB >= 8) {
+                    const int n_tail = (pa[1].total - pa[1].n_plain) / std::max(1, pa[1].s);
+                    int s0 = pa[1].s > 1 ? pa[1].s : std::min(std::min(16, pa[1].KB / 4), std::max(2, (n_pairs / 2 + t2 - 1) / t2));
+                    if (s0 > 1 && (n_tail + t2) * s0 <= max_units) {
+                        pa[1].s = s0;
+                        pa[1].total += t2 * (s0 - 1);
+                        ea.split0 = 1;
+                        ea.tail0 = n_tail;
+                        ea.n2 = t2 * s0;
+                    }
+                }
+                early->used = true;
+                early->add = (uint32_t)(t2 * pa[1].KB);
+            }
+        }
+        if (early->dry) return EF_OK;
+    }
     const int total = pa[0].total + pa[1].total;
     const int grid = 2 * std::min(total, n_pairs);
     if (2 + mtiles > EF_SCHED_WORDS) return ef_fail(ctx, EF_ERR_CAPACITY, "grouped FFN: too many token tiles in one wave");
@@ -1002,10 +1080,10 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     long long* kprof = (phase & 1) ? ctx->kprof1 : ctx->kprof2;
     if (relu)
         ffn_wave_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(ctx->tm_x, ctx->tm_h, ctx->tm_w, pa[0], pa[1], slot_rowlets,
-                                                                  bal ? 1 : 0, mtiles, sched, kprof, tab);
+                                                                  bal ? 1 : 0, mtiles, sched, kprof, ea, tab);
     else
         ffn_wave_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(ctx->tm_x, ctx->tm_h, ctx->tm_w, pa[0], pa[1], slot_rowlets,
-                                                                   bal ? 1 : 0, mtiles, sched, kprof, tab);
+                                                                   bal ? 1 : 0, mtiles, sched, kprof, ea, tab);
     ctx->launches++;
     EF_CUDA(ctx, cudaGetLastError());
     if (ctx->time_kernels) {

@@ -193,10 +193,14 @@ def test_switch_prefill_relu_top1(T):
 # ------------------------------------------------------------------------------------------------
 # decode traces: cache accounting bit-exact over many visits; outputs checked on sampled visits
 # ------------------------------------------------------------------------------------------------
-def run_decode(cfg, n_steps, horizon, check_out_every, policy="plec"):
+def run_decode(cfg, n_steps, horizon, check_out_every, policy="plec", early_release=None, launches=None, splitk=None):
     L, E = cfg.n_layers, cfg.n_experts
     r, ex = build_runner(cfg, horizon=horizon)
     r.ctx.ef_set_cache_policy(policy)
+    if early_release is not None:
+        r.ctx.ef_set_option(7, early_release)             # EF_OPT_EARLY_RELEASE
+    if splitk is not None:
+        r.ctx.ef_set_option(1, splitk)                    # EF_OPT_SPLITK
     tr = wl.routing_trace(cfg, n_steps)
     sim = CacheSim(L, E, cfg.n_slots, cfg.expert_bytes, horizon, policy=policy)
     nv = n_steps * L
@@ -240,8 +244,29 @@ def run_decode(cfg, n_steps, horizon, check_out_every, policy="plec"):
             hd = nxt
     r.ctx.ef_sync()
     st = r.ctx.ef_cache_get_stats()
+    if launches is not None:
+        launches.append(r.ctx.ef_launch_count())
     r.close()
     return st, sim
+
+
+@pytest.mark.parametrize("d_model,d_ff,T,splitk", [(256, 512, 16, None), (512, 3072, 16, None), (256, 512, 100, 1)],
+                         ids=["short_k", "long_k_split", "wider_tiles_no_split"])
+def test_first_victim_slot_is_handed_back_from_inside_the_hits_wave(d_model, d_ff, T, splitk):
+    """EF_OPT_EARLY_RELEASE: the hit whose slot the first pending copy overwrites runs inside the hits' wave (ticketed first)
+    and the copy waits on a device word its GEMM2 units bump, instead of on the event behind a launch of its own.  The
+    copy then lands in the slot WHILE that wave is still running: outputs are checked against the oracle after every
+    visit (a hand-back that came too early would feed the rest of the wave the next expert's weights), the slot table and
+    the counters are the simulator's with the option on and off, and with it on there are fewer launches.  (A wave hands a
+    slot back only when all its tiles are short, i.e. for decode-sized experts, and group 0's GEMM1 units are whole.)"""
+    cfg = wl.scaled(wl.CONFIGS["mixtral_decode"], d_model=d_model, d_ff=d_ff, T=T)
+    n = {}
+    for on in (1, 0):
+        L = []
+        st, sim = run_decode(cfg, n_steps=24, horizon=1, check_out_every=1, early_release=on, launches=L, splitk=splitk)
+        n[on] = (L[0], st)
+    assert n[1][1] == n[0][1]                   # accounting does not depend on the physical schedule
+    assert n[1][0] < n[0][0], n                 # the early path really ran: one launch fewer per visit with a first victim
 
 
 @pytest.mark.parametrize("horizon", [1, 0])

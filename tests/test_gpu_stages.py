@@ -388,7 +388,7 @@ def test_set_option_validates_keys_and_values():
     ctx = make_ctx()
     for key, good, bad in ((EF_OPT_SPLITK, (0, 1, 16), (-1, 17)), (EF_OPT_WAVE_BYTES, (0, 1 << 40), (-1,)),
                            (EF_OPT_CHUNK_MIN_BYTES, (0, 1), (-5,)), (EF_OPT_COPY_ORDER, (0, 1), (2, -1)),
-                           (EF_OPT_FUSED_WAVES, (0, 1), ()), (EF_OPT_TOKEN_SCHED_PATH, (0, 1), ())):
+                           (EF_OPT_FUSED_WAVES, (0, 1), ()), (EF_OPT_TOKEN_SCHED_PATH, (0, 1), ()), (7, (0, 1), ())):   # 7 = EF_OPT_EARLY_RELEASE
         for v in good:
             ctx.ef_set_option(key, v)
         for v in bad:
