@@ -649,13 +649,14 @@ struct MissBatcher {
     MissBatcher(ef_ctx* c, cudaStream_t s, const void* x, void* y, int n_misses)
         : ctx(c), st(s), x_perm(x), y_perm(y), remaining(n_misses) {
         min_wave = (int)std::max<int64_t>(1, std::min<int64_t>(EF_MAX_GROUPS, ctx->wave_bytes / ctx->W));
+        slot_wave.assign(ctx->cfg.n_slots, 0);
         target = next_target();
     }
     int next_target() const {
         if (ctx->wave_bytes == 0) return 1;
         int t = std::min(EF_MAX_GROUPS, std::max(min_wave, remaining / 2));
         // small experts: no trailing wave of one or two -- what is left joins this wave (see push)
-        if (!last_alone() && remaining - t < std::max(2, min_wave / 2) && remaining <= EF_MAX_GROUPS) t = std::max(t, remaining);
+        if (!last_alone() && remaining - t <= std::max(2, min_wave / 2) && remaining <= EF_MAX_GROUPS) t = std::max(t, remaining);
         return t;
     }
     bool last_alone() const { return ctx->chunk_min_bytes > 0 && ctx->W >= ctx->chunk_min_bytes; }
@@ -663,8 +664,12 @@ struct MissBatcher {
         for (const WaveItem& it : open) if (it.slot == slot) return true;
         return false;
     }
+    std::vector<int> slot_wave;   // per slot: sequence number of the miss wave that read it last (0: none of them)
+    int seq = 1;
     int32_t flush(bool last_of_visit = false) {
         if (open.empty()) return EF_OK;
+        for (const WaveItem& it : open) slot_wave[it.slot] = seq;
+        ++seq;
         int32_t rc = run_wave(ctx, st, x_perm, y_perm, open, last_of_visit);
         open.clear();
         target = next_target();
@@ -812,12 +817,39 @@ extern "C" int32_t ef_expert_ffn_grouped(ef_ctx* ctx, void* stream, int64_t visi
     MissBatcher mb(ctx, st, x_perm, y_perm, (int)(planA.size() + planB.size()));
     for (size_t i = 0; i < planA.size(); ++i)   // compute starts as the copies land, one grouped launch per batch
         if ((rc = mb.push(planA[i].item, planB.empty() && i + 1 == planA.size())) != EF_OK) return rc;
-    for (size_t i = 0; i < planB.size(); ++i) {
-        const Miss& m = planB[i];
-        // the copy into the slot waits for the "free" event of the wave that read it: that wave must be enqueued first
-        if (mb.holds_slot(m.item.slot) && (rc = mb.flush()) != EF_OK) return rc;
+    // The copy into a slot waits for the "free" event of the wave that read the slot last: that wave must be enqueued first.
+    // A miss whose slot belongs to a member of the OPEN wave therefore steps back behind the misses that can go now
+    // (EF_OPT_COPY_ORDER = 1; in policy copy order the open wave is launched early instead, as a small wave of its own): the
+    // link stays busy, and the open wave fills up to its target instead of being flushed with a handful of experts.  A miss
+    // never overtakes an earlier miss of the same slot (an earlier generation).  Among the misses that can go, the one
+    // whose slot was read by the OLDEST wave goes first: the copy stream is a FIFO, and a copy that has to wait for a wave
+    // that has only just been launched would hold up every copy behind it.
+    std::vector<char> done(planB.size(), 0);
+    size_t n_done = 0;
+    while (n_done < planB.size()) {
+        size_t pick = planB.size(), first_head = planB.size();
+        for (size_t i = 0; i < planB.size(); ++i) {
+            if (done[i]) continue;
+            bool head = true;                         // planB is in generation order: an earlier entry of the same slot goes first
+            for (size_t k = 0; k < i && head; ++k) head = done[k] || planB[k].item.slot != planB[i].item.slot;
+            if (!head) continue;
+            if (first_head == planB.size()) first_head = i;
+            if (ctx->copy_order != 1) {               // policy copy order: no overtaking
+                if (!mb.holds_slot(planB[i].item.slot)) pick = i;
+                break;
+            }
+            if (mb.holds_slot(planB[i].item.slot)) continue;
+            if (pick == planB.size() || mb.slot_wave[planB[i].item.slot] < mb.slot_wave[planB[pick].item.slot]) pick = i;
+        }
+        if (pick == planB.size()) {                   // whatever could go next waits for the open wave: launch it
+            if ((rc = mb.flush()) != EF_OK) return rc;
+            pick = first_head;
+        }
+        const Miss& m = planB[pick];
         if ((rc = enqueue_copy(ctx, m.item.slot, m.g)) != EF_OK) return rc;
-        if ((rc = mb.push(m.item, i + 1 == planB.size())) != EF_OK) return rc;
+        done[pick] = 1;
+        ++n_done;
+        if ((rc = mb.push(m.item, n_done == planB.size())) != EF_OK) return rc;
     }
     return mb.flush();
 }
