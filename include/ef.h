@@ -286,8 +286,8 @@ int32_t ef_get_launch_log(ef_ctx* ctx, ef_launch_record* out, int32_t max_record
  *                        and every counter are decided in policy order either way.
  * EF_OPT_EARLY_RELEASE   1 (default) = the hit whose slot the visit's first pending copy will overwrite is handed back from
  *                        INSIDE the hits' wave (its units are ticketed first and count themselves done on a device word
- *                        the copy stream waits for) when that wave consists of short (<= 128-token) tiles only, i.e. of
- *                        decode-sized experts; 0 = that hit always runs as a wave of its own first.
+ *                        the copy stream waits for) when that hit is a decode-sized expert (one token tile of <= 128 rows);
+ *                        0 = that hit always runs as a wave of its own first.
  *                        Physical scheduling only. */
 #define EF_OPT_SPLITK 1
 #define EF_OPT_WAVE_BYTES 2

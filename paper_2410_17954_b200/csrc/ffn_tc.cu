@@ -331,15 +331,16 @@ struct PhaseArgs {
 };
 
 // Early hand-back of ONE expert's slot (ef_internal.h, EfEarly): group 0 of the table is the hit whose slot the visit's first
-// pending copy will overwrite.  Its GEMM2 units -- canonical units [p0.total, p0.total + n2) -- are ticketed at position `a`
-// (one round of other GEMM1 units behind its own GEMM1 units, which are the first tickets) instead of behind every GEMM1
-// unit of the wave, and each of them adds its k-blocks to *flag once its MMAs have completed, i.e. once nothing of the unit
-// reads the slot any more; the copy stream waits for the sum (cuStreamWaitValue32), not for the end of the launch.
-// (a = the number of group 0's GEMM1 units: measured, one more round of other units in between changes nothing.)
+// pending copy will overwrite -- a decode-sized expert: ONE short token tile.  Its units are the first tickets of the launch:
+// [0, e1) its GEMM1 units, [e1, e1 + e2) its GEMM2 units (split s ways along K like a tail when split0), ahead of every unit
+// of the other groups, whose phases are planned and ordered as if group 0 were not in the wave.  Still deadlock-free: its
+// GEMM2 units depend only on lower tickets, which never wait.  Each of its GEMM2 units adds its k-blocks to *flag once its MMAs
+// have completed, i.e. once nothing of the unit reads the slot any more; the copy stream waits for the sum
+// (cuStreamWaitValue32), not for the end of the launch.
 struct EarlyArgs {
-    int32_t a, n2;          // n2 == 0: off
+    int32_t e1, e2;         // e1 == 0: off
     uint32_t* flag;
-    int32_t split0, t2, tail0;   // split0: group 0's t2 GEMM2 tiles are split p1.s ways; tail0 = split tiles of the phase's tail
+    int32_t split0, tail0;  // split0: group 0's GEMM2 tiles are split p1.s ways, workspace slots / counters from index tail0 on
 };
 
 struct Tile {
@@ -387,69 +388,72 @@ __device__ __host__ __forceinline__ int group_has_short(int rows, bool balanced)
 __device__ __forceinline__ Tile decode_tile(const EfWaveTable& tab, const SmemCtl* ctl, int unit, const PhaseArgs& p0,
                                             const PhaseArgs& p1, const EarlyArgs& early) {
     Tile t;
-    // ticket -> canonical unit (all GEMM1 units, then all GEMM2 units): group 0's GEMM2 units are pulled forward to ticket a
-    if (early.n2 > 0 && unit >= early.a && unit < p0.total + early.n2)
-        unit = unit < early.a + early.n2 ? p0.total + (unit - early.a) : unit - early.n2;
-    t.phase = unit >= p0.total ? 1 : 0;
-    const PhaseArgs& p = t.phase ? p1 : p0;
-    int u = unit - (t.phase ? p0.total : 0);
-    int g = 0, j;
-    t.kb0 = 0; t.kb1 = p.KB; t.tail = -1; t.split_j = 0;
-    int tile = -1;
-    if (t.phase == 1 && early.split0) {
-        // group 0's GEMM2 tiles -- the first t2 whole tiles of the phase -- are split s ways as well (each unit is then short
-        // enough for the slot to come back about as early as from a launch of its own); their workspace slots and arrival
-        // counters follow the tail's
-        if (u < early.t2 * p.s) {
-            tile = u / p.s;
-            t.split_j = u - tile * p.s;
-            t.tail = early.tail0 + tile;
+    t.tail = -1; t.split_j = 0;
+    int g = 0, j = 0;
+    if (unit < early.e1 + early.e2) {
+        // group 0's single short tile (early hand-back): its GEMM1 units, then its GEMM2 units
+        t.phase = unit >= early.e1 ? 1 : 0;
+        const PhaseArgs& p = t.phase ? p1 : p0;
+        t.kb0 = 0; t.kb1 = p.KB;
+        t.n_pair = unit - (t.phase ? early.e1 : 0);
+        if (t.phase == 1 && early.split0) {
+            const int k = t.n_pair;
+            t.n_pair = k / p.s;
+            t.split_j = k - t.n_pair * p.s;
+            t.tail = early.tail0 + t.n_pair;
             t.kb0 = (t.split_j * p.KB) / p.s;
             t.kb1 = ((t.split_j + 1) * p.KB) / p.s;
-        } else {
-            u -= early.t2 * (p.s - 1);
         }
-    }
-    if (tile >= 0) {
-    } else if (u < p.n_plain) {
-        tile = u;
-    } else {
-        const int v = u - p.n_plain;
-        t.tail = v / p.s;
-        t.split_j = v - t.tail * p.s;
-        tile = p.n_plain + t.tail;
-        t.kb0 = (t.split_j * p.KB) / p.s;
-        t.kb1 = ((t.split_j + 1) * p.KB) / p.s;
-    }
-    // Ticket order inside a phase: long (129..256-token) tiles are tensor-bound, short ones are bound by streaming their
-    // weight tile, so a launch with many short tiles (many-expert prefill) spreads them evenly among the long ones --
-    // both kinds are then in flight on different SMs at the same time -- and keeps only the last `tail_short` short
-    // tiles for the end of the list, where small units even out the finish (and where the split-K tail lives).
-    const int npn = p.n_pairs_n;
-    const int total_long = ctl->tl[tab.n] * npn, total_short = ctl->tsh[tab.n] * npn;
-    const int tail_short = min(total_short, (int)gridDim.x / 4);
-    const int spread = total_short - tail_short, first = total_long + spread;
-    bool is_short;
-    if (tile >= first) {
-        is_short = true;
-        tile = spread + (tile - first);
-    } else {
-        const int sb = (int)(((long long)tile * spread) / first), sb1 = (int)(((long long)(tile + 1) * spread) / first);
-        is_short = sb1 > sb;
-        tile = is_short ? sb : tile - sb;
-    }
-    if (!is_short) {
-        while (tile >= ctl->tl[g + 1] * npn) ++g;
-        const int local = tile - ctl->tl[g] * npn;
-        const int nl = ctl->g_long[g];
-        t.n_pair = local / nl;                  // n-major inside a group: the token tiles that share a weight tile are
-        j = local - t.n_pair * nl;              // claimed back to back and hit L2
-        t.is_long = 1;
-    } else {
-        while (tile >= ctl->tsh[g + 1] * npn) ++g;
-        t.n_pair = tile - ctl->tsh[g] * npn;
-        j = ctl->g_long[g];
         t.is_long = 0;
+    } else {
+        // the other groups (all groups when there is no early group): tickets in canonical order, all GEMM1 units, then all GEMM2 units
+        const int skip = early.e1 > 0 ? 1 : 0;      // group 0 is not part of this order
+        unit -= early.e1 + early.e2;
+        t.phase = unit >= p0.total ? 1 : 0;
+        const PhaseArgs& p = t.phase ? p1 : p0;
+        const int u = unit - (t.phase ? p0.total : 0);
+        int tile = u;
+        t.kb0 = 0; t.kb1 = p.KB;
+        if (u >= p.n_plain) {
+            const int v = u - p.n_plain;
+            t.tail = v / p.s;
+            t.split_j = v - t.tail * p.s;
+            tile = p.n_plain + t.tail;
+            t.kb0 = (t.split_j * p.KB) / p.s;
+            t.kb1 = ((t.split_j + 1) * p.KB) / p.s;
+        }
+        // Ticket order inside a phase: long (129..256-token) tiles are tensor-bound, short ones are bound by streaming their
+        // weight tile, so a launch with many short tiles (many-expert prefill) spreads them evenly among the long ones --
+        // both kinds are then in flight on different SMs at the same time -- and keeps only the last `tail_short` short
+        // tiles for the end of the list, where small units even out the finish (and where the split-K tail lives).
+        const int npn = p.n_pairs_n;
+        const int skip_short = skip * npn;          // the early group's tile is short and the first of the short tiles
+        const int total_long = ctl->tl[tab.n] * npn, total_short = ctl->tsh[tab.n] * npn - skip_short;
+        const int tail_short = min(total_short, (int)gridDim.x / 4);
+        const int spread = total_short - tail_short, first = total_long + spread;
+        bool is_short;
+        if (tile >= first) {
+            is_short = true;
+            tile = spread + (tile - first);
+        } else {
+            const int sb = (int)(((long long)tile * spread) / first), sb1 = (int)(((long long)(tile + 1) * spread) / first);
+            is_short = sb1 > sb;
+            tile = is_short ? sb : tile - sb;
+        }
+        if (!is_short) {
+            while (tile >= ctl->tl[g + 1] * npn) ++g;
+            const int local = tile - ctl->tl[g] * npn;
+            const int nl = ctl->g_long[g];
+            t.n_pair = local / nl;                  // n-major inside a group: the token tiles that share a weight tile are
+            j = local - t.n_pair * nl;              // claimed back to back and hit L2
+            t.is_long = 1;
+        } else {
+            tile += skip_short;
+            while (tile >= ctl->tsh[g + 1] * npn) ++g;
+            t.n_pair = tile - ctl->tsh[g] * npn;
+            j = ctl->g_long[g];
+            t.is_long = 0;
+        }
     }
     const int row_off = j * ctl->g_tile_rows[g];
     t.tid = ctl->tl[g] + ctl->tsh[g] + j;
@@ -636,7 +640,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
     const bool leader = rank == 0;
-    const int total_tiles = p0.total + p1.total;
+    const int total_tiles = early.e1 + early.e2 + p0.total + p1.total;
     int32_t* ready = sched + 2;
     // a GEMM2 unit waits for the h columns of all real weight tiles of GEMM1 (only when GEMM1 runs in this launch)
     const int ready_need = (p0.total > 0 && p1.total > 0) ? p0.n_tiles_n : 0;
@@ -812,7 +816,7 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
             }
             tc_fence_after();
             // the unit's MMAs have completed: neither CTA's stages of it are read any more (early hand-back, see EarlyArgs)
-            if (early.n2 > 0 && t.phase == 1 && t.g == 0 && leader && threadIdx.x == 4 * 32)
+            if (early.e1 > 0 && t.phase == 1 && t.g == 0 && leader && threadIdx.x == 4 * 32)
                 asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(early.flag), "r"((uint32_t)(t.kb1 - t.kb0)) : "memory");
             if (t.phase == 0)
                 epilogue_unit<kReluExperts ? 2 : 1>(t, p0, ctl, stg_base, tmem_base, rank, warp, lane, b0, nb, ready, ready_need > 0);
@@ -1005,59 +1009,52 @@ int32_t efk_ffn_tc(ef_ctx* ctx, cudaStream_t st, const void* x, void* y, const E
     pa[1] = PhaseArgs{(uint16_t*)y, d, d, f / BK, ntn2, (ntn2 + 1) / 2, d, (int)((int64_t)w1_rows * d / EF_ROWLET), 0, 0, 1, acc_f4,
                       ctx->splitk_ws + (size_t)kSlotFloats * 2 * ctx->splitk_max_units,
                       ctx->splitk_counters + 2 * 8 * ctx->splitk_max_units};
+    // Early hand-back of group 0's slot (EarlyArgs): group 0 must be ONE short tile (a decode-sized expert: a launch of its
+    // own for it is mostly launch, hand-over and tail -- measured on cfg 3: FFN time per step -6 %, step time +0.2 %; an expert
+    // of long tiles keeps its own launch, which is an efficient launch and hands the slot back 50-70 us earlier than a wave
+    // could, cfg 2: step time +0.3 % for -2 % FFN time).  Its units are ticketed ahead of the wave; the phases of the other
+    // groups are planned as if it were not there.
+    EarlyArgs ea{0, 0, nullptr, 0, 0};
+    bool early_on = false;
+    if (early) {
+        early->used = false;
+        early->add = 0;
+        early_on = early->want && phase == 3 && tab.n >= 2 && ctx->splitk_mode <= 1 && ctx->early_flag && tab.g[0].rows <= 128;
+    }
+    const int skip = early_on ? 1 : 0;
     for (int ph = 0; ph < 2; ++ph) {
         if (!(phase & (1 << ph))) continue;
         PhaseArgs& p = pa[ph];
-        const int tiles = mtiles * p.n_pairs_n;
+        const int tiles = (mtiles - skip) * p.n_pairs_n;
         // GEMM1 of a fused wave is followed by GEMM2 units that depend on it: its tail cannot be filled by them when the wave
         // is one token tile deep, so it is split like a launch of its own
-        const SplitPlan pl = plan_split(ctx, tiles, mshort * p.n_pairs_n, n_pairs, p.KB, avg_rows, max_units);
+        const double avg = early_on ? (double)(rows_total - tab.g[0].rows) / (mtiles - 1) : avg_rows;
+        const SplitPlan pl = plan_split(ctx, tiles, (mshort - skip) * p.n_pairs_n, n_pairs, p.KB, avg, max_units);
         p.n_plain = pl.n_plain;
         p.s = pl.s;
         p.total = pl.n_plain + pl.n_tail * pl.s;
     }
-    // Early hand-back of group 0's slot (EarlyArgs): only in a wave whose tiles are all SHORT (decode-sized experts: the
-    // canonical order of a phase is then group order, so group 0's units are its first ones, and a launch of its own for one
-    // such expert is mostly launch, hand-over and tail -- measured on cfg 3: FFN time per step -6 %, step time +0.2 %; for
-    // waves of long tiles a launch of its own is an efficient launch and hands the slot back 50-70 us earlier, cfg 2: step
-    // time +0.3 % for -2 % FFN time, so those keep it) and only when its GEMM1 units are whole and its GEMM2 units
-    // uniformly whole or uniformly split
-    EarlyArgs ea{0, 0, nullptr, 0, 0, 0};
-    if (early) {
-        early->used = false;
-        early->add = 0;
-        if (early->want && phase == 3 && tab.n >= 2 && ctx->splitk_mode <= 1 && ctx->early_flag) {
-            int wave_long = 0;
-            for (int i = 0; i < tab.n; ++i) wave_long += group_long_tiles(tab.g[i].rows, bal);
-            const int nt0 = group_long_tiles(tab.g[0].rows, bal) + group_has_short(tab.g[0].rows, bal);
-            const int n1 = nt0 * pa[0].n_pairs_n, t2 = nt0 * pa[1].n_pairs_n;
-            int n2 = 0;
-            if (wave_long == 0 && n1 <= pa[0].n_plain) {
-                if (t2 <= pa[1].n_plain) n2 = t2;
-                else if (pa[1].n_plain == 0) n2 = t2 * pa[1].s;
-            }
-            if (n2 > 0) {
-                ea = EarlyArgs{n1, n2, ctx->early_flag, 0, t2, 0};
-                // whole GEMM2 units of group 0: split them, with the tail's factor if the phase has a split tail, else
-                // with one that makes about half a round of units
-                if (n2 == t2 && pa[1].KB >= 8) {
-                    const int n_tail = (pa[1].total - pa[1].n_plain) / std::max(1, pa[1].s);
-                    int s0 = pa[1].s > 1 ? pa[1].s : std::min(std::min(16, pa[1].KB / 4), std::max(2, (n_pairs / 2 + t2 - 1) / t2));
-                    if (s0 > 1 && (n_tail + t2) * s0 <= max_units) {
-                        pa[1].s = s0;
-                        pa[1].total += t2 * (s0 - 1);
-                        ea.split0 = 1;
-                        ea.tail0 = n_tail;
-                        ea.n2 = t2 * s0;
-                    }
-                }
-                early->used = true;
-                early->add = (uint32_t)(t2 * pa[1].KB);
+    if (early_on) {
+        const int t2 = pa[1].n_pairs_n;            // group 0's GEMM2 tiles (pair units)
+        ea = EarlyArgs{pa[0].n_pairs_n, t2, ctx->early_flag, 0, 0};
+        // split them along K: with the tail's factor if the others' phase has a split tail, else with one that makes about
+        // half a round of units -- each unit is then short enough for the slot to come back about as early as from a launch
+        // of its own
+        if (pa[1].KB >= 8) {
+            const int n_tail = (pa[1].total - pa[1].n_plain) / std::max(1, pa[1].s);
+            const int s0 = pa[1].s > 1 ? pa[1].s : std::min(std::min(16, pa[1].KB / 4), std::max(2, (n_pairs / 2 + t2 - 1) / t2));
+            if (s0 > 1 && (n_tail + t2) * s0 <= max_units) {
+                pa[1].s = s0;
+                ea.split0 = 1;
+                ea.tail0 = n_tail;
+                ea.e2 = t2 * s0;
             }
         }
-        if (early->dry) return EF_OK;
+        early->used = true;
+        early->add = (uint32_t)(t2 * pa[1].KB);
     }
-    const int total = pa[0].total + pa[1].total;
+    if (early && early->dry) return EF_OK;
+    const int total = ea.e1 + ea.e2 + pa[0].total + pa[1].total;
     const int grid = 2 * std::min(total, n_pairs);
     if (2 + mtiles > EF_SCHED_WORDS) return ef_fail(ctx, EF_ERR_CAPACITY, "grouped FFN: too many token tiles in one wave");
     if (phase & 1) {

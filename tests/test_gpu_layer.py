@@ -258,7 +258,7 @@ def test_first_victim_slot_is_handed_back_from_inside_the_hits_wave(d_model, d_f
     copy then lands in the slot WHILE that wave is still running: outputs are checked against the oracle after every
     visit (a hand-back that came too early would feed the rest of the wave the next expert's weights), the slot table and
     the counters are the simulator's with the option on and off, and with it on there are fewer launches.  (A wave hands a
-    slot back only when all its tiles are short, i.e. for decode-sized experts, and group 0's GEMM1 units are whole.)"""
+    slot back only when the first victim is a decode-sized expert: one token tile of <= 128 rows.)"""
     cfg = wl.scaled(wl.CONFIGS["mixtral_decode"], d_model=d_model, d_ff=d_ff, T=T)
     n = {}
     for on in (1, 0):
