@@ -230,6 +230,20 @@ int32_t ef_reindex_rows(ef_ctx* ctx, void* stream, const void* src, const int32_
 /* The Hamming distance matrix of Eq. 6 alone: dist_out DEVICE uint16[N, N] (16-byte aligned), d_ij = number of
  * (layer, expert) entries in which r_i and r_j differ; S_ij = 1 - d_ij / LE.  N need not be even here. */
 int32_t ef_path_hamming(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, uint16_t* dist_out);
+/* ef_path_hamming for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same result, but the scratch -- the bit-packed paths, N * ceil(LE / 32) * 4 bytes --
+ * lives in a static device array inside the library instead of in a cudaMalloc'ed workspace.  The call makes no
+ * cudaMalloc, cudaFree or allocating library call: it launches two kernels on `stream`.
+ *   - Limit: N * ceil(LE / 32) * 4 <= EF_STATIC_SCRATCH_BYTES (1 MiB; e.g. N = 4096 tokens of LE = 2048 path entries);
+ *     beyond it the call fails with EF_ERR_CAPACITY and does nothing.  The array costs that much memory on every GPU that
+ *     loads the library, until the process exits.
+ *   - Its device address is resolved once per ctx at ef_create (cudaGetSymbolAddress with the ctx's device current); if
+ *     that failed, this call returns EF_ERR_CUDA with the reason.
+ *   - ONE array per device, shared by every call and every ctx on that device: two calls that overlap on the GPU (two
+ *     streams, two ctxs, two host threads) race on it and both results are undefined; calls on one stream are safe.  The
+ *     array keeps the last call's contents; nothing in it has to start at zero (every word read is written first). */
+#define EF_STATIC_SCRATCH_BYTES (1 << 20)
+int32_t ef_path_hamming_static(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE, uint16_t* dist_out);
 
 /* ---- misc ---------------------------------------------------------------------------------- */
 /* Wait for the copy stream and the device.  Synchronous. */

@@ -19,6 +19,7 @@ DECLARED_SYMBOLS = [
     "ef_expert_ffn_grouped", "ef_expert_ffn_grouped_resident", "ef_shared_ffn", "ef_combine", "ef_rmsnorm",
     "ef_cache_prefetch", "ef_cache_evict", "ef_cache_get_stats", "ef_cache_reset_stats", "ef_cache_snapshot",
     "ef_cache_clear", "ef_set_cache_policy", "ef_copy_busy_ms", "ef_token_schedule", "ef_reindex_rows", "ef_path_hamming",
+    "ef_path_hamming_static",
     "ef_sync", "ef_last_error", "ef_launch_count", "ef_set_kernel_timing", "ef_get_kernel_times", "ef_get_launch_log",
     "ef_set_option",
 ]
@@ -102,6 +103,7 @@ def load_library(diag: bool = False) -> ctypes.CDLL:
             "ef_token_schedule": [vp, vp, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp],
             "ef_reindex_rows": [vp, vp, vp, vp, i32, i64, vp],
             "ef_path_hamming": [vp, vp, vp, i32, i32, vp],
+            "ef_path_hamming_static": [vp, vp, vp, i32, i32, vp],
             "ef_set_cache_policy": [vp, i32],
             "ef_set_option": [vp, i32, i64],
         }
@@ -259,6 +261,11 @@ class EfContext:
         N = paths.shape[0]
         LE = paths.numel() // max(1, N)
         self._chk(self.lib.ef_path_hamming(self.h, _stream(), _dp(paths), N, LE, _dp(dist_out)))
+
+    def ef_path_hamming_static(self, paths, dist_out):
+        N = paths.shape[0]
+        LE = paths.numel() // max(1, N)
+        self._chk(self.lib.ef_path_hamming_static(self.h, _stream(), _dp(paths), N, LE, _dp(dist_out)))
 
     def ef_cache_get_stats(self) -> dict:
         st = CacheStats()

@@ -166,6 +166,7 @@ extern "C" int32_t ef_create(const ef_config* cfg, ef_ctx** out) {
             ctx->wait_value_fn = fn;
         }
     }
+    efk_token_sched_static_init(ctx);      // ef_path_hamming_static's scratch address; never fails ef_create
     int32_t rc = efk_ffn_tc_init(ctx);
     if (rc != EF_OK) {
         g_create_err = "ef_create: " + ctx->err;
@@ -981,6 +982,17 @@ extern "C" int32_t ef_path_hamming(ef_ctx* ctx, void* stream, const uint8_t* pat
     if (N == 0) return EF_OK;
     EF_ENTER_SCHED(ctx, (cudaStream_t)stream);
     return efk_path_hamming(ctx, (cudaStream_t)stream, paths, N, LE, dist_out);
+}
+
+extern "C" int32_t ef_path_hamming_static(ef_ctx* ctx, void* stream, const uint8_t* paths, int32_t N, int32_t LE,
+                                          uint16_t* dist_out) {
+    EF_CHECK_CTX(ctx);
+    if (N < 0 || (N > 0 && (!paths || !dist_out)) || LE < 1) return ef_fail(ctx, EF_ERR_INVALID_ARG, "ef_path_hamming_static: bad argument");
+    if (N > EF_TS_MAX_TOKENS || LE > 32767 || ((uintptr_t)dist_out & 15))
+        return ef_fail(ctx, EF_ERR_UNSUPPORTED, "ef_path_hamming_static: N <= %d, LE <= 32767, dist_out 16-byte aligned", EF_TS_MAX_TOKENS);
+    if (N == 0) return EF_OK;
+    EF_ENTER_SCHED(ctx, (cudaStream_t)stream);
+    return efk_path_hamming_static(ctx, (cudaStream_t)stream, paths, N, LE, dist_out);
 }
 
 extern "C" int32_t ef_cache_get_stats(ef_ctx* ctx, ef_cache_stats* out) {

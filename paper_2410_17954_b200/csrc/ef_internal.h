@@ -142,6 +142,8 @@ struct ef_ctx {
     void* ts_dist = nullptr;
     size_t ts_dist_bytes = 0;
     bool ts_small_attr = false;         // ts_small_kernel opted in to > 48 KB dynamic smem
+    void* ts_static_scratch = nullptr;  // device address of token_sched.cu's static scratch array (cudaGetSymbolAddress at ef_create)
+    int32_t ts_static_err = 0;          // the cudaError_t of that call
     int32_t ts_force_multi = 0;         // test hook (EF_OPT_TOKEN_SCHED_PATH): 1 = never take the single-CTA path
     // physical scheduling knobs (never part of the policy): ef_set_option(EF_OPT_WAVE_BYTES / EF_OPT_CHUNK_MIN_BYTES)
     int64_t wave_bytes = (int64_t)128 << 20;
@@ -200,6 +202,8 @@ int32_t efk_reindex_rows(ef_ctx* ctx, cudaStream_t st, const void* src, const in
                          void* dst);
 int32_t efk_path_hamming(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, uint16_t* dist_out);
 void efk_token_sched_free(ef_ctx* ctx);
+void efk_token_sched_static_init(ef_ctx* ctx);   // resolves the static scratch's device address; the ctx's device is current
+int32_t efk_path_hamming_static(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, uint16_t* dist_out);
 int32_t efk_ffn_tc_init(ef_ctx* ctx);   // build arena tensor maps, set smem attributes
 // Early hand-back of the slot of group 0 from INSIDE a fused wave (ffn_tc.cu, EarlyArgs): the launch adds `add` to
 // ctx->early_flag in total, the last of it as soon as nothing of the launch reads that slot any more.

@@ -443,6 +443,49 @@ int32_t ts_distances(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, 
 
 }  // namespace
 
+// ---- the no-allocation entry point (ef.h: ef_path_hamming_static) ------------------------------------------------------
+// Scratch for the bit-packed paths of ONE call, in the library's image instead of in cudaMalloc'ed memory:
+// EF_STATIC_SCRATCH_BYTES (1 MiB) on every GPU that loads the library, until the process exits.  In HOST code the name
+// below is a host-side stand-in, not a device address; the address is resolved once per device, at set-up (ef_create, with
+// the ctx's device current), by cudaGetSymbolAddress, and that pointer is what the kernels are given.
+static __device__ __align__(256) uint32_t g_ts_static_scratch[EF_STATIC_SCRATCH_BYTES / sizeof(uint32_t)];
+
+// set-up: called by ef_create with the ctx's device current.  A failure is remembered, not fatal: only
+// ef_path_hamming_static needs the address, and it reports the failure when it is called.
+void efk_token_sched_static_init(ef_ctx* ctx) {
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_ts_static_scratch);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        ptr = nullptr;
+    }
+    ctx->ts_static_scratch = ptr;
+    ctx->ts_static_err = (int32_t)e;
+}
+
+// No cudaMalloc, cudaFree or allocating library routine on this path: two kernel launches on the caller's stream.
+// Nothing in the scratch has to start at zero: ts_pack_kernel overwrites every word ts_hamming_kernel reads (rows < N,
+// words < Wd), so the previous call's contents are never seen.
+int32_t efk_path_hamming_static(ef_ctx* ctx, cudaStream_t st, const uint8_t* paths, int N, int LE, uint16_t* dist_out) {
+    const int Wd = (LE + 31) / 32;
+    const size_t need = (size_t)N * Wd * sizeof(uint32_t);
+    if (need > (size_t)EF_STATIC_SCRATCH_BYTES)
+        return ef_fail(ctx, EF_ERR_CAPACITY, "ef_path_hamming_static: N * ceil(LE / 32) * 4 = %zu bytes of packed paths exceed the static "
+                       "scratch of %d bytes (use ef_path_hamming, which allocates)", need, (int)EF_STATIC_SCRATCH_BYTES);
+    if (!ctx->ts_static_scratch)
+        return ef_fail(ctx, EF_ERR_CUDA, "ef_path_hamming_static: cudaGetSymbolAddress of the static scratch failed at ef_create: %s",
+                       cudaGetErrorString((cudaError_t)ctx->ts_static_err));
+    uint32_t* P = (uint32_t*)ctx->ts_static_scratch;
+    ts_pack_kernel<<<(N * 32 + 255) / 256, 256, 0, st>>>(paths, N, LE, Wd, P);
+    ctx->launches++;
+    EF_CUDA(ctx, cudaGetLastError());
+    const int nt = (N + TS_TILE - 1) / TS_TILE;
+    ts_hamming_kernel<<<dim3(nt, nt), 256, 0, st>>>(P, N, Wd, dist_out);
+    ctx->launches++;
+    EF_CUDA(ctx, cudaGetLastError());
+    return EF_OK;
+}
+
 void efk_token_sched_free(ef_ctx* ctx) {
     if (ctx->ts_state) cudaFree(ctx->ts_state);
     if (ctx->ts_small) cudaFree(ctx->ts_small);
