@@ -188,6 +188,12 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, ui
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.cta_group::2 [%0], [%1, {%3, %4}], [%2];"
         ::"r"(smem_u32(dst)), "l"(tm), "r"(bar), "r"(c0), "r"(c1) : "memory");
 }
+// one lane of a converged warp
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 // arrives, once the MMAs issued so far have completed, on the barrier at this offset in BOTH CTAs of the pair
@@ -744,9 +750,15 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
         }
     } else if (warp == 1) {
         // ===== MMA issuer (leader CTA only) =====
-        if (lane == 0 && leader) {
+        // The WHOLE warp runs this loop in step and one elected lane issues: every operand of a tcgen05 instruction is then a
+        // warp-uniform value the compiler keeps in uniform registers (values read from shared memory are made uniform with a
+        // shuffle from lane 0).  Issued from inside an `if (lane == 0)` region instead, each tcgen05.mma costs a loop of
+        // ELECT + 7 R2UR.BROADCAST (~74 clocks): more than the tensor time of an MMA of <= 128 tokens.
+        if (leader) {
             int stage = 0; uint32_t phase = 0;
             int buf = 0; uint32_t bphase = 0;          // bit b = phase of TMEM half b
+            const uint32_t tmem_u = (uint32_t)__shfl_sync(0xffffffffu, (int)tmem_base, 0);
+            const uint32_t smem_u = (uint32_t)__shfl_sync(0xffffffffu, (int)smem_u32(smem), 0);
             KPROF(long long kp_t0 = clock64(); long long kp_sched = 0, kp_tmem = 0, kp_full = 0; int kp_units = 0;)
             KTIME(long long kt[5] = {kt_entry, 0, 0, 0, 0}; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(kt[1]));)
             for (int it = 0;; ++it) {
@@ -754,46 +766,51 @@ ffn_wave_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__
                 KPROF(long long kp_a = clock64();)
                 mbar_wait(&ctl->sched_full[ss], (it / kSched) & 1);
                 KPROF(kp_sched += clock64() - kp_a;)
-                const int tile = ctl->sched_tile[ss];
-                mbar_arrive(&ctl->sched_empty[ss]);
+                const int tile = __shfl_sync(0xffffffffu, ctl->sched_tile[ss], 0);   // (also: every lane has read the slot)
+                if (lane == 0) mbar_arrive(&ctl->sched_empty[ss]);
                 if (tile >= total_tiles) break;
                 KPROF(++kp_units;)
                 const Tile t = decode_tile(tab, ctl, tile, p0, p1, early);
-                const int b0 = t.is_long ? 0 : buf, nb = t.is_long ? 2 : 1;
+                const int is_long = __shfl_sync(0xffffffffu, t.is_long, 0), n_mma = __shfl_sync(0xffffffffu, t.n_mma, 0);
+                const int kb0 = __shfl_sync(0xffffffffu, t.kb0, 0), kb1 = __shfl_sync(0xffffffffu, t.kb1, 0);
+                const int b0 = is_long ? 0 : buf, nb = is_long ? 2 : 1;
                 KPROF(long long kp_b = clock64();)
                 for (int h = 0; h < nb; ++h) mbar_wait_cluster(&ctl->tmem_empty[b0 + h], ((bphase >> (b0 + h)) & 1u) ^ 1u);
                 KPROF(kp_tmem += clock64() - kp_b;)
                 tc_fence_after();
-                const uint32_t d0 = tmem_base + (uint32_t)(b0 * 256);
-                const uint32_t d1 = d0 + (t.is_long ? 256u : 128u);
-                const uint32_t idesc = make_idesc(t.n_mma);
-                for (int kb = t.kb0; kb < t.kb1; ++kb) {
+                const uint32_t d0 = tmem_u + (uint32_t)(b0 * 256);
+                const uint32_t d1 = d0 + (is_long ? 256u : 128u);
+                const uint32_t idesc = make_idesc(n_mma);
+                for (int kb = kb0; kb < kb1; ++kb) {
                     KPROF(long long kp_c = clock64();)
                     mbar_wait(&ctl->full[stage], phase);
                     KPROF(kp_full += clock64() - kp_c;)
                     KTIME(if (t.phase == 1 && !kt[3]) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(kt[3]));)
                     tc_fence_after();
-                    const uint32_t sw = smem_u32(smem + (size_t)stage * STAGE_BYTES);
+                    const uint32_t sw = smem_u + (uint32_t)(stage * STAGE_BYTES);
                     const uint32_t sx = sw + W_BYTES;
+                    if (elect_one()) {
 #pragma unroll
-                    for (int k = 0; k < BK / 16; ++k) {
-                        const uint64_t xd = smem_desc(sx + k * 32);
-                        const uint32_t acc = (kb > t.kb0 || k > 0) ? 1u : 0u;
-                        tc_mma(d0, smem_desc(sw + k * 32), xd, idesc, acc);
-                        tc_mma(d1, smem_desc(sw + ACC_M * BK * 2 + k * 32), xd, idesc, acc);
+                        for (int k = 0; k < BK / 16; ++k) {
+                            const uint64_t xd = smem_desc(sx + k * 32);
+                            const uint32_t acc = (kb > kb0 || k > 0) ? 1u : 0u;
+                            tc_mma(d0, smem_desc(sw + k * 32), xd, idesc, acc);
+                            tc_mma(d1, smem_desc(sw + ACC_M * BK * 2 + k * 32), xd, idesc, acc);
+                        }
+                        tc_commit(&ctl->empty[stage]);    // frees the smem stage in both CTAs once these MMAs have read it
                     }
-                    tc_commit(&ctl->empty[stage]);    // frees the smem stage in both CTAs once these MMAs have read it
+                    __syncwarp();
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
-                for (int h = 0; h < nb; ++h) {
-                    tc_commit(&ctl->tmem_full[b0 + h]);
-                    bphase ^= 1u << (b0 + h);
-                }
-                buf = t.is_long ? 0 : (b0 ^ 1);
+                if (elect_one())
+                    for (int h = 0; h < nb; ++h) tc_commit(&ctl->tmem_full[b0 + h]);
+                __syncwarp();
+                for (int h = 0; h < nb; ++h) bphase ^= 1u << (b0 + h);
+                buf = is_long ? 0 : (b0 ^ 1);
                 KTIME(asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(kt[t.phase == 0 ? 2 : 4]));)
             }
-            KTIME(if (kprof) { long long* o = kprof + (size_t)(blockIdx.x >> 1) * 5; for (int i = 0; i < 5; ++i) o[i] = kt[i]; kprof = nullptr; })
-            KPROF(if (kprof) {
+            KTIME(if (kprof && lane == 0) { long long* o = kprof + (size_t)(blockIdx.x >> 1) * 5; for (int i = 0; i < 5; ++i) o[i] = kt[i]; kprof = nullptr; })
+            KPROF(if (kprof && lane == 0) {
                 long long* o = kprof + (size_t)(blockIdx.x >> 1) * 5;
                 o[0] = clock64() - kp_t0; o[1] = kp_sched; o[2] = kp_tmem; o[3] = kp_full; o[4] = kp_units;
             })
